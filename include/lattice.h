@@ -1,0 +1,148 @@
+/*
+ * lattice.h -- C ABI of the B200 (sm_100a) checkerboard Metropolis library.
+ *
+ * What is computed (arXiv:2503.14688, Bisson et al.; line numbers refer to the paper text
+ * PAPER.md as surveyed in SURVEY.md, readings in DESIGN.md):
+ *   - Hamiltonian H = -J sum_<xy> s_x s_y + Delta sum_x s_x^2, J = 1, periodic L x L square
+ *     lattice; spin-1/2 Ising (s = +-1) and spin-1 Blume-Capel (s in {-1,0,+1})
+ *     (Eq. 1).
+ *   - Metropolis dynamics with checkerboard decomposition and multispin coding
+ *     (PAPER.md:32-34): one sweep = black half-sweep ((i+j) even) then white half-sweep;
+ *     time is counted in full-lattice sweeps.
+ *   - Fully disordered start; a per-sweep inverse temperature beta(t): constant
+ *     for protocol 1, time-varying for protocol 2.
+ *   - Acceptance as a 32-bit integer compare: accept iff dE <= 0 or
+ *     u32(site) < floor(2^32 exp(-beta dE)).  u32(site) and every other random bit come from
+ *     Philox4x32-10 keyed by (seed, sweep, colour, site); random
+ *     numbers are generated in registers and never stored.
+ *   - Measurements as exact 64-bit integers: M = sum s, Q = sum s^2 and the axis correlation
+ *     sums S_x(r) = sum_{i,j} s(i,j) s(i,j+r), S_y(r) = sum_{i,j} s(i,j) s(i+r,j)
+ *     (Eq. 2); C(r) = (S_x+S_y)/(2 L^2), e = -(S_x(1)+S_y(1))/L^2 + Delta Q/L^2
+ *     (Eq. 3 with the sign fixed by E_eq = -sqrt 2), xi = I_2/I_1
+ *     (Eq. C1).
+ *
+ * Conventions
+ *   - Every pointer is a HOST pointer unless its name starts with `device_`.
+ *   - Every call that can fail returns an int status (LATTICE_OK == 0).  Outputs are written
+ *     only on LATTICE_OK.  Nothing throws or aborts across this boundary.
+ *   - A handle is not thread-safe; different handles are independent.
+ *   - The library runs only on a CUDA device; there is no CPU fallback.
+ */
+#ifndef LATTICE_H
+#define LATTICE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lattice lattice_t;              /* opaque; owned by the library */
+
+enum { LATTICE_ISING = 0, LATTICE_BLUME_CAPEL = 1 };
+enum {
+    LATTICE_OK = 0,
+    LATTICE_EINVAL = -1,    /* bad argument (see each call)                                */
+    LATTICE_ENOMEM = -2,    /* host or device scratch allocation failed                    */
+    LATTICE_ECUDA = -3,     /* a CUDA call or kernel failed; lattice_last_error() has text */
+    LATTICE_ESTATE = -4     /* call not allowed in the handle's current state              */
+};
+
+/* Bytes of device memory the packed state needs: L*L/8 (Ising, 1 bit/spin) or L*L/4
+ * (Blume-Capel, 2 bits/spin).  Returns 0 if L is not a positive multiple of 64 or the model
+ * is unknown.  Layout inside the buffer (32-bit words):
+ *   Ising:        [colour 0..1][row 0..L-1][word 0..L/64-1]
+ *   Blume-Capel:  [colour 0..1][plane 0 = nonzero, 1 = negative][row][word]
+ * Word k of a row holds the L/2 same-colour sites p = 32k..32k+31 (bit b <-> p = 32k+b),
+ * column j = 2p + ((i + colour) & 1). */
+size_t lattice_state_bytes(uint32_t L, int model);
+
+/* Create a lattice in caller-owned device memory and fill it with the disordered start
+ * (PAPER.md:65): Ising s = +-1 with probability 1/2, Blume-Capel uniform on {-1,0,+1}; t = 0.
+ *   out               receives the handle.
+ *   L                 lattice side, a multiple of 64, L <= 2^20.
+ *   model             LATTICE_ISING or LATTICE_BLUME_CAPEL.
+ *   delta             crystal field Delta of Eq. 1 (ignored for Ising; must be finite).
+ *   seed              Philox key.
+ *   device_buf        device pointer, 16-byte aligned, at least lattice_state_bytes(L, model)
+ *                     bytes.  The caller keeps ownership and must keep it alive until
+ *                     lattice_destroy; the library never frees it.
+ *   cuda_stream       a cudaStream_t (NULL = the legacy default stream).  Every kernel of this
+ *                     handle is launched on it.
+ * The RNG scheme defaults to 1 (bit-plane + tail).
+ * Errors: EINVAL (bad L/model/delta/buffer/alignment/out), ENOMEM, ECUDA. */
+int lattice_create(lattice_t **out, uint32_t L, int model, double delta, uint64_t seed,
+                   void *device_buf, size_t device_buf_bytes, void *cuda_stream);
+
+/* Select how u32(site) is derived from Philox4x32-10:
+ *   0 "quad":       one block per 4 consecutive same-colour sites, one 32-bit word each;
+ *   1 "plane+tail": top 8 bits from 8 bit-plane blocks shared by 128 sites, low 24 bits from a
+ *                   per-site block that is only evaluated when the top byte ties with the
+ *                   threshold's.  Same statistics, ~4x less RNG work.
+ * Only allowed at t == 0 (ESTATE otherwise).  EINVAL for an unknown scheme. */
+int lattice_set_rng_scheme(lattice_t *lat, int scheme);
+
+/* Run sweeps t .. t+n-1; sweep t+k uses beta[k] (host fp64 array of n entries; beta = 1/T).
+ * Thresholds floor(2^32 exp(-beta dE)) are rebuilt on the host whenever beta changes.
+ * Asynchronous on the handle's stream (beta is consumed before the call returns); t += n.
+ * Errors: EINVAL (NULL beta with n > 0, NaN or negative beta, t+n >= 2^32), ECUDA. */
+int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta);
+
+/* One colour (0 = black first, 1 = white) of sweep t at inverse temperature beta, without
+ * advancing t.  lattice_sweep(1, &beta) == half_sweep(0), half_sweep(1), t += 1.  For tests. */
+int lattice_half_sweep(lattice_t *lat, int colour, double beta);
+
+/* Exact integer measurements of the whole lattice, r = 1..r_max (1 <= r_max <= L/2):
+ *   *M = sum s, *Q = sum s^2 (= L^2 for Ising), Sx[r-1] = S_x(r), Sy[r-1] = S_y(r).
+ * Host outputs; synchronises the stream.  Errors: EINVAL, ENOMEM, ECUDA. */
+int lattice_measure(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx,
+                    int64_t *Sy);
+
+/* The same sums restricted to base sites in rows i0 .. i0+n_rows-1 (partners wrap
+ * periodically); the partial sums of a partition of the rows add up to lattice_measure.
+ * For spot checks at L = 2^20 and for future row-slab sharding. */
+int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t r_max,
+                         int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy);
+
+/* Unpacked -1/0/+1 windows, row-major h x w, global origin (i0, j0), periodic wrap.
+ * h, w <= L.  set_spins rejects values outside the model's alphabet (EINVAL).  Both
+ * synchronise the stream.  For tests, windowed replay and checkpoints. */
+int lattice_get_spins(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint32_t w,
+                      int8_t *out);
+int lattice_set_spins(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint32_t w,
+                      const int8_t *in);
+
+/* Sweeps done so far. */
+uint64_t lattice_time(const lattice_t *lat);
+/* Overwrite the sweep counter (checkpoint restore together with the packed words).
+ * EINVAL if t >= 2^32. */
+int lattice_set_time(lattice_t *lat, uint64_t t);
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+uint64_t lattice_launches(const lattice_t *lat);
+
+/* Host-only helpers (no device work).
+ * lattice_thresholds: acceptance thresholds in [0, 2^32] for inverse temperature beta;
+ *   Ising: out[0] = thr(dE = 4), out[1] = thr(dE = 8);
+ *   Blume-Capel: out[(code*2 + b)*9 + (h+4)], code = s+1, b = proposal bit, h = neighbour sum;
+ *   an entry equal to 2^32 means "always accept" (dE <= 0, or exp rounded to 1).
+ * lattice_xi: xi = I_2/I_1 of a single run (reading 14): C(r) = (Sx+Sy)/(2 L^2),
+ *   r_cut = (first r with Sx+Sy <= 0) - 1 or r_max, trapezoid weights (1/2 at r_cut),
+ *   ascending fp64 sums; returns 0 if r_cut < 1; *r_cut_out (may be NULL) receives r_cut.
+ * lattice_energy: e = -(Sx[0]+Sy[0])/L^2 + delta*Q/L^2. */
+void lattice_thresholds(int model, double delta, double beta, uint64_t *out);
+double lattice_xi(const int64_t *Sx, const int64_t *Sy, uint32_t r_max, int64_t Q, uint32_t L,
+                  uint32_t *r_cut_out);
+double lattice_energy(const int64_t *Sx, const int64_t *Sy, int64_t Q, double delta, uint32_t L);
+
+/* Frees the handle and its scratch; never the caller's device_buf. */
+int lattice_destroy(lattice_t *lat);
+
+const char *lattice_strerror(int status);
+/* Text of the last CUDA error seen by this handle ("" if none). */
+const char *lattice_last_error(const lattice_t *lat);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LATTICE_H */

@@ -1,0 +1,12 @@
+"""B200-native checkerboard Metropolis for the 2D Ising and Blume-Capel models.
+
+The product is the C-ABI CUDA library `liblattice.so` (include/lattice.h, csrc/); this package
+is its thin Python binding plus the seeded workload definitions.  There is no CPU fallback.
+"""
+from .binding import (BLUME_CAPEL, ISING, Lattice, LatticeError, energy, lib, state_bytes,
+                      thresholds, xi)
+from .buildlib import build
+from . import workloads
+
+__all__ = ["ISING", "BLUME_CAPEL", "Lattice", "LatticeError", "energy", "lib", "state_bytes",
+           "thresholds", "xi", "build", "workloads"]

@@ -1,0 +1,202 @@
+"""Thin ctypes binding of include/lattice.h: argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used for the
+device buffer and the stream, nothing else.  There is no CPU fallback: if the shared library is
+missing or no CUDA device is present, constructing a `Lattice` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import buildlib as _build
+
+ISING, BLUME_CAPEL = 0, 1
+OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
+
+_lib = None
+
+_u32p, _u64p, _i64p, _i8p, _f64p = (C.POINTER(C.c_uint32), C.POINTER(C.c_uint64),
+                                    C.POINTER(C.c_int64), C.POINTER(C.c_int8),
+                                    C.POINTER(C.c_double))
+_vp = C.c_void_p
+
+#: name -> (restype, argtypes); one entry per symbol declared in include/lattice.h
+SIGNATURES = {
+    "lattice_state_bytes": (C.c_size_t, [C.c_uint32, C.c_int]),
+    "lattice_create": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_double, C.c_uint64,
+                                 _vp, C.c_size_t, _vp]),
+    "lattice_set_rng_scheme": (C.c_int, [_vp, C.c_int]),
+    "lattice_sweep": (C.c_int, [_vp, C.c_uint64, _f64p]),
+    "lattice_half_sweep": (C.c_int, [_vp, C.c_int, C.c_double]),
+    "lattice_measure": (C.c_int, [_vp, C.c_uint32, _i64p, _i64p, _i64p, _i64p]),
+    "lattice_measure_rows": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint32, _i64p, _i64p,
+                                       _i64p, _i64p]),
+    "lattice_get_spins": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _i8p]),
+    "lattice_set_spins": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _i8p]),
+    "lattice_time": (C.c_uint64, [_vp]),
+    "lattice_set_time": (C.c_int, [_vp, C.c_uint64]),
+    "lattice_launches": (C.c_uint64, [_vp]),
+    "lattice_thresholds": (None, [C.c_int, C.c_double, C.c_double, _u64p]),
+    "lattice_xi": (C.c_double, [_i64p, _i64p, C.c_uint32, C.c_int64, C.c_uint32, _u32p]),
+    "lattice_energy": (C.c_double, [_i64p, _i64p, C.c_int64, C.c_double, C.c_uint32]),
+    "lattice_destroy": (C.c_int, [_vp]),
+    "lattice_strerror": (C.c_char_p, [C.c_int]),
+    "lattice_last_error": (C.c_char_p, [_vp]),
+}
+
+
+def lib() -> C.CDLL:
+    """Load liblattice.so (building it with nvcc if the sources are newer)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    if not os.path.exists(path):
+        raise RuntimeError(f"CUDA library {path} is missing and could not be built")
+    L = C.CDLL(path)
+    for name, (res, args) in SIGNATURES.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = L
+    return L
+
+
+class LatticeError(RuntimeError):
+    def __init__(self, what: str, status: int, detail: str = ""):
+        msg = lib().lattice_strerror(status).decode()
+        super().__init__(f"{what}: {msg} ({status}){': ' + detail if detail else ''}")
+        self.status = status
+
+
+def _p(a: np.ndarray, ty):
+    return a.ctypes.data_as(C.POINTER(ty))
+
+
+def state_bytes(L: int, model: int) -> int:
+    return int(lib().lattice_state_bytes(L, model))
+
+
+def thresholds(model: int, delta: float, beta: float) -> np.ndarray:
+    out = np.zeros(2 if model == ISING else 54, dtype=np.uint64)
+    lib().lattice_thresholds(model, float(delta), float(beta), _p(out, C.c_uint64))
+    return out
+
+
+def xi(Sx, Sy, Q: int, L: int):
+    Sx = np.ascontiguousarray(Sx, dtype=np.int64)
+    Sy = np.ascontiguousarray(Sy, dtype=np.int64)
+    rc = C.c_uint32(0)
+    v = lib().lattice_xi(_p(Sx, C.c_int64), _p(Sy, C.c_int64), Sx.size, int(Q), int(L), C.byref(rc))
+    return float(v), int(rc.value)
+
+
+def energy(Sx, Sy, Q: int, delta: float, L: int) -> float:
+    Sx = np.ascontiguousarray(Sx, dtype=np.int64)
+    Sy = np.ascontiguousarray(Sy, dtype=np.int64)
+    return float(lib().lattice_energy(_p(Sx, C.c_int64), _p(Sy, C.c_int64), int(Q), float(delta),
+                                      int(L)))
+
+
+class Lattice:
+    """A packed lattice in device memory (a torch.uint8 tensor owned by this object)."""
+
+    def __init__(self, L: int, model: int = ISING, delta: float = 0.0, seed: int = 0,
+                 scheme: int = 1, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2503_14688_b200 needs a CUDA device; there is no CPU path")
+        self.L, self.model, self.delta, self.seed = int(L), int(model), float(delta), int(seed)
+        nbytes = state_bytes(self.L, self.model)
+        if nbytes == 0:
+            raise LatticeError("lattice_state_bytes", EINVAL, f"L={L} model={model}")
+        self._torch = torch
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            self.buf = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = _vp()
+            rc = lib().lattice_create(C.byref(h), self.L, self.model, self.delta, self.seed,
+                                      _vp(self.buf.data_ptr()), nbytes, _vp(self.stream.cuda_stream))
+        if rc != OK:
+            raise LatticeError("lattice_create", rc)
+        self._h = h
+        if scheme != 1:
+            self._check(lib().lattice_set_rng_scheme(self._h, int(scheme)), "lattice_set_rng_scheme")
+        self.scheme = int(scheme)
+
+    # -- plumbing ---------------------------------------------------------------------------
+    def _check(self, rc: int, what: str) -> None:
+        if rc != OK:
+            detail = lib().lattice_last_error(self._h).decode() if rc == ECUDA else ""
+            raise LatticeError(what, rc, detail)
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            lib().lattice_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the path ---------------------------------------------------------------------------
+    @property
+    def time(self) -> int:
+        return int(lib().lattice_time(self._h))
+
+    @property
+    def launches(self) -> int:
+        return int(lib().lattice_launches(self._h))
+
+    def set_time(self, t: int) -> None:
+        self._check(lib().lattice_set_time(self._h, int(t)), "lattice_set_time")
+
+    def sweep(self, beta) -> None:
+        """Run len(beta) sweeps; beta is a host fp64 array (one entry per sweep)."""
+        b = np.ascontiguousarray(np.atleast_1d(beta), dtype=np.float64)
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_sweep(self._h, b.size, _p(b, C.c_double)), "lattice_sweep")
+
+    def half_sweep(self, colour: int, beta: float) -> None:
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_half_sweep(self._h, int(colour), float(beta)),
+                        "lattice_half_sweep")
+
+    def measure(self, r_max: int, rows=None):
+        """(M, Q, Sx[r_max], Sy[r_max]) as exact integers; rows = (i0, n_rows) for a slab."""
+        Sx = np.zeros(r_max, dtype=np.int64)
+        Sy = np.zeros(r_max, dtype=np.int64)
+        M, Q = C.c_int64(0), C.c_int64(0)
+        with self._torch.cuda.device(self.device):
+            if rows is None:
+                rc = lib().lattice_measure(self._h, r_max, C.byref(M), C.byref(Q),
+                                           _p(Sx, C.c_int64), _p(Sy, C.c_int64))
+            else:
+                rc = lib().lattice_measure_rows(self._h, rows[0], rows[1], r_max, C.byref(M),
+                                                C.byref(Q), _p(Sx, C.c_int64), _p(Sy, C.c_int64))
+        self._check(rc, "lattice_measure")
+        return int(M.value), int(Q.value), Sx, Sy
+
+    def get_spins(self, i0: int = 0, j0: int = 0, h: int | None = None, w: int | None = None):
+        h = self.L if h is None else h
+        w = self.L if w is None else w
+        out = np.zeros((h, w), dtype=np.int8)
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_get_spins(self._h, i0, j0, h, w, _p(out, C.c_int8)),
+                        "lattice_get_spins")
+        return out
+
+    def set_spins(self, spins, i0: int = 0, j0: int = 0) -> None:
+        s = np.ascontiguousarray(spins, dtype=np.int8)
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_set_spins(self._h, i0, j0, s.shape[0], s.shape[1],
+                                                _p(s, C.c_int8)), "lattice_set_spins")
+
+    def synchronize(self) -> None:
+        self.stream.synchronize()

@@ -1,0 +1,471 @@
+// lattice.cu -- host side of the C ABI declared in include/lattice.h.
+//
+// Everything the library computes on the device runs in the kernels of ising.cuh, bc.cuh and
+// measure.cuh; this file validates arguments, builds the integer acceptance thresholds on the
+// host (fp64, once per distinct beta), launches, and converts the device counters into the
+// signed sums the ABI returns.  There is no CPU implementation of any step of the path.
+#include "../../include/lattice.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "bc.cuh"
+#include "ising.cuh"
+#include "measure.cuh"
+#include "philox.cuh"
+
+using namespace lat;
+
+struct lattice {
+    uint32_t L;
+    uint32_t wpr;              // words per row per colour (per plane)
+    int model;
+    double delta;
+    uint64_t seed;
+    int scheme;
+    uint64_t t;
+    uint32_t *buf;             // caller-owned device memory
+    cudaStream_t stream;
+    uint64_t launches;
+    RoundKeys K;
+    // cached thresholds
+    bool have_beta;
+    double beta;
+    uint64_t thr64[54];
+    // device scratch
+    unsigned long long *d_cnt;
+    size_t cnt_cap;            // entries
+    int8_t *d_win;
+    size_t win_cap;            // bytes
+    char err[256];
+};
+
+namespace {
+
+const uint64_t TWO32 = 1ull << 32;
+
+bool model_ok(int m) { return m == LATTICE_ISING || m == LATTICE_BLUME_CAPEL; }
+
+int cuda_fail(lattice *lat, cudaError_t e, const char *what)
+{
+    if (lat) snprintf(lat->err, sizeof lat->err, "%s: %s", what, cudaGetErrorString(e));
+    return LATTICE_ECUDA;
+}
+
+#define CU(lat, call)                                                   \
+    do {                                                                \
+        cudaError_t e_ = (call);                                        \
+        if (e_ != cudaSuccess) return cuda_fail((lat), e_, #call);      \
+    } while (0)
+
+// Metropolis acceptance min(1, exp(-beta dE)) as an integer in [0, 2^32]:
+// floor(2^32 exp(-beta dE)) for dE > 0, 2^32 ("always") for dE <= 0 (reading 4).
+uint64_t threshold_of(double beta, double dE)
+{
+    if (dE <= 0.0) return TWO32;
+    const double x = std::floor(std::ldexp(std::exp(-(beta * dE)), 32));
+    if (!(x > 0.0)) return 0;
+    if (x >= 4294967296.0) return TWO32;
+    return (uint64_t)x;
+}
+
+void build_thresholds(int model, double delta, double beta, uint64_t *out)
+{
+    if (model == LATTICE_ISING) {
+        out[0] = threshold_of(beta, 4.0);
+        out[1] = threshold_of(beta, 8.0);
+        return;
+    }
+    for (int code = 0; code < 3; ++code)
+        for (int b = 0; b < 2; ++b)
+            for (int h = -4; h <= 4; ++h) {
+                const int s = code - 1, s2 = (code + 1 + b) % 3 - 1;
+                const double dE = (double)(s - s2) * (double)h + delta * (double)(s2 * s2 - s * s);
+                out[(code * 2 + b) * 9 + (h + 4)] = threshold_of(beta, dE);
+            }
+}
+
+void refresh_thresholds(lattice *lat, double beta)
+{
+    // bitwise comparison so that -0.0 / +0.0 or any other pair of distinct doubles rebuilds
+    if (lat->have_beta && std::memcmp(&lat->beta, &beta, sizeof beta) == 0) return;
+    build_thresholds(lat->model, lat->delta, beta, lat->thr64);
+    lat->beta = beta;
+    lat->have_beta = true;
+}
+
+uint32_t tile_log2(uint32_t nq)
+{
+    // widest power-of-two tile (<= 8 quads = one 128-byte line) that divides the row
+    uint32_t l = 0;
+    while (l < 3 && (nq % (2u << l)) == 0) ++l;
+    return l;
+}
+
+int launch_half_sweep(lattice *lat, int colour)
+{
+    const uint32_t L = lat->L, wpr = lat->wpr;
+    const size_t pw = (size_t)L * wpr;
+    const bool v4 = (wpr % 4u) == 0;
+    const uint32_t nq = wpr / 4u;
+    uint32_t tq_log2 = 0;
+    unsigned long long blocks;
+    if (v4) {
+        tq_log2 = tile_log2(nq);
+        const uint32_t tr = 256u >> tq_log2;
+        blocks = (unsigned long long)(nq >> tq_log2) * ((L + tr - 1) / tr);
+    } else {
+        blocks = (pw + 255) / 256;
+    }
+    if (blocks > 0x7fffffffull) return LATTICE_EINVAL;
+    const dim3 grid((unsigned)blocks), block(256);
+
+    if (lat->model == LATTICE_ISING) {
+        IsingArgs a;
+        a.tgt = lat->buf + (size_t)colour * pw;
+        a.opp = lat->buf + (size_t)(1 - colour) * pw;
+        a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
+        a.always4 = lat->thr64[0] >= TWO32; a.always8 = lat->thr64[1] >= TWO32;
+        a.thr4 = a.always4 ? 0xffffffffu : (uint32_t)lat->thr64[0];
+        a.thr8 = a.always8 ? 0xffffffffu : (uint32_t)lat->thr64[1];
+        a.tq_log2 = tq_log2;
+        a.K = lat->K;
+        if (v4) {
+            if (lat->scheme == 1) ising_half_sweep_v4<1><<<grid, block, 0, lat->stream>>>(a);
+            else ising_half_sweep_v4<0><<<grid, block, 0, lat->stream>>>(a);
+        } else {
+            if (lat->scheme == 1) ising_half_sweep_v1<1><<<grid, block, 0, lat->stream>>>(a);
+            else ising_half_sweep_v1<0><<<grid, block, 0, lat->stream>>>(a);
+        }
+    } else {
+        BCArgs a;
+        a.tnz = lat->buf + (size_t)(2 * colour) * pw;
+        a.tsg = lat->buf + (size_t)(2 * colour + 1) * pw;
+        a.onz = lat->buf + (size_t)(2 * (1 - colour)) * pw;
+        a.osg = lat->buf + (size_t)(2 * (1 - colour) + 1) * pw;
+        a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
+        a.tq_log2 = tq_log2;
+        a.always_mask = 0; a.decide_mask = 0;
+        for (int type = 0; type < 3; ++type)
+            for (int x = -4; x <= 4; ++x) {
+                // representative (code, b, h) of the (type, x) entry; the mirrored entry
+                // (s -> -s, h -> -h) has the identical dE
+                int idx;
+                if (type == BC_FLIP) idx = (2 * 2 + 0) * 9 + (x + 4);          // +1 -> -1, h = x
+                else if (type == BC_VACATE) idx = (2 * 2 + 1) * 9 + (x + 4);   // +1 -> 0,  h = x
+                else idx = (1 * 2 + 0) * 9 + (-x + 4);                         // 0 -> +1,  h = -x
+                const uint64_t th = lat->thr64[idx];
+                const int e = type * 9 + (x + 4);
+                a.thr[e] = 0;
+                if (th >= TWO32) a.always_mask |= 1u << e;
+                else if (th > 0) { a.decide_mask |= 1u << e; a.thr[e] = (uint32_t)th; }
+            }
+        a.K = lat->K;
+        if (v4) {
+            if (lat->scheme == 1) bc_half_sweep_v4<1><<<grid, block, 0, lat->stream>>>(a);
+            else bc_half_sweep_v4<0><<<grid, block, 0, lat->stream>>>(a);
+        } else {
+            if (lat->scheme == 1) bc_half_sweep_v1<1><<<grid, block, 0, lat->stream>>>(a);
+            else bc_half_sweep_v1<0><<<grid, block, 0, lat->stream>>>(a);
+        }
+    }
+    lat->launches += 1;
+    CU(lat, cudaGetLastError());
+    return LATTICE_OK;
+}
+
+int ensure_cnt(lattice *lat, size_t entries)
+{
+    if (lat->cnt_cap >= entries) return LATTICE_OK;
+    if (lat->d_cnt) cudaFree(lat->d_cnt);
+    lat->d_cnt = nullptr;
+    lat->cnt_cap = 0;
+    if (cudaMalloc(&lat->d_cnt, entries * sizeof(unsigned long long)) != cudaSuccess) {
+        cudaGetLastError();
+        return LATTICE_ENOMEM;
+    }
+    lat->cnt_cap = entries;
+    return LATTICE_OK;
+}
+
+int ensure_win(lattice *lat, size_t bytes)
+{
+    if (lat->win_cap >= bytes) return LATTICE_OK;
+    if (lat->d_win) cudaFree(lat->d_win);
+    lat->d_win = nullptr;
+    lat->win_cap = 0;
+    if (cudaMalloc(&lat->d_win, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return LATTICE_ENOMEM;
+    }
+    lat->win_cap = bytes;
+    return LATTICE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t lattice_state_bytes(uint32_t L, int model)
+{
+    if (L == 0 || (L % 64u) != 0 || L > (1u << 20) || !model_ok(model)) return 0;
+    const size_t n = (size_t)L * L;
+    return model == LATTICE_ISING ? n / 8 : n / 4;
+}
+
+int lattice_create(lattice_t **out, uint32_t L, int model, double delta, uint64_t seed,
+                   void *device_buf, size_t device_buf_bytes, void *cuda_stream)
+{
+    if (!out) return LATTICE_EINVAL;
+    const size_t need = lattice_state_bytes(L, model);
+    if (need == 0 || !std::isfinite(delta) || !device_buf || device_buf_bytes < need ||
+        ((uintptr_t)device_buf & 15u) != 0)
+        return LATTICE_EINVAL;
+    lattice *lat = new (std::nothrow) lattice();
+    if (!lat) return LATTICE_ENOMEM;
+    std::memset(lat, 0, sizeof *lat);
+    lat->L = L; lat->wpr = L / 64u; lat->model = model; lat->delta = delta; lat->seed = seed;
+    lat->scheme = 1; lat->t = 0;
+    lat->buf = (uint32_t *)device_buf;
+    lat->stream = (cudaStream_t)cuda_stream;
+    expand_round_keys(seed, lat->K);
+
+    const unsigned long long threads = 2ull * L * lat->wpr;
+    const unsigned long long blocks = (threads + 255) / 256;
+    if (model == LATTICE_ISING) {
+        IsingInitArgs a; a.buf = lat->buf; a.L = L; a.wpr = lat->wpr; a.K = lat->K;
+        ising_init_kernel<<<(unsigned)blocks, 256, 0, lat->stream>>>(a);
+    } else {
+        BCInitArgs a; a.buf = lat->buf; a.L = L; a.wpr = lat->wpr; a.K = lat->K;
+        bc_init_kernel<<<(unsigned)blocks, 256, 0, lat->stream>>>(a);
+    }
+    lat->launches += 1;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        fprintf(stderr, "lattice_create: init kernel launch failed: %s\n", cudaGetErrorString(e));
+        delete lat;
+        return LATTICE_ECUDA;
+    }
+    *out = lat;
+    return LATTICE_OK;
+}
+
+int lattice_set_rng_scheme(lattice_t *lat, int scheme)
+{
+    if (!lat || (scheme != 0 && scheme != 1)) return LATTICE_EINVAL;
+    if (lat->t != 0) return LATTICE_ESTATE;
+    lat->scheme = scheme;
+    return LATTICE_OK;
+}
+
+int lattice_half_sweep(lattice_t *lat, int colour, double beta)
+{
+    if (!lat || (colour != 0 && colour != 1) || std::isnan(beta) || beta < 0.0) return LATTICE_EINVAL;
+    if (lat->t >= 0xffffffffull) return LATTICE_EINVAL;
+    refresh_thresholds(lat, beta);
+    return launch_half_sweep(lat, colour);
+}
+
+int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta)
+{
+    if (!lat || (n && !beta)) return LATTICE_EINVAL;
+    if (lat->t + n >= TWO32) return LATTICE_EINVAL;
+    for (uint64_t k = 0; k < n; ++k)
+        if (std::isnan(beta[k]) || beta[k] < 0.0) return LATTICE_EINVAL;
+    for (uint64_t k = 0; k < n; ++k) {
+        refresh_thresholds(lat, beta[k]);
+        int rc = launch_half_sweep(lat, 0);      // black = (i+j) even first
+        if (rc) return rc;
+        rc = launch_half_sweep(lat, 1);
+        if (rc) return rc;
+        lat->t += 1;
+    }
+    return LATTICE_OK;
+}
+
+int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t r_max, int64_t *M,
+                         int64_t *Q, int64_t *Sx, int64_t *Sy)
+{
+    if (!lat || !M || !Q || !Sx || !Sy) return LATTICE_EINVAL;
+    const uint64_t L = lat->L;
+    if (r_max < 1 || r_max > L / 2 || i0 >= L || n_rows < 1 || n_rows > L || i0 + n_rows > L)
+        return LATTICE_EINVAL;
+    const size_t entries = 2 + 4 * (size_t)r_max;
+    int rc = ensure_cnt(lat, entries);
+    if (rc) return rc;
+    CU(lat, cudaMemsetAsync(lat->d_cnt, 0, entries * sizeof(unsigned long long), lat->stream));
+    MeasArgs a;
+    a.buf = lat->buf; a.L = lat->L; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
+    a.i0 = (uint32_t)i0; a.n_rows = (uint32_t)n_rows; a.r_max = r_max; a.r0 = 0; a.cnt = lat->d_cnt;
+    const unsigned long long words = 2ull * n_rows * lat->wpr;
+    unsigned bx = (unsigned)((words + 255) / 256);
+    {
+        const unsigned gx = bx > 148u * 16u ? 148u * 16u : bx;
+        measure_mq_kernel<<<gx, 256, 0, lat->stream>>>(a);
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+    }
+    // correlation passes: at most 65535 r values per launch in grid.y
+    {
+        unsigned gx = bx;
+        const unsigned long long cap = (148ull * 32ull + 2ull * r_max - 1) / (2ull * r_max);
+        if (gx > cap) gx = (unsigned)(cap ? cap : 1);
+        if (gx < 1) gx = 1;
+        for (uint32_t r0 = 0; r0 < r_max; r0 += 65535u) {
+            const uint32_t nr = (r_max - r0 < 65535u) ? r_max - r0 : 65535u;
+            a.r0 = r0;
+            measure_corr_kernel<<<dim3(gx, nr, 2), 256, 0, lat->stream>>>(a);
+            lat->launches += 1;
+            CU(lat, cudaGetLastError());
+        }
+    }
+    unsigned long long *h = (unsigned long long *)std::malloc(entries * sizeof(unsigned long long));
+    if (!h) return LATTICE_ENOMEM;
+    cudaError_t e = cudaMemcpyAsync(h, lat->d_cnt, entries * sizeof(unsigned long long),
+                                    cudaMemcpyDeviceToHost, lat->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(lat->stream);
+    if (e != cudaSuccess) { std::free(h); return cuda_fail(lat, e, "measure copy/sync"); }
+    const int64_t N = (int64_t)(n_rows * L);
+    if (lat->model == LATTICE_ISING) {
+        *M = 2 * (int64_t)h[0] - N;
+        *Q = N;
+        for (uint32_t r = 0; r < r_max; ++r) {
+            Sx[r] = N - 2 * (int64_t)h[2 + 2 * (size_t)r];
+            Sy[r] = N - 2 * (int64_t)h[2 + 2 * ((size_t)r_max + r)];
+        }
+    } else {
+        *M = (int64_t)h[0] - (int64_t)h[1];
+        *Q = (int64_t)h[0] + (int64_t)h[1];
+        for (uint32_t r = 0; r < r_max; ++r) {
+            Sx[r] = (int64_t)h[2 + 2 * (size_t)r] - 2 * (int64_t)h[3 + 2 * (size_t)r];
+            Sy[r] = (int64_t)h[2 + 2 * ((size_t)r_max + r)] - 2 * (int64_t)h[3 + 2 * ((size_t)r_max + r)];
+        }
+    }
+    std::free(h);
+    return LATTICE_OK;
+}
+
+int lattice_measure(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy)
+{
+    if (!lat) return LATTICE_EINVAL;
+    return lattice_measure_rows(lat, 0, lat->L, r_max, M, Q, Sx, Sy);
+}
+
+static int window_call(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint32_t w, int8_t *host,
+                       bool set)
+{
+    if (!lat || !host) return LATTICE_EINVAL;
+    const uint64_t L = lat->L;
+    if (h < 1 || w < 1 || h > L || w > L || i0 >= L || j0 >= L) return LATTICE_EINVAL;
+    const size_t bytes = (size_t)h * w;
+    if (set) {
+        for (size_t k = 0; k < bytes; ++k) {
+            const int v = host[k];
+            if (v < -1 || v > 1 || (lat->model == LATTICE_ISING && v == 0)) return LATTICE_EINVAL;
+        }
+    }
+    int rc = ensure_win(lat, bytes);
+    if (rc) return rc;
+    WindowArgs a;
+    a.buf = lat->buf; a.L = lat->L; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
+    a.i0 = (uint32_t)i0; a.j0 = (uint32_t)j0; a.h = h; a.w = w; a.spins = lat->d_win;
+    const unsigned long long blocks = (bytes + 255) / 256;
+    if (blocks > 0x7fffffffull) return LATTICE_EINVAL;
+    if (set) {
+        CU(lat, cudaMemcpyAsync(lat->d_win, host, bytes, cudaMemcpyHostToDevice, lat->stream));
+        set_spins_kernel<<<(unsigned)blocks, 256, 0, lat->stream>>>(a);
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+        CU(lat, cudaStreamSynchronize(lat->stream));
+    } else {
+        get_spins_kernel<<<(unsigned)blocks, 256, 0, lat->stream>>>(a);
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+        CU(lat, cudaMemcpyAsync(host, lat->d_win, bytes, cudaMemcpyDeviceToHost, lat->stream));
+        CU(lat, cudaStreamSynchronize(lat->stream));
+    }
+    return LATTICE_OK;
+}
+
+int lattice_get_spins(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint32_t w, int8_t *out)
+{
+    return window_call(lat, i0, j0, h, w, out, false);
+}
+
+int lattice_set_spins(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint32_t w, const int8_t *in)
+{
+    return window_call(lat, i0, j0, h, w, const_cast<int8_t *>(in), true);
+}
+
+uint64_t lattice_time(const lattice_t *lat) { return lat ? lat->t : 0; }
+
+int lattice_set_time(lattice_t *lat, uint64_t t)
+{
+    if (!lat || t >= TWO32) return LATTICE_EINVAL;
+    lat->t = t;
+    return LATTICE_OK;
+}
+
+uint64_t lattice_launches(const lattice_t *lat) { return lat ? lat->launches : 0; }
+
+void lattice_thresholds(int model, double delta, double beta, uint64_t *out)
+{
+    if (!out || !model_ok(model)) return;
+    build_thresholds(model, delta, beta, out);
+}
+
+double lattice_xi(const int64_t *Sx, const int64_t *Sy, uint32_t r_max, int64_t Q, uint32_t L,
+                  uint32_t *r_cut_out)
+{
+    (void)Q;   // the r = 0 term C(0) = Q/L^2 carries weight r^n = 0
+    uint32_t r_cut = r_max;
+    for (uint32_t r = 1; r <= r_max; ++r)
+        if (Sx[r - 1] + Sy[r - 1] <= 0) { r_cut = r - 1; break; }
+    if (r_cut_out) *r_cut_out = r_cut;
+    if (r_cut < 1) return 0.0;
+    const double norm = 2.0 * (double)L * (double)L;
+    double I1 = 0.0, I2 = 0.0;
+    for (uint32_t r = 1; r <= r_cut; ++r) {
+        const double C = (double)(Sx[r - 1] + Sy[r - 1]) / norm;
+        const double wgt = (r == r_cut) ? 0.5 : 1.0;
+        I1 += wgt * (double)r * C;
+        I2 += wgt * (double)r * (double)r * C;
+    }
+    return I2 / I1;
+}
+
+double lattice_energy(const int64_t *Sx, const int64_t *Sy, int64_t Q, double delta, uint32_t L)
+{
+    const double n = (double)L * (double)L;
+    return -((double)(Sx[0] + Sy[0])) / n + delta * (double)Q / n;
+}
+
+int lattice_destroy(lattice_t *lat)
+{
+    if (!lat) return LATTICE_EINVAL;
+    if (lat->d_cnt) cudaFree(lat->d_cnt);
+    if (lat->d_win) cudaFree(lat->d_win);
+    delete lat;
+    return LATTICE_OK;
+}
+
+const char *lattice_strerror(int status)
+{
+    switch (status) {
+    case LATTICE_OK: return "ok";
+    case LATTICE_EINVAL: return "invalid argument";
+    case LATTICE_ENOMEM: return "out of memory";
+    case LATTICE_ECUDA: return "CUDA error";
+    case LATTICE_ESTATE: return "call not allowed in this state";
+    default: return "unknown status";
+    }
+}
+
+const char *lattice_last_error(const lattice_t *lat) { return lat ? lat->err : ""; }
+
+}  // extern "C"

@@ -1,0 +1,250 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded inputs.  Spins and integer counts must match bit for bit; xi to 1e-12 relative
+(BASELINE.json north_star)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2503_14688_b200 as lat
+from paper_2503_14688_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+BETA_C = workloads.BETA_C_ISING
+NCPU = os.cpu_count() or 1
+
+
+@pytest.fixture(autouse=True)
+def _threads():
+    oracle.set_threads(NCPU)
+    yield
+    oracle.set_threads(1)
+
+
+def _same_measure(g, o, r_max, L, delta=0.0, rows=None):
+    Mg, Qg, Sxg, Syg = g.measure(r_max, rows)
+    Mo, Qo, Sxo, Syo = o.measure(r_max, rows)
+    assert (Mg, Qg) == (Mo, Qo)
+    assert np.array_equal(Sxg, Sxo) and np.array_equal(Syg, Syo)
+    if rows is None:
+        xg, rg = lat.xi(Sxg, Syg, Qg, L)
+        xo, ro = oracle.xi(Sxo, Syo, Qo, L)
+        assert rg == ro
+        assert xg == xo or abs(xg - xo) <= 1e-12 * abs(xo)          # north_star tolerance
+        eg, eo = lat.energy(Sxg, Syg, Qg, delta, L), oracle.energy(Sxo, Syo, Qo, delta, L)
+        assert eg == eo or abs(eg - eo) <= 1e-12 * abs(eo)
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+@pytest.mark.parametrize("L", [64, 128, 192, 256, 768, 1024])
+def test_initial_state(L, model):
+    g = lat.Lattice(L, model, 0.0, seed=77 + L)
+    o = oracle.OracleLattice(L, model, 0.0, seed=77 + L)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    _same_measure(g, o, min(L // 2, 48), L)
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_config1_ising_L64_whole_run(scheme):
+    """BASELINE.json config 1, whole: 2000 sweeps at beta_c, records at sweeps 2^k."""
+    w = workloads.CONFIGS["ising_L64"]
+    g = lat.Lattice(w.L, w.model, w.delta, w.seed, scheme)
+    o = oracle.OracleLattice(w.L, w.model, w.delta, w.seed, scheme)
+    done = 0
+    for t in w.measure_times():
+        beta = w.beta_schedule(t - done, done)
+        if t > done:
+            g.sweep(beta)
+            o.sweep(beta)
+            done = t
+        assert g.time == o.time == t
+        assert np.array_equal(g.get_spins(), o.get_spins()), t
+        _same_measure(g, o, w.r_max, w.L)
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+@pytest.mark.parametrize("L,sweeps", [(128, 300), (192, 100), (256, 200), (512, 100), (768, 40),
+                                      (2048, 24)])
+def test_ising_sweeps(L, sweeps, scheme):
+    g = lat.Lattice(L, lat.ISING, 0.0, 4242 + L, scheme)
+    o = oracle.OracleLattice(L, lat.ISING, 0.0, 4242 + L, scheme)
+    for n in (1, 1, sweeps - 2):
+        g.sweep([BETA_C] * n)
+        o.sweep([BETA_C] * n)
+        assert np.array_equal(g.get_spins(), o.get_spins())
+    _same_measure(g, o, min(L // 2, 64), L)
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+@pytest.mark.parametrize("L,delta,T,sweeps", [(64, 0.0, 1.6934, 400), (128, 0.0, 1.6934, 100),
+                                              (192, 0.7, 1.2, 60), (256, 0.0, 1.6934, 100),
+                                              (256, -1.3, 2.0, 60), (512, 1.965, 0.6, 40),
+                                              (1024, 0.0, 1.6934, 24), (256, -50.0, 1.5, 30)])
+def test_blume_capel_sweeps(L, delta, T, sweeps, scheme):
+    g = lat.Lattice(L, lat.BLUME_CAPEL, delta, 31 + L, scheme)
+    o = oracle.OracleLattice(L, lat.BLUME_CAPEL, delta, 31 + L, scheme)
+    for n in (1, 1, sweeps - 2):
+        g.sweep([1.0 / T] * n)
+        o.sweep([1.0 / T] * n)
+        assert np.array_equal(g.get_spins(), o.get_spins())
+    _same_measure(g, o, min(L // 2, 64), L, delta)
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_half_sweeps_and_extreme_temperatures(model, scheme):
+    L = 256
+    g = lat.Lattice(L, model, 0.3, 5, scheme)
+    o = oracle.OracleLattice(L, model, 0.3, 5, scheme)
+    for beta in (0.0, 0.0, math.inf, 1e-12, 40.0, 0.3, math.inf, 0.0):
+        for colour in (0, 1):
+            g.half_sweep(colour, beta)
+            o.half_sweep(colour, beta)
+            assert np.array_equal(g.get_spins(), o.get_spins()), (beta, colour)
+        g.sweep([beta])
+        o.sweep([beta])
+        assert np.array_equal(g.get_spins(), o.get_spins()), beta
+
+
+def test_ising_infinite_temperature_flips_every_spin():
+    g = lat.Lattice(512, lat.ISING, 0.0, 3)
+    s0 = g.get_spins()
+    M0, Q0, Sx0, Sy0 = g.measure(16)
+    g.sweep([0.0])
+    assert np.array_equal(g.get_spins(), -s0)
+    M1, Q1, Sx1, Sy1 = g.measure(16)
+    assert M1 == -M0 and np.array_equal(Sx0, Sx1) and np.array_equal(Sy0, Sy1)
+
+
+def test_zero_temperature_fixed_point_and_single_defect():
+    L = 256
+    g = lat.Lattice(L, lat.ISING, 0.0, 3)
+    up = np.ones((L, L), dtype=np.int8)
+    g.set_spins(up)
+    g.sweep([math.inf] * 3)
+    assert np.array_equal(g.get_spins(), up)
+    d = up.copy()
+    d[17, 33] = -1
+    d[200, 0] = -1
+    g.set_spins(d)
+    g.sweep([math.inf])
+    assert np.array_equal(g.get_spins(), up)
+    M, Q, Sx, Sy = g.measure(L // 2)
+    assert M == L * L and (Sx == L * L).all() and (Sy == L * L).all()
+
+
+@pytest.mark.parametrize("name", ["ising_L2p16_ramp", "bc_L2p15_ramp"])
+def test_protocol2_schedule_small(name):
+    """BASELINE.json config 5's beta(t) ramp on a small lattice: thresholds change every sweep."""
+    w = workloads.CONFIGS[name]
+    L = 256
+    g = lat.Lattice(L, w.model, w.delta, w.seed)
+    o = oracle.OracleLattice(L, w.model, w.delta, w.seed)
+    sched = w.beta_schedule(1100)
+    assert len(np.unique(sched)) == 1000
+    beta = sched[::11]                       # 100 distinct values spanning the ramp and the plateau
+    g.sweep(beta)
+    o.sweep(beta)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    _same_measure(g, o, 64, L, w.delta)
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+def test_special_states_and_set_get_roundtrip(model):
+    L = 128
+    g = lat.Lattice(L, model, 0.0, 9)
+    o = oracle.OracleLattice(L, model, 0.0, 9)
+    rng = np.random.default_rng(1)
+    vals = np.array([-1, 1] if model == lat.ISING else [-1, 0, 1], dtype=np.int8)
+    i, j = np.indices((L, L))
+    for s in (np.ones((L, L), np.int8), np.where((i + j) % 2 == 0, 1, -1).astype(np.int8),
+              np.where(i % 2 == 0, 1, -1).astype(np.int8), np.where(j % 4 < 2, 1, -1).astype(np.int8),
+              rng.choice(vals, (L, L))):
+        g.set_spins(s)
+        o.set_spins(s)
+        assert np.array_equal(g.get_spins(), s)
+        _same_measure(g, o, L // 2, L)
+    # windows with periodic wrap
+    win = rng.choice(vals, (40, 70))
+    g.set_spins(win, 100, 90)
+    o.set_spins(win, 100, 90)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    assert np.array_equal(g.get_spins(100, 90, 40, 70), win)
+    if model == lat.ISING:
+        with pytest.raises(lat.LatticeError):
+            g.set_spins(np.zeros((2, 2), np.int8))
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+def test_measure_rows_partition(model):
+    L = 256
+    g = lat.Lattice(L, model, 0.0, 21)
+    o = oracle.OracleLattice(L, model, 0.0, 21)
+    beta = BETA_C if model == lat.ISING else workloads.BETA_BC
+    g.sweep([beta] * 20)
+    o.sweep([beta] * 20)
+    tot = None
+    for i0, n in ((0, 1), (1, 100), (101, 155)):
+        _same_measure(g, o, 100, L, rows=(i0, n))
+        M, Q, Sx, Sy = g.measure(100, (i0, n))
+        part = np.concatenate([[M, Q], Sx, Sy])
+        tot = part if tot is None else tot + part
+    M, Q, Sx, Sy = g.measure(100)
+    assert np.array_equal(tot, np.concatenate([[M, Q], Sx, Sy]))
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+def test_determinism_and_checkpoint_resume(model):
+    L = 512
+    beta = [0.4] * 10
+    a = lat.Lattice(L, model, 0.2, 8)
+    a.sweep(beta + beta)
+    b = lat.Lattice(L, model, 0.2, 8)
+    b.sweep(beta)
+    snap, t = b.get_spins(), b.time
+    c = lat.Lattice(L, model, 0.2, 999)          # different start, then restored
+    c2 = lat.Lattice(L, model, 0.2, 8)
+    c2.set_spins(snap)
+    c2.set_time(t)
+    c2.sweep(beta)
+    assert np.array_equal(a.get_spins(), c2.get_spins())
+    assert not np.array_equal(a.get_spins(), c.get_spins())
+    a.close(); b.close(); c.close(); c2.close()
+
+
+def test_api_errors_on_device():
+    g = lat.Lattice(64, lat.ISING, 0.0, 1)
+    with pytest.raises(lat.LatticeError):
+        g.sweep([-0.1])
+    with pytest.raises(lat.LatticeError):
+        g.sweep([math.nan])
+    with pytest.raises(lat.LatticeError):
+        g.measure(33)
+    with pytest.raises(lat.LatticeError):
+        g.measure(0)
+    g.sweep([0.3])
+    with pytest.raises(lat.LatticeError) as e:
+        lat.binding.Lattice._check(g, lat.lib().lattice_set_rng_scheme(g._h, 0), "set_rng_scheme")
+    assert e.value.status == lat.binding.ESTATE
+    assert g.launches == 3                         # init + two half-sweeps
+
+
+def test_first_half_sweep_acceptance_closed_form():
+    """No oracle: on an i.i.d. start the first black half-sweep at beta_c flips a fraction
+    11/16 + (sqrt2-1)^2/4 + (sqrt2-1)^4/16 of the black spins (SURVEY 8c pins)."""
+    L = 4096
+    g = lat.Lattice(L, lat.ISING, 0.0, 12345)
+    s0 = g.get_spins()
+    g.half_sweep(0, BETA_C)
+    s1 = g.get_spins()
+    i, j = np.indices((L, L))
+    black = (i + j) % 2 == 0
+    assert np.array_equal(s0[~black], s1[~black])
+    frac = float((s0[black] != s1[black]).mean())
+    a = math.sqrt(2) - 1
+    want = 11 / 16 + a ** 2 / 4 + a ** 4 / 16
+    sigma = math.sqrt(want * (1 - want) / black.sum())
+    assert abs(frac - want) < 5 * sigma
