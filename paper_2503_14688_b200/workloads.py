@@ -44,7 +44,7 @@ class Workload:
             return np.full(n, self.beta_f, dtype=np.float64)
         # protocol 2: beta ramps linearly from 0.9*beta_f to beta_f over sweeps 0..999
         ramp = 0.9 * self.beta_f + (0.1 * self.beta_f) * (t / 999.0)
-        return np.where(t <= 999.0, ramp, self.beta_f).astype(np.float64)
+        return np.where(t < 999.0, ramp, self.beta_f).astype(np.float64)
 
     def measure_times(self, n: int | None = None) -> list[int]:
         """Sweep counts after which measurements are recorded: {0} u {2^k <= n} u {n}."""
