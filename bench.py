@@ -285,7 +285,7 @@ def main():
     alg_bytes = bpu * updates_per_step / 2          # per half-sweep launch
     achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
     in_l2 = lat.state_bytes(L, w.model) <= (126 << 20)
-    roofline = {"bound": "hbm", "kernel": "ising_half_sweep_v4" if w.model == 0 else "bc_half_sweep_v4",
+    roofline = {"bound": "hbm", "kernel": "ising_march_kernel" if w.model == 0 else "bc_half_sweep_v4",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": None, "peak_source": peak_src, "bytes_per_update": bpu,
                 "launch_ms": launch_ms, "l2_resident": in_l2}

@@ -16,6 +16,7 @@
 
 #include "bc.cuh"
 #include "ising.cuh"
+#include "ising_march.cuh"
 #include "measure.cuh"
 #include "philox.cuh"
 
@@ -107,8 +108,47 @@ uint32_t tile_log2(uint32_t nq)
     return l;
 }
 
+// Rows per thread of the marching kernels: the largest power of two <= 32 that divides L,
+// keeps the thread count a multiple of 32 (whole warps) and still leaves enough threads to
+// fill 148 SMs several times over; 2 (always valid for L % 256 == 0) for small lattices.
+uint32_t march_rows(uint32_t L, uint32_t nq)
+{
+    for (uint32_t R = 32; R > 2; R >>= 1) {
+        if (L % R) continue;
+        const unsigned long long threads = (unsigned long long)nq * (L / R);
+        if ((threads % 32u) == 0 && threads >= (1ull << 19)) return R;
+    }
+    return 2;
+}
+
+int launch_ising_march(lattice *lat, int colour)
+{
+    const uint32_t L = lat->L, wpr = lat->wpr, nq = wpr / 4u;
+    const size_t pw = (size_t)L * wpr;
+    IsingMarchArgs a;
+    a.tgt = lat->buf + (size_t)colour * pw;
+    a.opp = lat->buf + (size_t)(1 - colour) * pw;
+    a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
+    a.always4 = lat->thr64[0] >= TWO32; a.always8 = lat->thr64[1] >= TWO32;
+    a.thr4 = a.always4 ? 0xffffffffu : (uint32_t)lat->thr64[0];
+    a.thr8 = a.always8 ? 0xffffffffu : (uint32_t)lat->thr64[1];
+    a.top4 = a.thr4 >> 24; a.top8 = a.thr8 >> 24;
+    a.R = march_rows(L, nq);
+    a.threads = nq * (L / a.R);
+    a.K = lat->K;
+    build_plane_fold(lat->K, a.t, a.colour, TAG_ACC_PLANE, a.F);
+    const unsigned blocks = (a.threads + 255u) / 256u;
+    if (colour == 0) ising_march_kernel<0><<<blocks, 256, 0, lat->stream>>>(a);
+    else ising_march_kernel<1><<<blocks, 256, 0, lat->stream>>>(a);
+    lat->launches += 1;
+    CU(lat, cudaGetLastError());
+    return LATTICE_OK;
+}
+
 int launch_half_sweep(lattice *lat, int colour)
 {
+    if (lat->model == LATTICE_ISING && lat->scheme == 1 && (lat->wpr % 4u) == 0)
+        return launch_ising_march(lat, colour);
     const uint32_t L = lat->L, wpr = lat->wpr;
     const size_t pw = (size_t)L * wpr;
     const bool v4 = (wpr % 4u) == 0;
