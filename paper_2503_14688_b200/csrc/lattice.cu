@@ -339,30 +339,66 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
     int rc = ensure_cnt(lat, entries);
     if (rc) return rc;
     CU(lat, cudaMemsetAsync(lat->d_cnt, 0, entries * sizeof(unsigned long long), lat->stream));
-    MeasArgs a;
-    a.buf = lat->buf; a.L = lat->L; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
-    a.i0 = (uint32_t)i0; a.n_rows = (uint32_t)n_rows; a.r_max = r_max; a.r0 = 0; a.cnt = lat->d_cnt;
-    const unsigned long long words = 2ull * n_rows * lat->wpr;
-    unsigned bx = (unsigned)((words + 255) / 256);
-    {
-        const unsigned gx = bx > 148u * 16u ? 148u * 16u : bx;
-        measure_mq_kernel<<<gx, 256, 0, lat->stream>>>(a);
+    // Row-blocked kernels: the y axis (and M, Q) over the whole 16-row blocks of the slab, the
+    // x axis over every row when a row is a whole number of 16-word segments.  Whatever they do
+    // not cover (ragged rows, narrow lattices) goes through the generic kernels.
+    const uint32_t nblk = (uint32_t)(n_rows / MEAS_NB);
+    const uint32_t rows_blk = nblk * MEAS_NB;
+    const bool x_blk = (lat->wpr % MEAS_NB) == 0;
+    const unsigned chunks = (r_max + MEAS_RC - 1) / MEAS_RC;
+    MeasBlkArgs b;
+    b.buf = lat->buf; b.L = lat->L; b.wpr = lat->wpr; b.i0 = (uint32_t)i0; b.r_max = r_max; b.cnt = lat->d_cnt;
+    if (nblk) {
+        b.n = nblk;
+        const unsigned long long threads = 2ull * nblk * lat->wpr;
+        const dim3 grid((unsigned)((threads + 127) / 128), chunks);
+        if (lat->model == LATTICE_ISING) measure_y_kernel<0><<<grid, 128, 0, lat->stream>>>(b);
+        else measure_y_kernel<1><<<grid, 128, 0, lat->stream>>>(b);
         lat->launches += 1;
         CU(lat, cudaGetLastError());
     }
-    // correlation passes: at most 65535 r values per launch in grid.y
-    {
+    if (x_blk) {
+        b.n = (uint32_t)n_rows;
+        const unsigned long long threads = 2ull * n_rows * (lat->wpr / MEAS_NB);
+        const dim3 grid((unsigned)((threads + 127) / 128), chunks);
+        if (lat->model == LATTICE_ISING) measure_x_kernel<0><<<grid, 128, 0, lat->stream>>>(b);
+        else measure_x_kernel<1><<<grid, 128, 0, lat->stream>>>(b);
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+    }
+    MeasArgs a;
+    a.buf = lat->buf; a.L = lat->L; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
+    a.r_max = r_max; a.r0 = 0; a.axis0 = 0; a.cnt = lat->d_cnt;
+    auto generic = [&](uint32_t gi0, uint32_t gn, bool mq, uint32_t axis0, uint32_t naxes) -> int {
+        a.i0 = gi0; a.n_rows = gn; a.axis0 = axis0;
+        const unsigned long long words = 2ull * gn * lat->wpr;
+        const unsigned bx = (unsigned)((words + 255) / 256);
+        if (mq) {
+            const unsigned gx = bx > 148u * 16u ? 148u * 16u : bx;
+            measure_mq_kernel<<<gx, 256, 0, lat->stream>>>(a);
+            lat->launches += 1;
+            CU(lat, cudaGetLastError());
+        }
         unsigned gx = bx;
         const unsigned long long cap = (148ull * 32ull + 2ull * r_max - 1) / (2ull * r_max);
         if (gx > cap) gx = (unsigned)(cap ? cap : 1);
         if (gx < 1) gx = 1;
-        for (uint32_t r0 = 0; r0 < r_max; r0 += 65535u) {
+        for (uint32_t r0 = 0; r0 < r_max; r0 += 65535u) {     // at most 65535 r values in grid.y
             const uint32_t nr = (r_max - r0 < 65535u) ? r_max - r0 : 65535u;
             a.r0 = r0;
-            measure_corr_kernel<<<dim3(gx, nr, 2), 256, 0, lat->stream>>>(a);
+            measure_corr_kernel<<<dim3(gx, nr, naxes), 256, 0, lat->stream>>>(a);
             lat->launches += 1;
             CU(lat, cudaGetLastError());
         }
+        return LATTICE_OK;
+    };
+    if (rows_blk < n_rows) {            // ragged rows: M, Q, y axis (and x axis if not done above)
+        rc = generic((uint32_t)i0 + rows_blk, (uint32_t)n_rows - rows_blk, true, x_blk ? 1u : 0u, x_blk ? 1u : 2u);
+        if (rc) return rc;
+    }
+    if (!x_blk && rows_blk) {           // narrow lattice: x axis of the blocked rows
+        rc = generic((uint32_t)i0, rows_blk, false, 0u, 1u);
+        if (rc) return rc;
     }
     unsigned long long *h = (unsigned long long *)std::malloc(entries * sizeof(unsigned long long));
     if (!h) return LATTICE_ENOMEM;

@@ -26,6 +26,7 @@ struct MeasArgs {
     uint32_t i0, n_rows;             // base rows i0 .. i0+n_rows-1
     uint32_t r_max;
     uint32_t r0;                     // this launch covers r = r0+1 .. r0+gridDim.y
+    uint32_t axis0;                  // axis of blockIdx.z == 0 (0 = x, 1 = y)
     unsigned long long *cnt;
 };
 
@@ -81,10 +82,10 @@ __global__ void __launch_bounds__(256) measure_mq_kernel(const MeasArgs a)
     block_add2(c0, c1, a.cnt);
 }
 
-// grid = (blocks_x, n_r, 2): r = r0 + blockIdx.y + 1, blockIdx.z = axis (0 = x, 1 = y)
+// grid = (blocks_x, n_r, n_axes): r = r0 + blockIdx.y + 1, axis = axis0 + blockIdx.z (0 = x, 1 = y)
 __global__ void __launch_bounds__(256) measure_corr_kernel(const MeasArgs a)
 {
-    const uint32_t r = a.r0 + blockIdx.y + 1, axis = blockIdx.z;
+    const uint32_t r = a.r0 + blockIdx.y + 1, axis = a.axis0 + blockIdx.z;
     const uint32_t L = a.L, wpr = a.wpr;
     const unsigned long long per_colour = (unsigned long long)a.n_rows * wpr;
     const unsigned long long total = 2ull * per_colour;
@@ -123,6 +124,284 @@ __global__ void __launch_bounds__(256) measure_corr_kernel(const MeasArgs a)
         }
     }
     block_add2(c0, c1, a.cnt + 2 + 2 * ((size_t)axis * a.r_max + (r - 1)));
+}
+
+// ---- row-blocked kernels (the production measurement path) ----------------------------------
+//
+// The generic kernel above re-reads the lattice once per (r, axis) and pays one POPC per word.
+// The two kernels below keep 16 base words per thread in registers, slide the partner words
+// past them (one new row, or one more bit of funnel shift, per step of r) and reduce the 16
+// XOR words of one r with a carry-save adder tree (30 LOP3) before 5 POPCs, so the cost per
+// (word, r) is ~3 (y axis) to ~4 (x axis) ALU instructions and the lattice is read from DRAM
+// about once per chunk of MEAS_RC values of r.  Per-r counts are summed over the warp with
+// REDUX and accumulated in shared memory; one 64-bit atomic per (block, r) reaches global
+// memory.  blockIdx.y selects the chunk r = r0+1 .. r0+MEAS_RC, r0 = MEAS_RC * blockIdx.y.
+constexpr int MEAS_NB = 16;      // base words per thread (rows for the y axis, words for the x axis)
+constexpr int MEAS_RC = 64;      // values of r per chunk (even)
+
+// population count of 16 words as 5 bit-sliced words of weight 1, 2, 4, 8, 16
+__device__ __forceinline__ void csa(uint32_t a, uint32_t b, uint32_t c, uint32_t &s, uint32_t &cy)
+{
+    s = a ^ b ^ c;
+    cy = (a & b) | (a & c) | (b & c);
+}
+__device__ __forceinline__ uint32_t weighted_popc16(const uint32_t (&x)[16])
+{
+    uint32_t s[4], t[8], u[4], v[2];
+    // weight 1: 16 -> 1 (+ 8 of weight 2)
+    uint32_t a0, a1, a2, a3, a4, a5, a6;
+    csa(x[0], x[1], x[2], a0, t[0]);
+    csa(x[3], x[4], x[5], a1, t[1]);
+    csa(x[6], x[7], x[8], a2, t[2]);
+    csa(x[9], x[10], x[11], a3, t[3]);
+    csa(x[12], x[13], x[14], a4, t[4]);
+    csa(a0, a1, a2, a5, t[5]);
+    csa(a3, a4, x[15], a6, t[6]);
+    const uint32_t w1 = a5 ^ a6;
+    t[7] = a5 & a6;
+    // weight 2: 8 -> 1 (+ 4 of weight 4)
+    csa(t[0], t[1], t[2], s[0], u[0]);
+    csa(t[3], t[4], t[5], s[1], u[1]);
+    csa(s[0], s[1], t[6], s[2], u[2]);
+    const uint32_t w2 = s[2] ^ t[7];
+    u[3] = s[2] & t[7];
+    // weight 4: 4 -> 1 (+ 2 of weight 8)
+    csa(u[0], u[1], u[2], s[3], v[0]);
+    const uint32_t w4 = s[3] ^ u[3];
+    v[1] = s[3] & u[3];
+    // weight 8: 2 -> 1 (+ 1 of weight 16)
+    const uint32_t w8 = v[0] ^ v[1];
+    const uint32_t w16 = v[0] & v[1];
+    return __popc(w1) + 2u * __popc(w2) + 4u * __popc(w4) + 8u * __popc(w8) + 16u * __popc(w16);
+}
+
+struct MeasBlkArgs {
+    const uint32_t *buf;
+    uint32_t L, wpr;
+    uint32_t i0;                     // first base row
+    uint32_t n;                      // y kernel: number of 16-row blocks; x kernel: number of rows
+    uint32_t r_max;
+    unsigned long long *cnt;         // same layout as MeasArgs::cnt
+};
+
+template <int MODEL>
+__device__ __forceinline__ const uint32_t *blk_plane(const MeasBlkArgs &a, uint32_t colour, uint32_t plane)
+{
+    const size_t pw = (size_t)a.L * a.wpr;
+    return MODEL == 0 ? a.buf + (size_t)colour * pw : a.buf + (size_t)(2 * colour + plane) * pw;
+}
+
+// shared-memory accumulation of one r: counts summed over the live lanes of the warp
+__device__ __forceinline__ void add_r(unsigned int (*s_cnt)[2], uint32_t slot, uint32_t mask, uint32_t leader,
+                                      uint32_t lane, uint32_t c0, uint32_t c1, bool two)
+{
+    const uint32_t v0 = __reduce_add_sync(mask, c0);
+    const uint32_t v1 = two ? __reduce_add_sync(mask, c1) : 0u;
+    if (lane == leader) {
+        atomicAdd(&s_cnt[slot][0], v0);
+        if (two) atomicAdd(&s_cnt[slot][1], v1);
+    }
+}
+
+// y axis (and M, Q in chunk 0): thread = (colour c, 16-row block, word column k)
+template <int MODEL>
+__global__ void __launch_bounds__(128) measure_y_kernel(const MeasBlkArgs a)
+{
+    __shared__ unsigned int s_cnt[MEAS_RC][2];
+    __shared__ unsigned long long s_mq[2];
+    for (uint32_t t = threadIdx.x; t < MEAS_RC * 2; t += blockDim.x) (&s_cnt[0][0])[t] = 0;
+    if (threadIdx.x < 2) s_mq[threadIdx.x] = 0;
+    __syncthreads();
+    const uint32_t r0 = blockIdx.y * MEAS_RC;
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t per_colour = a.n * a.wpr;
+    const bool live = g < 2u * per_colour;
+    const uint32_t mask = __ballot_sync(0xffffffffu, live);
+    const uint32_t lane = threadIdx.x & 31u;
+    if (live) {
+        const uint32_t leader = __ffs(mask) - 1;
+        const uint32_t c = g >= per_colour ? 1u : 0u;
+        const uint32_t rem = g - c * per_colour;
+        const uint32_t rb = rem / a.wpr, k = rem - rb * a.wpr;
+        const uint32_t ib0 = a.i0 + MEAS_NB * rb;
+        const unsigned long long plane_words = (unsigned long long)a.L * a.wpr;
+        const uint32_t *bp0 = blk_plane<MODEL>(a, c, 0), *bp1 = blk_plane<MODEL>(a, c, 1);
+        const uint32_t *op0 = blk_plane<MODEL>(a, c ^ 1u, 0), *op1 = blk_plane<MODEL>(a, c ^ 1u, 1);
+
+        uint32_t B0[MEAS_NB], B1[MEAS_NB];          // base words (Ising: spins; BC: nz, sg)
+        {
+            unsigned long long o = (unsigned long long)ib0 * a.wpr + k;
+#pragma unroll
+            for (int j = 0; j < MEAS_NB; ++j) {
+                B0[j] = bp0[o];
+                B1[j] = MODEL ? bp1[o] : 0u;
+                o += a.wpr;
+            }
+        }
+        if (blockIdx.y == 0) {                       // M and Q of the base rows
+            uint32_t m0 = 0, m1 = 0;
+#pragma unroll
+            for (int j = 0; j < MEAS_NB; ++j) {
+                if (MODEL == 0) m0 += __popc(B0[j]);
+                else { m0 += __popc(B0[j] & ~B1[j]); m1 += __popc(B0[j] & B1[j]); }
+            }
+            const uint32_t v0 = __reduce_add_sync(mask, m0);
+            const uint32_t v1 = MODEL ? __reduce_add_sync(mask, m1) : 0u;
+            if (lane == leader) {
+                atomicAdd(&s_mq[0], (unsigned long long)v0);
+                if (MODEL) atomicAdd(&s_mq[1], (unsigned long long)v1);
+            }
+        }
+        // partner windows: odd r -> opposite colour rows ib0 + r + j, even r -> same colour.
+        // WO[x & 15] holds opposite-colour row ib0 + r0 + 1 + x, WS[x & 15] same-colour row
+        // ib0 + r0 + 2 + x; step m uses x = 2m .. 2m+15 of both.
+        uint32_t WO0[MEAS_NB], WO1[MEAS_NB], WS0[MEAS_NB], WS1[MEAS_NB];
+        unsigned long long oo = ((unsigned long long)((ib0 + r0 + 1u) % a.L)) * a.wpr + k;
+        unsigned long long os = ((unsigned long long)((ib0 + r0 + 2u) % a.L)) * a.wpr + k;
+#pragma unroll
+        for (int x = 0; x < MEAS_NB; ++x) {
+            WO0[x] = op0[oo]; WO1[x] = MODEL ? op1[oo] : 0u;
+            WS0[x] = bp0[os]; WS1[x] = MODEL ? bp1[os] : 0u;
+            oo += a.wpr; if (oo >= plane_words) oo -= plane_words;
+            os += a.wpr; if (os >= plane_words) os -= plane_words;
+        }
+        for (uint32_t mm = 0; mm < MEAS_RC / 2; mm += 8) {
+            if (r0 + 2 * mm + 1 > a.r_max) break;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const uint32_t r_odd = r0 + 2 * (mm + u) + 1;
+#pragma unroll
+                for (int par = 0; par < 2; ++par) {
+                    const uint32_t r = r_odd + par;
+                    if (r <= a.r_max) {
+                        uint32_t X[MEAS_NB], Y[MEAS_NB];
+#pragma unroll
+                        for (int j = 0; j < MEAS_NB; ++j) {
+                            const int sl = (j + 2 * u) & 15;
+                            const uint32_t p0 = par ? WS0[sl] : WO0[sl];
+                            const uint32_t p1 = par ? WS1[sl] : WO1[sl];
+                            if (MODEL == 0) X[j] = B0[j] ^ p0;
+                            else { X[j] = B0[j] & p0; Y[j] = X[j] & (B1[j] ^ p1); }
+                        }
+                        const uint32_t c0 = weighted_popc16(X);
+                        const uint32_t c1 = MODEL ? weighted_popc16(Y) : 0u;
+                        add_r(s_cnt, r - r0 - 1, mask, leader, lane, c0, c1, MODEL != 0);
+                    }
+                }
+                // slide both windows by two rows: slots (2u)&15 and (2u+1)&15 are free now
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int sl = (2 * u + e) & 15;
+                    WO0[sl] = op0[oo]; WO1[sl] = MODEL ? op1[oo] : 0u;
+                    WS0[sl] = bp0[os]; WS1[sl] = MODEL ? bp1[os] : 0u;
+                    oo += a.wpr; if (oo >= plane_words) oo -= plane_words;
+                    os += a.wpr; if (os >= plane_words) os -= plane_words;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (uint32_t t = threadIdx.x; t < MEAS_RC * 2; t += blockDim.x) {
+        const uint32_t r = r0 + (t >> 1) + 1;
+        const unsigned int v = (&s_cnt[0][0])[t];
+        if (r <= a.r_max && v) atomicAdd(a.cnt + 2 + 2 * ((size_t)a.r_max + (r - 1)) + (t & 1u), (unsigned long long)v);
+    }
+    if (threadIdx.x < 2 && s_mq[threadIdx.x]) atomicAdd(a.cnt + threadIdx.x, s_mq[threadIdx.x]);
+}
+
+// x axis: thread = (colour c, row i, segment of 16 words); requires wpr % 16 == 0.
+// r = 2d   -> same colour, bit shift d;   r = 2d+1 -> opposite colour, bit shift d + ((i+c)&1).
+// With r0/2 a multiple of 32 the chunk needs source words k0 + r0/64 + [0, 16] of each colour
+// and funnel shifts by 0..32 bits (clamped form).
+template <int MODEL>
+__global__ void __launch_bounds__(128) measure_x_kernel(const MeasBlkArgs a)
+{
+    __shared__ unsigned int s_cnt[MEAS_RC][2];
+    for (uint32_t t = threadIdx.x; t < MEAS_RC * 2; t += blockDim.x) (&s_cnt[0][0])[t] = 0;
+    __syncthreads();
+    const uint32_t r0 = blockIdx.y * MEAS_RC;
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t nseg = a.wpr / MEAS_NB;
+    const uint32_t per_colour = a.n * nseg;
+    const bool live = g < 2u * per_colour;
+    const uint32_t mask = __ballot_sync(0xffffffffu, live);
+    const uint32_t lane = threadIdx.x & 31u;
+    if (live) {
+        const uint32_t leader = __ffs(mask) - 1;
+        const uint32_t c = g >= per_colour ? 1u : 0u;
+        const uint32_t rem = g - c * per_colour;
+        const uint32_t ir = rem / nseg, sg = rem - ir * nseg;
+        const uint32_t i = a.i0 + ir, k0 = sg * MEAS_NB;
+        const uint32_t par = (i + c) & 1u;
+        const unsigned long long ro = (unsigned long long)i * a.wpr;
+        const uint32_t *bp0 = blk_plane<MODEL>(a, c, 0) + ro, *bp1 = blk_plane<MODEL>(a, c, 1) + ro;
+        const uint32_t *op0 = blk_plane<MODEL>(a, c ^ 1u, 0) + ro, *op1 = blk_plane<MODEL>(a, c ^ 1u, 1) + ro;
+
+        uint32_t B0[MEAS_NB], B1[MEAS_NB];
+#pragma unroll
+        for (int j = 0; j < MEAS_NB; j += 4) {
+            const uint4 v = *reinterpret_cast<const uint4 *>(bp0 + k0 + j);
+            B0[j] = v.x; B0[j + 1] = v.y; B0[j + 2] = v.z; B0[j + 3] = v.w;
+            if (MODEL) {
+                const uint4 w = *reinterpret_cast<const uint4 *>(bp1 + k0 + j);
+                B1[j] = w.x; B1[j + 1] = w.y; B1[j + 2] = w.z; B1[j + 3] = w.w;
+            } else { B1[j] = B1[j + 1] = B1[j + 2] = B1[j + 3] = 0u; }
+        }
+        uint32_t SS0[MEAS_NB + 1], SS1[MEAS_NB + 1], SO0[MEAS_NB + 1], SO1[MEAS_NB + 1];
+        {
+            uint32_t kk = k0 + (r0 >> 6);
+            if (kk >= a.wpr) kk -= a.wpr;
+#pragma unroll
+            for (int x = 0; x <= MEAS_NB; ++x) {
+                SS0[x] = bp0[kk]; SS1[x] = MODEL ? bp1[kk] : 0u;
+                SO0[x] = op0[kk]; SO1[x] = MODEL ? op1[kk] : 0u;
+                if (++kk == a.wpr) kk = 0;
+            }
+        }
+#pragma unroll 1
+        for (uint32_t b = 0; b < MEAS_RC / 2; ++b) {
+            const uint32_t r_odd = r0 + 2 * b + 1;
+            if (r_odd > a.r_max) break;
+            {   // r = 2d+1, d = r0/2 + b: opposite colour, shift b + par (0..32)
+                const uint32_t sh = b + par;
+                uint32_t X[MEAS_NB], Y[MEAS_NB];
+#pragma unroll
+                for (int j = 0; j < MEAS_NB; ++j) {
+                    const uint32_t p0 = __funnelshift_rc(SO0[j], SO0[j + 1], sh);
+                    if (MODEL == 0) X[j] = B0[j] ^ p0;
+                    else {
+                        const uint32_t p1 = __funnelshift_rc(SO1[j], SO1[j + 1], sh);
+                        X[j] = B0[j] & p0; Y[j] = X[j] & (B1[j] ^ p1);
+                    }
+                }
+                const uint32_t c0 = weighted_popc16(X);
+                const uint32_t c1 = MODEL ? weighted_popc16(Y) : 0u;
+                add_r(s_cnt, r_odd - r0 - 1, mask, leader, lane, c0, c1, MODEL != 0);
+            }
+            if (r_odd + 1 <= a.r_max) {   // r = 2d, d = r0/2 + b + 1: same colour, shift b + 1 (1..32)
+                const uint32_t sh = b + 1;
+                uint32_t X[MEAS_NB], Y[MEAS_NB];
+#pragma unroll
+                for (int j = 0; j < MEAS_NB; ++j) {
+                    const uint32_t p0 = __funnelshift_rc(SS0[j], SS0[j + 1], sh);
+                    if (MODEL == 0) X[j] = B0[j] ^ p0;
+                    else {
+                        const uint32_t p1 = __funnelshift_rc(SS1[j], SS1[j + 1], sh);
+                        X[j] = B0[j] & p0; Y[j] = X[j] & (B1[j] ^ p1);
+                    }
+                }
+                const uint32_t c0 = weighted_popc16(X);
+                const uint32_t c1 = MODEL ? weighted_popc16(Y) : 0u;
+                add_r(s_cnt, r_odd - r0, mask, leader, lane, c0, c1, MODEL != 0);
+            }
+        }
+    }
+    __syncthreads();
+    for (uint32_t t = threadIdx.x; t < MEAS_RC * 2; t += blockDim.x) {
+        const uint32_t r = r0 + (t >> 1) + 1;
+        const unsigned int v = (&s_cnt[0][0])[t];
+        if (r <= a.r_max && v) atomicAdd(a.cnt + 2 + 2 * (size_t)(r - 1) + (t & 1u), (unsigned long long)v);
+    }
 }
 
 // ---- unpacked windows (tests, windowed replay, checkpoints) --------------------------------

@@ -197,6 +197,21 @@ def test_measure_rows_partition(model):
 
 
 @pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+@pytest.mark.parametrize("L,r_max", [(1024, 512), (1536, 100), (2048, 131)])
+def test_measure_blocked_kernels_all_r_and_ragged_slabs(L, r_max, model):
+    """The row-blocked measurement kernels (16-row blocks, 16-word segments, chunks of 64 r):
+    every r up to L/2 on the whole lattice, and slabs whose row count is not a multiple of 16."""
+    g = lat.Lattice(L, model, 0.0, 1234 + L)
+    o = oracle.OracleLattice(L, model, 0.0, 1234 + L)
+    beta = BETA_C if model == lat.ISING else workloads.BETA_BC
+    g.sweep([beta] * 30)
+    o.sweep([beta] * 30)
+    _same_measure(g, o, r_max, L)
+    for i0, n in ((0, 16), (3, 45), (L - 33, 33), (500, 7)):
+        _same_measure(g, o, min(r_max, 70), L, rows=(i0, n))
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
 def test_determinism_and_checkpoint_resume(model):
     L = 512
     beta = [0.4] * 10
