@@ -258,10 +258,10 @@ def main():
     r_meas = max(1, min(r_meas, L // 2))
     meas = None
     if rank == 0:
-        # the generic correlation kernel re-reads the lattice once per (r, axis): bound the work
+        # ~3e12 (word, r) pairs/s per axis (profiles/): bound the default run to a few seconds
         words = L * L // 32
-        if words * r_meas > 1 << 36:
-            r_meas = max(1, (1 << 36) // words)
+        if words * r_meas > 1 << 42:
+            r_meas = max(1, (1 << 42) // words)
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record(g.stream)
         M, Q, Sx, Sy = g.measure(r_meas)

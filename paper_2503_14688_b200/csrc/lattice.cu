@@ -222,6 +222,7 @@ int launch_half_sweep(lattice *lat, int colour)
 int ensure_cnt(lattice *lat, size_t entries)
 {
     if (lat->cnt_cap >= entries) return LATTICE_OK;
+    if (entries < 2 + 4 * 4096) entries = 2 + 4 * 4096;      // one allocation serves r_max <= 4096
     if (lat->d_cnt) cudaFree(lat->d_cnt);
     lat->d_cnt = nullptr;
     lat->cnt_cap = 0;
@@ -328,6 +329,37 @@ int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta)
     return LATTICE_OK;
 }
 
+// device counters -> the signed sums of the ABI (synchronises the stream)
+static int finish_measure(lattice *lat, uint64_t n_rows, uint32_t r_max, size_t entries, int64_t *M,
+                          int64_t *Q, int64_t *Sx, int64_t *Sy)
+{
+    const uint64_t L = lat->L;
+    unsigned long long *h = (unsigned long long *)std::malloc(entries * sizeof(unsigned long long));
+    if (!h) return LATTICE_ENOMEM;
+    cudaError_t e = cudaMemcpyAsync(h, lat->d_cnt, entries * sizeof(unsigned long long),
+                                    cudaMemcpyDeviceToHost, lat->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(lat->stream);
+    if (e != cudaSuccess) { std::free(h); return cuda_fail(lat, e, "measure copy/sync"); }
+    const int64_t N = (int64_t)(n_rows * L);
+    if (lat->model == LATTICE_ISING) {
+        *M = 2 * (int64_t)h[0] - N;
+        *Q = N;
+        for (uint32_t r = 0; r < r_max; ++r) {
+            Sx[r] = N - 2 * (int64_t)h[2 + 2 * (size_t)r];
+            Sy[r] = N - 2 * (int64_t)h[2 + 2 * ((size_t)r_max + r)];
+        }
+    } else {
+        *M = (int64_t)h[0] - (int64_t)h[1];
+        *Q = (int64_t)h[0] + (int64_t)h[1];
+        for (uint32_t r = 0; r < r_max; ++r) {
+            Sx[r] = (int64_t)h[2 + 2 * (size_t)r] - 2 * (int64_t)h[3 + 2 * (size_t)r];
+            Sy[r] = (int64_t)h[2 + 2 * ((size_t)r_max + r)] - 2 * (int64_t)h[3 + 2 * ((size_t)r_max + r)];
+        }
+    }
+    std::free(h);
+    return LATTICE_OK;
+}
+
 int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t r_max, int64_t *M,
                          int64_t *Q, int64_t *Sx, int64_t *Sy)
 {
@@ -342,6 +374,20 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
     // Row-blocked kernels: the y axis (and M, Q) over the whole 16-row blocks of the slab, the
     // x axis over every row when a row is a whole number of 16-word segments.  Whatever they do
     // not cover (ragged rows, narrow lattices) goes through the generic kernels.
+    if (r_max == 1 && (lat->wpr % 4u) == 0) {
+        // the per-step record (e, m, q): one pass over the slab
+        MeasE1Args e1;
+        e1.buf = lat->buf; e1.L = lat->L; e1.wpr = lat->wpr; e1.i0 = (uint32_t)i0;
+        e1.n_rows = (uint32_t)n_rows; e1.cnt = lat->d_cnt;
+        const unsigned long long threads =
+            (unsigned long long)(lat->wpr / 4u) * ((n_rows + MEAS_E1_ROWS - 1) / MEAS_E1_ROWS);
+        const unsigned grid = (unsigned)((threads + 127) / 128);
+        if (lat->model == LATTICE_ISING) measure_e1_kernel<0><<<grid, 128, 0, lat->stream>>>(e1);
+        else measure_e1_kernel<1><<<grid, 128, 0, lat->stream>>>(e1);
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+        return finish_measure(lat, n_rows, r_max, entries, M, Q, Sx, Sy);
+    }
     const uint32_t nblk = (uint32_t)(n_rows / MEAS_NB);
     const uint32_t rows_blk = nblk * MEAS_NB;
     const bool x_blk = (lat->wpr % MEAS_NB) == 0;
@@ -400,30 +446,7 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
         rc = generic((uint32_t)i0, rows_blk, false, 0u, 1u);
         if (rc) return rc;
     }
-    unsigned long long *h = (unsigned long long *)std::malloc(entries * sizeof(unsigned long long));
-    if (!h) return LATTICE_ENOMEM;
-    cudaError_t e = cudaMemcpyAsync(h, lat->d_cnt, entries * sizeof(unsigned long long),
-                                    cudaMemcpyDeviceToHost, lat->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(lat->stream);
-    if (e != cudaSuccess) { std::free(h); return cuda_fail(lat, e, "measure copy/sync"); }
-    const int64_t N = (int64_t)(n_rows * L);
-    if (lat->model == LATTICE_ISING) {
-        *M = 2 * (int64_t)h[0] - N;
-        *Q = N;
-        for (uint32_t r = 0; r < r_max; ++r) {
-            Sx[r] = N - 2 * (int64_t)h[2 + 2 * (size_t)r];
-            Sy[r] = N - 2 * (int64_t)h[2 + 2 * ((size_t)r_max + r)];
-        }
-    } else {
-        *M = (int64_t)h[0] - (int64_t)h[1];
-        *Q = (int64_t)h[0] + (int64_t)h[1];
-        for (uint32_t r = 0; r < r_max; ++r) {
-            Sx[r] = (int64_t)h[2 + 2 * (size_t)r] - 2 * (int64_t)h[3 + 2 * (size_t)r];
-            Sy[r] = (int64_t)h[2 + 2 * ((size_t)r_max + r)] - 2 * (int64_t)h[3 + 2 * ((size_t)r_max + r)];
-        }
-    }
-    std::free(h);
-    return LATTICE_OK;
+    return finish_measure(lat, n_rows, r_max, entries, M, Q, Sx, Sy);
 }
 
 int lattice_measure(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy)

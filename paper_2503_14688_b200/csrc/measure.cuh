@@ -404,6 +404,145 @@ __global__ void __launch_bounds__(128) measure_x_kernel(const MeasBlkArgs a)
     }
 }
 
+// ---- r_max == 1: M, Q and the nearest-neighbour sums (the energy) in one pass ---------------
+//
+// The per-step record of a run (e, m, q) needs only r = 1.  One thread owns one 128-bit run of
+// both colours and marches down MEAS_E1_ROWS rows with the previous row in registers, so the
+// lattice is read from HBM exactly once (plus one row in MEAS_E1_ROWS and one side word per run):
+//   y axis: colour c of row i pairs with colour c^1 of row i+1 at the same packed position;
+//   x axis: r = 1 pairs colour c of row i with colour c^1 at p + ((i+c)&1): one of the two
+//           colours pairs in place, the other with the opposite colour shifted by one bit.
+// Requires wpr % 4 == 0.  Counts are reduced two rows at a time with the carry-save tree.
+constexpr int MEAS_E1_ROWS = 32;
+
+struct MeasE1Args {
+    const uint32_t *buf;
+    uint32_t L, wpr;
+    uint32_t i0, n_rows;
+    unsigned long long *cnt;         // [6]: MeasArgs::cnt layout with r_max = 1
+};
+
+template <int MODEL>
+struct E1Row {                       // one 128-bit run of both colours (+ planes) of one row
+    uint32_t a0[4], a1[4];           // colour 0: spins (Ising) or nz, sg (BC)
+    uint32_t b0[4], b1[4];           // colour 1
+};
+
+template <int MODEL>
+__device__ __forceinline__ void e1_load(const MeasE1Args &a, unsigned long long off, E1Row<MODEL> &r)
+{
+    const size_t pw = (size_t)a.L * a.wpr;
+    const uint4 x = *reinterpret_cast<const uint4 *>(a.buf + off);
+    r.a0[0] = x.x; r.a0[1] = x.y; r.a0[2] = x.z; r.a0[3] = x.w;
+    if (MODEL == 0) {
+        const uint4 y = *reinterpret_cast<const uint4 *>(a.buf + pw + off);
+        r.b0[0] = y.x; r.b0[1] = y.y; r.b0[2] = y.z; r.b0[3] = y.w;
+#pragma unroll
+        for (int w = 0; w < 4; ++w) { r.a1[w] = 0; r.b1[w] = 0; }
+    } else {
+        const uint4 xs = *reinterpret_cast<const uint4 *>(a.buf + pw + off);
+        const uint4 y = *reinterpret_cast<const uint4 *>(a.buf + 2 * pw + off);
+        const uint4 ys = *reinterpret_cast<const uint4 *>(a.buf + 3 * pw + off);
+        r.a1[0] = xs.x; r.a1[1] = xs.y; r.a1[2] = xs.z; r.a1[3] = xs.w;
+        r.b0[0] = y.x; r.b0[1] = y.y; r.b0[2] = y.z; r.b0[3] = y.w;
+        r.b1[0] = ys.x; r.b1[1] = ys.y; r.b1[2] = ys.z; r.b1[3] = ys.w;
+    }
+}
+
+template <int MODEL>
+__global__ void __launch_bounds__(128) measure_e1_kernel(const MeasE1Args a)
+{
+    const uint32_t nq = a.wpr >> 2;
+    const uint32_t nslab = (a.n_rows + MEAS_E1_ROWS - 1) / MEAS_E1_ROWS;
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t acc[6] = {0, 0, 0, 0, 0, 0};       // m0, m1, x0, x1, y0, y1 (MeasArgs::cnt order)
+    if (g < nq * nslab) {
+        const uint32_t q = g % nq, sl = g / nq;
+        const uint32_t kw = q << 2;
+        const uint32_t kn = (kw + 4 == a.wpr) ? 0 : kw + 4;       // word after the run (periodic)
+        const uint32_t ia = a.i0 + sl * MEAS_E1_ROWS;
+        const uint32_t nr = min((uint32_t)MEAS_E1_ROWS, a.i0 + a.n_rows - ia);
+        const size_t pw = (size_t)a.L * a.wpr;
+        unsigned long long ro = (unsigned long long)ia * a.wpr;
+        E1Row<MODEL> cur, nxt;
+        e1_load<MODEL>(a, ro + kw, cur);
+        for (uint32_t rr = 0; rr < nr; rr += 2) {
+            uint32_t XM[16], XN[16], XX[16], XXo[16], XY[16], XYo[16];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (rr + h < nr) {
+                    const uint32_t i = ia + rr + h;
+                    const unsigned long long rd = (i + 1 == a.L) ? 0ull : ro + a.wpr;
+                    e1_load<MODEL>(a, rd + kw, nxt);
+                    // x axis: colour (i&1) pairs in place; the other colour sees its partner
+                    // colour shifted down by one bit (partner at p+1)
+                    const uint32_t odd = i & 1u;
+                    // colour whose partner is shifted: c with (i+c)&1 == 1, i.e. c = 1 - odd;
+                    // its partner colour is `odd`: side word of colour `odd` (planes 0, 1)
+                    const uint32_t *sp = a.buf + (MODEL == 0 ? (size_t)odd * pw : (size_t)(2 * odd) * pw) + ro + kn;
+                    const uint32_t e0 = sp[0];
+                    const uint32_t e1 = MODEL ? sp[pw] : 0u;
+#pragma unroll
+                    for (int w = 0; w < 4; ++w) {
+                        const int o = 8 * h + w;
+                        // partner-colour words shifted by one bit
+                        const uint32_t p0lo = odd ? cur.b0[w] : cur.a0[w];
+                        const uint32_t p0hi = w < 3 ? (odd ? cur.b0[w < 3 ? w + 1 : 0] : cur.a0[w < 3 ? w + 1 : 0]) : e0;
+                        const uint32_t sh0 = __funnelshift_r(p0lo, p0hi, 1);
+                        const uint32_t t0 = odd ? cur.a0[w] : cur.b0[w];      // the shifted pairing's base colour
+                        if (MODEL == 0) {
+                            XM[o] = cur.a0[w]; XM[o + 4] = cur.b0[w];
+                            XX[o] = cur.a0[w] ^ cur.b0[w];                    // in-place pairing
+                            XX[o + 4] = t0 ^ sh0;
+                            XY[o] = cur.a0[w] ^ nxt.b0[w];
+                            XY[o + 4] = cur.b0[w] ^ nxt.a0[w];
+                        } else {
+                            const uint32_t p1lo = odd ? cur.b1[w] : cur.a1[w];
+                            const uint32_t p1hi = w < 3 ? (odd ? cur.b1[w < 3 ? w + 1 : 0] : cur.a1[w < 3 ? w + 1 : 0]) : e1;
+                            const uint32_t sh1 = __funnelshift_r(p1lo, p1hi, 1);
+                            const uint32_t t1 = odd ? cur.a1[w] : cur.b1[w];
+                            XM[o] = cur.a0[w] & ~cur.a1[w]; XM[o + 4] = cur.b0[w] & ~cur.b1[w];
+                            XN[o] = cur.a0[w] & cur.a1[w]; XN[o + 4] = cur.b0[w] & cur.b1[w];
+                            XX[o] = cur.a0[w] & cur.b0[w];
+                            XXo[o] = XX[o] & (cur.a1[w] ^ cur.b1[w]);
+                            XX[o + 4] = t0 & sh0;
+                            XXo[o + 4] = XX[o + 4] & (t1 ^ sh1);
+                            XY[o] = cur.a0[w] & nxt.b0[w];
+                            XYo[o] = XY[o] & (cur.a1[w] ^ nxt.b1[w]);
+                            XY[o + 4] = cur.b0[w] & nxt.a0[w];
+                            XYo[o + 4] = XY[o + 4] & (cur.b1[w] ^ nxt.a1[w]);
+                        }
+                    }
+                    cur = nxt;
+                    ro = rd;
+                } else {
+#pragma unroll
+                    for (int o = 8; o < 16; ++o) { XM[o] = XN[o] = XX[o] = XXo[o] = XY[o] = XYo[o] = 0; }
+                }
+            }
+            acc[0] += weighted_popc16(XM);
+            acc[2] += weighted_popc16(XX);
+            acc[4] += weighted_popc16(XY);
+            if (MODEL) {
+                acc[1] += weighted_popc16(XN);
+                acc[3] += weighted_popc16(XXo);
+                acc[5] += weighted_popc16(XYo);
+            }
+        }
+    }
+    __shared__ unsigned long long sh[6];
+    if (threadIdx.x < 6) sh[threadIdx.x] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < 6; ++e) {
+        if (MODEL == 0 && (e & 1)) continue;
+        const uint32_t v = __reduce_add_sync(0xffffffffu, acc[e]);
+        if ((threadIdx.x & 31u) == 0 && v) atomicAdd(&sh[e], (unsigned long long)v);
+    }
+    __syncthreads();
+    if (threadIdx.x < 6 && sh[threadIdx.x]) atomicAdd(a.cnt + threadIdx.x, sh[threadIdx.x]);
+}
+
 // ---- unpacked windows (tests, windowed replay, checkpoints) --------------------------------
 struct WindowArgs {
     uint32_t *buf;

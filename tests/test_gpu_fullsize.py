@@ -91,6 +91,8 @@ def _check_slab(g, w, i0, n, r_max):
     M, Q, Sx, Sy = g.measure(r_max, (i0, n))
     Mo, Qo, Sxo, Syo = _slab_counts(g, w, i0, n, rs)
     assert (M, Q) == (Mo, Qo)
+    M1, Q1, Sx1, Sy1 = g.measure(1, (i0, n))                 # the one-pass r_max = 1 kernel
+    assert (M1, Q1, Sx1[0], Sy1[0]) == (Mo, Qo, Sxo[1], Syo[1])
     for r in rs:
         assert Sx[r - 1] == Sxo[r], ("Sx", r)
         assert Sy[r - 1] == Syo[r], ("Sy", r)
@@ -133,6 +135,8 @@ def test_full_size_windowed_replay_and_slab_measurements(name, t_late, r_slab):
         part = np.concatenate([[M, Q], Sx, Sy])
         tot = part if tot is None else tot + part
     assert np.array_equal(tot, np.concatenate([[whole[0], whole[1]], whole[2], whole[3]]))
+    one = g.measure(1)
+    assert (one[0], one[1], one[2][0], one[3][0]) == (whole[0], whole[1], whole[2][0], whole[3][0])
     if w.model == lat.ISING:
         assert whole[1] == L * L
     g.close()

@@ -212,6 +212,21 @@ def test_measure_blocked_kernels_all_r_and_ragged_slabs(L, r_max, model):
 
 
 @pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+@pytest.mark.parametrize("L", [256, 768, 2048])
+def test_measure_r1_single_pass(L, model):
+    """r_max = 1 (the per-step record e, m, q) goes through the one-pass marching kernel."""
+    g = lat.Lattice(L, model, 0.4, 99 + L)
+    o = oracle.OracleLattice(L, model, 0.4, 99 + L)
+    _same_measure(g, o, 1, L, 0.4)
+    beta = BETA_C if model == lat.ISING else workloads.BETA_BC
+    g.sweep([beta] * 10)
+    o.sweep([beta] * 10)
+    _same_measure(g, o, 1, L, 0.4)
+    for i0, n in ((0, 1), (1, 1), (0, 32), (5, 64), (L - 71, 71), (31, 2), (L - 1, 1)):
+        _same_measure(g, o, 1, L, rows=(i0, n))
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
 def test_determinism_and_checkpoint_resume(model):
     L = 512
     beta = [0.4] * 10
