@@ -1,0 +1,277 @@
+// bc_march.cuh -- the production Blume-Capel half-sweep (RNG scheme 1, L a multiple of 256,
+// threshold tables with the "integer dE" structure that Delta = 0 gives).
+//
+// Paper: Eq. 1 with crystal field Delta; every run of the paper uses
+// Delta = 0.  Metropolis + checkerboard + multispin coding,
+// 32-bit acceptance compare.  Same packing, neighbour geometry, proposal rule and
+// acceptance rule as bc.cuh, which stays as the generic path (any Delta, scheme 0, narrow rows).
+//
+// With r the per-lane reference sign of bc.cuh and x = (#neighbours of sign r) - (#of sign -r),
+// the move types cost dE = 2x (flip), x - Delta (vacate), x + Delta (occupy).  When the host
+// finds that every entry with x <= 0 is "always" and vacate/occupy share their thresholds for
+// x = 1..4 (true for Delta = 0 at any beta), a lane that needs a random decision is in one of
+// 8 classes (F, x) with F = flip and x = 1..4, i.e. 3 bits per lane:
+//     F = flip,   Y1 = (x >= 3),   H0 = (x odd)
+// and bit k of the lane's threshold is a 3-input boolean function of those bits -- exactly one
+// LOP3 whose truth table (8 bits per plane) the host derives from the threshold table.  LOP3's
+// truth table is an immediate, so the kernel dispatches once per plane (warp-uniform, 256-way
+// jump table) to the LOP3 with the right immediate.  This replaces ~90 LOP3 per word of class
+// selection in bc.cuh by 1 per word per plane.
+//
+// Work layout as in ising_march.cuh: one thread owns a 128-bit run and marches down R rows with
+// the opposite-colour rows i-1, i, i+1 in registers; folded Philox bit-planes; ties (top byte of
+// u32 equal to the top byte of the lane's threshold) are queued per warp as one 64-bit entry per
+// tied lane and resolved 32 at a time, accepted late moves applied with global atomic XORs.
+#pragma once
+#include "bc.cuh"
+#include "ising_march.cuh"
+
+namespace lat {
+
+struct BCMarchArgs {
+    uint32_t *tnz, *tsg;            // colour being updated
+    const uint32_t *onz, *osg;      // opposite colour
+    uint32_t L, wpr, t, colour;
+    uint32_t R;                     // rows per thread (even, divides L)
+    uint32_t threads;               // (wpr/4) * (L/R), a multiple of 32
+    uint32_t lut[8];                // truth table of threshold bit (31-k) over (F, Y1, H0)
+    uint32_t lut_always;            // truth table of "threshold == 2^32" over (F, Y1, H0)
+    uint32_t thr[8];                // threshold of class (F<<2 | Y1<<1 | H0) (low 24 bits used)
+    uint32_t fbp;                   // folded counter word of the PROP plane
+    PlaneFold F;                    // folded ACC_PLANE stream of (t, colour)
+    RoundKeys K;
+};
+
+// out[w] = f(a[w], b[w], c[w]), w = 0..3, with f given by the runtime truth table `lut` (LOP3
+// convention: bit (a<<2 | b<<1 | c) of lut).  One PTX block: a 256-entry jump table (brx.idx)
+// into 256 groups of four LOP3 with the truth table as immediate.  Labels are scoped by the
+// braces, so the block can be inlined more than once.  lut should be warp-uniform.
+#define LAT_LC(h, l)                                                                              \
+    "L" #h #l ": lop3.b32 %0, %4, %8, %13, 0x" #h #l "; lop3.b32 %1, %5, %9, %14, 0x" #h #l       \
+    "; lop3.b32 %2, %6, %10, %15, 0x" #h #l "; lop3.b32 %3, %7, %11, %16, 0x" #h #l "; bra LE;\n\t"
+#define LAT_LR(h)                                                                                 \
+    LAT_LC(h, 0) LAT_LC(h, 1) LAT_LC(h, 2) LAT_LC(h, 3) LAT_LC(h, 4) LAT_LC(h, 5) LAT_LC(h, 6)    \
+    LAT_LC(h, 7) LAT_LC(h, 8) LAT_LC(h, 9) LAT_LC(h, a) LAT_LC(h, b) LAT_LC(h, c) LAT_LC(h, d)    \
+    LAT_LC(h, e) LAT_LC(h, f)
+#define LAT_TR(h)                                                                                 \
+    "L" #h "0, L" #h "1, L" #h "2, L" #h "3, L" #h "4, L" #h "5, L" #h "6, L" #h "7, L" #h        \
+    "8, L" #h "9, L" #h "a, L" #h "b, L" #h "c, L" #h "d, L" #h "e, L" #h "f"
+
+__device__ __forceinline__ void lut3_dispatch(uint32_t lut, const uint32_t (&a)[4], const uint32_t (&b)[4],
+                                              const uint32_t (&c)[4], uint32_t (&out)[4])
+{
+    asm("{\n\t"
+        "ts: .branchtargets " LAT_TR(0) ", " LAT_TR(1) ", " LAT_TR(2) ", " LAT_TR(3) ", " LAT_TR(4) ", "
+        LAT_TR(5) ", " LAT_TR(6) ", " LAT_TR(7) ", " LAT_TR(8) ", " LAT_TR(9) ", " LAT_TR(a) ", "
+        LAT_TR(b) ", " LAT_TR(c) ", " LAT_TR(d) ", " LAT_TR(e) ", " LAT_TR(f) ";\n\t"
+        "brx.idx %12, ts;\n\t"
+        LAT_LR(0) LAT_LR(1) LAT_LR(2) LAT_LR(3) LAT_LR(4) LAT_LR(5) LAT_LR(6) LAT_LR(7)
+        LAT_LR(8) LAT_LR(9) LAT_LR(a) LAT_LR(b) LAT_LR(c) LAT_LR(d) LAT_LR(e) LAT_LR(f)
+        "LE:\n\t"
+        "}"
+        : "=r"(out[0]), "=r"(out[1]), "=r"(out[2]), "=r"(out[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]), "r"(b[2]), "r"(b[3]),
+          "r"(lut & 0xffu), "r"(c[0]), "r"(c[1]), "r"(c[2]), "r"(c[3]));
+}
+
+#undef LAT_LC
+#undef LAT_LR
+#undef LAT_TR
+
+// per-warp queue of tied lanes: one 64-bit entry per lane
+//   bits 0..33 word offset of the lane's word, 34..38 bit, 39..41 class, 42 nz toggles, 43 sg toggles
+struct BCTieQueue {
+    const BCMarchArgs &a;
+    unsigned long long *q;      // [64 + 32] this warp's slice
+    uint32_t lane, pending;
+
+    __device__ __forceinline__ void resolve(uint32_t idx)
+    {
+        const unsigned long long e = q[idx];
+        const unsigned long long wo = e & 0x3ffffffffull;
+        const uint32_t bit = (uint32_t)(e >> 34) & 31u, cls = (uint32_t)(e >> 39) & 7u;
+        const unsigned long long P = (wo << 5) + bit;
+        const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
+                                        a.colour | (TAG_ACC_TAIL << 8), a.K);
+        if ((blk.x >> 8) < (a.thr[cls] & 0x00ffffffu)) {
+            if ((e >> 42) & 1u) atomicXor(a.tnz + wo, 1u << bit);
+            if ((e >> 43) & 1u) atomicXor(a.tsg + wo, 1u << bit);
+        }
+    }
+    // collective over the warp: every thread pushes its tied lanes (eq words) one at a time
+    __device__ __forceinline__ void push(uint32_t (&eq)[4], const uint32_t (&Fm)[4], const uint32_t (&Y1)[4],
+                                         const uint32_t (&H0)[4], const uint32_t (&nf)[4],
+                                         const uint32_t (&gg)[4], unsigned long long wo)
+    {
+        for (;;) {
+            const int w = eq[0] ? 0 : eq[1] ? 1 : eq[2] ? 2 : 3;
+            const uint32_t ew = eq[0] ? eq[0] : eq[1] ? eq[1] : eq[2] ? eq[2] : eq[3];
+            const uint32_t m = __ballot_sync(0xffffffffu, ew != 0);
+            if (m == 0) return;
+            if (ew) {
+                const uint32_t bit = __ffs(ew) - 1, bm = 1u << bit;
+                const uint32_t fw = w == 0 ? Fm[0] : w == 1 ? Fm[1] : w == 2 ? Fm[2] : Fm[3];
+                const uint32_t yw = w == 0 ? Y1[0] : w == 1 ? Y1[1] : w == 2 ? Y1[2] : Y1[3];
+                const uint32_t hw = w == 0 ? H0[0] : w == 1 ? H0[1] : w == 2 ? H0[2] : H0[3];
+                const uint32_t nw = w == 0 ? nf[0] : w == 1 ? nf[1] : w == 2 ? nf[2] : nf[3];
+                const uint32_t gw = w == 0 ? gg[0] : w == 1 ? gg[1] : w == 2 ? gg[2] : gg[3];
+                const uint32_t cls = (((fw >> bit) & 1u) << 2) | (((yw >> bit) & 1u) << 1) | ((hw >> bit) & 1u);
+                const unsigned long long e = (wo + (unsigned)w) | ((unsigned long long)bit << 34) |
+                                             ((unsigned long long)cls << 39) |
+                                             ((unsigned long long)((nw >> bit) & 1u) << 42) |
+                                             ((unsigned long long)((gw >> bit) & 1u) << 43);
+                q[pending + __popc(m & ((1u << lane) - 1u))] = e;
+                if (w == 0) eq[0] &= ~bm; else if (w == 1) eq[1] &= ~bm; else if (w == 2) eq[2] &= ~bm; else eq[3] &= ~bm;
+            }
+            pending += __popc(m);
+            __syncwarp();
+            if (pending >= 32) {
+                pending -= 32;
+                resolve(pending + lane);
+                __syncwarp();
+            }
+        }
+    }
+    __device__ __forceinline__ void drain()
+    {
+        __syncwarp();
+        if (lane < pending) resolve(lane);
+        pending = 0;
+    }
+};
+
+struct BCRow {
+    uint32_t nz[4], sg[4];
+};
+
+__device__ __forceinline__ void bcm_load(const uint32_t *nzp, const uint32_t *sgp, unsigned long long off, BCRow &v)
+{
+    const uint4 x = *reinterpret_cast<const uint4 *>(nzp + off);
+    const uint4 y = *reinterpret_cast<const uint4 *>(sgp + off);
+    v.nz[0] = x.x; v.nz[1] = x.y; v.nz[2] = x.z; v.nz[3] = x.w;
+    v.sg[0] = y.x; v.sg[1] = y.y; v.sg[2] = y.z; v.sg[3] = y.w;
+}
+
+// One row of one 128-bit run.  PAR == 0: side neighbour at p-1 (En, Es = word before the run),
+// PAR == 1: at p+1 (word after it).  Stores the updated words (ties treated as rejections) and
+// queues the ties.
+template <int PAR>
+__device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, unsigned long long wo,
+                                             const BCRow &U, const BCRow &C, const BCRow &D,
+                                             uint32_t En, uint32_t Es, BCTieQueue &queue)
+{
+    BCRow T;
+    bcm_load(a.tnz, a.tsg, wo, T);
+    const PlaneShared ps = plane_shared(G, a.F);
+    uint32_t Fm[4], Y1[4], H0[4], pos[4], nf[4], gg[4];
+    {
+        const uint4 pb = plane_block(ps, a.fbp, a.F, a.K);        // proposal bits
+        const uint32_t b[4] = {pb.x, pb.y, pb.z, pb.w};
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            uint32_t Sn, Ss;
+            if (PAR == 0) {
+                Sn = fsl1(w == 0 ? En : C.nz[w > 0 ? w - 1 : 0], C.nz[w]);
+                Ss = fsl1(w == 0 ? Es : C.sg[w > 0 ? w - 1 : 0], C.sg[w]);
+            } else {
+                Sn = fsr1(C.nz[w], w == 3 ? En : C.nz[w < 3 ? w + 1 : 0]);
+                Ss = fsr1(C.sg[w], w == 3 ? Es : C.sg[w < 3 ? w + 1 : 0]);
+            }
+            const uint32_t nz = T.nz[w], sg = T.sg[w], bw = b[w];
+            Fm[w] = nz & ~(sg ^ bw);                              // flip
+            nf[w] = ~Fm[w];                                       // nz toggles unless the move is a flip
+            gg[w] = Fm[w] | (nz & sg & ~bw) | (~nz & bw);         // sg toggles: flip, vacate of -1, occupy -1
+            const uint32_t r = (nz & sg) | (~nz & ~bw);
+            // x + 4 = sum over the 4 neighbours of [sign r] + [not sign -r], bit-sliced
+            const uint32_t a1 = U.nz[w] & ~(U.sg[w] ^ r), n1 = ~(U.nz[w] & (U.sg[w] ^ r));
+            const uint32_t a2 = D.nz[w] & ~(D.sg[w] ^ r), n2 = ~(D.nz[w] & (D.sg[w] ^ r));
+            const uint32_t a3 = C.nz[w] & ~(C.sg[w] ^ r), n3 = ~(C.nz[w] & (C.sg[w] ^ r));
+            const uint32_t a4 = Sn & ~(Ss ^ r), n4 = ~(Sn & (Ss ^ r));
+            const uint32_t s1 = a1 ^ a2 ^ a3, c1 = maj3m(a1, a2, a3);
+            const uint32_t s2 = n1 ^ n2 ^ n3, c2 = maj3m(n1, n2, n3);
+            const uint32_t s3 = s1 ^ s2 ^ a4, c3 = maj3m(s1, s2, a4);
+            const uint32_t h0 = s3 ^ n4, c4 = s3 & n4;            // weight 1 done
+            const uint32_t t1 = c1 ^ c2 ^ c3, d1 = maj3m(c1, c2, c3);
+            const uint32_t h1 = t1 ^ c4, d2 = t1 & c4;            // weight 2 done
+            const uint32_t h2 = d1 ^ d2, h3 = d1 & d2;            // weights 4, 8
+            H0[w] = h0;
+            Y1[w] = h3 | (h1 & h0);                               // x >= 3  (x+4 in {7, 8})
+            pos[w] = h3 | (h2 & (h1 | h0));                       // x >= 1  (x+4 >= 5)
+        }
+    }
+    uint32_t alw[4], acc[4], eq[4];
+    lut3_dispatch(a.lut_always, Fm, Y1, H0, alw);
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t need = pos[w] & ~alw[w];
+        alw[w] = ~need;                                           // x <= 0, or threshold 2^32
+        pos[w] = need;
+        eq[w] = need;
+        acc[w] = 0;
+    }
+#pragma unroll 1
+    for (int k = 7; k >= 0; --k) {
+        const uint4 b4 = plane_block(ps, a.F.fb[k], a.F, a.K);
+        const uint32_t b[4] = {b4.x, b4.y, b4.z, b4.w};
+        uint32_t tau[4];
+        lut3_dispatch(a.lut[k], Fm, Y1, H0, tau);
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            acc[w] = maj3m(tau[w], ~b[w], acc[w]);
+            eq[w] &= ~(b[w] ^ tau[w]);
+        }
+    }
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t ok = alw[w] | (acc[w] & pos[w]);           // a tied lane has acc = 0
+        T.nz[w] ^= ok & nf[w];
+        T.sg[w] ^= ok & gg[w];
+    }
+    *reinterpret_cast<uint4 *>(a.tnz + wo) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
+    *reinterpret_cast<uint4 *>(a.tsg + wo) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
+    queue.push(eq, Fm, Y1, H0, nf, gg, wo);
+}
+
+template <int COLOUR>
+__global__ void __launch_bounds__(256) bc_march_kernel(const BCMarchArgs a)
+{
+    __shared__ unsigned long long s_q[8][64];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t g = blockIdx.x * 256u + threadIdx.x;
+    if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
+    BCTieQueue queue{a, s_q[warp], lane, 0u};
+
+    const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
+    const uint32_t q = g % nq, s = g / nq;
+    const uint32_t kw = q << 2;
+    const uint32_t i0 = s * a.R;
+    const uint32_t iu = (i0 == 0) ? L - 1 : i0 - 1;
+    const uint32_t ke0 = (kw == 0) ? wpr - 1 : kw - 1;       // word before the run (periodic)
+    const uint32_t ke1 = (kw + 4 == wpr) ? 0 : kw + 4;       // word after it
+    unsigned long long ro = (unsigned long long)i0 * wpr;
+    BCRow U, C, D;
+    bcm_load(a.onz, a.osg, (unsigned long long)iu * wpr + kw, U);
+    bcm_load(a.onz, a.osg, ro + kw, C);
+    uint32_t G = i0 * nq + q;
+    for (uint32_t r = 0; r < a.R; r += 2) {
+        {   // row i0 + r: (i + colour) & 1 == COLOUR
+            const uint32_t i = i0 + r;
+            const unsigned long long rd = (i + 1 == L) ? 0ull : ro + wpr;
+            bcm_load(a.onz, a.osg, rd + kw, D);
+            const unsigned long long eo = ro + (COLOUR == 0 ? ke0 : ke1);
+            bc_march_row<COLOUR>(a, G, ro + kw, U, C, D, a.onz[eo], a.osg[eo], queue);
+            U = C; C = D; ro = rd; G += nq;
+        }
+        {   // row i0 + r + 1: the other parity
+            const uint32_t i = i0 + r + 1;
+            const unsigned long long rd = (i + 1 == L) ? 0ull : ro + wpr;
+            bcm_load(a.onz, a.osg, rd + kw, D);
+            const unsigned long long eo = ro + (COLOUR == 0 ? ke1 : ke0);
+            bc_march_row<COLOUR ^ 1>(a, G, ro + kw, U, C, D, a.onz[eo], a.osg[eo], queue);
+            U = C; C = D; ro = rd; G += nq;
+        }
+    }
+    queue.drain();
+}
+
+}  // namespace lat

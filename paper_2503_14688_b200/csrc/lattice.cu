@@ -15,6 +15,7 @@
 #include <new>
 
 #include "bc.cuh"
+#include "bc_march.cuh"
 #include "ising.cuh"
 #include "ising_march.cuh"
 #include "measure.cuh"
@@ -145,8 +146,66 @@ int launch_ising_march(lattice *lat, int colour)
     return LATTICE_OK;
 }
 
+// representative (code, b, h) entry of the 54-entry table for move type and x (bc.cuh): the
+// mirrored entry (s -> -s, h -> -h) has the identical dE
+int bc_entry(int type, int x)
+{
+    if (type == BC_FLIP) return (2 * 2 + 0) * 9 + (x + 4);          // +1 -> -1, h = x
+    if (type == BC_VACATE) return (2 * 2 + 1) * 9 + (x + 4);        // +1 -> 0,  h = x
+    return (1 * 2 + 0) * 9 + (-x + 4);                              // 0 -> +1,  h = -x
+}
+
+// bc_march.cuh applies when every x <= 0 entry is "always" and vacate/occupy share their
+// thresholds for x = 1..4 (Delta = 0 at any beta)
+bool bc_table_is_integer_dE(const lattice *lat)
+{
+    for (int type = 0; type < 3; ++type)
+        for (int x = -4; x <= 0; ++x)
+            if (lat->thr64[bc_entry(type, x)] < TWO32) return false;
+    for (int x = 1; x <= 4; ++x)
+        if (lat->thr64[bc_entry(BC_VACATE, x)] != lat->thr64[bc_entry(BC_OCCUPY, x)]) return false;
+    return true;
+}
+
+int launch_bc_march(lattice *lat, int colour)
+{
+    const uint32_t L = lat->L, wpr = lat->wpr, nq = wpr / 4u;
+    const size_t pw = (size_t)L * wpr;
+    BCMarchArgs a;
+    a.tnz = lat->buf + (size_t)(2 * colour) * pw;
+    a.tsg = lat->buf + (size_t)(2 * colour + 1) * pw;
+    a.onz = lat->buf + (size_t)(2 * (1 - colour)) * pw;
+    a.osg = lat->buf + (size_t)(2 * (1 - colour) + 1) * pw;
+    a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
+    a.R = march_rows(L, nq);
+    a.threads = nq * (L / a.R);
+    for (int k = 0; k < 8; ++k) a.lut[k] = 0;
+    a.lut_always = 0;
+    for (int F = 0; F < 2; ++F)
+        for (int x = 1; x <= 4; ++x) {
+            const uint32_t cls = (uint32_t)(F << 2) | (uint32_t)((x >= 3) << 1) | (uint32_t)(x & 1);
+            const uint64_t th = lat->thr64[bc_entry(F ? BC_FLIP : BC_VACATE, x)];
+            if (th >= TWO32) { a.lut_always |= 1u << cls; a.thr[cls] = 0xffffffffu; continue; }
+            a.thr[cls] = (uint32_t)th;
+            for (int k = 0; k < 8; ++k)
+                if ((th >> (31 - k)) & 1u) a.lut[k] |= 1u << cls;
+        }
+    a.K = lat->K;
+    build_plane_fold(lat->K, a.t, a.colour, TAG_ACC_PLANE, a.F);
+    a.fbp = (a.colour | (TAG_PROP_PLANE << 8)) ^ lat->K.k1[0];
+    const unsigned blocks = (a.threads + 255u) / 256u;
+    if (colour == 0) bc_march_kernel<0><<<blocks, 256, 0, lat->stream>>>(a);
+    else bc_march_kernel<1><<<blocks, 256, 0, lat->stream>>>(a);
+    lat->launches += 1;
+    CU(lat, cudaGetLastError());
+    return LATTICE_OK;
+}
+
 int launch_half_sweep(lattice *lat, int colour)
 {
+    if (lat->model == LATTICE_BLUME_CAPEL && lat->scheme == 1 && (lat->wpr % 4u) == 0 &&
+        bc_table_is_integer_dE(lat))
+        return launch_bc_march(lat, colour);
     if (lat->model == LATTICE_ISING && lat->scheme == 1 && (lat->wpr % 4u) == 0)
         return launch_ising_march(lat, colour);
     const uint32_t L = lat->L, wpr = lat->wpr;
