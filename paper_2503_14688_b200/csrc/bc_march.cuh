@@ -233,7 +233,7 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
 }
 
 template <int COLOUR>
-__global__ void __launch_bounds__(256) bc_march_kernel(const BCMarchArgs a)
+__global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
 {
     __shared__ unsigned long long s_q[8][64];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
