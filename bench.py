@@ -13,10 +13,12 @@ One JSON line is printed by rank 0:
   e2e       the same metric through the C-ABI with host buffers every step: the step's beta goes
             in as a host fp64 array and the step's result (M, Q, S_x(1), S_y(1) -> e, m) comes
             back to host memory (lattice_sweep + lattice_measure), all inside the timed region
-  roofline  HBM roofline of the dominant kernel (Ising half-sweep): algorithmic bytes
-            (0.375 B/update: read both colours once, write one) / mean launch time, against the
-            measured copy bandwidth in MEASURED_PEAKS.json; roofline_alu is the integer-issue
-            roofline of the same kernel
+  roofline  the binding roofline of the dominant kernel (the half-sweep): "bound": "alu" -- thread-
+            instructions of the 16-lane integer dispatch class per launch / mean launch time,
+            against 148 SM x 64 lanes x the sampled SM clock
+  roofline_hbm  the HBM roofline BASELINE.json's metric asks for: algorithmic bytes (0.375
+            B/update Ising, 0.75 BC: read both colours once, write one) / mean launch time,
+            against the measured copy bandwidth in MEASURED_PEAKS.json
   cpu_baseline  the oracle, as it stands, on the host cores over a bounded sample
   measure   the measurement pass (M, Q, C(r) on both axes) timed separately after the sweeps
 
@@ -47,10 +49,15 @@ from paper_2503_14688_b200 import workloads  # noqa: E402
 METRIC = "spin updates/ns per B200 (Ising & Blume-Capel) and % of HBM roofline"
 UNIT = "spin updates/ns"
 BYTES_PER_UPDATE = {workloads.ISING: 0.375, workloads.BLUME_CAPEL: 0.75}
-# thread-instructions issued per spin update by the dominant kernel (from the ncu capture named
-# in DESIGN.md "Rooflines"; updated whenever the kernel changes)
-INSTR_PER_UPDATE = {workloads.ISING: None, workloads.BLUME_CAPEL: None}
-SM_COUNT, ISSUE_LANES_PER_CLK_PER_SM = 148, 128
+# Integer-pipe roofline of the dominant kernel: thread-instructions of the
+# half-rate class (ALU pipe: LOP3/SHF/SEL/ISETP..., plus IMAD.WIDE/IMAD.HI, which block the same
+# 16-lane dispatch for two cycles) per spin update, from the committed ncu captures under
+# profiles/ (sm__inst_executed_pipe_alu + IMAD.WIDE/HI counts / updates per launch).
+HALF_RATE_INSTR_PER_UPDATE = {workloads.ISING: 4.00, workloads.BLUME_CAPEL: 5.54}
+#: DRAM bytes per update measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum) / updates
+DRAM_BYTES_PER_UPDATE_NCU = {workloads.ISING: 0.363, workloads.BLUME_CAPEL: 0.667}
+SM_COUNT, HALF_RATE_LANES_PER_CLK_PER_SM = 148, 64
+KERNEL = {workloads.ISING: "ising_march_kernel", workloads.BLUME_CAPEL: "bc_march_kernel"}
 
 
 def measured_peaks():
@@ -285,10 +292,21 @@ def main():
     alg_bytes = bpu * updates_per_step / 2          # per half-sweep launch
     achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
     in_l2 = lat.state_bytes(L, w.model) <= (126 << 20)
-    roofline = {"bound": "hbm", "kernel": "ising_march_kernel" if w.model == 0 else "bc_half_sweep_v4",
-                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "bytes_per_update": bpu,
-                "launch_ms": launch_ms, "l2_resident": in_l2}
+    roofline_hbm = {"bound": "hbm", "kernel": KERNEL[w.model], "achieved": achieved, "peak": peak,
+                    "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                    "bytes_per_update": bpu, "launch_ms": launch_ms, "l2_resident": in_l2}
+    # the binding roofline: the 16-lane integer dispatch (ALU pipe + IMAD.WIDE), DESIGN.md section 6
+    mhz = clocks.get("sm_mhz") or sm_max
+    ipu = HALF_RATE_INSTR_PER_UPDATE[w.model]
+    peak_alu = SM_COUNT * HALF_RATE_LANES_PER_CLK_PER_SM * mhz * 1e6 / 1e12
+    ach_alu = ipu * (updates_per_step / 2) / (launch_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": KERNEL[w.model], "achieved": ach_alu, "peak": peak_alu,
+                "unit": "T thread-instr/s", "frac": ach_alu / peak_alu,
+                "traffic": DRAM_BYTES_PER_UPDATE_NCU[w.model] * updates_per_step / 2,
+                "traffic_source": "ncu dram bytes per update (profiles/) x updates per launch",
+                "instr_per_update": ipu, "sm_mhz": mhz, "launch_ms": launch_ms,
+                "peak_source": "148 SM x 64 lanes/clk (ALU + IMAD.WIDE dispatch) x sampled SM clock",
+                "hbm_frac": achieved / peak, "hbm_achieved_GBs": achieved, "hbm_peak_GBs": peak}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -303,18 +321,11 @@ def main():
                 "d2h_bytes_per_step": 8 * (2 + 4 * 1), "ms_per_step": e2e_ms / args.steps,
                 "what": "lattice_sweep(1, host beta) + lattice_measure(r_max=1) -> host int64"},
         "roofline": roofline,
+        "roofline_hbm": roofline_hbm,
         "measure": meas,
     }
-    ipu = INSTR_PER_UPDATE[w.model]
-    if ipu:
-        mhz = clocks.get("sm_mhz") or sm_max
-        peak_alu = SM_COUNT * ISSUE_LANES_PER_CLK_PER_SM * mhz * 1e6 / 1e12
-        ach_alu = ipu * value / world * 1e9 / 1e12
-        line["roofline_alu"] = {"bound": "alu", "achieved": ach_alu, "peak": peak_alu,
-                                "unit": "T thread-instr/s", "frac": ach_alu / peak_alu,
-                                "instr_per_update": ipu, "sm_mhz": mhz}
     if not args.no_cpu_baseline:
-        Ls, ns = min(L, 4096), 8
+        Ls, ns = min(L, 4096), 96
         rate, dt, cores = oracle_rate(w, Ls, ns, args.scheme)
         line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"{ns} sweeps of a {Ls}x{Ls} lattice of the same model, "
