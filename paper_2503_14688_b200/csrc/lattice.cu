@@ -130,17 +130,26 @@ int launch_ising_march(lattice *lat, int colour)
     a.tgt = lat->buf + (size_t)colour * pw;
     a.opp = lat->buf + (size_t)(1 - colour) * pw;
     a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
-    a.always4 = lat->thr64[0] >= TWO32; a.always8 = lat->thr64[1] >= TWO32;
-    a.thr4 = a.always4 ? 0xffffffffu : (uint32_t)lat->thr64[0];
-    a.thr8 = a.always8 ? 0xffffffffu : (uint32_t)lat->thr64[1];
-    a.top4 = a.thr4 >> 24; a.top8 = a.thr8 >> 24;
+    const bool always4 = lat->thr64[0] >= TWO32, always8 = lat->thr64[1] >= TWO32;
+    a.thr4 = always4 ? 0xffffffffu : (uint32_t)lat->thr64[0];
+    a.thr8 = always8 ? 0xffffffffu : (uint32_t)lat->thr64[1];
+    a.mask4 = always4 ? 0u : 0xffffffffu;
+    a.mask8 = always8 ? 0u : 0xffffffffu;
+    for (int p = 0; p < 8; ++p)
+        a.pcase[p] = ((a.thr4 >> (31 - p)) & 1u) | (((a.thr8 >> (31 - p)) & 1u) << 1);
     a.R = march_rows(L, nq);
     a.threads = nq * (L / a.R);
     a.K = lat->K;
     build_plane_fold(lat->K, a.t, a.colour, TAG_ACC_PLANE, a.F);
     const unsigned blocks = (a.threads + 255u) / 256u;
-    if (colour == 0) ising_march_kernel<0><<<blocks, 256, 0, lat->stream>>>(a);
-    else ising_march_kernel<1><<<blocks, 256, 0, lat->stream>>>(a);
+    const bool edge = always4 || always8;
+    if (colour == 0) {
+        if (edge) ising_march_kernel<0, true><<<blocks, 256, 0, lat->stream>>>(a);
+        else ising_march_kernel<0, false><<<blocks, 256, 0, lat->stream>>>(a);
+    } else {
+        if (edge) ising_march_kernel<1, true><<<blocks, 256, 0, lat->stream>>>(a);
+        else ising_march_kernel<1, false><<<blocks, 256, 0, lat->stream>>>(a);
+    }
     lat->launches += 1;
     CU(lat, cudaGetLastError());
     return LATTICE_OK;
