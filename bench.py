@@ -191,6 +191,7 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_2503_14688_b200 as lat
+    from paper_2503_14688_b200 import replicas
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -204,16 +205,13 @@ def main():
 
     w = workloads.CONFIGS[args.workload]
     L = args.L or pick_L(w, torch, dev)
-    if world > 1:                               # all replicas use the same size
-        t = torch.tensor([L], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MIN)
-        L = int(t.item())
-    g = lat.Lattice(L, w.model, w.delta, seed=w.seed + 1000 * rank, scheme=args.scheme, device=str(dev))
+    L = replicas.agree_min(L, dev)              # all replicas use the same size
+    g = lat.Lattice(L, w.model, w.delta, seed=replicas.replica_seed(w.seed, rank), scheme=args.scheme,
+                    device=str(dev))
     updates_per_step = L * L
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier()
         torch.cuda.synchronize(dev)
 
     def timed(fn, steps, start_t):
@@ -224,11 +222,7 @@ def main():
             fn(start_t + k)
         ev1.record(g.stream)
         torch.cuda.synchronize(dev)
-        ms = ev0.elapsed_time(ev1)
-        if world > 1:
-            t = torch.tensor([ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = replicas.max_over_ranks(ev0.elapsed_time(ev1), dev)
         barrier()
         return ms
 
@@ -284,8 +278,8 @@ def main():
             dist.destroy_process_group()
         return
 
-    value = world * updates_per_step * args.steps / (ms * 1e6)
-    e2e_value = world * updates_per_step * args.steps / (e2e_ms * 1e6)
+    value = replicas.job_rate(updates_per_step * args.steps, world, ms)
+    e2e_value = replicas.job_rate(updates_per_step * args.steps, world, e2e_ms)
     peak, peak_src, sm_max = measured_peaks()
     bpu = BYTES_PER_UPDATE[w.model]
     launch_ms = ms / max(launches, 1)

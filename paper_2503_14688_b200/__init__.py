@@ -6,7 +6,7 @@ is its thin Python binding plus the seeded workload definitions.  There is no CP
 from .binding import (BLUME_CAPEL, ISING, Lattice, LatticeError, energy, lib, state_bytes,
                       thresholds, xi)
 from .buildlib import build
-from . import workloads
+from . import replicas, workloads
 
 __all__ = ["ISING", "BLUME_CAPEL", "Lattice", "LatticeError", "energy", "lib", "state_bytes",
-           "thresholds", "xi", "build", "workloads"]
+           "thresholds", "xi", "build", "workloads", "replicas"]
