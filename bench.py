@@ -51,11 +51,15 @@ UNIT = "spin updates/ns"
 BYTES_PER_UPDATE = {workloads.ISING: 0.375, workloads.BLUME_CAPEL: 0.75}
 # Integer-pipe roofline of the dominant kernel: thread-instructions of the
 # half-rate class (ALU pipe: LOP3/SHF/SEL/ISETP..., plus IMAD.WIDE/IMAD.HI, which block the same
-# 16-lane dispatch for two cycles) per spin update, from the committed ncu captures under
-# profiles/ (sm__inst_executed_pipe_alu + IMAD.WIDE/HI counts / updates per launch).
-HALF_RATE_INSTR_PER_UPDATE = {workloads.ISING: 4.00, workloads.BLUME_CAPEL: 5.54}
+# 16-lane dispatch for two cycles) per spin update.
+#   ALGORITHMIC: the floor of the method under the RNG contract (folded Philox planes, 2 LOP3 per
+#   word per plane of compare, class logic, 2^-8 tails), the analogue of algorithmic bytes;
+#   EXECUTED: from the committed ncu captures under profiles/ (sm__inst_executed_pipe_alu +
+#   IMAD.WIDE/HI counts / updates per launch).
+ALG_HALF_RATE_INSTR_PER_UPDATE = {workloads.ISING: 2.98, workloads.BLUME_CAPEL: 4.46}
+EXE_HALF_RATE_INSTR_PER_UPDATE = {workloads.ISING: 3.62, workloads.BLUME_CAPEL: 5.54}
 #: DRAM bytes per update measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum) / updates
-DRAM_BYTES_PER_UPDATE_NCU = {workloads.ISING: 0.363, workloads.BLUME_CAPEL: 0.667}
+DRAM_BYTES_PER_UPDATE_NCU = {workloads.ISING: 0.385, workloads.BLUME_CAPEL: 0.667}
 SM_COUNT, HALF_RATE_LANES_PER_CLK_PER_SM = 148, 64
 KERNEL = {workloads.ISING: "ising_march_kernel", workloads.BLUME_CAPEL: "bc_march_kernel"}
 
@@ -291,14 +295,16 @@ def main():
                     "bytes_per_update": bpu, "launch_ms": launch_ms, "l2_resident": in_l2}
     # the binding roofline: the 16-lane integer dispatch (ALU pipe + IMAD.WIDE), DESIGN.md section 6
     mhz = clocks.get("sm_mhz") or sm_max
-    ipu = HALF_RATE_INSTR_PER_UPDATE[w.model]
+    ipu, ipu_exe = ALG_HALF_RATE_INSTR_PER_UPDATE[w.model], EXE_HALF_RATE_INSTR_PER_UPDATE[w.model]
     peak_alu = SM_COUNT * HALF_RATE_LANES_PER_CLK_PER_SM * mhz * 1e6 / 1e12
     ach_alu = ipu * (updates_per_step / 2) / (launch_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": KERNEL[w.model], "achieved": ach_alu, "peak": peak_alu,
                 "unit": "T thread-instr/s", "frac": ach_alu / peak_alu,
                 "traffic": DRAM_BYTES_PER_UPDATE_NCU[w.model] * updates_per_step / 2,
                 "traffic_source": "ncu dram bytes per update (profiles/) x updates per launch",
-                "instr_per_update": ipu, "sm_mhz": mhz, "launch_ms": launch_ms,
+                "instr_per_update": ipu, "executed_instr_per_update": ipu_exe,
+                "executed_frac": ach_alu / peak_alu * ipu_exe / ipu,
+                "sm_mhz": mhz, "launch_ms": launch_ms,
                 "peak_source": "148 SM x 64 lanes/clk (ALU + IMAD.WIDE dispatch) x sampled SM clock",
                 "hbm_frac": achieved / peak, "hbm_achieved_GBs": achieved, "hbm_peak_GBs": peak}
     line = {
