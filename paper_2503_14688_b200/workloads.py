@@ -33,8 +33,11 @@ class Workload:
     seed: int
     sweeps: int
     r_max: int
-    protocol: int = 1                      # 1: constant beta; 2: ramp (BASELINE.json config 5)
+    protocol: int = 1                      # 1: constant beta; 2: ramp (BASELINE.json config 5);
+                                           # 3: the paper's two-step protocol (Table II)
     beta_f: float = field(default=BETA_C_ISING)
+    beta_1: float = 0.0                    # protocol 3: 1/T_1 for sweeps t < t_switch
+    t_switch: int = 0
 
     def beta_schedule(self, n: int | None = None, start: int = 0) -> np.ndarray:
         """beta[t] for sweeps start..start+n-1 as fp64 (what `lattice_sweep` takes)."""
@@ -42,6 +45,9 @@ class Workload:
         t = np.arange(start, start + n, dtype=np.float64)
         if self.protocol == 1:
             return np.full(n, self.beta_f, dtype=np.float64)
+        if self.protocol == 3:
+            # T_1 until t_switch, then T_2 (beta_f = 1/T_2)
+            return np.where(t < float(self.t_switch), self.beta_1, self.beta_f).astype(np.float64)
         # protocol 2: beta ramps linearly from 0.9*beta_f to beta_f over sweeps 0..999
         ramp = 0.9 * self.beta_f + (0.1 * self.beta_f) * (t / 999.0)
         return np.where(t < 999.0, ramp, self.beta_f).astype(np.float64)
@@ -80,4 +86,12 @@ CONFIGS: dict[str, Workload] = {
                                  1024, protocol=2, beta_f=BETA_C_ISING / 1.01),
     "bc_L2p15_ramp": Workload("bc_L2p15_ramp", BLUME_CAPEL, 1 << 15, 0.0, SEED_BASE + 6, 20000,
                               1024, protocol=2, beta_f=BETA_BC / 1.01),
+    # the paper's own two-step schedules (Table II, PAPER.md:142-153;
+    # the middle t_switch of each model).  Same API, a different beta array.
+    "ising_L2p16_twostep": Workload("ising_L2p16_twostep", ISING, 1 << 16, 0.0, SEED_BASE + 7,
+                                    3_000_000, 1024, protocol=3, beta_f=1.0 / 2.27414861561203,
+                                    beta_1=1.0 / 1.66, t_switch=4467),
+    "bc_L2p16_twostep": Workload("bc_L2p16_twostep", BLUME_CAPEL, 1 << 16, 0.0, SEED_BASE + 8,
+                                 2_097_152, 1024, protocol=3, beta_f=1.0 / 1.69661396797728,
+                                 beta_1=1.0 / 1.24, t_switch=41270),
 }

@@ -152,6 +152,28 @@ def test_protocol2_schedule_small(name):
     _same_measure(g, o, 64, L, w.delta)
 
 
+@pytest.mark.parametrize("name", ["ising_L2p16_twostep", "bc_L2p16_twostep"])
+def test_paper_two_step_schedule_small(name):
+    """The paper's protocol 2 (Table II): T_1 until t_switch, then T_2 -- on a
+    small lattice, across the switch (set_time moves both sides next to t_switch)."""
+    w = workloads.CONFIGS[name]
+    L = 256
+    g = lat.Lattice(L, w.model, w.delta, w.seed)
+    o = oracle.OracleLattice(L, w.model, w.delta, w.seed)
+    t0 = w.t_switch - 12
+    sched = w.beta_schedule(30, t0)
+    assert sched[11] == w.beta_1 and sched[12] == w.beta_f and len(np.unique(sched)) == 2
+    g.sweep(w.beta_schedule(10))
+    o.sweep(w.beta_schedule(10))
+    g.set_time(t0)
+    o.close()
+    o = oracle.OracleLattice.window(L, w.model, w.delta, w.seed, 1, t0, 0, 0, g.get_spins())
+    g.sweep(sched)
+    o.sweep(sched)
+    assert g.time == o.time == t0 + 30
+    assert np.array_equal(g.get_spins(), o.get_spins())
+
+
 @pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
 def test_special_states_and_set_get_roundtrip(model):
     L = 128
