@@ -178,10 +178,11 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
                 Ss = fsr1(C.sg[w], w == 3 ? Es : C.sg[w < 3 ? w + 1 : 0]);
             }
             const uint32_t nz = T.nz[w], sg = T.sg[w], bw = b[w];
-            Fm[w] = nz & ~(sg ^ bw);                              // flip
+            Fm[w] = lop3<0x90>(nz, sg, bw);                       // flip: nz & ~(sg ^ b)
             nf[w] = ~Fm[w];                                       // nz toggles unless the move is a flip
-            gg[w] = Fm[w] | (nz & sg & ~bw) | (~nz & bw);         // sg toggles: flip, vacate of -1, occupy -1
-            const uint32_t r = (nz & sg) | (~nz & ~bw);
+            // sg toggles on flip, vacate of -1, occupy to -1: Fm | (nz & sg & ~b) | (~nz & b)
+            gg[w] = lop3<0xDA>(nz, sg, bw);
+            const uint32_t r = lop3<0xC5>(nz, sg, bw);            // (nz & sg) | (~nz & ~b)
             // x + 4 = sum over the 4 neighbours of [sign r] + [not sign -r], bit-sliced
             const uint32_t a1 = U.nz[w] & ~(U.sg[w] ^ r), n1 = ~(U.nz[w] & (U.sg[w] ^ r));
             const uint32_t a2 = D.nz[w] & ~(D.sg[w] ^ r), n2 = ~(D.nz[w] & (D.sg[w] ^ r));
@@ -209,9 +210,9 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
         eq[w] = need;
         acc[w] = 0;
     }
-#pragma unroll 1
+#pragma unroll 1                     // unrolling replicates the 256-entry tables: slower (I-cache)
     for (int k = 7; k >= 0; --k) {
-        const uint4 b4 = plane_block(ps, a.F.fb[k], a.F, a.K);
+        const uint4 b4 = plane_block(ps, a.F.fb[0] ^ ((uint32_t)k << 16), a.F, a.K);
         const uint32_t b[4] = {b4.x, b4.y, b4.z, b4.w};
         uint32_t tau[4];
         lut3_dispatch(a.lut[k], Fm, Y1, H0, tau);

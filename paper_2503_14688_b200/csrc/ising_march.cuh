@@ -66,6 +66,16 @@ __host__ __device__ __forceinline__ uint32_t maj3m(uint32_t a, uint32_t b, uint3
 }
 
 #ifdef __CUDACC__
+// f(a, b, c) with the truth table LUT (bit (a<<2 | b<<1 | c)): one LOP3 where the compiler's own
+// decomposition of a 3-input expression would take two or three
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(r) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return r;
+}
+
 // One plane of the bit-serial compare for the 4 words of a run (see the header comment).
 // pcase = t4 | t8 << 1 (warp-uniform).  LOP3 truth tables, inputs (a, b, c) <-> (0xF0, 0xCC, 0xAA):
 //   acc' = f(c8, b, acc):  tau = 0: ~b & acc = 0x22;  tau = ~c8: 0x2B;  tau = c8: 0xB2;  tau = 1: ~b | acc = 0xBB
@@ -171,9 +181,9 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
         const uint32_t c1 = maj3m(U[w], D[w], C[w]);
         const uint32_t t = T[w];
         // k >= 3:  t = 1: c1 & (s1 | S);   t = 0: ~c1 & ~(s1 & S)
-        const uint32_t m = (t & (s1 | S)) | (~t & ~(s1 & S));
-        uint32_t nd = ~(c1 ^ t) & m;
-        uint32_t k4 = nd & ~(s1 ^ S);                                         // k == 4
+        const uint32_t m = lop3<0xE7>(t, s1, S);         // (t & (s1 | S)) | (~t & ~(s1 & S))
+        uint32_t nd = lop3<0x82>(c1, t, m);              // ~(c1 ^ t) & m
+        uint32_t k4 = lop3<0x90>(nd, s1, S);             // nd & ~(s1 ^ S): k == 4
         if (EDGE) {
             // classes whose threshold is 2^32 flip unconditionally: drop them from need
             const uint32_t k3 = nd & ~k4;
@@ -187,12 +197,13 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
     const PlaneShared ps = plane_shared(G, a.F);
 #pragma unroll
     for (int k = 7; k >= 0; --k) {
-        const uint4 b4 = plane_block(ps, a.F.fb[k], a.F, a.K);
+        // fb[k] = fb[0] ^ (k << 16): the plane index enters as an immediate of the first XOR
+        const uint4 b4 = plane_block(ps, a.F.fb[0] ^ ((uint32_t)k << 16), a.F, a.K);
         plane_compare(a.pcase[k], c8, b4, acc, eq);
     }
     // lanes outside need flip unconditionally (dE <= 0); a tied lane has acc = 0 and stays put
 #pragma unroll
-    for (int w = 0; w < 4; ++w) T[w] ^= ~need[w] | acc[w];
+    for (int w = 0; w < 4; ++w) T[w] = lop3<0x4B>(T[w], need[w], acc[w]);    // T ^ (~need | acc)
     *reinterpret_cast<uint4 *>(a.tgt + wo) = make_uint4(T[0], T[1], T[2], T[3]);
     queue.push(eq, c8, wo);
 }
