@@ -22,9 +22,10 @@
 //     warp-uniform pair (bit_k(thr4), bit_k(thr8)): a 4-way brx.idx per plane picks the LOP3
 //     immediates (inline PTX);
 //   * the rare lanes whose top random byte ties with the threshold's (2^-8 per deciding lane)
-//     are pushed, one 64-bit entry per lane, into a per-warp queue in shared memory; whenever 32
-//     entries are pending the warp resolves them, one tail Philox block per thread, and applies
-//     the accepted flips with a global atomic XOR on the already-stored word.
+//     are not resolved in place; the words that contain them are pushed (loop-free, one ballot
+//     per word) into a per-warp queue in shared memory; whenever 32 entries are pending the
+//     warp resolves them, one entry per thread (tail Philox block per tied lane), and applies the
+//     accepted flips with a global atomic XOR on the already-stored word.
 #pragma once
 #include "ising.cuh"
 
@@ -103,49 +104,53 @@ __device__ __forceinline__ void plane_compare(uint32_t pcase, const uint32_t (&c
 }
 #undef LAT_PL
 
-// Per-warp queue of tied lanes, one 64-bit entry per lane:
-//   bits 0..34 word offset of the lane's word in the colour array, 35..39 bit, 40 class (1 = dE 8).
-// At most 31 entries are pending before a push round and a round adds at most 32, so 64 slots
-// are enough.  Entries are resolved 32 at a time, one tail Philox block per thread.
+// Per-warp queue of words that contain tied lanes.  One 128-bit entry per word:
+//   x = the tied lanes of the word, y = which of them are class dE = 8, (z, w) = word offset.
+// Pushing is loop-free (one ballot per word of the run); the bits of a word are only
+// enumerated when the entry is resolved, 32 entries at a time, one entry per thread.  At most
+// 31 entries are pending before a row and a row adds at most 4 x 32.
+constexpr int TIE_Q_SLOTS = 160;
+
 struct WarpTieQueue {
     const IsingMarchArgs &a;
-    unsigned long long *q;     // [64] this warp's slice
+    uint4 *q;                  // [TIE_Q_SLOTS] this warp's slice
     uint32_t lane, pending;
 
     __device__ __forceinline__ void resolve(uint32_t idx)
     {
-        const unsigned long long e = q[idx];
-        const unsigned long long wo = e & 0x7ffffffffull;
-        const uint32_t bit = (uint32_t)(e >> 35) & 31u;
-        const unsigned long long P = (wo << 5) + bit;
-        const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
-                                        a.colour | (TAG_ACC_TAIL << 8), a.K);
-        const uint32_t thr = ((e >> 40) & 1u) ? a.thr8 : a.thr4;
-        if ((blk.x >> 8) < (thr & 0x00ffffffu)) atomicXor(a.tgt + wo, 1u << bit);
+        const uint4 e = q[idx];
+        const unsigned long long wo = ((unsigned long long)e.w << 32) | e.z;
+        uint32_t ties = e.x, flip = 0;
+        while (ties) {
+            const uint32_t bit = __ffs(ties) - 1;
+            ties &= ties - 1;
+            const unsigned long long P = (wo << 5) + bit;
+            const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
+                                            a.colour | (TAG_ACC_TAIL << 8), a.K);
+            const uint32_t thr = ((e.y >> bit) & 1u) ? a.thr8 : a.thr4;
+            if ((blk.x >> 8) < (thr & 0x00ffffffu)) flip |= 1u << bit;
+        }
+        if (flip) atomicXor(a.tgt + wo, flip);
     }
-    // collective over the warp: every thread pushes its tied lanes (eq words), one per round
-    __device__ __forceinline__ void push(uint32_t (&eq)[4], const uint32_t (&c8)[4], unsigned long long wo)
+    // collective over the warp: queue the words of this run that hold ties
+    __device__ __forceinline__ void push(const uint32_t (&eq)[4], const uint32_t (&c8)[4], unsigned long long wo)
     {
-        for (;;) {
-            const int w = eq[0] ? 0 : eq[1] ? 1 : eq[2] ? 2 : 3;
-            const uint32_t ew = eq[0] ? eq[0] : eq[1] ? eq[1] : eq[2] ? eq[2] : eq[3];
-            const uint32_t m = __ballot_sync(0xffffffffu, ew != 0);
-            if (m == 0) return;
-            if (ew) {
-                const uint32_t bit = __ffs(ew) - 1, bm = 1u << bit;
-                const uint32_t cw = w == 0 ? c8[0] : w == 1 ? c8[1] : w == 2 ? c8[2] : c8[3];
-                q[pending + __popc(m & ((1u << lane) - 1u))] =
-                    (wo + (unsigned)w) | ((unsigned long long)bit << 35) |
-                    ((unsigned long long)((cw >> bit) & 1u) << 40);
-                if (w == 0) eq[0] &= ~bm; else if (w == 1) eq[1] &= ~bm; else if (w == 2) eq[2] &= ~bm; else eq[3] &= ~bm;
+        const uint32_t below = (1u << lane) - 1u;
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const bool has = eq[w] != 0;
+            const uint32_t m = __ballot_sync(0xffffffffu, has);
+            if (has) {
+                const unsigned long long o = wo + (unsigned)w;
+                q[pending + __popc(m & below)] = make_uint4(eq[w], c8[w], (uint32_t)o, (uint32_t)(o >> 32));
             }
             pending += __popc(m);
+        }
+        __syncwarp();
+        while (pending >= 32) {
+            pending -= 32;
+            resolve(pending + lane);
             __syncwarp();
-            if (pending >= 32) {
-                pending -= 32;
-                resolve(pending + lane);
-                __syncwarp();
-            }
         }
     }
     __device__ __forceinline__ void drain()
@@ -211,7 +216,7 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
 template <int COLOUR, bool EDGE>
 __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a)
 {
-    __shared__ unsigned long long s_q[8][64];
+    __shared__ uint4 s_q[8][TIE_Q_SLOTS];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;
     if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
