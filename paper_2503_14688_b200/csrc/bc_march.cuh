@@ -20,8 +20,8 @@
 //
 // Work layout as in ising_march.cuh: one thread owns a 128-bit run and marches down R rows with
 // the opposite-colour rows i-1, i, i+1 in registers; folded Philox bit-planes; ties (top byte of
-// u32 equal to the top byte of the lane's threshold) are queued per warp as one 64-bit entry per
-// tied lane and resolved 32 at a time, accepted late moves applied with global atomic XORs.
+// u32 equal to the top byte of the lane's threshold) are queued per warp, one entry per word that
+// holds ties, and resolved 32 entries at a time, accepted late moves applied with global atomic XORs.
 #pragma once
 #include "bc.cuh"
 #include "ising_march.cuh"
@@ -78,58 +78,55 @@ __device__ __forceinline__ void lut3_dispatch(uint32_t lut, const uint32_t (&a)[
 #undef LAT_LR
 #undef LAT_TR
 
-// per-warp queue of tied lanes: one 64-bit entry per lane
-//   bits 0..33 word offset of the lane's word, 34..38 bit, 39..41 class, 42 nz toggles, 43 sg toggles
+// Per-warp queue of words that contain tied lanes (same scheme as WarpTieQueue in
+// ising_march.cuh).  Two 128-bit halves per entry:
+//   [0] = (tied lanes, F, Y1, H0 of the word)    [1] = (nz-toggle mask, sg-toggle mask, word offset)
+// Pushing is loop-free (one ballot per word); the tied lanes of a word are enumerated when the
+// entry is resolved, 32 entries at a time, one entry per thread.
 struct BCTieQueue {
     const BCMarchArgs &a;
-    unsigned long long *q;      // [64 + 32] this warp's slice
+    uint4 *q;                   // [2 * TIE_Q_SLOTS] this warp's slice
     uint32_t lane, pending;
 
     __device__ __forceinline__ void resolve(uint32_t idx)
     {
-        const unsigned long long e = q[idx];
-        const unsigned long long wo = e & 0x3ffffffffull;
-        const uint32_t bit = (uint32_t)(e >> 34) & 31u, cls = (uint32_t)(e >> 39) & 7u;
-        const unsigned long long P = (wo << 5) + bit;
-        const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
-                                        a.colour | (TAG_ACC_TAIL << 8), a.K);
-        if ((blk.x >> 8) < (a.thr[cls] & 0x00ffffffu)) {
-            if ((e >> 42) & 1u) atomicXor(a.tnz + wo, 1u << bit);
-            if ((e >> 43) & 1u) atomicXor(a.tsg + wo, 1u << bit);
+        const uint4 e0 = q[2 * idx], e1 = q[2 * idx + 1];
+        const unsigned long long wo = ((unsigned long long)e1.w << 32) | e1.z;
+        uint32_t ties = e0.x, hit = 0;
+        while (ties) {
+            const uint32_t bit = __ffs(ties) - 1;
+            ties &= ties - 1;
+            const uint32_t cls = (((e0.y >> bit) & 1u) << 2) | (((e0.z >> bit) & 1u) << 1) | ((e0.w >> bit) & 1u);
+            const unsigned long long P = (wo << 5) + bit;
+            const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
+                                            a.colour | (TAG_ACC_TAIL << 8), a.K);
+            if ((blk.x >> 8) < (a.thr[cls] & 0x00ffffffu)) hit |= 1u << bit;
         }
+        if (hit & e1.x) atomicXor(a.tnz + wo, hit & e1.x);
+        if (hit & e1.y) atomicXor(a.tsg + wo, hit & e1.y);
     }
-    // collective over the warp: every thread pushes its tied lanes (eq words) one at a time
-    __device__ __forceinline__ void push(uint32_t (&eq)[4], const uint32_t (&Fm)[4], const uint32_t (&Y1)[4],
+    __device__ __forceinline__ void push(const uint32_t (&eq)[4], const uint32_t (&Fm)[4], const uint32_t (&Y1)[4],
                                          const uint32_t (&H0)[4], const uint32_t (&nf)[4],
                                          const uint32_t (&gg)[4], unsigned long long wo)
     {
-        for (;;) {
-            const int w = eq[0] ? 0 : eq[1] ? 1 : eq[2] ? 2 : 3;
-            const uint32_t ew = eq[0] ? eq[0] : eq[1] ? eq[1] : eq[2] ? eq[2] : eq[3];
-            const uint32_t m = __ballot_sync(0xffffffffu, ew != 0);
-            if (m == 0) return;
-            if (ew) {
-                const uint32_t bit = __ffs(ew) - 1, bm = 1u << bit;
-                const uint32_t fw = w == 0 ? Fm[0] : w == 1 ? Fm[1] : w == 2 ? Fm[2] : Fm[3];
-                const uint32_t yw = w == 0 ? Y1[0] : w == 1 ? Y1[1] : w == 2 ? Y1[2] : Y1[3];
-                const uint32_t hw = w == 0 ? H0[0] : w == 1 ? H0[1] : w == 2 ? H0[2] : H0[3];
-                const uint32_t nw = w == 0 ? nf[0] : w == 1 ? nf[1] : w == 2 ? nf[2] : nf[3];
-                const uint32_t gw = w == 0 ? gg[0] : w == 1 ? gg[1] : w == 2 ? gg[2] : gg[3];
-                const uint32_t cls = (((fw >> bit) & 1u) << 2) | (((yw >> bit) & 1u) << 1) | ((hw >> bit) & 1u);
-                const unsigned long long e = (wo + (unsigned)w) | ((unsigned long long)bit << 34) |
-                                             ((unsigned long long)cls << 39) |
-                                             ((unsigned long long)((nw >> bit) & 1u) << 42) |
-                                             ((unsigned long long)((gw >> bit) & 1u) << 43);
-                q[pending + __popc(m & ((1u << lane) - 1u))] = e;
-                if (w == 0) eq[0] &= ~bm; else if (w == 1) eq[1] &= ~bm; else if (w == 2) eq[2] &= ~bm; else eq[3] &= ~bm;
+        const uint32_t below = (1u << lane) - 1u;
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const bool has = eq[w] != 0;
+            const uint32_t m = __ballot_sync(0xffffffffu, has);
+            if (has) {
+                const unsigned long long o = wo + (unsigned)w;
+                const uint32_t slot = pending + __popc(m & below);
+                q[2 * slot] = make_uint4(eq[w], Fm[w], Y1[w], H0[w]);
+                q[2 * slot + 1] = make_uint4(nf[w], gg[w], (uint32_t)o, (uint32_t)(o >> 32));
             }
             pending += __popc(m);
+        }
+        __syncwarp();
+        while (pending >= 32) {
+            pending -= 32;
+            resolve(pending + lane);
             __syncwarp();
-            if (pending >= 32) {
-                pending -= 32;
-                resolve(pending + lane);
-                __syncwarp();
-            }
         }
     }
     __device__ __forceinline__ void drain()
@@ -236,7 +233,7 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
 template <int COLOUR>
 __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
 {
-    __shared__ unsigned long long s_q[8][64];
+    __shared__ uint4 s_q[8][2 * TIE_Q_SLOTS];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;
     if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
