@@ -146,14 +146,15 @@ def run_reference(args):
     if rank != 0:
         return
     w = workloads.CONFIGS[args.workload]
-    Ls = min(w.L, 2048)
+    Ls, ns = min(w.L, 4096), 8                   # one step = 8 sweeps of a 4096 x 4096 sample (~1 s)
     for _ in range(args.warmup):
         oracle_rate(w, 256, 1)
     t0 = time.perf_counter()
-    rates = [oracle_rate(w, Ls, 1) for _ in range(args.steps)]
+    rates = [oracle_rate(w, Ls, ns) for _ in range(args.steps)]
     wall = time.perf_counter() - t0
-    value = Ls * Ls * args.steps / sum(r[1] for r in rates) / 1e9
-    sample = f"{args.steps} steps, each one sweep of a {Ls}x{Ls} {w.name}-shaped lattice (scheme 1)"
+    value = Ls * Ls * ns * args.steps / sum(r[1] for r in rates) / 1e9
+    sample = (f"{args.steps} steps, each {ns} sweeps of a {Ls}x{Ls} {w.name}-shaped lattice "
+              f"(same model, beta, RNG scheme 1)")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(args.steps, 1),
