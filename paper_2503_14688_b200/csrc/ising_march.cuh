@@ -166,11 +166,11 @@ struct WarpTieQueue {
 // PAR == 1: the word after it).  Stores the updated words with every tie treated as a rejection
 // and queues the ties.  EDGE: some class has threshold 2^32 (beta = 0): mask it out of `need`.
 template <int PAR, bool EDGE>
-__device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, unsigned long long wo,
+__device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, unsigned long long wo, uint32_t *tp,
                                           const uint4 &U4, const uint4 &C4, const uint4 &D4, uint32_t E,
                                           WarpTieQueue &queue)
 {
-    const uint4 T4 = *reinterpret_cast<const uint4 *>(a.tgt + wo);
+    const uint4 T4 = *reinterpret_cast<const uint4 *>(tp);       // tp == a.tgt + wo
     uint32_t T[4] = {T4.x, T4.y, T4.z, T4.w};
     const uint32_t U[4] = {U4.x, U4.y, U4.z, U4.w};
     const uint32_t C[4] = {C4.x, C4.y, C4.z, C4.w};
@@ -209,7 +209,7 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
     // lanes outside need flip unconditionally (dE <= 0); a tied lane has acc = 0 and stays put
 #pragma unroll
     for (int w = 0; w < 4; ++w) T[w] = lop3<0x4B>(T[w], need[w], acc[w]);    // T ^ (~need | acc)
-    *reinterpret_cast<uint4 *>(a.tgt + wo) = make_uint4(T[0], T[1], T[2], T[3]);
+    *reinterpret_cast<uint4 *>(tp) = make_uint4(T[0], T[1], T[2], T[3]);
     queue.push(eq, c8, wo);
 }
 
@@ -231,27 +231,31 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
     const uint32_t ke0 = (kw == 0) ? wpr - 1 : kw - 1;
     const uint32_t ke1 = (kw + 4 == wpr) ? 0 : kw + 4;
 
-    unsigned long long ro = (unsigned long long)i0 * wpr;            // word offset of row i
+    const unsigned long long ro = (unsigned long long)i0 * wpr;      // word offset of row i0
     uint4 U = *reinterpret_cast<const uint4 *>(a.opp + (unsigned long long)iu * wpr + kw);
     uint4 C = *reinterpret_cast<const uint4 *>(a.opp + ro + kw);
     uint32_t G = i0 * nq + q;                                        // (i*(L/2) + 32 kw) >> 7
+    // running pointers: the slab's own rows never wrap; only row i+1 of the last lattice row does
+    const uint32_t *op = a.opp + ro;                                 // row i of the opposite colour
+    uint32_t *tp = a.tgt + ro + kw;                                  // this run in row i
+    unsigned long long wo = ro + kw;
+    uint32_t left = L - i0;                                          // rows from i to the lattice end
 
     for (uint32_t r = 0; r < a.R; r += 2) {
         {   // row i0 + r: (i + colour) & 1 == COLOUR because i0 and r are even
-            const uint32_t i = i0 + r;
-            const unsigned long long rd = (i + 1 == L) ? 0ull : ro + wpr;
-            const uint4 D = *reinterpret_cast<const uint4 *>(a.opp + rd + kw);
-            const uint32_t E = a.opp[ro + (COLOUR == 0 ? ke0 : ke1)];
-            march_row<COLOUR, EDGE>(a, G, ro + kw, U, C, D, E, queue);
-            U = C; C = D; ro = rd; G += nq;
+            const uint32_t *dn = op + wpr;                           // row i + 1 (left >= 2 here)
+            const uint4 D = *reinterpret_cast<const uint4 *>(dn + kw);
+            const uint32_t E = op[COLOUR == 0 ? ke0 : ke1];
+            march_row<COLOUR, EDGE>(a, G, wo, tp, U, C, D, E, queue);
+            U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
-        {   // row i0 + r + 1: the other parity
-            const uint32_t i = i0 + r + 1;
-            const unsigned long long rd = (i + 1 == L) ? 0ull : ro + wpr;
-            const uint4 D = *reinterpret_cast<const uint4 *>(a.opp + rd + kw);
-            const uint32_t E = a.opp[ro + (COLOUR == 0 ? ke1 : ke0)];
-            march_row<COLOUR ^ 1, EDGE>(a, G, ro + kw, U, C, D, E, queue);
-            U = C; C = D; ro = rd; G += nq;
+        {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
+            left -= 2;
+            const uint32_t *dn = left ? op + wpr : a.opp;
+            const uint4 D = *reinterpret_cast<const uint4 *>(dn + kw);
+            const uint32_t E = op[COLOUR == 0 ? ke1 : ke0];
+            march_row<COLOUR ^ 1, EDGE>(a, G, wo, tp, U, C, D, E, queue);
+            U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
     }
     queue.drain();
