@@ -154,11 +154,12 @@ __device__ __forceinline__ void bcm_load(const uint32_t *nzp, const uint32_t *sg
 // queues the ties.
 template <int PAR>
 __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, unsigned long long wo,
+                                             uint32_t *tn, uint32_t *ts,
                                              const BCRow &U, const BCRow &C, const BCRow &D,
                                              uint32_t En, uint32_t Es, BCTieQueue &queue)
 {
     BCRow T;
-    bcm_load(a.tnz, a.tsg, wo, T);
+    bcm_load(tn, ts, 0, T);                                       // tn == a.tnz + wo, ts == a.tsg + wo
     const PlaneShared ps = plane_shared(G, a.F);
     uint32_t Fm[4], Y1[4], H0[4], pos[4], nf[4], gg[4];
     {
@@ -225,8 +226,8 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
         T.nz[w] ^= ok & nf[w];
         T.sg[w] ^= ok & gg[w];
     }
-    *reinterpret_cast<uint4 *>(a.tnz + wo) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
-    *reinterpret_cast<uint4 *>(a.tsg + wo) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
+    *reinterpret_cast<uint4 *>(tn) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
+    *reinterpret_cast<uint4 *>(ts) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
     queue.push(eq, Fm, Y1, H0, nf, gg, wo);
 }
 
@@ -246,27 +247,33 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
     const uint32_t iu = (i0 == 0) ? L - 1 : i0 - 1;
     const uint32_t ke0 = (kw == 0) ? wpr - 1 : kw - 1;       // word before the run (periodic)
     const uint32_t ke1 = (kw + 4 == wpr) ? 0 : kw + 4;       // word after it
-    unsigned long long ro = (unsigned long long)i0 * wpr;
+    const unsigned long long ro = (unsigned long long)i0 * wpr;
     BCRow U, C, D;
     bcm_load(a.onz, a.osg, (unsigned long long)iu * wpr + kw, U);
     bcm_load(a.onz, a.osg, ro + kw, C);
     uint32_t G = i0 * nq + q;
+    // running pointers: the slab's own rows never wrap; only row i+1 of the last lattice row does
+    // (the sg plane sits one plane stride pw = L * wpr words after the nz plane)
+    const unsigned long long pw = (unsigned long long)L * wpr;
+    const uint32_t *on = a.onz + ro;                                // row i of the opposite colour (nz)
+    uint32_t *tn = a.tnz + ro + kw;                                 // this run in row i (nz)
+    unsigned long long wo = ro + kw;
+    uint32_t left = L - i0;
     for (uint32_t r = 0; r < a.R; r += 2) {
         {   // row i0 + r: (i + colour) & 1 == COLOUR
-            const uint32_t i = i0 + r;
-            const unsigned long long rd = (i + 1 == L) ? 0ull : ro + wpr;
-            bcm_load(a.onz, a.osg, rd + kw, D);
-            const unsigned long long eo = ro + (COLOUR == 0 ? ke0 : ke1);
-            bc_march_row<COLOUR>(a, G, ro + kw, U, C, D, a.onz[eo], a.osg[eo], queue);
-            U = C; C = D; ro = rd; G += nq;
+            const uint32_t *dn = on + wpr;
+            bcm_load(dn, dn + pw, kw, D);
+            const uint32_t ke = COLOUR == 0 ? ke0 : ke1;
+            bc_march_row<COLOUR>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+            U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
-        {   // row i0 + r + 1: the other parity
-            const uint32_t i = i0 + r + 1;
-            const unsigned long long rd = (i + 1 == L) ? 0ull : ro + wpr;
-            bcm_load(a.onz, a.osg, rd + kw, D);
-            const unsigned long long eo = ro + (COLOUR == 0 ? ke1 : ke0);
-            bc_march_row<COLOUR ^ 1>(a, G, ro + kw, U, C, D, a.onz[eo], a.osg[eo], queue);
-            U = C; C = D; ro = rd; G += nq;
+        {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
+            left -= 2;
+            const uint32_t *dn = left ? on + wpr : a.onz;
+            bcm_load(dn, dn + pw, kw, D);
+            const uint32_t ke = COLOUR == 0 ? ke1 : ke0;
+            bc_march_row<COLOUR ^ 1>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+            U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
     }
     queue.drain();
