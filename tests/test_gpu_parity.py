@@ -248,6 +248,30 @@ def test_measure_r1_single_pass(L, model):
         _same_measure(g, o, 1, L, rows=(i0, n))
 
 
+def test_randomised_parity_sweep_of_parameters():
+    """Seeded random (model, L, scheme, beta schedule, Delta, seed) cases: spins and counts after a
+    few sweeps, bit for bit.  Covers the generic kernels (L not a multiple of 256, scheme 0,
+    Delta != 0) next to the marching ones, and per-sweep threshold changes."""
+    rng = np.random.default_rng(20250314)
+    for case in range(24):
+        model = int(rng.integers(0, 2))
+        L = int(rng.choice([64, 128, 192, 256, 320, 512, 768]))
+        scheme = int(rng.integers(0, 2))
+        delta = float(rng.choice([0.0, 0.0, rng.uniform(-2, 2)])) if model == lat.BLUME_CAPEL else 0.0
+        seed = int(rng.integers(0, 2 ** 63))
+        n = int(rng.integers(3, 9))
+        beta = rng.uniform(0.0, 1.2, size=n)
+        if case % 5 == 0:
+            beta[int(rng.integers(0, n))] = 0.0                 # an "always accept" sweep in the middle
+        g = lat.Lattice(L, model, delta, seed, scheme)
+        o = oracle.OracleLattice(L, model, delta, seed, scheme)
+        g.sweep(beta)
+        o.sweep(beta)
+        assert np.array_equal(g.get_spins(), o.get_spins()), (case, model, L, scheme, delta, seed)
+        _same_measure(g, o, int(rng.integers(1, L // 2 + 1)), L, delta)
+        g.close(); o.close()
+
+
 @pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
 def test_determinism_and_checkpoint_resume(model):
     L = 512
