@@ -75,6 +75,30 @@ size_t lattice_state_bytes(uint32_t L, int model);
 int lattice_create(lattice_t **out, uint32_t L, int model, double delta, uint64_t seed,
                    void *device_buf, size_t device_buf_bytes, void *cuda_stream);
 
+/* ---- Row-slab domain decomposition (the paper's third level of parallelism, PAPER.md:32-34;
+ * SURVEY.md section 8(f) NEXT-1) -------------------------------------------
+ * A slab owns global rows row0 .. row0+n_rows-1 of a periodic L x L lattice and keeps one halo
+ * row above and below them: layout [colour][n_rows + 2][L/64] 32-bit words, local row l being
+ * global row (row0 - 1 + l) mod L.  Random numbers are keyed by GLOBAL (row, column), so N slabs
+ * evolve bit for bit like the whole lattice.  Every half-sweep kernel stores the slab's first
+ * and last own row a second time, directly into the neighbour slabs' halo rows (and applies late
+ * tie flips there with atomics): those pointers may be peer-GPU memory (NVLink P2P), so the halo
+ * exchange is fused into the update kernel and needs no copy or collective.  The caller orders
+ * the half-sweeps: all slabs finish colour c (and its mirrors) before any starts colour 1-c.
+ * Restrictions (round 1): Ising, RNG scheme 1, L a multiple of 256, row0 and n_rows multiples
+ * of 64; lattice_measure only with r_max == 1 (partial sums over the own rows: add them up);
+ * windows of get/set_spins must stay inside the slab's rows (halos included). */
+size_t lattice_slab_bytes(uint32_t L, int model, uint32_t n_rows);      /* 0 if not supported */
+/* Like lattice_create for the slab; own rows AND halos receive the disordered start. */
+int lattice_create_slab(lattice_t **out, uint32_t L, int model, double delta, uint64_t seed,
+                        uint32_t row0, uint32_t n_rows, void *device_buf, size_t device_buf_bytes,
+                        void *cuda_stream);
+/* Device buffers (and n_rows) of the slabs that own the rows above and below this one (this
+ * slab's own buffer twice when it is the only slab).  Required before the first half-sweep
+ * (ESTATE otherwise).  The buffers must stay valid and, if on another GPU, peer-accessible. */
+int lattice_slab_set_neighbours(lattice_t *lat, void *device_up_buf, uint32_t up_n_rows,
+                                void *device_down_buf, uint32_t down_n_rows);
+
 /* Select how u32(site) is derived from Philox4x32-10:
  *   0 "quad":       one block per 4 consecutive same-colour sites, one 32-bit word each;
  *   1 "plane+tail": top 8 bits from 8 bit-plane blocks shared by 128 sites, low 24 bits from a

@@ -28,6 +28,10 @@ SIGNATURES = {
     "lattice_state_bytes": (C.c_size_t, [C.c_uint32, C.c_int]),
     "lattice_create": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_double, C.c_uint64,
                                  _vp, C.c_size_t, _vp]),
+    "lattice_slab_bytes": (C.c_size_t, [C.c_uint32, C.c_int, C.c_uint32]),
+    "lattice_create_slab": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_double, C.c_uint64,
+                                      C.c_uint32, C.c_uint32, _vp, C.c_size_t, _vp]),
+    "lattice_slab_set_neighbours": (C.c_int, [_vp, _vp, C.c_uint32, _vp, C.c_uint32]),
     "lattice_set_rng_scheme": (C.c_int, [_vp, C.c_int]),
     "lattice_sweep": (C.c_int, [_vp, C.c_uint64, _f64p]),
     "lattice_half_sweep": (C.c_int, [_vp, C.c_int, C.c_double]),
@@ -105,22 +109,32 @@ class Lattice:
     """A packed lattice in device memory (a torch.uint8 tensor owned by this object)."""
 
     def __init__(self, L: int, model: int = ISING, delta: float = 0.0, seed: int = 0,
-                 scheme: int = 1, device: str = "cuda:0", stream=None):
+                 scheme: int = 1, device: str = "cuda:0", stream=None, slab=None):
+        """slab = (row0, n_rows) creates a row slab of the L x L lattice (include/lattice.h)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2503_14688_b200 needs a CUDA device; there is no CPU path")
         self.L, self.model, self.delta, self.seed = int(L), int(model), float(delta), int(seed)
-        nbytes = state_bytes(self.L, self.model)
+        self.slab = None if slab is None else (int(slab[0]), int(slab[1]))
+        if self.slab is None:
+            nbytes = state_bytes(self.L, self.model)
+        else:
+            nbytes = int(lib().lattice_slab_bytes(self.L, self.model, self.slab[1]))
         if nbytes == 0:
-            raise LatticeError("lattice_state_bytes", EINVAL, f"L={L} model={model}")
+            raise LatticeError("lattice_state_bytes", EINVAL, f"L={L} model={model} slab={slab}")
         self._torch = torch
         self.device = torch.device(device)
         with torch.cuda.device(self.device):
             self.buf = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = _vp()
-            rc = lib().lattice_create(C.byref(h), self.L, self.model, self.delta, self.seed,
-                                      _vp(self.buf.data_ptr()), nbytes, _vp(self.stream.cuda_stream))
+            if self.slab is None:
+                rc = lib().lattice_create(C.byref(h), self.L, self.model, self.delta, self.seed,
+                                          _vp(self.buf.data_ptr()), nbytes, _vp(self.stream.cuda_stream))
+            else:
+                rc = lib().lattice_create_slab(C.byref(h), self.L, self.model, self.delta, self.seed,
+                                               self.slab[0], self.slab[1], _vp(self.buf.data_ptr()),
+                                               nbytes, _vp(self.stream.cuda_stream))
         if rc != OK:
             raise LatticeError("lattice_create", rc)
         self._h = h
@@ -154,6 +168,13 @@ class Lattice:
     def launches(self) -> int:
         return int(lib().lattice_launches(self._h))
 
+    def set_neighbours(self, up: "Lattice", down: "Lattice") -> None:
+        """Row-slab mode: the slabs owning the rows above / below (self twice for a single slab)."""
+        self._check(lib().lattice_slab_set_neighbours(self._h, _vp(up.buf.data_ptr()), up.slab[1],
+                                                      _vp(down.buf.data_ptr()), down.slab[1]),
+                    "lattice_slab_set_neighbours")
+        self._nbr = (up, down)                       # keep the neighbours' buffers alive
+
     def set_time(self, t: int) -> None:
         self._check(lib().lattice_set_time(self._h, int(t)), "lattice_set_time")
 
@@ -184,6 +205,8 @@ class Lattice:
         return int(M.value), int(Q.value), Sx, Sy
 
     def get_spins(self, i0: int = 0, j0: int = 0, h: int | None = None, w: int | None = None):
+        if self.slab is not None and h is None:
+            i0, h = self.slab                        # a slab's default window: its own rows
         h = self.L if h is None else h
         w = self.L if w is None else w
         out = np.zeros((h, w), dtype=np.int8)

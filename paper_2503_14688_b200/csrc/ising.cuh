@@ -232,4 +232,27 @@ __global__ void __launch_bounds__(256) ising_init_kernel(const IsingInitArgs a)
     a.buf[g] = pick(blk, (uint32_t)(P0 >> 5) & 3u);
 }
 
+// Row-slab variant of the disordered start: the slab holds local rows 0 .. rows-1 per colour,
+// local row l being global row (row_base + l) mod L (local rows 0 and rows-1 are halo rows).
+// Keying uses global coordinates, so the halos are born consistent with their owners.
+struct IsingSlabInitArgs {
+    uint32_t *buf;            // [2][rows][wpr]
+    uint32_t L, wpr, rows, row_base;
+    RoundKeys K;
+};
+
+__global__ void __launch_bounds__(256) ising_init_slab_kernel(const IsingSlabInitArgs a)
+{
+    const unsigned long long words = (unsigned long long)a.rows * a.wpr;   // per colour
+    const unsigned long long g = (unsigned long long)blockIdx.x * 256u + threadIdx.x;
+    if (g >= 2 * words) return;
+    const uint32_t colour = g >= words;
+    const unsigned long long wi = g - (colour ? words : 0);
+    const uint32_t li = (uint32_t)(wi / a.wpr), k = (uint32_t)(wi % a.wpr);
+    const uint32_t gi = (a.row_base + li) % a.L;
+    const unsigned long long P0 = ((unsigned long long)gi * a.wpr + k) << 5;
+    const uint4 blk = philox_unit(P0 >> 7, 0, colour, TAG_INIT_PLANE, 0, a.K);
+    a.buf[g] = pick(blk, (uint32_t)(P0 >> 5) & 3u);
+}
+
 }  // namespace lat

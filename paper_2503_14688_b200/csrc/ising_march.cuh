@@ -34,7 +34,13 @@ namespace lat {
 struct IsingMarchArgs {
     uint32_t *tgt;            // colour being updated   [L][wpr]
     const uint32_t *opp;      // opposite colour        [L][wpr]
-    uint32_t L, wpr;
+    uint32_t L, wpr;          // L = rows allocated per colour (lattice side, or n_rows + 2 for a slab)
+    // row-slab mode (all zero / null for a whole lattice):
+    uint32_t row_off;         // local index of the first own row (1: local row 0 is a halo row)
+    uint32_t g_off;           // added to the RNG unit index: (global row of local row 0) * (wpr/4)
+    long long p_off;          // global minus local word offset, for the tail keying
+    uint32_t *mir_up;         // where the first / last own row of tgt is mirrored: the neighbour
+    uint32_t *mir_dn;         // slabs' halo rows (possibly peer-GPU memory), same [wpr] layout
     uint32_t t, colour;
     uint32_t thr4, thr8;      // thresholds for dE = 4, 8 (low 24 bits used by the tails)
     uint32_t mask4, mask8;    // 0 if the class flips unconditionally (threshold == 2^32), else ~0
@@ -116,24 +122,30 @@ struct WarpTieQueue {
     uint4 *q;                  // [TIE_Q_SLOTS] this warp's slice
     uint32_t lane, pending;
 
+    // entry.w = word offset bits 32..35 | column word << 4 | mirror flag << 30 (1 = up, 2 = down)
     __device__ __forceinline__ void resolve(uint32_t idx)
     {
         const uint4 e = q[idx];
-        const unsigned long long wo = ((unsigned long long)e.w << 32) | e.z;
+        const unsigned long long wo = ((unsigned long long)(e.w & 0xFu) << 32) | e.z;
         uint32_t ties = e.x, flip = 0;
         while (ties) {
             const uint32_t bit = __ffs(ties) - 1;
             ties &= ties - 1;
-            const unsigned long long P = (wo << 5) + bit;
+            const unsigned long long P = ((wo + a.p_off) << 5) + bit;
             const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
                                             a.colour | (TAG_ACC_TAIL << 8), a.K);
             const uint32_t thr = ((e.y >> bit) & 1u) ? a.thr8 : a.thr4;
             if ((blk.x >> 8) < (thr & 0x00ffffffu)) flip |= 1u << bit;
         }
-        if (flip) atomicXor(a.tgt + wo, flip);
+        if (flip) {
+            atomicXor(a.tgt + wo, flip);
+            const uint32_t mf = e.w >> 30;
+            if (mf) atomicXor((mf == 1 ? a.mir_up : a.mir_dn) + ((e.w >> 4) & 0x3ffffu), flip);
+        }
     }
     // collective over the warp: queue the words of this run that hold ties
-    __device__ __forceinline__ void push(const uint32_t (&eq)[4], const uint32_t (&c8)[4], unsigned long long wo)
+    __device__ __forceinline__ void push(const uint32_t (&eq)[4], const uint32_t (&c8)[4], unsigned long long wo,
+                                         uint32_t mir_tag)
     {
         const uint32_t below = (1u << lane) - 1u;
 #pragma unroll
@@ -142,7 +154,8 @@ struct WarpTieQueue {
             const uint32_t m = __ballot_sync(0xffffffffu, has);
             if (has) {
                 const unsigned long long o = wo + (unsigned)w;
-                q[pending + __popc(m & below)] = make_uint4(eq[w], c8[w], (uint32_t)o, (uint32_t)(o >> 32));
+                q[pending + __popc(m & below)] =
+                    make_uint4(eq[w], c8[w], (uint32_t)o, (uint32_t)(o >> 32) | (mir_tag + ((unsigned)w << 4)));
             }
             pending += __popc(m);
         }
@@ -165,10 +178,12 @@ struct WarpTieQueue {
 // i+1 at the same packed position; E: the side word (PAR == 0: the word before the run,
 // PAR == 1: the word after it).  Stores the updated words with every tie treated as a rejection
 // and queues the ties.  EDGE: some class has threshold 2^32 (beta = 0): mask it out of `need`.
+// mir / mir_tag: slab mode only -- where this row is mirrored (null: nowhere) and the queue tag
+// (column word << 4 | flag << 30) that lets a late flip reach the mirror too.
 template <int PAR, bool EDGE>
 __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, unsigned long long wo, uint32_t *tp,
                                           const uint4 &U4, const uint4 &C4, const uint4 &D4, uint32_t E,
-                                          WarpTieQueue &queue)
+                                          WarpTieQueue &queue, uint32_t *mir = nullptr, uint32_t mir_tag = 0)
 {
     const uint4 T4 = *reinterpret_cast<const uint4 *>(tp);       // tp == a.tgt + wo
     uint32_t T[4] = {T4.x, T4.y, T4.z, T4.w};
@@ -210,10 +225,11 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
 #pragma unroll
     for (int w = 0; w < 4; ++w) T[w] = lop3<0x4B>(T[w], need[w], acc[w]);    // T ^ (~need | acc)
     *reinterpret_cast<uint4 *>(tp) = make_uint4(T[0], T[1], T[2], T[3]);
-    queue.push(eq, c8, wo);
+    if (mir) *reinterpret_cast<uint4 *>(mir) = make_uint4(T[0], T[1], T[2], T[3]);
+    queue.push(eq, c8, wo, mir_tag);
 }
 
-template <int COLOUR, bool EDGE>
+template <int COLOUR, bool EDGE, bool SLAB>
 __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a)
 {
     __shared__ uint4 s_q[8][TIE_Q_SLOTS];
@@ -225,7 +241,7 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
     const uint32_t q = g % nq, s = g / nq;
     const uint32_t kw = q << 2;
-    const uint32_t i0 = s * a.R;
+    const uint32_t i0 = s * a.R + (SLAB ? a.row_off : 0u);
     const uint32_t iu = (i0 == 0) ? L - 1 : i0 - 1;
     // side words: PAR == 0 reads the word before the run, PAR == 1 the word after it (periodic)
     const uint32_t ke0 = (kw == 0) ? wpr - 1 : kw - 1;
@@ -234,7 +250,10 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
     const unsigned long long ro = (unsigned long long)i0 * wpr;      // word offset of row i0
     uint4 U = *reinterpret_cast<const uint4 *>(a.opp + (unsigned long long)iu * wpr + kw);
     uint4 C = *reinterpret_cast<const uint4 *>(a.opp + ro + kw);
-    uint32_t G = i0 * nq + q;                                        // (i*(L/2) + 32 kw) >> 7
+    uint32_t G = i0 * nq + q + (SLAB ? a.g_off : 0u);                // (global i*(L/2) + 32 kw) >> 7
+    // slab mode: the first own row is mirrored into the upper neighbour's halo, the last into the
+    // lower neighbour's (this slab's own halos when it is the only one)
+    const bool top = SLAB && s == 0, bot = SLAB && (s + 1) * nq == a.threads;
     // running pointers: the slab's own rows never wrap; only row i+1 of the last lattice row does
     const uint32_t *op = a.opp + ro;                                 // row i of the opposite colour
     uint32_t *tp = a.tgt + ro + kw;                                  // this run in row i
@@ -246,7 +265,10 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
             const uint32_t *dn = op + wpr;                           // row i + 1 (left >= 2 here)
             const uint4 D = *reinterpret_cast<const uint4 *>(dn + kw);
             const uint32_t E = op[COLOUR == 0 ? ke0 : ke1];
-            march_row<COLOUR, EDGE>(a, G, wo, tp, U, C, D, E, queue);
+            if (SLAB && top && r == 0)
+                march_row<COLOUR, EDGE>(a, G, wo, tp, U, C, D, E, queue, a.mir_up + kw, (kw << 4) | (1u << 30));
+            else
+                march_row<COLOUR, EDGE>(a, G, wo, tp, U, C, D, E, queue);
             U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
         {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
@@ -254,7 +276,10 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
             const uint32_t *dn = left ? op + wpr : a.opp;
             const uint4 D = *reinterpret_cast<const uint4 *>(dn + kw);
             const uint32_t E = op[COLOUR == 0 ? ke1 : ke0];
-            march_row<COLOUR ^ 1, EDGE>(a, G, wo, tp, U, C, D, E, queue);
+            if (SLAB && bot && r + 2 == a.R)
+                march_row<COLOUR ^ 1, EDGE>(a, G, wo, tp, U, C, D, E, queue, a.mir_dn + kw, (kw << 4) | (2u << 30));
+            else
+                march_row<COLOUR ^ 1, EDGE>(a, G, wo, tp, U, C, D, E, queue);
             U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
     }

@@ -24,7 +24,13 @@
 using namespace lat;
 
 struct lattice {
-    uint32_t L;
+    uint32_t L;                // lattice side (global)
+    uint32_t rows;             // rows allocated per colour/plane: L, or n_own + 2 for a row slab
+    uint32_t n_own;            // rows this handle updates: L, or the slab's n_rows
+    uint32_t row0;             // global index of the first own row (0 for a whole lattice)
+    bool slab;
+    uint32_t *mir_up[2], *mir_dn[2];   // slab: per colour, the neighbours' halo rows
+    bool have_nbr;
     uint32_t wpr;              // words per row per colour (per plane)
     int model;
     double delta;
@@ -124,12 +130,17 @@ uint32_t march_rows(uint32_t L, uint32_t nq)
 
 int launch_ising_march(lattice *lat, int colour)
 {
-    const uint32_t L = lat->L, wpr = lat->wpr, nq = wpr / 4u;
-    const size_t pw = (size_t)L * wpr;
+    const uint32_t wpr = lat->wpr, nq = wpr / 4u;
+    const size_t pw = (size_t)lat->rows * wpr;
     IsingMarchArgs a;
     a.tgt = lat->buf + (size_t)colour * pw;
     a.opp = lat->buf + (size_t)(1 - colour) * pw;
-    a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
+    a.L = lat->rows; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
+    a.row_off = lat->slab ? 1u : 0u;
+    a.g_off = lat->slab ? (lat->row0 - 1u) * nq : 0u;                 // mod 2^32 on purpose
+    a.p_off = lat->slab ? ((long long)lat->row0 - 1) * (long long)wpr : 0;
+    a.mir_up = lat->slab ? lat->mir_up[colour] : nullptr;
+    a.mir_dn = lat->slab ? lat->mir_dn[colour] : nullptr;
     const bool always4 = lat->thr64[0] >= TWO32, always8 = lat->thr64[1] >= TWO32;
     a.thr4 = always4 ? 0xffffffffu : (uint32_t)lat->thr64[0];
     a.thr8 = always8 ? 0xffffffffu : (uint32_t)lat->thr64[1];
@@ -137,19 +148,21 @@ int launch_ising_march(lattice *lat, int colour)
     a.mask8 = always8 ? 0u : 0xffffffffu;
     for (int p = 0; p < 8; ++p)
         a.pcase[p] = ((a.thr4 >> (31 - p)) & 1u) | (((a.thr8 >> (31 - p)) & 1u) << 1);
-    a.R = march_rows(L, nq);
-    a.threads = nq * (L / a.R);
+    a.R = march_rows(lat->n_own, nq);
+    a.threads = nq * (lat->n_own / a.R);
     a.K = lat->K;
     build_plane_fold(lat->K, a.t, a.colour, TAG_ACC_PLANE, a.F);
     const unsigned blocks = (a.threads + 255u) / 256u;
     const bool edge = always4 || always8;
-    if (colour == 0) {
-        if (edge) ising_march_kernel<0, true><<<blocks, 256, 0, lat->stream>>>(a);
-        else ising_march_kernel<0, false><<<blocks, 256, 0, lat->stream>>>(a);
+#define LAT_LAUNCH_MARCH(C, E, S) ising_march_kernel<C, E, S><<<blocks, 256, 0, lat->stream>>>(a)
+    if (lat->slab) {
+        if (colour == 0) { if (edge) LAT_LAUNCH_MARCH(0, true, true); else LAT_LAUNCH_MARCH(0, false, true); }
+        else { if (edge) LAT_LAUNCH_MARCH(1, true, true); else LAT_LAUNCH_MARCH(1, false, true); }
     } else {
-        if (edge) ising_march_kernel<1, true><<<blocks, 256, 0, lat->stream>>>(a);
-        else ising_march_kernel<1, false><<<blocks, 256, 0, lat->stream>>>(a);
+        if (colour == 0) { if (edge) LAT_LAUNCH_MARCH(0, true, false); else LAT_LAUNCH_MARCH(0, false, false); }
+        else { if (edge) LAT_LAUNCH_MARCH(1, true, false); else LAT_LAUNCH_MARCH(1, false, false); }
     }
+#undef LAT_LAUNCH_MARCH
     lat->launches += 1;
     CU(lat, cudaGetLastError());
     return LATTICE_OK;
@@ -212,6 +225,10 @@ int launch_bc_march(lattice *lat, int colour)
 
 int launch_half_sweep(lattice *lat, int colour)
 {
+    if (lat->slab) {
+        if (!lat->have_nbr) return LATTICE_ESTATE;
+        return launch_ising_march(lat, colour);          // create_slab admits only this path
+    }
     if (lat->model == LATTICE_BLUME_CAPEL && lat->scheme == 1 && (lat->wpr % 4u) == 0 &&
         bc_table_is_integer_dE(lat))
         return launch_bc_march(lat, colour);
@@ -339,6 +356,7 @@ int lattice_create(lattice_t **out, uint32_t L, int model, double delta, uint64_
     if (!lat) return LATTICE_ENOMEM;
     std::memset(lat, 0, sizeof *lat);
     lat->L = L; lat->wpr = L / 64u; lat->model = model; lat->delta = delta; lat->seed = seed;
+    lat->rows = L; lat->n_own = L; lat->row0 = 0; lat->slab = false;
     lat->scheme = 1; lat->t = 0;
     lat->buf = (uint32_t *)device_buf;
     lat->stream = (cudaStream_t)cuda_stream;
@@ -364,10 +382,67 @@ int lattice_create(lattice_t **out, uint32_t L, int model, double delta, uint64_
     return LATTICE_OK;
 }
 
+size_t lattice_slab_bytes(uint32_t L, int model, uint32_t n_rows)
+{
+    if (lattice_state_bytes(L, model) == 0 || model != LATTICE_ISING || (L % 256u) != 0) return 0;
+    if (n_rows == 0 || (n_rows % 64u) != 0 || n_rows > L) return 0;
+    return (size_t)2 * (n_rows + 2) * (L / 64u) * sizeof(uint32_t);
+}
+
+int lattice_create_slab(lattice_t **out, uint32_t L, int model, double delta, uint64_t seed,
+                        uint32_t row0, uint32_t n_rows, void *device_buf, size_t device_buf_bytes,
+                        void *cuda_stream)
+{
+    if (!out) return LATTICE_EINVAL;
+    const size_t need = lattice_slab_bytes(L, model, n_rows);
+    if (need == 0 || !std::isfinite(delta) || !device_buf || device_buf_bytes < need ||
+        ((uintptr_t)device_buf & 15u) != 0 || (row0 % 64u) != 0 || (uint64_t)row0 + n_rows > L)
+        return LATTICE_EINVAL;
+    lattice *lat = new (std::nothrow) lattice();
+    if (!lat) return LATTICE_ENOMEM;
+    std::memset(lat, 0, sizeof *lat);
+    lat->L = L; lat->wpr = L / 64u; lat->model = model; lat->delta = delta; lat->seed = seed;
+    lat->rows = n_rows + 2; lat->n_own = n_rows; lat->row0 = row0; lat->slab = true;
+    lat->scheme = 1; lat->t = 0;
+    lat->buf = (uint32_t *)device_buf;
+    lat->stream = (cudaStream_t)cuda_stream;
+    expand_round_keys(seed, lat->K);
+    IsingSlabInitArgs a;
+    a.buf = lat->buf; a.L = L; a.wpr = lat->wpr; a.rows = lat->rows;
+    a.row_base = (row0 + L - 1u) % L; a.K = lat->K;
+    const unsigned long long threads = 2ull * lat->rows * lat->wpr;
+    ising_init_slab_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, lat->stream>>>(a);
+    lat->launches += 1;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        fprintf(stderr, "lattice_create_slab: init kernel launch failed: %s\n", cudaGetErrorString(e));
+        delete lat;
+        return LATTICE_ECUDA;
+    }
+    *out = lat;
+    return LATTICE_OK;
+}
+
+int lattice_slab_set_neighbours(lattice_t *lat, void *device_up_buf, uint32_t up_n_rows,
+                                void *device_down_buf, uint32_t down_n_rows)
+{
+    if (!lat || !lat->slab || !device_up_buf || !device_down_buf || up_n_rows == 0 || down_n_rows == 0)
+        return LATTICE_EINVAL;
+    const size_t wpr = lat->wpr;
+    for (int c = 0; c < 2; ++c) {
+        // upper neighbour: its bottom halo (local row up_n_rows + 1); lower neighbour: its top halo
+        lat->mir_up[c] = (uint32_t *)device_up_buf + (size_t)c * (up_n_rows + 2) * wpr + (size_t)(up_n_rows + 1) * wpr;
+        lat->mir_dn[c] = (uint32_t *)device_down_buf + (size_t)c * (down_n_rows + 2) * wpr;
+    }
+    lat->have_nbr = true;
+    return LATTICE_OK;
+}
+
 int lattice_set_rng_scheme(lattice_t *lat, int scheme)
 {
     if (!lat || (scheme != 0 && scheme != 1)) return LATTICE_EINVAL;
     if (lat->t != 0) return LATTICE_ESTATE;
+    if (lat->slab && scheme != 1) return LATTICE_EINVAL;
     lat->scheme = scheme;
     return LATTICE_OK;
 }
@@ -435,6 +510,10 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
     const uint64_t L = lat->L;
     if (r_max < 1 || r_max > L / 2 || i0 >= L || n_rows < 1 || n_rows > L || i0 + n_rows > L)
         return LATTICE_EINVAL;
+    // a row slab measures its own rows only, and only r = 1 (row i+1 of the last own row is the
+    // lower halo); larger r along y would need r_max halo rows
+    if (lat->slab && (r_max != 1 || i0 < lat->row0 || i0 + n_rows > (uint64_t)lat->row0 + lat->n_own))
+        return LATTICE_EINVAL;
     const size_t entries = 2 + 4 * (size_t)r_max;
     int rc = ensure_cnt(lat, entries);
     if (rc) return rc;
@@ -445,7 +524,9 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
     if (r_max == 1 && (lat->wpr % 4u) == 0) {
         // the per-step record (e, m, q): one pass over the slab
         MeasE1Args e1;
-        e1.buf = lat->buf; e1.L = lat->L; e1.wpr = lat->wpr; e1.i0 = (uint32_t)i0;
+        e1.buf = lat->buf; e1.rows = lat->rows; e1.wpr = lat->wpr;
+        e1.i0 = lat->slab ? (uint32_t)(i0 - lat->row0) + 1u : (uint32_t)i0;      // local row index
+        e1.par_off = lat->slab ? ((lat->row0 + 1u) & 1u) : 0u;
         e1.n_rows = (uint32_t)n_rows; e1.cnt = lat->d_cnt;
         const unsigned long long threads =
             (unsigned long long)(lat->wpr / 4u) * ((n_rows + MEAS_E1_ROWS - 1) / MEAS_E1_ROWS);
@@ -520,7 +601,7 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
 int lattice_measure(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy)
 {
     if (!lat) return LATTICE_EINVAL;
-    return lattice_measure_rows(lat, 0, lat->L, r_max, M, Q, Sx, Sy);
+    return lattice_measure_rows(lat, lat->row0, lat->n_own, r_max, M, Q, Sx, Sy);
 }
 
 static int window_call(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint32_t w, int8_t *host,
@@ -529,6 +610,12 @@ static int window_call(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uin
     if (!lat || !host) return LATTICE_EINVAL;
     const uint64_t L = lat->L;
     if (h < 1 || w < 1 || h > L || w > L || i0 >= L || j0 >= L) return LATTICE_EINVAL;
+    const uint32_t row_base = lat->slab ? (lat->row0 + lat->L - 1u) % lat->L : 0u;
+    if (lat->slab) {
+        // rows of the window must lie inside the slab's allocation (own rows and the two halos)
+        const uint64_t li = (i0 + L - row_base) % L;
+        if (li + h > lat->rows) return LATTICE_EINVAL;
+    }
     const size_t bytes = (size_t)h * w;
     if (set) {
         for (size_t k = 0; k < bytes; ++k) {
@@ -540,6 +627,7 @@ static int window_call(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uin
     if (rc) return rc;
     WindowArgs a;
     a.buf = lat->buf; a.L = lat->L; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
+    a.rows = lat->rows; a.row_base = row_base;
     a.i0 = (uint32_t)i0; a.j0 = (uint32_t)j0; a.h = h; a.w = w; a.spins = lat->d_win;
     const unsigned long long blocks = (bytes + 255) / 256;
     if (blocks > 0x7fffffffull) return LATTICE_EINVAL;

@@ -417,8 +417,9 @@ constexpr int MEAS_E1_ROWS = 32;
 
 struct MeasE1Args {
     const uint32_t *buf;
-    uint32_t L, wpr;
-    uint32_t i0, n_rows;
+    uint32_t rows, wpr;              // rows allocated per plane (L, or n_rows + 2 for a row slab)
+    uint32_t i0, n_rows;             // local index of the first base row, number of base rows
+    uint32_t par_off;                // parity of the global row of local row 0 (0 for a whole lattice)
     unsigned long long *cnt;         // [6]: MeasArgs::cnt layout with r_max = 1
 };
 
@@ -431,7 +432,7 @@ struct E1Row {                       // one 128-bit run of both colours (+ plane
 template <int MODEL>
 __device__ __forceinline__ void e1_load(const MeasE1Args &a, unsigned long long off, E1Row<MODEL> &r)
 {
-    const size_t pw = (size_t)a.L * a.wpr;
+    const size_t pw = (size_t)a.rows * a.wpr;
     const uint4 x = *reinterpret_cast<const uint4 *>(a.buf + off);
     r.a0[0] = x.x; r.a0[1] = x.y; r.a0[2] = x.z; r.a0[3] = x.w;
     if (MODEL == 0) {
@@ -462,7 +463,7 @@ __global__ void __launch_bounds__(128) measure_e1_kernel(const MeasE1Args a)
         const uint32_t kn = (kw + 4 == a.wpr) ? 0 : kw + 4;       // word after the run (periodic)
         const uint32_t ia = a.i0 + sl * MEAS_E1_ROWS;
         const uint32_t nr = min((uint32_t)MEAS_E1_ROWS, a.i0 + a.n_rows - ia);
-        const size_t pw = (size_t)a.L * a.wpr;
+        const size_t pw = (size_t)a.rows * a.wpr;
         unsigned long long ro = (unsigned long long)ia * a.wpr;
         E1Row<MODEL> cur, nxt;
         e1_load<MODEL>(a, ro + kw, cur);
@@ -472,11 +473,11 @@ __global__ void __launch_bounds__(128) measure_e1_kernel(const MeasE1Args a)
             for (int h = 0; h < 2; ++h) {
                 if (rr + h < nr) {
                     const uint32_t i = ia + rr + h;
-                    const unsigned long long rd = (i + 1 == a.L) ? 0ull : ro + a.wpr;
+                    const unsigned long long rd = (i + 1 == a.rows) ? 0ull : ro + a.wpr;
                     e1_load<MODEL>(a, rd + kw, nxt);
                     // x axis: colour (i&1) pairs in place; the other colour sees its partner
                     // colour shifted down by one bit (partner at p+1)
-                    const uint32_t odd = i & 1u;
+                    const uint32_t odd = (i + a.par_off) & 1u;      // parity of the global row
                     // colour whose partner is shifted: c with (i+c)&1 == 1, i.e. c = 1 - odd;
                     // its partner colour is `odd`: side word of colour `odd` (planes 0, 1)
                     const uint32_t *sp = a.buf + (MODEL == 0 ? (size_t)odd * pw : (size_t)(2 * odd) * pw) + ro + kn;
@@ -547,6 +548,8 @@ __global__ void __launch_bounds__(128) measure_e1_kernel(const MeasE1Args a)
 struct WindowArgs {
     uint32_t *buf;
     uint32_t L, wpr, model;
+    uint32_t rows, row_base;         // rows allocated per plane and the global row of local row 0
+                                     // (L and 0 for a whole lattice; n_rows + 2 and row0 - 1 for a slab)
     uint32_t i0, j0, h, w;
     int8_t *spins;                   // device, row-major h x w
 };
@@ -556,7 +559,8 @@ __device__ __forceinline__ void site_addr(const WindowArgs &a, uint32_t i, uint3
 {
     colour = (i + j) & 1u;
     const uint32_t p = j >> 1;
-    word = (size_t)i * a.wpr + (p >> 5);
+    const uint32_t li = i >= a.row_base ? i - a.row_base : i + a.L - a.row_base;   // local row
+    word = (size_t)li * a.wpr + (p >> 5);
     bit = p & 31u;
 }
 
@@ -567,7 +571,7 @@ __global__ void __launch_bounds__(256) get_spins_kernel(const WindowArgs a)
     const uint32_t i = (uint32_t)((a.i0 + g / a.w) % a.L), j = (uint32_t)((a.j0 + g % a.w) % a.L);
     size_t word; uint32_t bit, colour;
     site_addr(a, i, j, word, bit, colour);
-    const size_t pw = (size_t)a.L * a.wpr;
+    const size_t pw = (size_t)a.rows * a.wpr;
     if (a.model == 0) {
         a.spins[g] = ((a.buf[(size_t)colour * pw + word] >> bit) & 1u) ? 1 : -1;
     } else {
@@ -584,7 +588,7 @@ __global__ void __launch_bounds__(256) set_spins_kernel(const WindowArgs a)
     const uint32_t i = (uint32_t)((a.i0 + g / a.w) % a.L), j = (uint32_t)((a.j0 + g % a.w) % a.L);
     size_t word; uint32_t bit, colour;
     site_addr(a, i, j, word, bit, colour);
-    const size_t pw = (size_t)a.L * a.wpr;
+    const size_t pw = (size_t)a.rows * a.wpr;
     const int s = a.spins[g];
     const uint32_t m = 1u << bit;
     if (a.model == 0) {

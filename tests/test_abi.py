@@ -122,3 +122,25 @@ def test_product_never_imports_the_oracle():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 assert not pat.search(open(os.path.join(dirpath, f)).read()), f
+
+
+def test_slab_bytes_and_create_slab_argument_checks():
+    """Row-slab mode (include/lattice.h): sizes and the checks made before touching a device."""
+    import ctypes as C
+    L = lat.lib()
+    wpr = 1024 // 64
+    assert L.lattice_slab_bytes(1024, lat.ISING, 256) == 2 * (256 + 2) * wpr * 4
+    assert L.lattice_slab_bytes(1024, lat.ISING, 1024) == 2 * (1024 + 2) * wpr * 4
+    for bad in [(1000, lat.ISING, 64), (64, lat.ISING, 64), (1024, lat.ISING, 100), (1024, lat.ISING, 0),
+                (1024, lat.ISING, 2048), (1024, lat.BLUME_CAPEL, 256), (1024, 7, 256)]:
+        assert L.lattice_slab_bytes(*bad) == 0, bad
+    h = C.c_void_p()
+    fake = C.c_void_p(0x10000)
+    n = L.lattice_slab_bytes(1024, lat.ISING, 256)
+    for args in [(1024, lat.ISING, 0.0, 1, 32, 256, fake, n, None),        # row0 not a multiple of 64
+                 (1024, lat.ISING, 0.0, 1, 896, 256, fake, n, None),       # runs past the last row
+                 (1024, lat.ISING, 0.0, 1, 0, 256, fake, n - 1, None),     # buffer too small
+                 (1024, lat.ISING, 0.0, 1, 0, 256, None, n, None),         # no buffer
+                 (1024, lat.ISING, float("nan"), 1, 0, 256, fake, n, None)]:
+        assert L.lattice_create_slab(C.byref(h), *args) == lat.binding.EINVAL, args
+    assert L.lattice_slab_set_neighbours(None, fake, 64, fake, 64) == lat.binding.EINVAL

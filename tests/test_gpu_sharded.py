@@ -1,0 +1,75 @@
+"""Row-slab domain decomposition (include/lattice.h): N slabs with fused halo mirroring evolve
+bit for bit like the whole lattice and like the oracle.  All slabs sit on one GPU here (the
+mirror pointers are then ordinary device memory; across GPUs they are NVLink peer pointers)."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2503_14688_b200 as lat
+from paper_2503_14688_b200 import workloads
+from paper_2503_14688_b200.sharded import ShardedLattice
+
+pytestmark = pytest.mark.gpu
+BETA_C = workloads.BETA_C_ISING
+
+
+@pytest.mark.parametrize("L,n_slabs", [(256, 1), (256, 2), (256, 4), (1024, 2), (1024, 16), (2048, 8)])
+def test_sharded_equals_unsharded_and_oracle(L, n_slabs):
+    seed = 777 + L + n_slabs
+    sh = ShardedLattice(L, n_slabs, seed)
+    g = lat.Lattice(L, lat.ISING, 0.0, seed)
+    assert np.array_equal(sh.get_spins(), g.get_spins())            # the disordered start
+    beta = [BETA_C] * 6 + [0.0, 0.3, 5.0, np.inf] + [BETA_C / 1.01] * 6
+    sh.sweep(beta)
+    g.sweep(beta)
+    assert sh.time == g.time == len(beta)
+    assert np.array_equal(sh.get_spins(), g.get_spins())
+    M, Q, Sx, Sy = g.measure(1)
+    assert sh.measure() == (M, Q, int(Sx[0]), int(Sy[0]))
+    if L <= 1024:
+        o = oracle.OracleLattice(L, oracle.ISING, 0.0, seed)
+        o.sweep(beta)
+        assert np.array_equal(sh.get_spins(), o.get_spins())
+    # halos are the neighbours' boundary rows (the mirror stores and the late tie flips landed)
+    rows = L // n_slabs
+    for k, s in enumerate(sh.slabs):
+        own = s.get_spins()
+        up_last = sh.slabs[(k - 1) % n_slabs].get_spins()[-1]
+        dn_first = sh.slabs[(k + 1) % n_slabs].get_spins()[0]
+        assert np.array_equal(s.get_spins((k * rows - 1) % L, 0, 1, L)[0], up_last)
+        assert np.array_equal(s.get_spins((k * rows + rows) % L, 0, 1, L)[0], dn_first)
+        assert own.shape == (rows, L)
+    sh.close(); g.close()
+
+
+def test_sharded_many_sweeps_many_ties_across_boundaries():
+    """Long enough that hundreds of tied lanes fall on mirrored boundary rows."""
+    L, n_slabs, seed = 512, 8, 31337
+    sh = ShardedLattice(L, n_slabs, seed)
+    g = lat.Lattice(L, lat.ISING, 0.0, seed)
+    for _ in range(5):
+        sh.sweep([BETA_C] * 40)
+        g.sweep([BETA_C] * 40)
+        assert np.array_equal(sh.get_spins(), g.get_spins())
+    sh.close(); g.close()
+
+
+def test_slab_api_errors():
+    L = 256
+    with pytest.raises(lat.LatticeError):
+        lat.Lattice(L, lat.ISING, 0.0, 1, slab=(0, 100))             # n_rows not a multiple of 64
+    with pytest.raises(lat.LatticeError):
+        lat.Lattice(L, lat.ISING, 0.0, 1, slab=(32, 64))             # row0 not a multiple of 64
+    with pytest.raises(lat.LatticeError):
+        lat.Lattice(L, lat.BLUME_CAPEL, 0.0, 1, slab=(0, 64))        # Ising only in round 1
+    s = lat.Lattice(L, lat.ISING, 0.0, 1, slab=(64, 128))
+    with pytest.raises(lat.LatticeError) as e:
+        s.half_sweep(0, 0.4)                                         # neighbours not set
+    assert e.value.status == lat.binding.ESTATE
+    with pytest.raises(lat.LatticeError):
+        s.measure(2)                                                 # only r_max = 1 on a slab
+    with pytest.raises(lat.LatticeError):
+        s.get_spins(0, 0, 8, L)                                      # rows outside the slab
+    assert s.get_spins().shape == (128, L)
+    assert s.get_spins(63, 0, 130, L).shape == (130, L)              # own rows and both halos
+    s.close()
