@@ -296,4 +296,37 @@ __global__ void __launch_bounds__(256) bc_init_kernel(const BCInitArgs a)
     a.buf[(size_t)(2 * colour + 1) * words + wi] = sg;
 }
 
+// Row-slab variant of the disordered start (see ising_init_slab_kernel): local rows 0 .. rows-1,
+// local row l = global row (row_base + l) mod L, keyed by global coordinates.
+struct BCSlabInitArgs {
+    uint32_t *buf;            // [2 colours][2 planes][rows][wpr]
+    uint32_t L, wpr, rows, row_base;
+    RoundKeys K;
+};
+
+__global__ void __launch_bounds__(256) bc_init_slab_kernel(const BCSlabInitArgs a)
+{
+    const unsigned long long words = (unsigned long long)a.rows * a.wpr;   // per colour per plane
+    const unsigned long long g = (unsigned long long)blockIdx.x * 256u + threadIdx.x;
+    if (g >= 2 * words) return;
+    const uint32_t colour = g >= words;
+    const unsigned long long wi = g - (colour ? words : 0);
+    const uint32_t li = (uint32_t)(wi / a.wpr), k = (uint32_t)(wi % a.wpr);
+    const uint32_t gi = (a.row_base + li) % a.L;
+    const unsigned long long P0 = ((unsigned long long)gi * a.wpr + k) << 5;
+    uint32_t nz = 0, sg = 0;
+#pragma unroll 1
+    for (int q = 0; q < 8; ++q) {
+        const uint4 blk = philox_unit((P0 >> 2) + q, 0, colour, TAG_INIT_QUAD, 0, a.K);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t code = __umulhi(pick(blk, j), 3u);
+            nz |= (uint32_t)(code != 1u) << (4 * q + j);
+            sg |= (uint32_t)(code == 0u) << (4 * q + j);
+        }
+    }
+    a.buf[(size_t)(2 * colour) * words + wi] = nz;
+    a.buf[(size_t)(2 * colour + 1) * words + wi] = sg;
+}
+
 }  // namespace lat

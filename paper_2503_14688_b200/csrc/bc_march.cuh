@@ -31,7 +31,11 @@ namespace lat {
 struct BCMarchArgs {
     uint32_t *tnz, *tsg;            // colour being updated
     const uint32_t *onz, *osg;      // opposite colour
-    uint32_t L, wpr, t, colour;
+    uint32_t L, wpr, t, colour;     // L = rows allocated per plane (lattice side, or n_rows + 2 for a slab)
+    // row-slab mode (same meaning as in IsingMarchArgs; zero / null for a whole lattice)
+    uint32_t row_off, g_off;
+    long long p_off;
+    uint32_t *mir_up_nz, *mir_up_sg, *mir_dn_nz, *mir_dn_sg;
     uint32_t R;                     // rows per thread (even, divides L)
     uint32_t threads;               // (wpr/4) * (L/R), a multiple of 32
     uint32_t lut[8];                // truth table of threshold bit (31-k) over (F, Y1, H0)
@@ -88,26 +92,34 @@ struct BCTieQueue {
     uint4 *q;                   // [2 * TIE_Q_SLOTS] this warp's slice
     uint32_t lane, pending;
 
+    // e1.w = word offset bits 32..35 | column word << 4 | mirror flag << 30 (1 = up, 2 = down)
     __device__ __forceinline__ void resolve(uint32_t idx)
     {
         const uint4 e0 = q[2 * idx], e1 = q[2 * idx + 1];
-        const unsigned long long wo = ((unsigned long long)e1.w << 32) | e1.z;
+        const unsigned long long wo = ((unsigned long long)(e1.w & 0xFu) << 32) | e1.z;
         uint32_t ties = e0.x, hit = 0;
         while (ties) {
             const uint32_t bit = __ffs(ties) - 1;
             ties &= ties - 1;
             const uint32_t cls = (((e0.y >> bit) & 1u) << 2) | (((e0.z >> bit) & 1u) << 1) | ((e0.w >> bit) & 1u);
-            const unsigned long long P = (wo << 5) + bit;
+            const unsigned long long P = ((wo + a.p_off) << 5) + bit;
             const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
                                             a.colour | (TAG_ACC_TAIL << 8), a.K);
             if ((blk.x >> 8) < (a.thr[cls] & 0x00ffffffu)) hit |= 1u << bit;
         }
-        if (hit & e1.x) atomicXor(a.tnz + wo, hit & e1.x);
-        if (hit & e1.y) atomicXor(a.tsg + wo, hit & e1.y);
+        const uint32_t dnz = hit & e1.x, dsg = hit & e1.y;
+        if (dnz) atomicXor(a.tnz + wo, dnz);
+        if (dsg) atomicXor(a.tsg + wo, dsg);
+        const uint32_t mf = e1.w >> 30;
+        if (mf && (dnz | dsg)) {
+            const uint32_t col = (e1.w >> 4) & 0x3ffffu;
+            if (dnz) atomicXor((mf == 1 ? a.mir_up_nz : a.mir_dn_nz) + col, dnz);
+            if (dsg) atomicXor((mf == 1 ? a.mir_up_sg : a.mir_dn_sg) + col, dsg);
+        }
     }
     __device__ __forceinline__ void push(const uint32_t (&eq)[4], const uint32_t (&Fm)[4], const uint32_t (&Y1)[4],
                                          const uint32_t (&H0)[4], const uint32_t (&nf)[4],
-                                         const uint32_t (&gg)[4], unsigned long long wo)
+                                         const uint32_t (&gg)[4], unsigned long long wo, uint32_t mir_tag)
     {
         const uint32_t below = (1u << lane) - 1u;
 #pragma unroll
@@ -118,7 +130,8 @@ struct BCTieQueue {
                 const unsigned long long o = wo + (unsigned)w;
                 const uint32_t slot = pending + __popc(m & below);
                 q[2 * slot] = make_uint4(eq[w], Fm[w], Y1[w], H0[w]);
-                q[2 * slot + 1] = make_uint4(nf[w], gg[w], (uint32_t)o, (uint32_t)(o >> 32));
+                q[2 * slot + 1] = make_uint4(nf[w], gg[w], (uint32_t)o,
+                                             (uint32_t)(o >> 32) | (mir_tag + ((unsigned)w << 4)));
             }
             pending += __popc(m);
         }
@@ -156,7 +169,9 @@ template <int PAR>
 __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, unsigned long long wo,
                                              uint32_t *tn, uint32_t *ts,
                                              const BCRow &U, const BCRow &C, const BCRow &D,
-                                             uint32_t En, uint32_t Es, BCTieQueue &queue)
+                                             uint32_t En, uint32_t Es, BCTieQueue &queue,
+                                             uint32_t *mir_nz = nullptr, uint32_t *mir_sg = nullptr,
+                                             uint32_t mir_tag = 0)
 {
     BCRow T;
     bcm_load(tn, ts, 0, T);                                       // tn == a.tnz + wo, ts == a.tsg + wo
@@ -228,10 +243,14 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
     }
     *reinterpret_cast<uint4 *>(tn) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
     *reinterpret_cast<uint4 *>(ts) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
-    queue.push(eq, Fm, Y1, H0, nf, gg, wo);
+    if (mir_nz) {       // slab mode: this row is also a neighbour's halo row
+        *reinterpret_cast<uint4 *>(mir_nz) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
+        *reinterpret_cast<uint4 *>(mir_sg) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
+    }
+    queue.push(eq, Fm, Y1, H0, nf, gg, wo, mir_tag);
 }
 
-template <int COLOUR>
+template <int COLOUR, bool SLAB>
 __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
 {
     __shared__ uint4 s_q[8][2 * TIE_Q_SLOTS];
@@ -243,7 +262,7 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
     const uint32_t q = g % nq, s = g / nq;
     const uint32_t kw = q << 2;
-    const uint32_t i0 = s * a.R;
+    const uint32_t i0 = s * a.R + (SLAB ? a.row_off : 0u);
     const uint32_t iu = (i0 == 0) ? L - 1 : i0 - 1;
     const uint32_t ke0 = (kw == 0) ? wpr - 1 : kw - 1;       // word before the run (periodic)
     const uint32_t ke1 = (kw + 4 == wpr) ? 0 : kw + 4;       // word after it
@@ -251,7 +270,8 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
     BCRow U, C, D;
     bcm_load(a.onz, a.osg, (unsigned long long)iu * wpr + kw, U);
     bcm_load(a.onz, a.osg, ro + kw, C);
-    uint32_t G = i0 * nq + q;
+    uint32_t G = i0 * nq + q + (SLAB ? a.g_off : 0u);
+    const bool top = SLAB && s == 0, bot = SLAB && (s + 1) * nq == a.threads;
     // running pointers: the slab's own rows never wrap; only row i+1 of the last lattice row does
     // (the sg plane sits one plane stride pw = L * wpr words after the nz plane)
     const unsigned long long pw = (unsigned long long)L * wpr;
@@ -264,7 +284,11 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
             const uint32_t *dn = on + wpr;
             bcm_load(dn, dn + pw, kw, D);
             const uint32_t ke = COLOUR == 0 ? ke0 : ke1;
-            bc_march_row<COLOUR>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+            if (SLAB && top && r == 0)
+                bc_march_row<COLOUR>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
+                                     a.mir_up_nz + kw, a.mir_up_sg + kw, (kw << 4) | (1u << 30));
+            else
+                bc_march_row<COLOUR>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
             U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
         {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
@@ -272,7 +296,11 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
             const uint32_t *dn = left ? on + wpr : a.onz;
             bcm_load(dn, dn + pw, kw, D);
             const uint32_t ke = COLOUR == 0 ? ke1 : ke0;
-            bc_march_row<COLOUR ^ 1>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+            if (SLAB && bot && r + 2 == a.R)
+                bc_march_row<COLOUR ^ 1>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
+                                         a.mir_dn_nz + kw, a.mir_dn_sg + kw, (kw << 4) | (2u << 30));
+            else
+                bc_march_row<COLOUR ^ 1>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
             U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
     }

@@ -29,7 +29,7 @@ struct lattice {
     uint32_t n_own;            // rows this handle updates: L, or the slab's n_rows
     uint32_t row0;             // global index of the first own row (0 for a whole lattice)
     bool slab;
-    uint32_t *mir_up[2], *mir_dn[2];   // slab: per colour, the neighbours' halo rows
+    uint32_t *mir_up[2][2], *mir_dn[2][2];   // slab: per colour and plane, the neighbours' halo rows
     bool have_nbr;
     uint32_t wpr;              // words per row per colour (per plane)
     int model;
@@ -139,8 +139,8 @@ int launch_ising_march(lattice *lat, int colour)
     a.row_off = lat->slab ? 1u : 0u;
     a.g_off = lat->slab ? (lat->row0 - 1u) * nq : 0u;                 // mod 2^32 on purpose
     a.p_off = lat->slab ? ((long long)lat->row0 - 1) * (long long)wpr : 0;
-    a.mir_up = lat->slab ? lat->mir_up[colour] : nullptr;
-    a.mir_dn = lat->slab ? lat->mir_dn[colour] : nullptr;
+    a.mir_up = lat->slab ? lat->mir_up[colour][0] : nullptr;
+    a.mir_dn = lat->slab ? lat->mir_dn[colour][0] : nullptr;
     const bool always4 = lat->thr64[0] >= TWO32, always8 = lat->thr64[1] >= TWO32;
     a.thr4 = always4 ? 0xffffffffu : (uint32_t)lat->thr64[0];
     a.thr8 = always8 ? 0xffffffffu : (uint32_t)lat->thr64[1];
@@ -191,16 +191,23 @@ bool bc_table_is_integer_dE(const lattice *lat)
 
 int launch_bc_march(lattice *lat, int colour)
 {
-    const uint32_t L = lat->L, wpr = lat->wpr, nq = wpr / 4u;
-    const size_t pw = (size_t)L * wpr;
+    const uint32_t wpr = lat->wpr, nq = wpr / 4u;
+    const size_t pw = (size_t)lat->rows * wpr;
     BCMarchArgs a;
     a.tnz = lat->buf + (size_t)(2 * colour) * pw;
     a.tsg = lat->buf + (size_t)(2 * colour + 1) * pw;
     a.onz = lat->buf + (size_t)(2 * (1 - colour)) * pw;
     a.osg = lat->buf + (size_t)(2 * (1 - colour) + 1) * pw;
-    a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
-    a.R = march_rows(L, nq);
-    a.threads = nq * (L / a.R);
+    a.L = lat->rows; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
+    a.row_off = lat->slab ? 1u : 0u;
+    a.g_off = lat->slab ? (lat->row0 - 1u) * nq : 0u;
+    a.p_off = lat->slab ? ((long long)lat->row0 - 1) * (long long)wpr : 0;
+    a.mir_up_nz = lat->slab ? lat->mir_up[colour][0] : nullptr;
+    a.mir_up_sg = lat->slab ? lat->mir_up[colour][1] : nullptr;
+    a.mir_dn_nz = lat->slab ? lat->mir_dn[colour][0] : nullptr;
+    a.mir_dn_sg = lat->slab ? lat->mir_dn[colour][1] : nullptr;
+    a.R = march_rows(lat->n_own, nq);
+    a.threads = nq * (lat->n_own / a.R);
     for (int k = 0; k < 8; ++k) a.lut[k] = 0;
     a.lut_always = 0;
     for (int F = 0; F < 2; ++F)
@@ -216,8 +223,13 @@ int launch_bc_march(lattice *lat, int colour)
     build_plane_fold(lat->K, a.t, a.colour, TAG_ACC_PLANE, a.F);
     a.fbp = (a.colour | (TAG_PROP_PLANE << 8)) ^ lat->K.k1[0];
     const unsigned blocks = (a.threads + 255u) / 256u;
-    if (colour == 0) bc_march_kernel<0><<<blocks, 256, 0, lat->stream>>>(a);
-    else bc_march_kernel<1><<<blocks, 256, 0, lat->stream>>>(a);
+    if (lat->slab) {
+        if (colour == 0) bc_march_kernel<0, true><<<blocks, 256, 0, lat->stream>>>(a);
+        else bc_march_kernel<1, true><<<blocks, 256, 0, lat->stream>>>(a);
+    } else {
+        if (colour == 0) bc_march_kernel<0, false><<<blocks, 256, 0, lat->stream>>>(a);
+        else bc_march_kernel<1, false><<<blocks, 256, 0, lat->stream>>>(a);
+    }
     lat->launches += 1;
     CU(lat, cudaGetLastError());
     return LATTICE_OK;
@@ -227,7 +239,11 @@ int launch_half_sweep(lattice *lat, int colour)
 {
     if (lat->slab) {
         if (!lat->have_nbr) return LATTICE_ESTATE;
-        return launch_ising_march(lat, colour);          // create_slab admits only this path
+        if (lat->model == LATTICE_ISING) return launch_ising_march(lat, colour);
+        // Blume-Capel slabs run only the marching kernel: tables without the Delta = 0 structure
+        // (bc_march.cuh) are not supported in slab mode
+        if (!bc_table_is_integer_dE(lat)) return LATTICE_EINVAL;
+        return launch_bc_march(lat, colour);
     }
     if (lat->model == LATTICE_BLUME_CAPEL && lat->scheme == 1 && (lat->wpr % 4u) == 0 &&
         bc_table_is_integer_dE(lat))
@@ -384,9 +400,10 @@ int lattice_create(lattice_t **out, uint32_t L, int model, double delta, uint64_
 
 size_t lattice_slab_bytes(uint32_t L, int model, uint32_t n_rows)
 {
-    if (lattice_state_bytes(L, model) == 0 || model != LATTICE_ISING || (L % 256u) != 0) return 0;
+    if (lattice_state_bytes(L, model) == 0 || (L % 256u) != 0) return 0;
     if (n_rows == 0 || (n_rows % 64u) != 0 || n_rows > L) return 0;
-    return (size_t)2 * (n_rows + 2) * (L / 64u) * sizeof(uint32_t);
+    const size_t planes = model == LATTICE_ISING ? 2 : 4;
+    return planes * (n_rows + 2) * (L / 64u) * sizeof(uint32_t);
 }
 
 int lattice_create_slab(lattice_t **out, uint32_t L, int model, double delta, uint64_t seed,
@@ -407,11 +424,19 @@ int lattice_create_slab(lattice_t **out, uint32_t L, int model, double delta, ui
     lat->buf = (uint32_t *)device_buf;
     lat->stream = (cudaStream_t)cuda_stream;
     expand_round_keys(seed, lat->K);
-    IsingSlabInitArgs a;
-    a.buf = lat->buf; a.L = L; a.wpr = lat->wpr; a.rows = lat->rows;
-    a.row_base = (row0 + L - 1u) % L; a.K = lat->K;
     const unsigned long long threads = 2ull * lat->rows * lat->wpr;
-    ising_init_slab_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, lat->stream>>>(a);
+    const unsigned blocks = (unsigned)((threads + 255) / 256);
+    if (model == LATTICE_ISING) {
+        IsingSlabInitArgs a;
+        a.buf = lat->buf; a.L = L; a.wpr = lat->wpr; a.rows = lat->rows;
+        a.row_base = (row0 + L - 1u) % L; a.K = lat->K;
+        ising_init_slab_kernel<<<blocks, 256, 0, lat->stream>>>(a);
+    } else {
+        BCSlabInitArgs a;
+        a.buf = lat->buf; a.L = L; a.wpr = lat->wpr; a.rows = lat->rows;
+        a.row_base = (row0 + L - 1u) % L; a.K = lat->K;
+        bc_init_slab_kernel<<<blocks, 256, 0, lat->stream>>>(a);
+    }
     lat->launches += 1;
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
@@ -429,11 +454,14 @@ int lattice_slab_set_neighbours(lattice_t *lat, void *device_up_buf, uint32_t up
     if (!lat || !lat->slab || !device_up_buf || !device_down_buf || up_n_rows == 0 || down_n_rows == 0)
         return LATTICE_EINVAL;
     const size_t wpr = lat->wpr;
-    for (int c = 0; c < 2; ++c) {
-        // upper neighbour: its bottom halo (local row up_n_rows + 1); lower neighbour: its top halo
-        lat->mir_up[c] = (uint32_t *)device_up_buf + (size_t)c * (up_n_rows + 2) * wpr + (size_t)(up_n_rows + 1) * wpr;
-        lat->mir_dn[c] = (uint32_t *)device_down_buf + (size_t)c * (down_n_rows + 2) * wpr;
-    }
+    const int planes = lat->model == LATTICE_ISING ? 1 : 2;
+    for (int c = 0; c < 2; ++c)
+        for (int p = 0; p < planes; ++p) {
+            // upper neighbour: its bottom halo (local row up_n_rows + 1); lower neighbour: its top halo
+            lat->mir_up[c][p] = (uint32_t *)device_up_buf + (size_t)(planes * c + p) * (up_n_rows + 2) * wpr +
+                                (size_t)(up_n_rows + 1) * wpr;
+            lat->mir_dn[c][p] = (uint32_t *)device_down_buf + (size_t)(planes * c + p) * (down_n_rows + 2) * wpr;
+        }
     lat->have_nbr = true;
     return LATTICE_OK;
 }

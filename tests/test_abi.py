@@ -131,8 +131,9 @@ def test_slab_bytes_and_create_slab_argument_checks():
     wpr = 1024 // 64
     assert L.lattice_slab_bytes(1024, lat.ISING, 256) == 2 * (256 + 2) * wpr * 4
     assert L.lattice_slab_bytes(1024, lat.ISING, 1024) == 2 * (1024 + 2) * wpr * 4
+    assert L.lattice_slab_bytes(1024, lat.BLUME_CAPEL, 256) == 4 * (256 + 2) * wpr * 4
     for bad in [(1000, lat.ISING, 64), (64, lat.ISING, 64), (1024, lat.ISING, 100), (1024, lat.ISING, 0),
-                (1024, lat.ISING, 2048), (1024, lat.BLUME_CAPEL, 256), (1024, 7, 256)]:
+                (1024, lat.ISING, 2048), (1024, 7, 256)]:
         assert L.lattice_slab_bytes(*bad) == 0, bad
     h = C.c_void_p()
     fake = C.c_void_p(0x10000)

@@ -13,13 +13,15 @@ pytestmark = pytest.mark.gpu
 BETA_C = workloads.BETA_C_ISING
 
 
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
 @pytest.mark.parametrize("L,n_slabs", [(256, 1), (256, 2), (256, 4), (1024, 2), (1024, 16), (2048, 8)])
-def test_sharded_equals_unsharded_and_oracle(L, n_slabs):
+def test_sharded_equals_unsharded_and_oracle(L, n_slabs, model):
     seed = 777 + L + n_slabs
-    sh = ShardedLattice(L, n_slabs, seed)
-    g = lat.Lattice(L, lat.ISING, 0.0, seed)
+    sh = ShardedLattice(L, n_slabs, seed, model=model)
+    g = lat.Lattice(L, model, 0.0, seed)
     assert np.array_equal(sh.get_spins(), g.get_spins())            # the disordered start
-    beta = [BETA_C] * 6 + [0.0, 0.3, 5.0, np.inf] + [BETA_C / 1.01] * 6
+    bc = BETA_C if model == lat.ISING else workloads.BETA_BC
+    beta = [bc] * 6 + [0.0, 0.3, 5.0, np.inf] + [bc / 1.01] * 6
     sh.sweep(beta)
     g.sweep(beta)
     assert sh.time == g.time == len(beta)
@@ -27,7 +29,7 @@ def test_sharded_equals_unsharded_and_oracle(L, n_slabs):
     M, Q, Sx, Sy = g.measure(1)
     assert sh.measure() == (M, Q, int(Sx[0]), int(Sy[0]))
     if L <= 1024:
-        o = oracle.OracleLattice(L, oracle.ISING, 0.0, seed)
+        o = oracle.OracleLattice(L, model, 0.0, seed)
         o.sweep(beta)
         assert np.array_equal(sh.get_spins(), o.get_spins())
     # halos are the neighbours' boundary rows (the mirror stores and the late tie flips landed)
@@ -42,14 +44,16 @@ def test_sharded_equals_unsharded_and_oracle(L, n_slabs):
     sh.close(); g.close()
 
 
-def test_sharded_many_sweeps_many_ties_across_boundaries():
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+def test_sharded_many_sweeps_many_ties_across_boundaries(model):
     """Long enough that hundreds of tied lanes fall on mirrored boundary rows."""
     L, n_slabs, seed = 512, 8, 31337
-    sh = ShardedLattice(L, n_slabs, seed)
-    g = lat.Lattice(L, lat.ISING, 0.0, seed)
+    sh = ShardedLattice(L, n_slabs, seed, model=model)
+    g = lat.Lattice(L, model, 0.0, seed)
+    bc = BETA_C if model == lat.ISING else workloads.BETA_BC
     for _ in range(5):
-        sh.sweep([BETA_C] * 40)
-        g.sweep([BETA_C] * 40)
+        sh.sweep([bc] * 40)
+        g.sweep([bc] * 40)
         assert np.array_equal(sh.get_spins(), g.get_spins())
     sh.close(); g.close()
 
@@ -60,8 +64,11 @@ def test_slab_api_errors():
         lat.Lattice(L, lat.ISING, 0.0, 1, slab=(0, 100))             # n_rows not a multiple of 64
     with pytest.raises(lat.LatticeError):
         lat.Lattice(L, lat.ISING, 0.0, 1, slab=(32, 64))             # row0 not a multiple of 64
+    b = lat.Lattice(L, lat.BLUME_CAPEL, 0.7, 1, slab=(0, 256))      # Delta != 0: no marching table
+    b.set_neighbours(b, b)
     with pytest.raises(lat.LatticeError):
-        lat.Lattice(L, lat.BLUME_CAPEL, 0.0, 1, slab=(0, 64))        # Ising only in round 1
+        b.half_sweep(0, 0.5)
+    b.close()
     s = lat.Lattice(L, lat.ISING, 0.0, 1, slab=(64, 128))
     with pytest.raises(lat.LatticeError) as e:
         s.half_sweep(0, 0.4)                                         # neighbours not set
