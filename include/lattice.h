@@ -100,6 +100,17 @@ int lattice_create_slab(lattice_t **out, uint32_t L, int model, double delta, ui
 int lattice_slab_set_neighbours(lattice_t *lat, void *device_up_buf, uint32_t up_n_rows,
                                 void *device_down_buf, uint32_t down_n_rows);
 
+/* One process per GPU: the mirror pointers of lattice_slab_set_neighbours must then come from
+ * another process.  These helpers allocate a slab buffer that can be exported (cudaMalloc on the
+ * current device, so that the IPC handle maps the buffer itself), export it as a 64-byte CUDA IPC
+ * handle (sent to the neighbours by any means, e.g. torch.distributed), and open a neighbour's
+ * handle as a device pointer valid in this process.  Errors: EINVAL (NULL), ECUDA. */
+int lattice_device_alloc(void **device_ptr, size_t bytes);
+int lattice_device_free(void *device_ptr);
+int lattice_ipc_export(const void *device_ptr, unsigned char handle[64]);
+int lattice_ipc_open(const unsigned char handle[64], void **device_ptr);
+int lattice_ipc_close(void *device_ptr);
+
 /* Select how u32(site) is derived from Philox4x32-10:
  *   0 "quad":       one block per 4 consecutive same-colour sites, one 32-bit word each;
  *   1 "plane+tail": top 8 bits from 8 bit-plane blocks shared by 128 sites, low 24 bits from a

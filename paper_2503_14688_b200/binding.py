@@ -32,6 +32,11 @@ SIGNATURES = {
     "lattice_create_slab": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_double, C.c_uint64,
                                       C.c_uint32, C.c_uint32, _vp, C.c_size_t, _vp]),
     "lattice_slab_set_neighbours": (C.c_int, [_vp, _vp, C.c_uint32, _vp, C.c_uint32]),
+    "lattice_device_alloc": (C.c_int, [C.POINTER(_vp), C.c_size_t]),
+    "lattice_device_free": (C.c_int, [_vp]),
+    "lattice_ipc_export": (C.c_int, [_vp, C.POINTER(C.c_ubyte)]),
+    "lattice_ipc_open": (C.c_int, [C.POINTER(C.c_ubyte), C.POINTER(_vp)]),
+    "lattice_ipc_close": (C.c_int, [_vp]),
     "lattice_set_rng_scheme": (C.c_int, [_vp, C.c_int]),
     "lattice_sweep": (C.c_int, [_vp, C.c_uint64, _f64p]),
     "lattice_half_sweep": (C.c_int, [_vp, C.c_int, C.c_double]),
@@ -80,6 +85,20 @@ def _p(a: np.ndarray, ty):
     return a.ctypes.data_as(C.POINTER(ty))
 
 
+def ipc_open(handle: bytes) -> int:
+    """Map another process's exportable buffer into this process; returns its device address."""
+    h = (C.c_ubyte * 64).from_buffer_copy(handle)
+    p = _vp()
+    rc = lib().lattice_ipc_open(h, C.byref(p))
+    if rc != OK:
+        raise LatticeError("lattice_ipc_open", rc)
+    return p.value
+
+
+def ipc_close(ptr: int) -> None:
+    lib().lattice_ipc_close(_vp(ptr))
+
+
 def state_bytes(L: int, model: int) -> int:
     return int(lib().lattice_state_bytes(L, model))
 
@@ -109,8 +128,10 @@ class Lattice:
     """A packed lattice in device memory (a torch.uint8 tensor owned by this object)."""
 
     def __init__(self, L: int, model: int = ISING, delta: float = 0.0, seed: int = 0,
-                 scheme: int = 1, device: str = "cuda:0", stream=None, slab=None):
-        """slab = (row0, n_rows) creates a row slab of the L x L lattice (include/lattice.h)."""
+                 scheme: int = 1, device: str = "cuda:0", stream=None, slab=None, exportable=False):
+        """slab = (row0, n_rows) creates a row slab of the L x L lattice (include/lattice.h);
+        exportable = True allocates the buffer with lattice_device_alloc so that it can be shared
+        with other processes through a CUDA IPC handle (`ipc_handle`)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2503_14688_b200 needs a CUDA device; there is no CPU path")
@@ -124,16 +145,24 @@ class Lattice:
             raise LatticeError("lattice_state_bytes", EINVAL, f"L={L} model={model} slab={slab}")
         self._torch = torch
         self.device = torch.device(device)
+        self._own_ptr = None
         with torch.cuda.device(self.device):
-            self.buf = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            if exportable:
+                p = _vp()
+                rc = lib().lattice_device_alloc(C.byref(p), nbytes)
+                if rc != OK:
+                    raise LatticeError("lattice_device_alloc", rc)
+                self._own_ptr, self.buf = p.value, None
+            else:
+                self.buf = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = _vp()
             if self.slab is None:
                 rc = lib().lattice_create(C.byref(h), self.L, self.model, self.delta, self.seed,
-                                          _vp(self.buf.data_ptr()), nbytes, _vp(self.stream.cuda_stream))
+                                          _vp(self.data_ptr), nbytes, _vp(self.stream.cuda_stream))
             else:
                 rc = lib().lattice_create_slab(C.byref(h), self.L, self.model, self.delta, self.seed,
-                                               self.slab[0], self.slab[1], _vp(self.buf.data_ptr()),
+                                               self.slab[0], self.slab[1], _vp(self.data_ptr),
                                                nbytes, _vp(self.stream.cuda_stream))
         if rc != OK:
             raise LatticeError("lattice_create", rc)
@@ -148,10 +177,27 @@ class Lattice:
             detail = lib().lattice_last_error(self._h).decode() if rc == ECUDA else ""
             raise LatticeError(what, rc, detail)
 
+    @property
+    def data_ptr(self) -> int:
+        """Device address of the packed state."""
+        return self._own_ptr if self._own_ptr is not None else self.buf.data_ptr()
+
+    def ipc_handle(self) -> bytes:
+        """64-byte CUDA IPC handle of an exportable buffer, for a neighbour in another process."""
+        if self._own_ptr is None:
+            raise RuntimeError("create the Lattice with exportable=True")
+        h = (C.c_ubyte * 64)()
+        self._check(lib().lattice_ipc_export(_vp(self._own_ptr), h), "lattice_ipc_export")
+        return bytes(h)
+
     def close(self) -> None:
         if getattr(self, "_h", None):
             lib().lattice_destroy(self._h)
             self._h = None
+            if self._own_ptr is not None:
+                self.synchronize()
+                lib().lattice_device_free(_vp(self._own_ptr))
+                self._own_ptr = None
 
     def __del__(self):
         try:
@@ -170,10 +216,13 @@ class Lattice:
 
     def set_neighbours(self, up: "Lattice", down: "Lattice") -> None:
         """Row-slab mode: the slabs owning the rows above / below (self twice for a single slab)."""
-        self._check(lib().lattice_slab_set_neighbours(self._h, _vp(up.buf.data_ptr()), up.slab[1],
-                                                      _vp(down.buf.data_ptr()), down.slab[1]),
-                    "lattice_slab_set_neighbours")
+        self.set_neighbour_ptrs(up.data_ptr, up.slab[1], down.data_ptr, down.slab[1])
         self._nbr = (up, down)                       # keep the neighbours' buffers alive
+
+    def set_neighbour_ptrs(self, up_ptr: int, up_rows: int, down_ptr: int, down_rows: int) -> None:
+        """The same with raw device addresses (e.g. opened from another process's IPC handle)."""
+        self._check(lib().lattice_slab_set_neighbours(self._h, _vp(up_ptr), up_rows, _vp(down_ptr), down_rows),
+                    "lattice_slab_set_neighbours")
 
     def set_time(self, t: int) -> None:
         self._check(lib().lattice_set_time(self._h, int(t)), "lattice_set_time")

@@ -466,6 +466,47 @@ int lattice_slab_set_neighbours(lattice_t *lat, void *device_up_buf, uint32_t up
     return LATTICE_OK;
 }
 
+int lattice_device_alloc(void **device_ptr, size_t bytes)
+{
+    if (!device_ptr || bytes == 0) return LATTICE_EINVAL;
+    if (cudaMalloc(device_ptr, bytes) != cudaSuccess) { cudaGetLastError(); return LATTICE_ENOMEM; }
+    return LATTICE_OK;
+}
+
+int lattice_device_free(void *device_ptr)
+{
+    if (!device_ptr) return LATTICE_EINVAL;
+    return cudaFree(device_ptr) == cudaSuccess ? LATTICE_OK : LATTICE_ECUDA;
+}
+
+int lattice_ipc_export(const void *device_ptr, unsigned char handle[64])
+{
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handles are 64 bytes");
+    if (!device_ptr || !handle) return LATTICE_EINVAL;
+    cudaIpcMemHandle_t h;
+    if (cudaIpcGetMemHandle(&h, const_cast<void *>(device_ptr)) != cudaSuccess) { cudaGetLastError(); return LATTICE_ECUDA; }
+    std::memcpy(handle, &h, 64);
+    return LATTICE_OK;
+}
+
+int lattice_ipc_open(const unsigned char handle[64], void **device_ptr)
+{
+    if (!device_ptr || !handle) return LATTICE_EINVAL;
+    cudaIpcMemHandle_t h;
+    std::memcpy(&h, handle, 64);
+    if (cudaIpcOpenMemHandle(device_ptr, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) {
+        cudaGetLastError();
+        return LATTICE_ECUDA;
+    }
+    return LATTICE_OK;
+}
+
+int lattice_ipc_close(void *device_ptr)
+{
+    if (!device_ptr) return LATTICE_EINVAL;
+    return cudaIpcCloseMemHandle(device_ptr) == cudaSuccess ? LATTICE_OK : LATTICE_ECUDA;
+}
+
 int lattice_set_rng_scheme(lattice_t *lat, int scheme)
 {
     if (!lat || (scheme != 0 && scheme != 1)) return LATTICE_EINVAL;

@@ -97,3 +97,93 @@ class ShardedLattice:
     def close(self) -> None:
         for s in self.slabs:
             s.close()
+
+
+# ---- one process per GPU ---------------------------------------------------------------------
+def neighbour_ranks(rank: int, world: int):
+    """(up, down): the ranks that own the rows above / below rank's slab (periodic)."""
+    return (rank - 1) % world, (rank + 1) % world
+
+
+def exchange_handles(my_handle: bytes, group=None):
+    """All-gather the 64-byte IPC handles over torch.distributed (any backend) and return
+    (handle of the upper neighbour, handle of the lower neighbour)."""
+    import torch.distributed as dist
+    rank, world = dist.get_rank(group), dist.get_world_size(group)
+    handles = [None] * world
+    dist.all_gather_object(handles, bytes(my_handle), group=group)
+    if any(h is None or len(h) != 64 for h in handles):
+        raise RuntimeError("a rank did not contribute a 64-byte handle")
+    up, down = neighbour_ranks(rank, world)
+    return handles[up], handles[down]
+
+
+class SlabRank:
+    """This process's slab of an L x L lattice sharded over the ranks of a torch.distributed
+    group, one rank per GPU.  Buffers are shared through CUDA IPC handles, so the half-sweep
+    kernel of each rank writes its boundary rows straight into its neighbours' halo rows
+    (NVLink P2P); the only collectives are the barrier that orders the colours and the u64
+    all-reduce of the measurement counts."""
+
+    def __init__(self, L: int, seed: int = 0, model: int = lat.ISING, delta: float = 0.0,
+                 device: str = "cuda:0", group=None):
+        import torch
+        import torch.distributed as dist
+        self._torch, self._dist, self.group = torch, dist, group
+        self.rank, self.world = dist.get_rank(group), dist.get_world_size(group)
+        if L % self.world:
+            raise ValueError("the number of ranks must divide L")
+        rows = L // self.world
+        self.L, self.rows = L, rows
+        self.lat = lat.Lattice(L, model, delta, seed, device=device, slab=(self.rank * rows, rows),
+                               exportable=True)
+        self._opened = []
+        if self.world == 1:
+            self.lat.set_neighbours(self.lat, self.lat)
+        else:
+            h_up, h_down = exchange_handles(self.lat.ipc_handle(), group)
+            with torch.cuda.device(self.lat.device):
+                p_up = lat.ipc_open(h_up)
+                p_down = p_up if self.world == 2 else lat.ipc_open(h_down)   # one mapping per buffer
+            self._opened = [p_up] if self.world == 2 else [p_up, p_down]
+            self.lat.set_neighbour_ptrs(p_up, rows, p_down, rows)
+        self._t = 0
+        self._fence()
+
+    def _fence(self) -> None:
+        self.lat.synchronize()
+        if self.world > 1:
+            self._dist.barrier(self.group)
+
+    @property
+    def time(self) -> int:
+        return self._t
+
+    def sweep(self, beta) -> None:
+        for b in np.atleast_1d(np.asarray(beta, dtype=np.float64)):
+            for colour in (0, 1):
+                self.lat.half_sweep(colour, float(b))
+                self._fence()                        # every rank's mirrors have landed
+            self._t += 1
+            self.lat.set_time(self._t)
+
+    def measure(self):
+        """(M, Q, S_x(1), S_y(1)) of the whole lattice on every rank."""
+        M, Q, Sx, Sy = self.lat.measure(1)
+        t = self._torch.tensor([M, Q, int(Sx[0]), int(Sy[0])], dtype=self._torch.int64)
+        if self.world > 1:
+            if self._dist.get_backend(self.group) == "nccl":
+                t = t.to(self.lat.device)
+            self._dist.all_reduce(t, op=self._dist.ReduceOp.SUM, group=self.group)
+        return tuple(int(x) for x in t.cpu())
+
+    def get_spins(self) -> np.ndarray:
+        """This rank's own rows."""
+        return self.lat.get_spins()
+
+    def close(self) -> None:
+        self._fence()
+        for p in self._opened:
+            lat.ipc_close(p)
+        self._opened = []
+        self.lat.close()

@@ -80,3 +80,57 @@ def test_slab_api_errors():
     assert s.get_spins().shape == (128, L)
     assert s.get_spins(63, 0, 130, L).shape == (130, L)              # own rows and both halos
     s.close()
+
+
+RANK_WORKER = r'''
+import os, sys
+sys.path.insert(0, sys.argv[1])
+import numpy as np
+import torch.distributed as dist
+import paper_2503_14688_b200 as lat
+from paper_2503_14688_b200 import sharded, workloads
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+L, model, seed = int(sys.argv[2]), int(sys.argv[3]), 4711
+dist.init_process_group("gloo", rank=rank, world_size=world)
+beta = [workloads.BETA_C_ISING if model == 0 else workloads.BETA_BC] * 12 + [0.0, 0.7]
+s = sharded.SlabRank(L, seed, model)
+s.sweep(beta)
+counts = s.measure()
+parts = [None] * world
+dist.all_gather_object(parts, s.get_spins())
+if rank == 0:
+    g = lat.Lattice(L, model, 0.0, seed)
+    g.sweep(beta)
+    assert np.array_equal(np.concatenate(parts, axis=0), g.get_spins())
+    M, Q, Sx, Sy = g.measure(1)
+    assert counts == (M, Q, int(Sx[0]), int(Sy[0])), (counts, M, Q, Sx, Sy)
+    g.close()
+s.close()
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+'''
+
+
+@pytest.mark.parametrize("world,L,model", [(2, 512, lat.ISING), (3, 768, lat.ISING), (2, 512, lat.BLUME_CAPEL)])
+def test_one_process_per_slab_through_cuda_ipc(tmp_path, world, L, model):
+    """One process per slab (as one process per GPU would run it), neighbours' halo rows reached
+    through CUDA IPC handles exchanged over torch.distributed (gloo), colours ordered by
+    barriers.  All processes share this box's single GPU; no kernel waits on another process."""
+    import os, socket, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "rank_worker.py"
+    script.write_text(RANK_WORKER)
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    procs = []
+    for rank in range(world):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script), root, str(L), str(model)], env=env,
+                                      stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
+    outs = [p.communicate(timeout=300)[0] for p in procs]
+    for rank, (p, out) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0, out
+        assert f"ok {rank}" in out
