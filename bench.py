@@ -167,6 +167,61 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_sharded(args):
+    """One L x L lattice in row slabs, one rank per GPU: the optional
+    strong-scaling mode.  The default N > 1 mode stays independent replicas."""
+    import torch
+    import torch.distributed as dist
+    from paper_2503_14688_b200 import replicas
+    from paper_2503_14688_b200.sharded import SlabRank
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0")) % max(torch.cuda.device_count(), 1)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29533")
+    if args.dist_backend == "nccl":
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=dev)
+    else:
+        dist.init_process_group("gloo", rank=rank, world_size=world)
+    w = workloads.CONFIGS[args.workload]
+    L = args.L or w.L
+    free, _ = torch.cuda.mem_get_info(dev)
+    per_spin = 8 if w.model == workloads.ISING else 4
+    while L > 256 * world and L * L // per_spin // world > free - (2 << 30):
+        L //= 2
+    L = replicas.agree_min(L, dev if args.dist_backend == "nccl" else "cpu")
+    s = SlabRank(L, w.seed, w.model, w.delta, device=str(dev))
+    sched = w.beta_schedule(args.warmup + args.steps)
+    s.sweep(sched[:args.warmup])
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    dist.barrier()
+    n0 = s.lat.launches
+    ev0.record(s.lat.stream)
+    s.sweep(sched[args.warmup:])
+    ev1.record(s.lat.stream)
+    launches = s.lat.launches - n0
+    torch.cuda.synchronize(dev)
+    ms = replicas.max_over_ranks(ev0.elapsed_time(ev1), dev if args.dist_backend == "nccl" else "cpu")
+    counts = s.measure()
+    if rank == 0:
+        line = {"metric": METRIC, "value": L * L * args.steps / (ms * 1e6), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+                "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "u32",
+                "data": "synthetic",
+                "config": {"workload": w.name if L == w.L else f"{w.name}@L={L}", "L": L,
+                           "parallelism": f"row slabs x{world}, halo rows mirrored by the update kernel",
+                           "rows_per_rank": L // world},
+                "gpu_launches": int(launches),
+                "record": {"M": counts[0], "Q": counts[1], "Sx1": counts[2], "Sy1": counts[3]}}
+        print(json.dumps(line))
+    s.close()
+    dist.destroy_process_group()
+
+
 def pick_L(w, torch, dev):
     """Largest power-of-two L <= w.L whose packed state fits in the free device memory."""
     free, _ = torch.cuda.mem_get_info(dev)
@@ -189,9 +244,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--measure-rmax", type=int, default=-1,
                     help="r_max of the separately timed measurement pass (-1: the workload's)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: ONE lattice in row slabs over the ranks (strong scaling, fused halo "
+                         "mirroring over peer memory) instead of independent replicas")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"])
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sharded:
+        return run_sharded(args)
 
     import torch
     import torch.distributed as dist
