@@ -241,7 +241,7 @@ __device__ __forceinline__ void bc_update_run(const BCArgs &a, uint32_t i, uint3
 }
 
 template <int SCHEME>
-__global__ void __launch_bounds__(256) bc_half_sweep_v4(const BCArgs a)
+__global__ void __launch_bounds__(256, 2) bc_half_sweep_v4(const BCArgs a)
 {
     const uint32_t tq = 1u << a.tq_log2;
     const uint32_t tr = 256u >> a.tq_log2;
