@@ -100,6 +100,17 @@ int lattice_create_slab(lattice_t **out, uint32_t L, int model, double delta, ui
 int lattice_slab_set_neighbours(lattice_t *lat, void *device_up_buf, uint32_t up_n_rows,
                                 void *device_down_buf, uint32_t down_n_rows);
 
+/* A measurement-only handle over a caller-assembled buffer [colour(/plane)][rows][L/64] that is
+ * NOT periodic along y: lattice_measure_rows(view, i0, n, r_max, ...) requires
+ * i0 + n + r_max <= rows (partner rows i + r are read from the buffer as they are); the x axis
+ * stays periodic within a row.  This is how a slab measures C(r) for r > 1: its own rows followed
+ * by the next r_max rows of the lattice (copied from the slabs below, lattice_device_copy works on
+ * peer / IPC pointers), base rows 0 .. n_rows-1.  No other call is allowed on a view except
+ * lattice_destroy.  Row parity matters for odd r along x: rows must start at an EVEN global row. */
+int lattice_view(lattice_t **out, uint32_t L, int model, uint32_t rows, void *device_buf,
+                 size_t device_buf_bytes, void *cuda_stream);
+int lattice_device_copy(void *device_dst, const void *device_src, size_t bytes, void *cuda_stream);
+
 /* One process per GPU: the mirror pointers of lattice_slab_set_neighbours must then come from
  * another process.  These helpers allocate a slab buffer that can be exported (cudaMalloc on the
  * current device, so that the IPC handle maps the buffer itself), export it as a 64-byte CUDA IPC

@@ -32,6 +32,8 @@ SIGNATURES = {
     "lattice_create_slab": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_double, C.c_uint64,
                                       C.c_uint32, C.c_uint32, _vp, C.c_size_t, _vp]),
     "lattice_slab_set_neighbours": (C.c_int, [_vp, _vp, C.c_uint32, _vp, C.c_uint32]),
+    "lattice_view": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_uint32, _vp, C.c_size_t, _vp]),
+    "lattice_device_copy": (C.c_int, [_vp, _vp, C.c_size_t, _vp]),
     "lattice_device_alloc": (C.c_int, [C.POINTER(_vp), C.c_size_t]),
     "lattice_device_free": (C.c_int, [_vp]),
     "lattice_ipc_export": (C.c_int, [_vp, C.POINTER(C.c_ubyte)]),
@@ -122,6 +124,33 @@ def energy(Sx, Sy, Q: int, delta: float, L: int) -> float:
     Sy = np.ascontiguousarray(Sy, dtype=np.int64)
     return float(lib().lattice_energy(_p(Sx, C.c_int64), _p(Sy, C.c_int64), int(Q), float(delta),
                                       int(L)))
+
+
+def measure_buffer(L: int, model: int, rows: int, n_base: int, r_max: int, ptr: int, nbytes: int,
+                   stream_ptr: int = 0):
+    """(M, Q, Sx[r_max], Sy[r_max]) over base rows 0 .. n_base-1 of a caller-assembled buffer
+    [colour(/plane)][rows][L/64] that is not periodic along y (include/lattice.h, lattice_view)."""
+    h = _vp()
+    rc = lib().lattice_view(C.byref(h), L, model, rows, _vp(ptr), nbytes, _vp(stream_ptr))
+    if rc != OK:
+        raise LatticeError("lattice_view", rc)
+    try:
+        Sx = np.zeros(r_max, dtype=np.int64)
+        Sy = np.zeros(r_max, dtype=np.int64)
+        M, Q = C.c_int64(0), C.c_int64(0)
+        rc = lib().lattice_measure_rows(h, 0, n_base, r_max, C.byref(M), C.byref(Q),
+                                        _p(Sx, C.c_int64), _p(Sy, C.c_int64))
+        if rc != OK:
+            raise LatticeError("lattice_measure_rows", rc)
+        return int(M.value), int(Q.value), Sx, Sy
+    finally:
+        lib().lattice_destroy(h)
+
+
+def device_copy(dst: int, src: int, nbytes: int, stream_ptr: int = 0) -> None:
+    rc = lib().lattice_device_copy(_vp(dst), _vp(src), nbytes, _vp(stream_ptr))
+    if rc != OK:
+        raise LatticeError("lattice_device_copy", rc)
 
 
 class Lattice:

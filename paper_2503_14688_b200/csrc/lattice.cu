@@ -29,6 +29,7 @@ struct lattice {
     uint32_t n_own;            // rows this handle updates: L, or the slab's n_rows
     uint32_t row0;             // global index of the first own row (0 for a whole lattice)
     bool slab;
+    bool view;                 // handle over a caller-assembled [planes][rows][wpr] buffer: measurement only
     uint32_t *mir_up[2][2], *mir_dn[2][2];   // slab: per colour and plane, the neighbours' halo rows
     bool have_nbr;
     uint32_t wpr;              // words per row per colour (per plane)
@@ -237,6 +238,7 @@ int launch_bc_march(lattice *lat, int colour)
 
 int launch_half_sweep(lattice *lat, int colour)
 {
+    if (lat->view) return LATTICE_ESTATE;
     if (lat->slab) {
         if (!lat->have_nbr) return LATTICE_ESTATE;
         if (lat->model == LATTICE_ISING) return launch_ising_march(lat, colour);
@@ -466,6 +468,34 @@ int lattice_slab_set_neighbours(lattice_t *lat, void *device_up_buf, uint32_t up
     return LATTICE_OK;
 }
 
+int lattice_view(lattice_t **out, uint32_t L, int model, uint32_t rows, void *device_buf,
+                 size_t device_buf_bytes, void *cuda_stream)
+{
+    if (!out || lattice_state_bytes(L, model) == 0 || rows == 0 || !device_buf ||
+        ((uintptr_t)device_buf & 15u) != 0)
+        return LATTICE_EINVAL;
+    const size_t planes = model == LATTICE_ISING ? 2 : 4;
+    if (device_buf_bytes < planes * rows * (size_t)(L / 64u) * sizeof(uint32_t)) return LATTICE_EINVAL;
+    lattice *lat = new (std::nothrow) lattice();
+    if (!lat) return LATTICE_ENOMEM;
+    std::memset(lat, 0, sizeof *lat);
+    lat->L = L; lat->wpr = L / 64u; lat->model = model; lat->delta = 0.0; lat->seed = 0;
+    lat->rows = rows; lat->n_own = rows; lat->row0 = 0; lat->slab = false; lat->view = true;
+    lat->scheme = 1; lat->t = 0;
+    lat->buf = (uint32_t *)device_buf;
+    lat->stream = (cudaStream_t)cuda_stream;
+    *out = lat;
+    return LATTICE_OK;
+}
+
+int lattice_device_copy(void *device_dst, const void *device_src, size_t bytes, void *cuda_stream)
+{
+    if (!device_dst || !device_src) return LATTICE_EINVAL;
+    if (bytes == 0) return LATTICE_OK;
+    return cudaMemcpyAsync(device_dst, device_src, bytes, cudaMemcpyDeviceToDevice,
+                           (cudaStream_t)cuda_stream) == cudaSuccess ? LATTICE_OK : LATTICE_ECUDA;
+}
+
 int lattice_device_alloc(void **device_ptr, size_t bytes)
 {
     if (!device_ptr || bytes == 0) return LATTICE_EINVAL;
@@ -577,12 +607,15 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
 {
     if (!lat || !M || !Q || !Sx || !Sy) return LATTICE_EINVAL;
     const uint64_t L = lat->L;
-    if (r_max < 1 || r_max > L / 2 || i0 >= L || n_rows < 1 || n_rows > L || i0 + n_rows > L)
+    const uint64_t R = lat->view ? lat->rows : L;                 // rows that can be base rows
+    if (r_max < 1 || r_max > L / 2 || i0 >= R || n_rows < 1 || n_rows > R || i0 + n_rows > R)
         return LATTICE_EINVAL;
     // a row slab measures its own rows only, and only r = 1 (row i+1 of the last own row is the
     // lower halo); larger r along y would need r_max halo rows
     if (lat->slab && (r_max != 1 || i0 < lat->row0 || i0 + n_rows > (uint64_t)lat->row0 + lat->n_own))
         return LATTICE_EINVAL;
+    // a view is not periodic along y: the partner rows i + r must lie inside the buffer
+    if (lat->view && i0 + n_rows + r_max > lat->rows) return LATTICE_EINVAL;
     const size_t entries = 2 + 4 * (size_t)r_max;
     int rc = ensure_cnt(lat, entries);
     if (rc) return rc;
@@ -611,7 +644,8 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
     const bool x_blk = (lat->wpr % MEAS_NB) == 0;
     const unsigned chunks = (r_max + MEAS_RC - 1) / MEAS_RC;
     MeasBlkArgs b;
-    b.buf = lat->buf; b.L = lat->L; b.wpr = lat->wpr; b.i0 = (uint32_t)i0; b.r_max = r_max; b.cnt = lat->d_cnt;
+    // the kernels' "L" is the number of rows per plane (plane stride, y wrap): rows == L for a lattice
+    b.buf = lat->buf; b.L = lat->rows; b.wpr = lat->wpr; b.i0 = (uint32_t)i0; b.r_max = r_max; b.cnt = lat->d_cnt;
     if (nblk) {
         b.n = nblk;
         const unsigned long long threads = 2ull * nblk * lat->wpr;
@@ -631,7 +665,7 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
         CU(lat, cudaGetLastError());
     }
     MeasArgs a;
-    a.buf = lat->buf; a.L = lat->L; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
+    a.buf = lat->buf; a.L = lat->rows; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
     a.r_max = r_max; a.r0 = 0; a.axis0 = 0; a.cnt = lat->d_cnt;
     auto generic = [&](uint32_t gi0, uint32_t gn, bool mq, uint32_t axis0, uint32_t naxes) -> int {
         a.i0 = gi0; a.n_rows = gn; a.axis0 = axis0;

@@ -83,13 +83,43 @@ class ShardedLattice:
             for s in self.slabs:
                 s.set_time(self._t)
 
-    def measure(self):
-        """(M, Q, S_x(1), S_y(1)) of the whole lattice: the slabs' partial sums added up."""
-        tot = np.zeros(4, dtype=np.int64)
-        for s in self.slabs:
-            M, Q, Sx, Sy = s.measure(1)
-            tot += np.array([M, Q, Sx[0], Sy[0]], dtype=np.int64)
-        return tuple(int(x) for x in tot)
+    def measure(self, r_max: int = 1):
+        """Whole-lattice counts, the slabs' partial sums added up: (M, Q, S_x(1), S_y(1)) for
+        r_max == 1 (one pass per slab), else (M, Q, Sx[r_max], Sy[r_max]): every slab measures a
+        temporary buffer of its own rows followed by the next r_max rows of the lattice."""
+        if r_max == 1:
+            tot = np.zeros(4, dtype=np.int64)
+            for s in self.slabs:
+                M, Q, Sx, Sy = s.measure(1)
+                tot += np.array([M, Q, Sx[0], Sy[0]], dtype=np.int64)
+            return tuple(int(x) for x in tot)
+        torch = self._torch
+        rows = self.L // self.n
+        wpr = self.L // 64
+        planes = 2 if self.model == lat.ISING else 4
+        M = Q = 0
+        Sx = np.zeros(r_max, dtype=np.int64)
+        Sy = np.zeros(r_max, dtype=np.int64)
+        self.synchronize()
+        for k, s in enumerate(self.slabs):
+            # own rows, then r_max rows from the slabs below (possibly several, periodic)
+            pieces = []
+            for p in range(planes):
+                own = s.buf.view(planes, rows + 2, wpr * 4)[p, 1:rows + 1]
+                ext, need, j = [own], r_max, k
+                while need > 0:
+                    j = (j + 1) % self.n
+                    nb = self.slabs[j].buf.view(planes, rows + 2, wpr * 4)[p, 1:1 + min(need, rows)]
+                    ext.append(nb.to(s.device))
+                    need -= min(need, rows)
+                pieces.append(torch.cat(ext, dim=0))
+            with torch.cuda.device(s.device):
+                buf = torch.stack(pieces, dim=0).contiguous()
+                torch.cuda.current_stream(s.device).synchronize()
+                m, q, sx, sy = lat.measure_buffer(self.L, self.model, rows + r_max, rows, r_max,
+                                                  buf.data_ptr(), buf.numel(), s.stream.cuda_stream)
+            M += m; Q += q; Sx += sx; Sy += sy
+        return M, Q, Sx, Sy
 
     def get_spins(self) -> np.ndarray:
         return np.concatenate([s.get_spins() for s in self.slabs], axis=0)
@@ -146,6 +176,7 @@ class SlabRank:
                 p_up = lat.ipc_open(h_up)
                 p_down = p_up if self.world == 2 else lat.ipc_open(h_down)   # one mapping per buffer
             self._opened = [p_up] if self.world == 2 else [p_up, p_down]
+            self._down_ptr = p_down
             self.lat.set_neighbour_ptrs(p_up, rows, p_down, rows)
         self._t = 0
         self._fence()
@@ -167,15 +198,43 @@ class SlabRank:
             self._t += 1
             self.lat.set_time(self._t)
 
-    def measure(self):
-        """(M, Q, S_x(1), S_y(1)) of the whole lattice on every rank."""
-        M, Q, Sx, Sy = self.lat.measure(1)
-        t = self._torch.tensor([M, Q, int(Sx[0]), int(Sy[0])], dtype=self._torch.int64)
+    def _all_reduce(self, values):
+        t = self._torch.tensor(values, dtype=self._torch.int64)
         if self.world > 1:
             if self._dist.get_backend(self.group) == "nccl":
                 t = t.to(self.lat.device)
             self._dist.all_reduce(t, op=self._dist.ReduceOp.SUM, group=self.group)
-        return tuple(int(x) for x in t.cpu())
+        return t.cpu().numpy()
+
+    def measure(self, r_max: int = 1):
+        """Whole-lattice counts on every rank: (M, Q, S_x(1), S_y(1)) for r_max == 1, else
+        (M, Q, Sx[r_max], Sy[r_max]) with r_max <= rows per rank (the partner rows come from the
+        lower neighbour's buffer through its IPC mapping)."""
+        if r_max == 1:
+            M, Q, Sx, Sy = self.lat.measure(1)
+            return tuple(int(x) for x in self._all_reduce([M, Q, int(Sx[0]), int(Sy[0])]))
+        if r_max > self.rows:
+            raise ValueError("r_max must not exceed the rows per rank")
+        rows, wpr = self.rows, self.L // 64
+        planes = 2 if self.lat.model == lat.ISING else 4
+        row_bytes, plane_bytes = wpr * 4, (rows + 2) * wpr * 4
+        ext_rows = rows + r_max
+        nbytes = planes * ext_rows * row_bytes
+        down = self._down_ptr if self.world > 1 else self.lat.data_ptr
+        self._fence()                                 # every rank's state is final
+        with self._torch.cuda.device(self.lat.device):
+            buf = self._torch.empty(nbytes, dtype=self._torch.uint8, device=self.lat.device)
+            st = self.lat.stream.cuda_stream
+            for p in range(planes):
+                dst = buf.data_ptr() + p * ext_rows * row_bytes
+                lat.device_copy(dst, self.lat.data_ptr + p * plane_bytes + row_bytes, rows * row_bytes, st)
+                lat.device_copy(dst + rows * row_bytes, down + p * plane_bytes + row_bytes,
+                                r_max * row_bytes, st)
+            M, Q, Sx, Sy = lat.measure_buffer(self.L, self.lat.model, ext_rows, rows, r_max,
+                                              buf.data_ptr(), nbytes, st)
+        self._fence()                                 # neighbours may sweep again
+        tot = self._all_reduce([M, Q] + Sx.tolist() + Sy.tolist())
+        return int(tot[0]), int(tot[1]), tot[2:2 + r_max].copy(), tot[2 + r_max:].copy()
 
     def get_spins(self) -> np.ndarray:
         """This rank's own rows."""

@@ -145,3 +145,24 @@ def test_slab_bytes_and_create_slab_argument_checks():
                  (1024, lat.ISING, float("nan"), 1, 0, 256, fake, n, None)]:
         assert L.lattice_create_slab(C.byref(h), *args) == lat.binding.EINVAL, args
     assert L.lattice_slab_set_neighbours(None, fake, 64, fake, 64) == lat.binding.EINVAL
+
+
+def test_view_and_copy_argument_checks():
+    import ctypes as C
+    L = lat.lib()
+    h = C.c_void_p()
+    fake = C.c_void_p(0x10000)
+    need = 2 * 300 * (1024 // 64) * 4
+    assert L.lattice_view(C.byref(h), 1024, lat.ISING, 300, fake, need - 1, None) == lat.binding.EINVAL
+    assert L.lattice_view(C.byref(h), 1000, lat.ISING, 300, fake, need, None) == lat.binding.EINVAL
+    assert L.lattice_view(C.byref(h), 1024, lat.ISING, 0, fake, need, None) == lat.binding.EINVAL
+    assert L.lattice_view(C.byref(h), 1024, lat.ISING, 300, None, need, None) == lat.binding.EINVAL
+    assert L.lattice_view(C.byref(h), 1024, lat.ISING, 300, fake, need, None) == lat.binding.OK
+    M, Q = C.c_int64(), C.c_int64()
+    S = (C.c_int64 * 64)()
+    # base rows + r_max must fit in the view (it is not periodic along y); checked before any launch
+    assert L.lattice_measure_rows(h, 0, 280, 40, C.byref(M), C.byref(Q), S, S) == lat.binding.EINVAL
+    assert L.lattice_half_sweep(h, 0, 0.4) == lat.binding.ESTATE          # a view cannot be swept
+    assert L.lattice_destroy(h) == lat.binding.OK
+    assert L.lattice_device_copy(None, fake, 16, None) == lat.binding.EINVAL
+    assert L.lattice_device_copy(fake, fake, 0, None) == lat.binding.OK

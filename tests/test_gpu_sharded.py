@@ -28,6 +28,11 @@ def test_sharded_equals_unsharded_and_oracle(L, n_slabs, model):
     assert np.array_equal(sh.get_spins(), g.get_spins())
     M, Q, Sx, Sy = g.measure(1)
     assert sh.measure() == (M, Q, int(Sx[0]), int(Sy[0]))
+    # C(r) for r > 1: own rows + the next r_max rows of the lattice, per slab (r_max may span slabs)
+    for r_max in (2, 37, min(L // 2, L // n_slabs + 5)):
+        Mg, Qg, Sxg, Syg = g.measure(r_max)
+        Ms, Qs, Sxs, Sys = sh.measure(r_max)
+        assert (Ms, Qs) == (Mg, Qg) and np.array_equal(Sxs, Sxg) and np.array_equal(Sys, Syg), r_max
     if L <= 1024:
         o = oracle.OracleLattice(L, model, 0.0, seed)
         o.sweep(beta)
@@ -96,6 +101,7 @@ beta = [workloads.BETA_C_ISING if model == 0 else workloads.BETA_BC] * 12 + [0.0
 s = sharded.SlabRank(L, seed, model)
 s.sweep(beta)
 counts = s.measure()
+corr = s.measure(40)
 parts = [None] * world
 dist.all_gather_object(parts, s.get_spins())
 if rank == 0:
@@ -104,6 +110,8 @@ if rank == 0:
     assert np.array_equal(np.concatenate(parts, axis=0), g.get_spins())
     M, Q, Sx, Sy = g.measure(1)
     assert counts == (M, Q, int(Sx[0]), int(Sy[0])), (counts, M, Q, Sx, Sy)
+    M, Q, Sx, Sy = g.measure(40)
+    assert corr[0] == M and corr[1] == Q and np.array_equal(corr[2], Sx) and np.array_equal(corr[3], Sy)
     g.close()
 s.close()
 dist.barrier()
