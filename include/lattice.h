@@ -87,7 +87,8 @@ int lattice_create(lattice_t **out, uint32_t L, int model, double delta, uint64_
  * the half-sweeps: all slabs finish colour c (and its mirrors) before any starts colour 1-c.
  * Restrictions (round 1): RNG scheme 1, L a multiple of 256, row0 and n_rows multiples of 64;
  * Blume-Capel only with threshold tables of the Delta = 0 structure (half-sweeps return EINVAL
- * otherwise); Blume-Capel layout [colour][plane][n_rows + 2][L/64]; lattice_measure only with r_max == 1 (partial sums over the own rows: add them up);
+ * otherwise); Blume-Capel layout [colour][plane][n_rows + 2][L/64]; lattice_measure on a slab
+ * only with r_max == 1 (partial sums over the own rows: add them up; for r > 1 see lattice_view);
  * windows of get/set_spins must stay inside the slab's rows (halos included). */
 size_t lattice_slab_bytes(uint32_t L, int model, uint32_t n_rows);      /* 0 if not supported */
 /* Like lattice_create for the slab; own rows AND halos receive the disordered start. */
