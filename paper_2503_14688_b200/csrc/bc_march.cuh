@@ -87,6 +87,7 @@ __device__ __forceinline__ void lut3_dispatch(uint32_t lut, const uint32_t (&a)[
 //   [0] = (tied lanes, F, Y1, H0 of the word)    [1] = (nz-toggle mask, sg-toggle mask, word offset)
 // Pushing is loop-free (one ballot per word); the tied lanes of a word are enumerated when the
 // entry is resolved, 32 entries at a time, one entry per thread.
+template <bool SLAB>
 struct BCTieQueue {
     const BCMarchArgs &a;
     uint4 *q;                   // [2 * TIE_Q_SLOTS] this warp's slice
@@ -102,7 +103,7 @@ struct BCTieQueue {
             const uint32_t bit = __ffs(ties) - 1;
             ties &= ties - 1;
             const uint32_t cls = (((e0.y >> bit) & 1u) << 2) | (((e0.z >> bit) & 1u) << 1) | ((e0.w >> bit) & 1u);
-            const unsigned long long P = ((wo + a.p_off) << 5) + bit;
+            const unsigned long long P = ((SLAB ? wo + a.p_off : wo) << 5) + bit;
             const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
                                             a.colour | (TAG_ACC_TAIL << 8), a.K);
             if ((blk.x >> 8) < (a.thr[cls] & 0x00ffffffu)) hit |= 1u << bit;
@@ -110,7 +111,7 @@ struct BCTieQueue {
         const uint32_t dnz = hit & e1.x, dsg = hit & e1.y;
         if (dnz) atomicXor(a.tnz + wo, dnz);
         if (dsg) atomicXor(a.tsg + wo, dsg);
-        const uint32_t mf = e1.w >> 30;
+        const uint32_t mf = SLAB ? e1.w >> 30 : 0u;
         if (mf && (dnz | dsg)) {
             const uint32_t col = (e1.w >> 4) & 0x3ffffu;
             if (dnz) atomicXor((mf == 1 ? a.mir_up_nz : a.mir_dn_nz) + col, dnz);
@@ -131,7 +132,8 @@ struct BCTieQueue {
                 const uint32_t slot = pending + __popc(m & below);
                 q[2 * slot] = make_uint4(eq[w], Fm[w], Y1[w], H0[w]);
                 q[2 * slot + 1] = make_uint4(nf[w], gg[w], (uint32_t)o,
-                                             (uint32_t)(o >> 32) | (mir_tag + ((unsigned)w << 4)));
+                                             SLAB ? (uint32_t)(o >> 32) | (mir_tag + ((unsigned)w << 4))
+                                                  : (uint32_t)(o >> 32));
             }
             pending += __popc(m);
         }
@@ -165,11 +167,11 @@ __device__ __forceinline__ void bcm_load(const uint32_t *nzp, const uint32_t *sg
 // One row of one 128-bit run.  PAR == 0: side neighbour at p-1 (En, Es = word before the run),
 // PAR == 1: at p+1 (word after it).  Stores the updated words (ties treated as rejections) and
 // queues the ties.
-template <int PAR>
+template <int PAR, bool SLAB>
 __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, unsigned long long wo,
                                              uint32_t *tn, uint32_t *ts,
                                              const BCRow &U, const BCRow &C, const BCRow &D,
-                                             uint32_t En, uint32_t Es, BCTieQueue &queue,
+                                             uint32_t En, uint32_t Es, BCTieQueue<SLAB> &queue,
                                              uint32_t *mir_nz = nullptr, uint32_t *mir_sg = nullptr,
                                              uint32_t mir_tag = 0)
 {
@@ -243,7 +245,7 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
     }
     *reinterpret_cast<uint4 *>(tn) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
     *reinterpret_cast<uint4 *>(ts) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
-    if (mir_nz) {       // slab mode: this row is also a neighbour's halo row
+    if (SLAB && mir_nz) {       // slab mode: this row is also a neighbour's halo row
         *reinterpret_cast<uint4 *>(mir_nz) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
         *reinterpret_cast<uint4 *>(mir_sg) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
     }
@@ -257,7 +259,7 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;
     if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
-    BCTieQueue queue{a, s_q[warp], lane, 0u};
+    BCTieQueue<SLAB> queue{a, s_q[warp], lane, 0u};
 
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
     const uint32_t q = g % nq, s = g / nq;
@@ -285,10 +287,10 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
             bcm_load(dn, dn + pw, kw, D);
             const uint32_t ke = COLOUR == 0 ? ke0 : ke1;
             if (SLAB && top && r == 0)
-                bc_march_row<COLOUR>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
+                bc_march_row<COLOUR, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
                                      a.mir_up_nz + kw, a.mir_up_sg + kw, (kw << 4) | (1u << 30));
             else
-                bc_march_row<COLOUR>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+                bc_march_row<COLOUR, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
             U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
         {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
@@ -297,10 +299,10 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
             bcm_load(dn, dn + pw, kw, D);
             const uint32_t ke = COLOUR == 0 ? ke1 : ke0;
             if (SLAB && bot && r + 2 == a.R)
-                bc_march_row<COLOUR ^ 1>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
+                bc_march_row<COLOUR ^ 1, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
                                          a.mir_dn_nz + kw, a.mir_dn_sg + kw, (kw << 4) | (2u << 30));
             else
-                bc_march_row<COLOUR ^ 1>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+                bc_march_row<COLOUR ^ 1, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
             U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
     }

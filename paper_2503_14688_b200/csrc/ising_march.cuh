@@ -117,6 +117,7 @@ __device__ __forceinline__ void plane_compare(uint32_t pcase, const uint32_t (&c
 // 31 entries are pending before a row and a row adds at most 4 x 32.
 constexpr int TIE_Q_SLOTS = 160;
 
+template <bool SLAB>
 struct WarpTieQueue {
     const IsingMarchArgs &a;
     uint4 *q;                  // [TIE_Q_SLOTS] this warp's slice
@@ -131,7 +132,7 @@ struct WarpTieQueue {
         while (ties) {
             const uint32_t bit = __ffs(ties) - 1;
             ties &= ties - 1;
-            const unsigned long long P = ((wo + a.p_off) << 5) + bit;
+            const unsigned long long P = ((SLAB ? wo + a.p_off : wo) << 5) + bit;
             const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
                                             a.colour | (TAG_ACC_TAIL << 8), a.K);
             const uint32_t thr = ((e.y >> bit) & 1u) ? a.thr8 : a.thr4;
@@ -139,7 +140,7 @@ struct WarpTieQueue {
         }
         if (flip) {
             atomicXor(a.tgt + wo, flip);
-            const uint32_t mf = e.w >> 30;
+            const uint32_t mf = SLAB ? e.w >> 30 : 0u;
             if (mf) atomicXor((mf == 1 ? a.mir_up : a.mir_dn) + ((e.w >> 4) & 0x3ffffu), flip);
         }
     }
@@ -155,7 +156,8 @@ struct WarpTieQueue {
             if (has) {
                 const unsigned long long o = wo + (unsigned)w;
                 q[pending + __popc(m & below)] =
-                    make_uint4(eq[w], c8[w], (uint32_t)o, (uint32_t)(o >> 32) | (mir_tag + ((unsigned)w << 4)));
+                    make_uint4(eq[w], c8[w], (uint32_t)o,
+                               SLAB ? (uint32_t)(o >> 32) | (mir_tag + ((unsigned)w << 4)) : (uint32_t)(o >> 32));
             }
             pending += __popc(m);
         }
@@ -180,10 +182,10 @@ struct WarpTieQueue {
 // and queues the ties.  EDGE: some class has threshold 2^32 (beta = 0): mask it out of `need`.
 // mir / mir_tag: slab mode only -- where this row is mirrored (null: nowhere) and the queue tag
 // (column word << 4 | flag << 30) that lets a late flip reach the mirror too.
-template <int PAR, bool EDGE>
+template <int PAR, bool EDGE, bool SLAB>
 __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, unsigned long long wo, uint32_t *tp,
                                           const uint4 &U4, const uint4 &C4, const uint4 &D4, uint32_t E,
-                                          WarpTieQueue &queue, uint32_t *mir = nullptr, uint32_t mir_tag = 0)
+                                          WarpTieQueue<SLAB> &queue, uint32_t *mir = nullptr, uint32_t mir_tag = 0)
 {
     const uint4 T4 = *reinterpret_cast<const uint4 *>(tp);       // tp == a.tgt + wo
     uint32_t T[4] = {T4.x, T4.y, T4.z, T4.w};
@@ -225,7 +227,7 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
 #pragma unroll
     for (int w = 0; w < 4; ++w) T[w] = lop3<0x4B>(T[w], need[w], acc[w]);    // T ^ (~need | acc)
     *reinterpret_cast<uint4 *>(tp) = make_uint4(T[0], T[1], T[2], T[3]);
-    if (mir) *reinterpret_cast<uint4 *>(mir) = make_uint4(T[0], T[1], T[2], T[3]);
+    if (SLAB && mir) *reinterpret_cast<uint4 *>(mir) = make_uint4(T[0], T[1], T[2], T[3]);
     queue.push(eq, c8, wo, mir_tag);
 }
 
@@ -236,7 +238,7 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;
     if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
-    WarpTieQueue queue{a, s_q[warp], lane, 0u};
+    WarpTieQueue<SLAB> queue{a, s_q[warp], lane, 0u};
 
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
     const uint32_t q = g % nq, s = g / nq;
@@ -266,9 +268,9 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
             const uint4 D = *reinterpret_cast<const uint4 *>(dn + kw);
             const uint32_t E = op[COLOUR == 0 ? ke0 : ke1];
             if (SLAB && top && r == 0)
-                march_row<COLOUR, EDGE>(a, G, wo, tp, U, C, D, E, queue, a.mir_up + kw, (kw << 4) | (1u << 30));
+                march_row<COLOUR, EDGE, SLAB>(a, G, wo, tp, U, C, D, E, queue, a.mir_up + kw, (kw << 4) | (1u << 30));
             else
-                march_row<COLOUR, EDGE>(a, G, wo, tp, U, C, D, E, queue);
+                march_row<COLOUR, EDGE, SLAB>(a, G, wo, tp, U, C, D, E, queue);
             U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
         {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
@@ -277,9 +279,9 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
             const uint4 D = *reinterpret_cast<const uint4 *>(dn + kw);
             const uint32_t E = op[COLOUR == 0 ? ke1 : ke0];
             if (SLAB && bot && r + 2 == a.R)
-                march_row<COLOUR ^ 1, EDGE>(a, G, wo, tp, U, C, D, E, queue, a.mir_dn + kw, (kw << 4) | (2u << 30));
+                march_row<COLOUR ^ 1, EDGE, SLAB>(a, G, wo, tp, U, C, D, E, queue, a.mir_dn + kw, (kw << 4) | (2u << 30));
             else
-                march_row<COLOUR ^ 1, EDGE>(a, G, wo, tp, U, C, D, E, queue);
+                march_row<COLOUR ^ 1, EDGE, SLAB>(a, G, wo, tp, U, C, D, E, queue);
             U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
     }
