@@ -292,7 +292,7 @@ def main():
         barrier()
         return ms
 
-    sched = w.beta_schedule(2 * (args.warmup + args.steps) + 2)
+    sched = w.beta_schedule(2 * (args.warmup + args.steps) + 16)
 
     def step_device(t):
         g.sweep(sched[t:t + 1])
@@ -319,6 +319,18 @@ def main():
     step_e2e(tdone)
     e2e_ms = timed(step_e2e, args.steps, tdone + 1)
     tdone += 1 + args.steps
+
+    # ---- worst-case input: the all-up state (every site has 4 aligned neighbours, so every
+    # lane needs a random decision and ties are ~3x more frequent than after the quench) ----------
+    worst = None
+    if world == 1:
+        g.fill(1)
+        nw = max(2, min(4, args.steps))
+        g.sweep(sched[tdone:tdone + 1])
+        worst_ms = timed(step_device, nw, tdone + 1)
+        tdone += 1 + nw
+        worst = {"value": updates_per_step * nw / (worst_ms * 1e6), "unit": UNIT, "steps": nw,
+                 "input": "all spins up at t0 (SURVEY.md 8(d) worst case), then the same sweeps"}
 
     # ---- measurement pass, timed separately --------------------------------------------------
     r_meas = w.r_max if args.measure_rmax < 0 else args.measure_rmax
@@ -384,6 +396,7 @@ def main():
                 "what": "lattice_sweep(1, host beta) + lattice_measure(r_max=1) -> host int64"},
         "roofline": roofline,
         "roofline_hbm": roofline_hbm,
+        "worst_case": worst,
         "measure": meas,
     }
     if not args.no_cpu_baseline:

@@ -161,6 +161,12 @@ int lattice_get_spins(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint
 int lattice_set_spins(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint32_t w,
                       const int8_t *in);
 
+/* Set every spin of the lattice (or slab, halos included) to `spin` (+1 / -1, or 0 for
+ * Blume-Capel): the ordered states used as worst-case throughput inputs (every site has 4 aligned
+ * neighbours, so every lane needs a random decision) and in tests.  Asynchronous on the stream.
+ * EINVAL if the value is not in the model's alphabet. */
+int lattice_fill(lattice_t *lat, int spin);
+
 /* Sweeps done so far. */
 uint64_t lattice_time(const lattice_t *lat);
 /* Overwrite the sweep counter (checkpoint restore together with the packed words).

@@ -47,6 +47,7 @@ SIGNATURES = {
                                        _i64p, _i64p]),
     "lattice_get_spins": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _i8p]),
     "lattice_set_spins": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _i8p]),
+    "lattice_fill": (C.c_int, [_vp, C.c_int]),
     "lattice_time": (C.c_uint64, [_vp]),
     "lattice_set_time": (C.c_int, [_vp, C.c_uint64]),
     "lattice_launches": (C.c_uint64, [_vp]),
@@ -298,6 +299,11 @@ class Lattice:
         with self._torch.cuda.device(self.device):
             self._check(lib().lattice_set_spins(self._h, i0, j0, s.shape[0], s.shape[1],
                                                 _p(s, C.c_int8)), "lattice_set_spins")
+
+    def fill(self, spin: int) -> None:
+        """Every spin := spin (an ordered state: worst-case throughput input, tests)."""
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_fill(self._h, int(spin)), "lattice_fill")
 
     def synchronize(self) -> None:
         self.stream.synchronize()

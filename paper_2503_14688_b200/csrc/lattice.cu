@@ -760,6 +760,23 @@ int lattice_set_spins(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint
     return window_call(lat, i0, j0, h, w, const_cast<int8_t *>(in), true);
 }
 
+int lattice_fill(lattice_t *lat, int spin)
+{
+    if (!lat || lat->view || spin < -1 || spin > 1 || (lat->model == LATTICE_ISING && spin == 0))
+        return LATTICE_EINVAL;
+    const size_t plane = (size_t)lat->rows * lat->wpr * sizeof(uint32_t);
+    if (lat->model == LATTICE_ISING) {
+        CU(lat, cudaMemsetAsync(lat->buf, spin > 0 ? 0xFF : 0x00, 2 * plane, lat->stream));
+    } else {
+        for (int c = 0; c < 2; ++c) {
+            char *base = (char *)lat->buf + (size_t)(2 * c) * plane;
+            CU(lat, cudaMemsetAsync(base, spin != 0 ? 0xFF : 0x00, plane, lat->stream));            // nz
+            CU(lat, cudaMemsetAsync(base + plane, spin < 0 ? 0xFF : 0x00, plane, lat->stream));     // sg
+        }
+    }
+    return LATTICE_OK;
+}
+
 uint64_t lattice_time(const lattice_t *lat) { return lat ? lat->t : 0; }
 
 int lattice_set_time(lattice_t *lat, uint64_t t)

@@ -248,6 +248,30 @@ def test_measure_r1_single_pass(L, model):
         _same_measure(g, o, 1, L, rows=(i0, n))
 
 
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+def test_fill_ordered_states_and_sweep_from_them(model):
+    """lattice_fill: ordered states (bench.py's worst-case input), then sweeps against the oracle."""
+    L = 512
+    g = lat.Lattice(L, model, 0.0, 77)
+    o = oracle.OracleLattice(L, model, 0.0, 77)
+    for spin in ([1, -1] if model == lat.ISING else [1, 0, -1]):
+        g.fill(spin)
+        want = np.full((L, L), spin, dtype=np.int8)
+        assert np.array_equal(g.get_spins(), want)
+        M, Q, Sx, Sy = g.measure(8)
+        assert M == spin * L * L and Q == abs(spin) * L * L and (Sx == Q).all() and (Sy == Q).all()
+        o.set_spins(want)
+        beta = [BETA_C if model == lat.ISING else workloads.BETA_BC] * 6
+        g.sweep(beta)
+        o.sweep(beta)
+        assert np.array_equal(g.get_spins(), o.get_spins()), spin
+    if model == lat.ISING:
+        with pytest.raises(lat.LatticeError):
+            g.fill(0)
+    with pytest.raises(lat.LatticeError):
+        g.fill(2)
+
+
 def test_randomised_parity_sweep_of_parameters():
     """Seeded random (model, L, scheme, beta schedule, Delta, seed) cases: spins and counts after a
     few sweeps, bit for bit.  Covers the generic kernels (L not a multiple of 256, scheme 0,
