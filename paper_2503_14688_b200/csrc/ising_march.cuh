@@ -231,15 +231,11 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
     queue.push(eq, c8, wo, mir_tag);
 }
 
+// The march of one thread: rows i0 .. i0+R-1 of run q, g = s * (wpr/4) + q (ties are queued, not
+// drained).
 template <int COLOUR, bool EDGE, bool SLAB>
-__global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a)
+__device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g, WarpTieQueue<SLAB> &queue)
 {
-    __shared__ uint4 s_q[8][TIE_Q_SLOTS];
-    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t g = blockIdx.x * 256u + threadIdx.x;
-    if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
-    WarpTieQueue<SLAB> queue{a, s_q[warp], lane, 0u};
-
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
     const uint32_t q = g % nq, s = g / nq;
     const uint32_t kw = q << 2;
@@ -285,6 +281,17 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
             U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
     }
+}
+
+template <int COLOUR, bool EDGE, bool SLAB>
+__global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a)
+{
+    __shared__ uint4 s_q[8][TIE_Q_SLOTS];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t g = blockIdx.x * 256u + threadIdx.x;
+    if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
+    WarpTieQueue<SLAB> queue{a, s_q[warp], lane, 0u};
+    march_thread<COLOUR, EDGE, SLAB>(a, g, queue);
     queue.drain();
 }
 #endif

@@ -18,6 +18,7 @@
 #include "bc_march.cuh"
 #include "ising.cuh"
 #include "ising_march.cuh"
+#include "ising_persist.cuh"
 #include "measure.cuh"
 #include "philox.cuh"
 
@@ -51,6 +52,9 @@ struct lattice {
     size_t cnt_cap;            // entries
     int8_t *d_win;
     size_t win_cap;            // bytes
+    SweepParams *d_sp;         // per-sweep parameters of the persistent kernel
+    size_t sp_cap;             // entries
+    int persist_blocks;        // co-resident blocks of ising_persist_kernel (0: not yet queried, -1: unavailable)
     char err[256];
 };
 
@@ -554,19 +558,99 @@ int lattice_half_sweep(lattice_t *lat, int colour, double beta)
     return launch_half_sweep(lat, colour);
 }
 
+// Cache-resident Ising lattices: all n sweeps in one cooperative launch (ising_persist.cuh).
+// Returns 1 if the path does not apply (the caller then launches the half-sweeps one by one).
+static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
+{
+    if (lat->model != LATTICE_ISING || lat->scheme != 1 || lat->slab || lat->view || (lat->wpr % 4u) != 0 ||
+        lat->L > 8192u || n < 2 || lat->persist_blocks < 0)
+        return 1;
+    if (lat->persist_blocks == 0) {
+        int dev = 0, coop = 0, sms = 0, per_sm = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_persist_kernel<false>, 256, 0) != cudaSuccess ||
+            per_sm < 1) {
+            cudaGetLastError();
+            lat->persist_blocks = -1;
+            return 1;
+        }
+        int per_sm_e = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_e, ising_persist_kernel<true>, 256, 0);
+        if (per_sm_e >= 1 && per_sm_e < per_sm) per_sm = per_sm_e;
+        lat->persist_blocks = per_sm * sms;
+    }
+    const uint32_t L = lat->L, wpr = lat->wpr, nq = wpr / 4u;
+    const size_t pw = (size_t)L * wpr;
+    if (lat->sp_cap < n) {
+        if (lat->d_sp) cudaFree(lat->d_sp);
+        lat->d_sp = nullptr; lat->sp_cap = 0;
+        const size_t cap = n < 1024 ? 1024 : n;
+        if (cudaMalloc(&lat->d_sp, cap * sizeof(SweepParams)) != cudaSuccess) { cudaGetLastError(); return LATTICE_ENOMEM; }
+        lat->sp_cap = cap;
+    }
+    SweepParams *h = (SweepParams *)std::malloc(n * sizeof(SweepParams));
+    if (!h) return LATTICE_ENOMEM;
+    bool edge = false;
+    for (uint64_t k = 0; k < n; ++k) {
+        refresh_thresholds(lat, beta[k]);
+        const bool always4 = lat->thr64[0] >= TWO32, always8 = lat->thr64[1] >= TWO32;
+        SweepParams &p = h[k];
+        p.thr4 = always4 ? 0xffffffffu : (uint32_t)lat->thr64[0];
+        p.thr8 = always8 ? 0xffffffffu : (uint32_t)lat->thr64[1];
+        p.mask4 = always4 ? 0u : 0xffffffffu;
+        p.mask8 = always8 ? 0u : 0xffffffffu;
+        for (int q = 0; q < 8; ++q)
+            p.pcase[q] = ((p.thr4 >> (31 - q)) & 1u) | (((p.thr8 >> (31 - q)) & 1u) << 1);
+        edge = edge || always4 || always8;
+    }
+    // pageable source: the copy is staged before the call returns, so h can be freed right away
+    const cudaError_t ce = cudaMemcpyAsync(lat->d_sp, h, n * sizeof(SweepParams), cudaMemcpyHostToDevice, lat->stream);
+    std::free(h);
+    if (ce != cudaSuccess) return cuda_fail(lat, ce, "sweep parameter upload");
+
+    IsingMarchArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t;
+    a.R = march_rows(L, nq);
+    a.threads = nq * (L / a.R);
+    a.K = lat->K;
+    uint32_t *buf0 = lat->buf, *buf1 = lat->buf + pw;
+    const SweepParams *sp = lat->d_sp;
+    uint32_t ns = (uint32_t)n;
+    unsigned blocks = (a.threads + 255u) / 256u;
+    if (blocks > (unsigned)lat->persist_blocks) blocks = (unsigned)lat->persist_blocks;
+    void *args[] = {&a, &buf0, &buf1, &sp, &ns};
+    const void *fn = edge ? (const void *)ising_persist_kernel<true> : (const void *)ising_persist_kernel<false>;
+    const cudaError_t le = cudaLaunchCooperativeKernel(fn, dim3(blocks), dim3(256), args, 0, lat->stream);
+    if (le != cudaSuccess) return cuda_fail(lat, le, "cudaLaunchCooperativeKernel");
+    lat->launches += 1;
+    lat->t += n;
+    return LATTICE_OK;
+}
+
 int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta)
 {
     if (!lat || (n && !beta)) return LATTICE_EINVAL;
     if (lat->t + n >= TWO32) return LATTICE_EINVAL;
     for (uint64_t k = 0; k < n; ++k)
         if (std::isnan(beta[k]) || beta[k] < 0.0) return LATTICE_EINVAL;
-    for (uint64_t k = 0; k < n; ++k) {
-        refresh_thresholds(lat, beta[k]);
-        int rc = launch_half_sweep(lat, 0);      // black = (i+j) even first
-        if (rc) return rc;
-        rc = launch_half_sweep(lat, 1);
-        if (rc) return rc;
-        lat->t += 1;
+    for (uint64_t done = 0; done < n;) {
+        // cache-resident Ising lattices: up to 65536 sweeps per cooperative launch
+        const uint64_t chunk = n - done < 65536 ? n - done : 65536;
+        const int rc = sweep_persistent(lat, chunk, beta + done);
+        if (rc == LATTICE_OK) { done += chunk; continue; }
+        if (rc != 1) return rc;
+        for (uint64_t k = done; k < n; ++k) {
+            refresh_thresholds(lat, beta[k]);
+            int rc2 = launch_half_sweep(lat, 0);      // black = (i+j) even first
+            if (rc2) return rc2;
+            rc2 = launch_half_sweep(lat, 1);
+            if (rc2) return rc2;
+            lat->t += 1;
+        }
+        break;
     }
     return LATTICE_OK;
 }
@@ -825,6 +909,7 @@ int lattice_destroy(lattice_t *lat)
     if (!lat) return LATTICE_EINVAL;
     if (lat->d_cnt) cudaFree(lat->d_cnt);
     if (lat->d_win) cudaFree(lat->d_win);
+    if (lat->d_sp) cudaFree(lat->d_sp);
     delete lat;
     return LATTICE_OK;
 }

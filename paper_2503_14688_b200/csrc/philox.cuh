@@ -67,6 +67,9 @@ struct PlaneFold {
     uint32_t fb[8];           // ctr3(colour, tag, k) ^ k1[0], k = 0..7
 };
 
+#ifdef __CUDACC__
+__host__ __device__
+#endif
 static inline void build_plane_fold(const RoundKeys &K, uint32_t t, uint32_t colour, uint32_t tag,
                                     PlaneFold &f)
 {
