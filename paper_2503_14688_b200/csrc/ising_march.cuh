@@ -283,6 +283,45 @@ __device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g
     }
 }
 
+// One row per thread, for lattices too small to fill the GPU with marching threads (there the
+// time of a half-sweep is the latency of ONE thread's rows, so fewer rows per thread is faster
+// even though every thread now loads all three neighbour rows itself).  g enumerates
+// (row slot s, run q) with the even rows first and the odd rows after them, so that every warp
+// works on rows of one parity (wpr/4 * L/2 is a multiple of 32) and the branch is warp-uniform.
+template <int COLOUR, bool EDGE>
+__device__ __forceinline__ void row_thread(const IsingMarchArgs &a, uint32_t g, WarpTieQueue<false> &queue)
+{
+    const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2, half = L >> 1;
+    const uint32_t q = g % nq, s = g / nq;
+    const uint32_t i = s < half ? 2u * s : 2u * (s - half) + 1u;
+    const uint32_t kw = q << 2;
+    const uint32_t iu = (i == 0) ? L - 1 : i - 1, id = (i + 1 == L) ? 0 : i + 1;
+    const unsigned long long ro = (unsigned long long)i * wpr;
+    const uint4 U = *reinterpret_cast<const uint4 *>(a.opp + (unsigned long long)iu * wpr + kw);
+    const uint4 C = *reinterpret_cast<const uint4 *>(a.opp + ro + kw);
+    const uint4 D = *reinterpret_cast<const uint4 *>(a.opp + (unsigned long long)id * wpr + kw);
+    const uint32_t G = i * nq + q;
+    if (((i + COLOUR) & 1u) == 0) {
+        const uint32_t E = a.opp[ro + ((kw == 0) ? wpr - 1 : kw - 1)];
+        march_row<0, EDGE, false>(a, G, ro + kw, a.tgt + ro + kw, U, C, D, E, queue);
+    } else {
+        const uint32_t E = a.opp[ro + ((kw + 4 == wpr) ? 0 : kw + 4)];
+        march_row<1, EDGE, false>(a, G, ro + kw, a.tgt + ro + kw, U, C, D, E, queue);
+    }
+}
+
+template <int COLOUR, bool EDGE>
+__global__ void __launch_bounds__(256) ising_row_kernel(const IsingMarchArgs a)
+{
+    __shared__ uint4 s_q[8][TIE_Q_SLOTS];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t g = blockIdx.x * 256u + threadIdx.x;
+    if (g - lane >= a.threads) return;          // a.threads = wpr/4 * L, a multiple of 32
+    WarpTieQueue<false> queue{a, s_q[warp], lane, 0u};
+    row_thread<COLOUR, EDGE>(a, g, queue);
+    queue.drain();
+}
+
 template <int COLOUR, bool EDGE, bool SLAB>
 __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a)
 {

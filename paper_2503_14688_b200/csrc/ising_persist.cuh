@@ -8,7 +8,7 @@
 // dominates.  Here the grid is launched once (cudaLaunchCooperativeKernel, every block resident), loops over the
 // sweeps and colours itself and separates the half-sweeps with a grid-wide barrier; the lattice
 // stays in L2.  What is computed is exactly what n launches of ising_march_kernel compute: the
-// same march_thread() runs, with the per-half-sweep arguments (sweep index, colour, folded
+// same march_thread() (or, for the smallest lattices, row_thread()) runs, with the per-half-sweep arguments (sweep index, colour, folded
 // Philox constants, thresholds) rebuilt in shared memory by one thread per block from a
 // per-sweep table the host uploads.
 #pragma once
@@ -24,7 +24,7 @@ struct SweepParams {          // what changes from sweep to sweep (built on the 
 };
 
 #ifdef __CUDACC__
-template <bool EDGE>
+template <bool EDGE, bool ONE_ROW>
 __global__ void __launch_bounds__(256) ising_persist_kernel(const IsingMarchArgs a0, uint32_t *buf0,
                                                             uint32_t *buf1, const SweepParams *sp,
                                                             uint32_t n_sweeps)
@@ -55,8 +55,13 @@ __global__ void __launch_bounds__(256) ising_persist_kernel(const IsingMarchArgs
             __syncthreads();
             WarpTieQueue<false> queue{a, s_q[warp], lane, 0u};
             for (uint32_t g = blockIdx.x * 256u + threadIdx.x; g - lane < a0.threads; g += stride) {
-                if (colour == 0) march_thread<0, EDGE, false>(a, g, queue);
-                else march_thread<1, EDGE, false>(a, g, queue);
+                if (ONE_ROW) {
+                    if (colour == 0) row_thread<0, EDGE>(a, g, queue);
+                    else row_thread<1, EDGE>(a, g, queue);
+                } else {
+                    if (colour == 0) march_thread<0, EDGE, false>(a, g, queue);
+                    else march_thread<1, EDGE, false>(a, g, queue);
+                }
             }
             queue.drain();
             __threadfence();

@@ -133,6 +133,14 @@ uint32_t march_rows(uint32_t L, uint32_t nq)
     return 2;
 }
 
+// One row per thread (ising_row_kernel) when marching threads would not fill the GPU: the
+// half-sweep time is then one thread's latency, which is proportional to its rows.
+bool ising_one_row(const lattice *lat)
+{
+    const unsigned long long marching = (unsigned long long)(lat->wpr / 4u) * (lat->L / 2u);   // R = 2
+    return !lat->slab && marching < 148ull * 256ull;      // measured: helps up to L = 4096
+}
+
 int launch_ising_march(lattice *lat, int colour)
 {
     const uint32_t wpr = lat->wpr, nq = wpr / 4u;
@@ -163,6 +171,12 @@ int launch_ising_march(lattice *lat, int colour)
     if (lat->slab) {
         if (colour == 0) { if (edge) LAT_LAUNCH_MARCH(0, true, true); else LAT_LAUNCH_MARCH(0, false, true); }
         else { if (edge) LAT_LAUNCH_MARCH(1, true, true); else LAT_LAUNCH_MARCH(1, false, true); }
+    } else if (ising_one_row(lat)) {
+        a.R = 1;
+        a.threads = nq * lat->L;
+        const unsigned rb = (a.threads + 255u) / 256u;
+        if (colour == 0) { if (edge) ising_row_kernel<0, true><<<rb, 256, 0, lat->stream>>>(a); else ising_row_kernel<0, false><<<rb, 256, 0, lat->stream>>>(a); }
+        else { if (edge) ising_row_kernel<1, true><<<rb, 256, 0, lat->stream>>>(a); else ising_row_kernel<1, false><<<rb, 256, 0, lat->stream>>>(a); }
     } else {
         if (colour == 0) { if (edge) LAT_LAUNCH_MARCH(0, true, false); else LAT_LAUNCH_MARCH(0, false, false); }
         else { if (edge) LAT_LAUNCH_MARCH(1, true, false); else LAT_LAUNCH_MARCH(1, false, false); }
@@ -570,15 +584,19 @@ static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
         if (cudaGetDevice(&dev) != cudaSuccess ||
             cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop ||
             cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_persist_kernel<false>, 256, 0) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_persist_kernel<false, false>, 256, 0) != cudaSuccess ||
             per_sm < 1) {
             cudaGetLastError();
             lat->persist_blocks = -1;
             return 1;
         }
-        int per_sm_e = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_e, ising_persist_kernel<true>, 256, 0);
-        if (per_sm_e >= 1 && per_sm_e < per_sm) per_sm = per_sm_e;
+        int o[3] = {0, 0, 0};
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o[0], ising_persist_kernel<true, false>, 256, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o[1], ising_persist_kernel<false, true>, 256, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o[2], ising_persist_kernel<true, true>, 256, 0);
+        for (int k = 0; k < 3; ++k)
+            if (o[k] < per_sm) per_sm = o[k];
+        if (per_sm < 1) { lat->persist_blocks = -1; return 1; }
         lat->persist_blocks = per_sm * sms;
     }
     const uint32_t L = lat->L, wpr = lat->wpr, nq = wpr / 4u;
@@ -613,7 +631,8 @@ static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
     IsingMarchArgs a;
     std::memset(&a, 0, sizeof a);
     a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t;
-    a.R = march_rows(L, nq);
+    const bool one_row = ising_one_row(lat);
+    a.R = one_row ? 1u : march_rows(L, nq);
     a.threads = nq * (L / a.R);
     a.K = lat->K;
     uint32_t *buf0 = lat->buf, *buf1 = lat->buf + pw;
@@ -622,7 +641,8 @@ static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
     unsigned blocks = (a.threads + 255u) / 256u;
     if (blocks > (unsigned)lat->persist_blocks) blocks = (unsigned)lat->persist_blocks;
     void *args[] = {&a, &buf0, &buf1, &sp, &ns};
-    const void *fn = edge ? (const void *)ising_persist_kernel<true> : (const void *)ising_persist_kernel<false>;
+    const void *fn = one_row ? (edge ? (const void *)ising_persist_kernel<true, true> : (const void *)ising_persist_kernel<false, true>)
+                             : (edge ? (const void *)ising_persist_kernel<true, false> : (const void *)ising_persist_kernel<false, false>);
     const cudaError_t le = cudaLaunchCooperativeKernel(fn, dim3(blocks), dim3(256), args, 0, lat->stream);
     if (le != cudaSuccess) return cuda_fail(lat, le, "cudaLaunchCooperativeKernel");
     lat->launches += 1;
