@@ -59,7 +59,7 @@ BYTES_PER_UPDATE = {workloads.ISING: 0.375, workloads.BLUME_CAPEL: 0.75}
 ALG_HALF_RATE_INSTR_PER_UPDATE = {workloads.ISING: 2.98, workloads.BLUME_CAPEL: 4.46}
 EXE_HALF_RATE_INSTR_PER_UPDATE = {workloads.ISING: 3.39, workloads.BLUME_CAPEL: 5.30}
 #: DRAM bytes per update measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum) / updates
-DRAM_BYTES_PER_UPDATE_NCU = {workloads.ISING: 0.385, workloads.BLUME_CAPEL: 0.667}
+DRAM_BYTES_PER_UPDATE_NCU = {workloads.ISING: 0.383, workloads.BLUME_CAPEL: 0.667}
 SM_COUNT, HALF_RATE_LANES_PER_CLK_PER_SM = 148, 64
 KERNEL = {workloads.ISING: "ising_march_kernel", workloads.BLUME_CAPEL: "bc_march_kernel"}
 
