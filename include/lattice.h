@@ -117,6 +117,10 @@ int lattice_device_copy(void *device_dst, const void *device_src, size_t bytes, 
  * current device, so that the IPC handle maps the buffer itself), export it as a 64-byte CUDA IPC
  * handle (sent to the neighbours by any means, e.g. torch.distributed), and open a neighbour's
  * handle as a device pointer valid in this process.  Errors: EINVAL (NULL), ECUDA. */
+/* One process driving several GPUs: let kernels running on `device` store into memory of
+ * `peer_device` (cudaDeviceEnablePeerAccess; already-enabled is not an error).  ECUDA if the two
+ * devices cannot reach each other. */
+int lattice_enable_peer_access(int device, int peer_device);
 int lattice_device_alloc(void **device_ptr, size_t bytes);
 int lattice_device_free(void *device_ptr);
 int lattice_ipc_export(const void *device_ptr, unsigned char handle[64]);

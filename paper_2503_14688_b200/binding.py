@@ -34,6 +34,7 @@ SIGNATURES = {
     "lattice_slab_set_neighbours": (C.c_int, [_vp, _vp, C.c_uint32, _vp, C.c_uint32]),
     "lattice_view": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_uint32, _vp, C.c_size_t, _vp]),
     "lattice_device_copy": (C.c_int, [_vp, _vp, C.c_size_t, _vp]),
+    "lattice_enable_peer_access": (C.c_int, [C.c_int, C.c_int]),
     "lattice_device_alloc": (C.c_int, [C.POINTER(_vp), C.c_size_t]),
     "lattice_device_free": (C.c_int, [_vp]),
     "lattice_ipc_export": (C.c_int, [_vp, C.POINTER(C.c_ubyte)]),
@@ -86,6 +87,12 @@ class LatticeError(RuntimeError):
 
 def _p(a: np.ndarray, ty):
     return a.ctypes.data_as(C.POINTER(ty))
+
+
+def enable_peer_access(device: int, peer_device: int) -> None:
+    rc = lib().lattice_enable_peer_access(int(device), int(peer_device))
+    if rc != OK:
+        raise LatticeError("lattice_enable_peer_access", rc, f"{device} -> {peer_device}")
 
 
 def ipc_open(handle: bytes) -> int:

@@ -514,6 +514,20 @@ int lattice_device_copy(void *device_dst, const void *device_src, size_t bytes, 
                            (cudaStream_t)cuda_stream) == cudaSuccess ? LATTICE_OK : LATTICE_ECUDA;
 }
 
+int lattice_enable_peer_access(int device, int peer_device)
+{
+    if (device < 0 || peer_device < 0) return LATTICE_EINVAL;
+    if (device == peer_device) return LATTICE_OK;
+    int prev = 0, can = 0;
+    if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return LATTICE_ECUDA; }
+    if (cudaDeviceCanAccessPeer(&can, device, peer_device) != cudaSuccess || !can) { cudaGetLastError(); return LATTICE_ECUDA; }
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return LATTICE_ECUDA; }
+    const cudaError_t e = cudaDeviceEnablePeerAccess(peer_device, 0);
+    cudaGetLastError();                                   // clears "already enabled" too
+    cudaSetDevice(prev);
+    return (e == cudaSuccess || e == cudaErrorPeerAccessAlreadyEnabled) ? LATTICE_OK : LATTICE_ECUDA;
+}
+
 int lattice_device_alloc(void **device_ptr, size_t bytes)
 {
     if (!device_ptr || bytes == 0) return LATTICE_EINVAL;

@@ -9,8 +9,8 @@ different devices (NVLink P2P through NVSwitch), so the transfer rides on the up
 What this driver adds is ordering: every slab finishes colour c before any slab starts colour
 1 - c (stream order on one device, events across devices).
 
-One process drives all devices of the node (torch enables peer access on the first cross-device
-copy).  Random numbers are keyed by global (row, column): the result is bit-identical to the
+`ShardedLattice`: one process drives all devices of the node (peer access enabled explicitly);
+`SlabRank`: one process per GPU.  Random numbers are keyed by global (row, column): the result is bit-identical to the
 unsharded lattice for any number of slabs (tests/test_gpu_sharded.py).
 """
 from __future__ import annotations
@@ -37,10 +37,9 @@ class ShardedLattice:
         self._multi_device = len({str(s.device) for s in self.slabs}) > 1
         for k, s in enumerate(self.slabs):
             up, down = self.slabs[(k - 1) % n_slabs], self.slabs[(k + 1) % n_slabs]
-            if self._multi_device:
-                for nb in (up, down):                 # one tiny copy makes torch enable peer access
-                    if nb.device != s.device:
-                        s.buf[:16].copy_(nb.buf[:16].to(s.device, copy=True) * 0 + s.buf[:16])
+            for nb in (up, down):                     # kernels of s store into nb's halo rows
+                if nb.device != s.device:
+                    lat.enable_peer_access(s.device.index, nb.device.index)
             s.set_neighbours(up, down)
         self._t = 0
         self.synchronize()
