@@ -46,6 +46,8 @@ def lib() -> C.CDLL:
     sig = {
         "oracle_philox4x32_10": (None, [u32p, u32p, u32p]),
         "oracle_u32": (C.c_uint32, [C.c_uint64, C.c_int, C.c_uint32, C.c_int, C.c_uint64]),
+        "oracle_u64": (C.c_uint64, [C.c_uint64, C.c_uint32, C.c_int, C.c_uint64]),
+        "oracle_thresholds64": (None, [C.c_int, C.c_double, C.c_double, u64p, C.POINTER(C.c_ubyte)]),
         "oracle_proposal_bit": (C.c_int, [C.c_uint64, C.c_uint32, C.c_int, C.c_uint64]),
         "oracle_initial_spin": (C.c_int, [C.c_uint64, C.c_int, C.c_uint32, C.c_uint64, C.c_uint64]),
         "oracle_thresholds": (None, [C.c_int, C.c_double, C.c_double, u64p]),
@@ -92,6 +94,19 @@ def philox4x32_10(ctr, key) -> np.ndarray:
 
 def u32(seed, scheme, t, colour, P) -> int:
     return int(lib().oracle_u32(seed, scheme, t, colour, P))
+
+
+def u64(seed, t, colour, P) -> int:
+    return int(lib().oracle_u64(seed, t, colour, P))
+
+
+def thresholds64(model, delta, beta):
+    """(thr[n] on the 2^64 scale, always[n]) for scheme 2."""
+    n = 2 if model == ISING else 54
+    thr = np.zeros(n, dtype=np.uint64)
+    alw = np.zeros(n, dtype=np.uint8)
+    lib().oracle_thresholds64(model, float(delta), float(beta), _p(thr, C.c_uint64), _p(alw, C.c_ubyte))
+    return thr, alw
 
 
 def proposal_bit(seed, t, colour, P) -> int:

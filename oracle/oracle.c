@@ -91,6 +91,25 @@ uint32_t oracle_u32(uint64_t seed, int scheme, uint32_t t, int colour, uint64_t 
     return u;
 }
 
+/* Scheme 2 ("plane + 56-bit tail", 64-bit thresholds): the same top byte
+ * and the same tail block as scheme 1, but 56 tail bits instead of 24:
+ *   u64 = top byte << 56 | (tail word 0 >> 8) << 32 | tail word 1.
+ * Its top 32 bits are scheme 1's u32.  Lifts the 2^-32 floor on acceptance probabilities that
+ * PAPER.md:159 mentions to 2^-64. */
+uint64_t oracle_u64(uint64_t seed, uint32_t t, int colour, uint64_t P)
+{
+    uint32_t blk[4];
+    uint64_t u = 0;
+    for (int k = 0; k < 8; ++k) {
+        keyed_block(seed, P >> 7, t, colour, TAG_ACC_PLANE, k, blk);
+        u |= (uint64_t)lane_bit(blk, P) << (63 - k);
+    }
+    keyed_block(seed, P, t, colour, TAG_ACC_TAIL, 0, blk);
+    u |= (uint64_t)(blk[0] >> 8) << 32;
+    u |= (uint64_t)blk[1];
+    return u;
+}
+
 int oracle_proposal_bit(uint64_t seed, uint32_t t, int colour, uint64_t P)
 {
     uint32_t blk[4];
@@ -147,6 +166,39 @@ void oracle_thresholds(int model, double delta, double beta, uint64_t *out)
                 /* Eq. (1): dE = -(s2 - s)*h + Delta*(s2^2 - s^2) */
                 double dE = (double)(s - s2) * (double)h + delta * (double)(s2 * s2 - s * s);
                 out[(code * 2 + b) * 9 + (h + 4)] = threshold(beta, dE);
+            }
+}
+
+/* 64-bit thresholds (scheme 2): thr = floor(2^64 * exp(-beta*dE)); *always = 1 when dE <= 0 or
+ * the product rounds to 2^64 (then thr is meaningless).  exp() carries 53 significant bits and
+ * the scaling is exact, so floor(thr / 2^32) equals the 32-bit threshold of the same dE. */
+static uint64_t threshold64(double beta, double dE, unsigned char *always)
+{
+    *always = 0;
+    if (dE <= 0.0) { *always = 1; return 0; }
+    double p = exp(-(beta * dE));
+    double x = floor(ldexp(p, 64));
+    if (!(x > 0.0)) return 0;
+    if (x >= 18446744073709551616.0) { *always = 1; return 0; }
+    return (uint64_t)x;
+}
+
+void oracle_thresholds64(int model, double delta, double beta, uint64_t *thr, unsigned char *always)
+{
+    if (model == ORACLE_ISING) {
+        thr[0] = threshold64(beta, 4.0, &always[0]);
+        thr[1] = threshold64(beta, 8.0, &always[1]);
+        return;
+    }
+    for (int code = 0; code < 3; ++code)
+        for (int b = 0; b < 2; ++b)
+            for (int h = -4; h <= 4; ++h) {
+                int s = code - 1;
+                int code2 = (code + 1 + b) % 3;
+                int s2 = code2 - 1;
+                double dE = (double)(s - s2) * (double)h + delta * (double)(s2 * s2 - s * s);
+                int e = (code * 2 + b) * 9 + (h + 4);
+                thr[e] = threshold64(beta, dE, &always[e]);
             }
 }
 
@@ -208,7 +260,7 @@ int oracle_window_create(oracle_lattice_t **out, uint32_t Lg, int model, double 
 {
     if (!out || Lg < 2 || (Lg & 1u) || !valid_model(model) || !isfinite(delta)) return ORACLE_EINVAL;
     if (h < 1 || w < 1 || h > Lg || w > Lg || i0 >= Lg || j0 >= Lg || !spins) return ORACLE_EINVAL;
-    if (scheme != 0 && scheme != 1) return ORACLE_EINVAL;
+    if (scheme < 0 || scheme > 2) return ORACLE_EINVAL;
     if (outside < -1 || outside > 1 || (model == ORACLE_ISING && outside == 0)) return ORACLE_EINVAL;
     oracle_lattice_t *lat = (oracle_lattice_t *)calloc(1, sizeof *lat);
     if (!lat) return ORACLE_ENOMEM;
@@ -224,7 +276,7 @@ int oracle_window_create(oracle_lattice_t **out, uint32_t Lg, int model, double 
 
 int oracle_set_rng_scheme(oracle_lattice_t *lat, int scheme)
 {
-    if (!lat || (scheme != 0 && scheme != 1)) return ORACLE_EINVAL;
+    if (!lat || scheme < 0 || scheme > 2) return ORACLE_EINVAL;
     if (lat->t != 0) return ORACLE_ESTATE;
     lat->scheme = scheme;
     return ORACLE_OK;
@@ -258,8 +310,10 @@ int oracle_half_sweep(oracle_lattice_t *lat, int colour, double beta)
 {
     if (!lat || (colour != 0 && colour != 1) || isnan(beta) || beta < 0.0) return ORACLE_EINVAL;
     if (lat->t >= 0xffffffffull) return ORACLE_EINVAL;
-    uint64_t thr[54];
+    uint64_t thr[54], thr64[54];
+    unsigned char alw64[54];
     oracle_thresholds(lat->model, lat->delta, beta, thr);
+    oracle_thresholds64(lat->model, lat->delta, beta, thr64, alw64);
     const uint32_t t = (uint32_t)lat->t;
     const uint64_t half = lat->Lg / 2;
 
@@ -276,22 +330,32 @@ int oracle_half_sweep(oracle_lattice_t *lat, int colour, double beta)
             int hsum = spin_at(lat, a - 1, b) + spin_at(lat, a + 1, b) +
                        spin_at(lat, a, b - 1) + spin_at(lat, a, b + 1);
             uint64_t th;
-            int s_new;
+            int s_new, entry = -1;           /* entry: index into the tables, -1: dE <= 0 (Ising) */
             if (lat->model == ORACLE_ISING) {
                 /* 2. dE = 2*sigma*h in {-8,-4,0,4,8} */
                 int dE = 2 * s * hsum;
                 th = dE <= 0 ? ((uint64_t)1 << 32) : (dE == 4 ? thr[0] : thr[1]);
+                if (dE > 0) entry = dE == 4 ? 0 : 1;
                 s_new = -s;
             } else {
                 int bit = oracle_proposal_bit(lat->seed, t, colour, P);
                 int code = s + 1;
                 int code2 = (code + 1 + bit) % 3;
                 s_new = code2 - 1;
-                th = thr[(code * 2 + bit) * 9 + (hsum + 4)];
+                entry = (code * 2 + bit) * 9 + (hsum + 4);
+                th = thr[entry];
             }
-            /* 3. accept iff dE <= 0 (th = 2^32) or u32 < th */
-            uint32_t u = oracle_u32(lat->seed, lat->scheme, t, colour, P);
-            if ((uint64_t)u < th) lat->s[(uint64_t)a * lat->w + (uint64_t)b] = (int8_t)s_new;
+            int accept;
+            if (lat->scheme == 2) {
+                /* 3'. 64-bit compare: accept iff dE <= 0 / "always", or u64 < thr64 */
+                if (entry < 0 || alw64[entry]) accept = 1;
+                else accept = oracle_u64(lat->seed, t, colour, P) < thr64[entry];
+            } else {
+                /* 3. accept iff dE <= 0 (th = 2^32) or u32 < th */
+                uint32_t u = oracle_u32(lat->seed, lat->scheme, t, colour, P);
+                accept = (uint64_t)u < th;
+            }
+            if (accept) lat->s[(uint64_t)a * lat->w + (uint64_t)b] = (int8_t)s_new;
         }
     }
     return ORACLE_OK;

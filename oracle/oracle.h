@@ -46,7 +46,9 @@ void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t
 /* The acceptance random number of one site: a pure function of (seed, scheme, t, c, P).
  * P = i*(L/2) + (j>>1) is the same-colour linear index. */
 uint32_t oracle_u32(uint64_t seed, int scheme, uint32_t t, int colour, uint64_t P);
-/* Blume-Capel proposal bit of one site (both schemes). */
+/* Scheme 2: the 64-bit acceptance number of one site (top 32 bits = scheme 1's u32). */
+uint64_t oracle_u64(uint64_t seed, uint32_t t, int colour, uint64_t P);
+/* Blume-Capel proposal bit of one site (all schemes). */
 int oracle_proposal_bit(uint64_t seed, uint32_t t, int colour, uint64_t P);
 /* Initial spin (-1/0/+1) of global site (i,j) for a lattice of side L. */
 int oracle_initial_spin(uint64_t seed, int model, uint32_t L, uint64_t i, uint64_t j);
@@ -55,6 +57,9 @@ int oracle_initial_spin(uint64_t seed, int model, uint32_t L, uint64_t i, uint64
  * Ising: out[0] = thr(dE=4), out[1] = thr(dE=8).
  * Blume-Capel: out[(code*2+b)*9 + (h+4)], 54 entries. */
 void oracle_thresholds(int model, double delta, double beta, uint64_t *out);
+/* Scheme 2: thresholds on the 2^64 scale, same indexing; always[e] = 1 where the move is always
+ * accepted (dE <= 0 or the product rounds to 2^64). */
+void oracle_thresholds64(int model, double delta, double beta, uint64_t *thr, unsigned char *always);
 
 /* Whole periodic L x L lattice (any even L >= 2), disordered start, t = 0. */
 int oracle_create(oracle_lattice_t **out, uint32_t L, int model, double delta, uint64_t seed);
@@ -65,7 +70,7 @@ int oracle_create(oracle_lattice_t **out, uint32_t L, int model, double delta, u
 int oracle_window_create(oracle_lattice_t **out, uint32_t Lg, int model, double delta,
                          uint64_t seed, int scheme, uint64_t t0, uint64_t i0, uint64_t j0,
                          uint32_t h, uint32_t w, const int8_t *spins, int outside);
-int oracle_set_rng_scheme(oracle_lattice_t *, int scheme);      /* 0 = quad, 1 = plane+tail */
+int oracle_set_rng_scheme(oracle_lattice_t *, int scheme);      /* 0 = quad, 1 = plane+tail, 2 = plane+tail56 */
 int oracle_sweep(oracle_lattice_t *, uint64_t n, const double *beta);
 /* One colour of sweep t at inverse temperature beta; does not advance t.  A sweep is
  * half_sweep(0) then half_sweep(1) then t += 1. */

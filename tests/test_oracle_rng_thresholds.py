@@ -213,3 +213,59 @@ def test_detailed_balance_from_threshold_table_ising_4x4():
             np.add.at(new, y, w)
         pi = new
     assert np.allclose(pi, ex["prob"], rtol=1e-7, atol=1e-15)
+
+
+# ---- scheme 2: 56-bit tails and 64-bit thresholds ----------------------
+BETA_C = math.log(1.0 + math.sqrt(2.0)) / 2.0
+def test_scheme2_u64_extends_scheme1_u32():
+    """u64 = top byte | 56 tail bits: its top 32 bits are scheme 1's u32, the next 32 bits are
+    word 1 of the site's own tail block."""
+    seed = 2503146884
+    for t, c, P in [(0, 0, 0), (5, 1, 12345), (2 ** 31 + 7, 0, 2 ** 38 + 99), (17, 1, 127), (17, 1, 128)]:
+        u = oracle.u64(seed, t, c, P)
+        assert u >> 32 == oracle.u32(seed, 1, t, c, P)
+        tail = oracle.philox4x32_10([P & 0xFFFFFFFF, P >> 32, t, c | (4 << 8)],
+                                    [seed & 0xFFFFFFFF, seed >> 32])
+        assert u & 0xFFFFFFFF == int(tail[1])
+
+
+def test_thresholds64_refine_the_32_bit_table():
+    """floor(thr64 / 2^32) == thr32 entry by entry (same fp64 exp, exact scaling), "always" flags
+    agree except where only the 32-bit product rounds up, and closed forms at beta_c hold to the
+    53 bits exp() carries."""
+    import math
+    from fractions import Fraction
+    for model, delta, beta in [(oracle.ISING, 0.0, BETA_C), (oracle.BLUME_CAPEL, 0.0, 1 / 1.6934),
+                               (oracle.BLUME_CAPEL, 0.7, 0.9), (oracle.ISING, 0.0, 1e-12)]:
+        t32 = oracle.thresholds(model, delta, beta)
+        t64, alw = oracle.thresholds64(model, delta, beta)
+        for a, b, f in zip(t32, t64, alw):
+            if f:
+                assert int(a) == 2 ** 32
+            elif int(a) < 2 ** 32:
+                assert int(b) >> 32 == int(a)
+    t64, alw = oracle.thresholds64(oracle.ISING, 0.0, BETA_C)
+    r2 = Fraction(math.isqrt(2 * 10 ** 60), 10 ** 30)        # sqrt 2 to 30 digits
+    for thr, power in zip(t64, (2, 4)):
+        exact = (r2 - 1) ** power * 2 ** 64
+        assert abs(int(thr) - exact) / exact < 2 ** -50
+    # low temperature: the 32-bit table says "never", the 64-bit one still has a probability
+    t32 = oracle.thresholds(oracle.ISING, 0.0, 3.0)
+    t64, alw = oracle.thresholds64(oracle.ISING, 0.0, 3.0)
+    assert int(t32[1]) == 0 and int(t64[1]) == math.floor(math.ldexp(math.exp(-24.0), 64)) > 0
+    t64, alw = oracle.thresholds64(oracle.ISING, 0.0, 0.0)
+    assert alw.tolist() == [1, 1]
+    t64, alw = oracle.thresholds64(oracle.ISING, 0.0, math.inf)
+    assert t64.tolist() == [0, 0] and alw.tolist() == [0, 0]
+
+
+@pytest.mark.parametrize("model,beta", [(oracle.ISING, BETA_C), (oracle.BLUME_CAPEL, 1 / 1.6934)])
+def test_scheme2_trajectory_equals_scheme1_when_no_32_bit_tie_occurs(model, beta):
+    """The decisions of schemes 1 and 2 differ only if u32 == thr32 (probability 2^-32 per
+    decision): on a small run the trajectories are identical, which pins the 64-bit path to the
+    pinned 32-bit one."""
+    a = oracle.OracleLattice(32, model, 0.0, seed=11, scheme=1)
+    b = oracle.OracleLattice(32, model, 0.0, seed=11, scheme=2)
+    a.sweep([beta] * 200)
+    b.sweep([beta] * 200)
+    assert np.array_equal(a.get_spins(), b.get_spins())
