@@ -132,6 +132,12 @@ int lattice_ipc_close(void *device_ptr);
  *   1 "plane+tail": top 8 bits from 8 bit-plane blocks shared by 128 sites, low 24 bits from a
  *                   per-site block that is only evaluated when the top byte ties with the
  *                   threshold's.  Same statistics, ~4x less RNG work.
+ *   2 "plane+tail56": scheme 1 with 64-bit thresholds floor(2^64 exp(-beta dE)) and 56 tail bits
+ *                   (words 0 and 1 of the same tail block): u64 = top byte | 56 tail bits; lifts the
+ *                   2^-32 floor on acceptance probabilities to 2^-64.  Identical to
+ *                   scheme 1 unless u32 == thr32.  Marching kernels only: EINVAL unless L is a
+ *                   multiple of 256; Blume-Capel half-sweeps return EINVAL for tables without the
+ *                   Delta = 0 structure.
  * Only allowed at t == 0 (ESTATE otherwise).  EINVAL for an unknown scheme. */
 int lattice_set_rng_scheme(lattice_t *lat, int scheme);
 
@@ -189,6 +195,9 @@ uint64_t lattice_launches(const lattice_t *lat);
  *   ascending fp64 sums; returns 0 if r_cut < 1; *r_cut_out (may be NULL) receives r_cut.
  * lattice_energy: e = -(Sx[0]+Sy[0])/L^2 + delta*Q/L^2. */
 void lattice_thresholds(int model, double delta, double beta, uint64_t *out);
+/* Scheme 2: thresholds on the 2^64 scale (same indexing); always[e] = 1 where the move is always
+ * accepted (dE <= 0, or the product rounds to 2^64), thr[e] is then 0. */
+void lattice_thresholds64(int model, double delta, double beta, uint64_t *thr, unsigned char *always);
 double lattice_xi(const int64_t *Sx, const int64_t *Sy, uint32_t r_max, int64_t Q, uint32_t L,
                   uint32_t *r_cut_out);
 double lattice_energy(const int64_t *Sx, const int64_t *Sy, int64_t Q, double delta, uint32_t L);

@@ -4,9 +4,9 @@ The product is the C-ABI CUDA library `liblattice.so` (include/lattice.h, csrc/)
 is its thin Python binding plus the seeded workload definitions.  There is no CPU fallback.
 """
 from .binding import (BLUME_CAPEL, ISING, Lattice, LatticeError, energy, lib, state_bytes,
-                      thresholds, xi)
+                      thresholds, thresholds64, xi)
 from .buildlib import build
 from . import replicas, workloads
 
 __all__ = ["ISING", "BLUME_CAPEL", "Lattice", "LatticeError", "energy", "lib", "state_bytes",
-           "thresholds", "xi", "build", "workloads", "replicas"]
+           "thresholds", "thresholds64", "xi", "build", "workloads", "replicas"]

@@ -53,6 +53,7 @@ SIGNATURES = {
     "lattice_set_time": (C.c_int, [_vp, C.c_uint64]),
     "lattice_launches": (C.c_uint64, [_vp]),
     "lattice_thresholds": (None, [C.c_int, C.c_double, C.c_double, _u64p]),
+    "lattice_thresholds64": (None, [C.c_int, C.c_double, C.c_double, _u64p, C.POINTER(C.c_ubyte)]),
     "lattice_xi": (C.c_double, [_i64p, _i64p, C.c_uint32, C.c_int64, C.c_uint32, _u32p]),
     "lattice_energy": (C.c_double, [_i64p, _i64p, C.c_int64, C.c_double, C.c_uint32]),
     "lattice_destroy": (C.c_int, [_vp]),
@@ -117,6 +118,15 @@ def thresholds(model: int, delta: float, beta: float) -> np.ndarray:
     out = np.zeros(2 if model == ISING else 54, dtype=np.uint64)
     lib().lattice_thresholds(model, float(delta), float(beta), _p(out, C.c_uint64))
     return out
+
+
+def thresholds64(model: int, delta: float, beta: float):
+    """(thr, always) of RNG scheme 2: thresholds on the 2^64 scale."""
+    n = 2 if model == ISING else 54
+    thr = np.zeros(n, dtype=np.uint64)
+    alw = np.zeros(n, dtype=np.uint8)
+    lib().lattice_thresholds64(model, float(delta), float(beta), _p(thr, C.c_uint64), _p(alw, C.c_ubyte))
+    return thr, alw
 
 
 def xi(Sx, Sy, Q: int, L: int):

@@ -40,7 +40,8 @@ struct BCMarchArgs {
     uint32_t threads;               // (wpr/4) * (L/R), a multiple of 32
     uint32_t lut[8];                // truth table of threshold bit (31-k) over (F, Y1, H0)
     uint32_t lut_always;            // truth table of "threshold == 2^32" over (F, Y1, H0)
-    uint32_t thr[8];                // threshold of class (F<<2 | Y1<<1 | H0) (low 24 bits used)
+    unsigned long long thr[8];      // threshold of class (F<<2 | Y1<<1 | H0) on the 2^64 scale (scheme 1:
+                                    // thr32 << 32); the low 56 bits are compared with the 56 tail bits
     uint32_t fbp;                   // folded counter word of the PROP plane
     PlaneFold F;                    // folded ACC_PLANE stream of (t, colour)
     RoundKeys K;
@@ -106,7 +107,8 @@ struct BCTieQueue {
             const unsigned long long P = ((SLAB ? wo + a.p_off : wo) << 5) + bit;
             const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
                                             a.colour | (TAG_ACC_TAIL << 8), a.K);
-            if ((blk.x >> 8) < (a.thr[cls] & 0x00ffffffu)) hit |= 1u << bit;
+            const unsigned long long u56 = ((unsigned long long)(blk.x >> 8) << 32) | blk.y;
+            if (u56 < (a.thr[cls] & 0x00ffffffffffffffull)) hit |= 1u << bit;
         }
         const uint32_t dnz = hit & e1.x, dsg = hit & e1.y;
         if (dnz) atomicXor(a.tnz + wo, dnz);

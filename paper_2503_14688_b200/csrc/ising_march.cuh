@@ -42,7 +42,8 @@ struct IsingMarchArgs {
     uint32_t *mir_up;         // where the first / last own row of tgt is mirrored: the neighbour
     uint32_t *mir_dn;         // slabs' halo rows (possibly peer-GPU memory), same [wpr] layout
     uint32_t t, colour;
-    uint32_t thr4, thr8;      // thresholds for dE = 4, 8 (low 24 bits used by the tails)
+    unsigned long long thr4, thr8;   // thresholds for dE = 4, 8 on the 2^64 scale (scheme 1: thr32 << 32):
+                              // top byte -> pcase, low 56 bits -> compared with the 56 tail bits
     uint32_t mask4, mask8;    // 0 if the class flips unconditionally (threshold == 2^32), else ~0
     uint32_t pcase[8];        // plane k: bit_k(thr4) | bit_k(thr8) << 1, bit_k = bit (31-k)
     uint32_t R;               // rows per thread (even, divides L)
@@ -135,8 +136,11 @@ struct WarpTieQueue {
             const unsigned long long P = ((SLAB ? wo + a.p_off : wo) << 5) + bit;
             const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
                                             a.colour | (TAG_ACC_TAIL << 8), a.K);
-            const uint32_t thr = ((e.y >> bit) & 1u) ? a.thr8 : a.thr4;
-            if ((blk.x >> 8) < (thr & 0x00ffffffu)) flip |= 1u << bit;
+            // low 56 bits: (tail word 0 >> 8) : tail word 1 against the threshold's (for scheme 1
+            // the threshold's low word is 0, so word 1 never decides: u32 < thr32 exactly)
+            const unsigned long long thr = ((e.y >> bit) & 1u) ? a.thr8 : a.thr4;
+            const unsigned long long u56 = ((unsigned long long)(blk.x >> 8) << 32) | blk.y;
+            if (u56 < (thr & 0x00ffffffffffffffull)) flip |= 1u << bit;
         }
         if (flip) {
             atomicXor(a.tgt + wo, flip);

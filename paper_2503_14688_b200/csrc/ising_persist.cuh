@@ -19,7 +19,8 @@
 namespace lat {
 
 struct SweepParams {          // what changes from sweep to sweep (built on the host, fp64 -> u32)
-    uint32_t thr4, thr8, mask4, mask8;
+    unsigned long long thr4, thr8;
+    uint32_t mask4, mask8;
     uint32_t pcase[8];
 };
 

@@ -46,7 +46,9 @@ struct lattice {
     // cached thresholds
     bool have_beta;
     double beta;
-    uint64_t thr64[54];
+    uint64_t thr64[54];        // 32-bit scale, 2^32 = always (schemes 0, 1; lattice_thresholds)
+    uint64_t thrT[54];         // the marching kernels' thresholds on the 2^64 scale (scheme 1: thr64 << 32)
+    bool alwT[54];             // ... and their "always accept" flags
     // device scratch
     unsigned long long *d_cnt;
     size_t cnt_cap;            // entries
@@ -87,6 +89,34 @@ uint64_t threshold_of(double beta, double dE)
     return (uint64_t)x;
 }
 
+// scheme 2: floor(2^64 exp(-beta dE)); *always when dE <= 0 or the product rounds to 2^64
+uint64_t threshold64_of(double beta, double dE, bool *always)
+{
+    *always = false;
+    if (dE <= 0.0) { *always = true; return 0; }
+    const double x = std::floor(std::ldexp(std::exp(-(beta * dE)), 64));
+    if (!(x > 0.0)) return 0;
+    if (x >= 18446744073709551616.0) { *always = true; return 0; }
+    return (uint64_t)x;
+}
+
+void build_thresholds64(int model, double delta, double beta, uint64_t *thr, bool *always)
+{
+    if (model == LATTICE_ISING) {
+        thr[0] = threshold64_of(beta, 4.0, &always[0]);
+        thr[1] = threshold64_of(beta, 8.0, &always[1]);
+        return;
+    }
+    for (int code = 0; code < 3; ++code)
+        for (int b = 0; b < 2; ++b)
+            for (int h = -4; h <= 4; ++h) {
+                const int s = code - 1, s2 = (code + 1 + b) % 3 - 1;
+                const double dE = (double)(s - s2) * (double)h + delta * (double)(s2 * s2 - s * s);
+                const int e = (code * 2 + b) * 9 + (h + 4);
+                thr[e] = threshold64_of(beta, dE, &always[e]);
+            }
+}
+
 void build_thresholds(int model, double delta, double beta, uint64_t *out)
 {
     if (model == LATTICE_ISING) {
@@ -108,6 +138,16 @@ void refresh_thresholds(lattice *lat, double beta)
     // bitwise comparison so that -0.0 / +0.0 or any other pair of distinct doubles rebuilds
     if (lat->have_beta && std::memcmp(&lat->beta, &beta, sizeof beta) == 0) return;
     build_thresholds(lat->model, lat->delta, beta, lat->thr64);
+    const int n = lat->model == LATTICE_ISING ? 2 : 54;
+    if (lat->scheme == 2) {
+        build_thresholds64(lat->model, lat->delta, beta, lat->thrT, lat->alwT);
+    } else {
+        // u32 < thr32  <=>  (u32 << 32 | anything) < (thr32 << 32): one 64-bit compare serves both
+        for (int e = 0; e < n; ++e) {
+            lat->alwT[e] = lat->thr64[e] >= TWO32;
+            lat->thrT[e] = lat->alwT[e] ? 0 : lat->thr64[e] << 32;
+        }
+    }
     lat->beta = beta;
     lat->have_beta = true;
 }
@@ -154,13 +194,13 @@ int launch_ising_march(lattice *lat, int colour)
     a.p_off = lat->slab ? ((long long)lat->row0 - 1) * (long long)wpr : 0;
     a.mir_up = lat->slab ? lat->mir_up[colour][0] : nullptr;
     a.mir_dn = lat->slab ? lat->mir_dn[colour][0] : nullptr;
-    const bool always4 = lat->thr64[0] >= TWO32, always8 = lat->thr64[1] >= TWO32;
-    a.thr4 = always4 ? 0xffffffffu : (uint32_t)lat->thr64[0];
-    a.thr8 = always8 ? 0xffffffffu : (uint32_t)lat->thr64[1];
+    const bool always4 = lat->alwT[0], always8 = lat->alwT[1];
+    a.thr4 = lat->thrT[0];
+    a.thr8 = lat->thrT[1];
     a.mask4 = always4 ? 0u : 0xffffffffu;
     a.mask8 = always8 ? 0u : 0xffffffffu;
     for (int p = 0; p < 8; ++p)
-        a.pcase[p] = ((a.thr4 >> (31 - p)) & 1u) | (((a.thr8 >> (31 - p)) & 1u) << 1);
+        a.pcase[p] = (uint32_t)((a.thr4 >> (63 - p)) & 1u) | ((uint32_t)((a.thr8 >> (63 - p)) & 1u) << 1);
     a.R = march_rows(lat->n_own, nq);
     a.threads = nq * (lat->n_own / a.R);
     a.K = lat->K;
@@ -202,9 +242,11 @@ bool bc_table_is_integer_dE(const lattice *lat)
 {
     for (int type = 0; type < 3; ++type)
         for (int x = -4; x <= 0; ++x)
-            if (lat->thr64[bc_entry(type, x)] < TWO32) return false;
+            if (!lat->alwT[bc_entry(type, x)]) return false;
     for (int x = 1; x <= 4; ++x)
-        if (lat->thr64[bc_entry(BC_VACATE, x)] != lat->thr64[bc_entry(BC_OCCUPY, x)]) return false;
+        if (lat->thrT[bc_entry(BC_VACATE, x)] != lat->thrT[bc_entry(BC_OCCUPY, x)] ||
+            lat->alwT[bc_entry(BC_VACATE, x)] != lat->alwT[bc_entry(BC_OCCUPY, x)])
+            return false;
     return true;
 }
 
@@ -232,11 +274,11 @@ int launch_bc_march(lattice *lat, int colour)
     for (int F = 0; F < 2; ++F)
         for (int x = 1; x <= 4; ++x) {
             const uint32_t cls = (uint32_t)(F << 2) | (uint32_t)((x >= 3) << 1) | (uint32_t)(x & 1);
-            const uint64_t th = lat->thr64[bc_entry(F ? BC_FLIP : BC_VACATE, x)];
-            if (th >= TWO32) { a.lut_always |= 1u << cls; a.thr[cls] = 0xffffffffu; continue; }
-            a.thr[cls] = (uint32_t)th;
+            const int e = bc_entry(F ? BC_FLIP : BC_VACATE, x);
+            a.thr[cls] = lat->thrT[e];
+            if (lat->alwT[e]) { a.lut_always |= 1u << cls; continue; }
             for (int k = 0; k < 8; ++k)
-                if ((th >> (31 - k)) & 1u) a.lut[k] |= 1u << cls;
+                if ((lat->thrT[e] >> (63 - k)) & 1u) a.lut[k] |= 1u << cls;
         }
     a.K = lat->K;
     build_plane_fold(lat->K, a.t, a.colour, TAG_ACC_PLANE, a.F);
@@ -265,11 +307,12 @@ int launch_half_sweep(lattice *lat, int colour)
         if (!bc_table_is_integer_dE(lat)) return LATTICE_EINVAL;
         return launch_bc_march(lat, colour);
     }
-    if (lat->model == LATTICE_BLUME_CAPEL && lat->scheme == 1 && (lat->wpr % 4u) == 0 &&
+    if (lat->model == LATTICE_BLUME_CAPEL && lat->scheme >= 1 && (lat->wpr % 4u) == 0 &&
         bc_table_is_integer_dE(lat))
         return launch_bc_march(lat, colour);
-    if (lat->model == LATTICE_ISING && lat->scheme == 1 && (lat->wpr % 4u) == 0)
+    if (lat->model == LATTICE_ISING && lat->scheme >= 1 && (lat->wpr % 4u) == 0)
         return launch_ising_march(lat, colour);
+    if (lat->scheme == 2) return LATTICE_EINVAL;      // the generic kernels compare 32 bits only
     const uint32_t L = lat->L, wpr = lat->wpr;
     const size_t pw = (size_t)L * wpr;
     const bool v4 = (wpr % 4u) == 0;
@@ -571,10 +614,12 @@ int lattice_ipc_close(void *device_ptr)
 
 int lattice_set_rng_scheme(lattice_t *lat, int scheme)
 {
-    if (!lat || (scheme != 0 && scheme != 1)) return LATTICE_EINVAL;
+    if (!lat || scheme < 0 || scheme > 2) return LATTICE_EINVAL;
     if (lat->t != 0) return LATTICE_ESTATE;
-    if (lat->slab && scheme != 1) return LATTICE_EINVAL;
+    if (lat->slab && scheme == 0) return LATTICE_EINVAL;
+    if (scheme == 2 && (lat->wpr % 4u) != 0) return LATTICE_EINVAL;   // marching kernels only
     lat->scheme = scheme;
+    lat->have_beta = false;                                           // thresholds depend on the scheme
     return LATTICE_OK;
 }
 
@@ -590,7 +635,7 @@ int lattice_half_sweep(lattice_t *lat, int colour, double beta)
 // Returns 1 if the path does not apply (the caller then launches the half-sweeps one by one).
 static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
 {
-    if (lat->model != LATTICE_ISING || lat->scheme != 1 || lat->slab || lat->view || (lat->wpr % 4u) != 0 ||
+    if (lat->model != LATTICE_ISING || lat->scheme < 1 || lat->slab || lat->view || (lat->wpr % 4u) != 0 ||
         lat->L > 8192u || n < 2 || lat->persist_blocks < 0)
         return 1;
     if (lat->persist_blocks == 0) {
@@ -627,14 +672,14 @@ static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
     bool edge = false;
     for (uint64_t k = 0; k < n; ++k) {
         refresh_thresholds(lat, beta[k]);
-        const bool always4 = lat->thr64[0] >= TWO32, always8 = lat->thr64[1] >= TWO32;
+        const bool always4 = lat->alwT[0], always8 = lat->alwT[1];
         SweepParams &p = h[k];
-        p.thr4 = always4 ? 0xffffffffu : (uint32_t)lat->thr64[0];
-        p.thr8 = always8 ? 0xffffffffu : (uint32_t)lat->thr64[1];
+        p.thr4 = lat->thrT[0];
+        p.thr8 = lat->thrT[1];
         p.mask4 = always4 ? 0u : 0xffffffffu;
         p.mask8 = always8 ? 0u : 0xffffffffu;
         for (int q = 0; q < 8; ++q)
-            p.pcase[q] = ((p.thr4 >> (31 - q)) & 1u) | (((p.thr8 >> (31 - q)) & 1u) << 1);
+            p.pcase[q] = (uint32_t)((p.thr4 >> (63 - q)) & 1u) | ((uint32_t)((p.thr8 >> (63 - q)) & 1u) << 1);
         edge = edge || always4 || always8;
     }
     // pageable source: the copy is staged before the call returns, so h can be freed right away
@@ -910,6 +955,15 @@ void lattice_thresholds(int model, double delta, double beta, uint64_t *out)
 {
     if (!out || !model_ok(model)) return;
     build_thresholds(model, delta, beta, out);
+}
+
+void lattice_thresholds64(int model, double delta, double beta, uint64_t *thr, unsigned char *always)
+{
+    if (!thr || !always || !model_ok(model)) return;
+    bool a[54];
+    build_thresholds64(model, delta, beta, thr, a);
+    const int n = model == LATTICE_ISING ? 2 : 54;
+    for (int e = 0; e < n; ++e) always[e] = a[e] ? 1 : 0;
 }
 
 double lattice_xi(const int64_t *Sx, const int64_t *Sy, uint32_t r_max, int64_t Q, uint32_t L,

@@ -166,3 +166,14 @@ def test_view_and_copy_argument_checks():
     assert L.lattice_destroy(h) == lat.binding.OK
     assert L.lattice_device_copy(None, fake, 16, None) == lat.binding.EINVAL
     assert L.lattice_device_copy(fake, fake, 0, None) == lat.binding.OK
+
+
+@pytest.mark.parametrize("model,delta", [(lat.ISING, 0.0), (lat.BLUME_CAPEL, 0.0), (lat.BLUME_CAPEL, -1.3),
+                                         (lat.BLUME_CAPEL, 0.7)])
+def test_thresholds64_equal_oracle(model, delta):
+    """RNG scheme 2: the library's 64-bit thresholds equal the oracle's, entry by entry."""
+    import math
+    for beta in (0.0, 1e-12, 0.2, workloads.BETA_C_ISING, workloads.BETA_BC, 1.0, 3.0, 11.0, 50.0, math.inf):
+        tg, ag = lat.thresholds64(model, delta, beta)
+        to, ao = oracle.thresholds64(model, delta, beta)
+        assert np.array_equal(tg, to) and np.array_equal(ag, ao), beta

@@ -272,6 +272,37 @@ def test_fill_ordered_states_and_sweep_from_them(model):
         g.fill(2)
 
 
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+@pytest.mark.parametrize("L", [256, 512, 1024])
+def test_scheme2_64_bit_thresholds(L, model):
+    """RNG scheme 2 (56-bit tails, 64-bit thresholds) against the oracle's scheme 2, including
+    temperatures so low that the 32-bit table has only zeros where the 64-bit one does not."""
+    g = lat.Lattice(L, model, 0.0, 2024 + L, scheme=2)
+    o = oracle.OracleLattice(L, model, 0.0, 2024 + L, scheme=2)
+    bc = BETA_C if model == lat.ISING else workloads.BETA_BC
+    beta = [bc] * 8 + [3.0, 3.0, 0.0, 0.05, 25.0, math.inf] + [bc / 1.01] * 8
+    g.sweep(beta[:5])                       # several calls: launch path and persistent path
+    g.sweep(beta[5:6])
+    g.sweep(beta[6:])
+    o.sweep(beta)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    _same_measure(g, o, 32, L)
+    # scheme 2 differs from scheme 1 only on a 2^-32 tie: same trajectory here
+    g1 = lat.Lattice(L, model, 0.0, 2024 + L, scheme=1)
+    g1.sweep(beta)
+    assert np.array_equal(g.get_spins(), g1.get_spins())
+    g.close(); g1.close(); o.close()
+
+
+def test_scheme2_needs_marching_kernels():
+    with pytest.raises(lat.LatticeError):
+        lat.Lattice(64, lat.ISING, 0.0, 1, scheme=2)                 # L not a multiple of 256
+    b = lat.Lattice(256, lat.BLUME_CAPEL, 0.5, 1, scheme=2)          # Delta != 0: generic table
+    with pytest.raises(lat.LatticeError):
+        b.sweep([0.5])
+    b.close()
+
+
 def test_randomised_parity_sweep_of_parameters():
     """Seeded random (model, L, scheme, beta schedule, Delta, seed) cases: spins and counts after a
     few sweeps, bit for bit.  Covers the generic kernels (L not a multiple of 256, scheme 0,
