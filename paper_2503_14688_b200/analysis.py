@@ -1,0 +1,162 @@
+"""Estimator layer: from many independent runs to xi(t) and z.
+
+Host-side fp64 analysis of the integer counts the CUDA path returns; nothing here touches the
+device.  It restates the procedures of the paper:
+
+* errors by the jackknife over independent realisations (App. C, D);
+* the coherence length xi = I_2 / I_1, I_n = int_0^inf r^n C(r) dr (Eq. C1) with
+  the paper's three steps: (i) r_cut where C(r_cut + 1) drops below three
+  times its error; (ii) r* = argmax r^2 C, r_min / r_max the first r where r^2 C falls below
+  0.9 / (1/3) of that maximum; (iii) if r_max - r_min <= 8 integrate the data up to r_cut, else
+  fit F(r) = A exp[-(r/xi_F)^beta] / sqrt(r) (Eq. C2) on [r_min, r_max], integrate the data up
+  to r_max and F from r_max to 20 xi_F.  Our C(r) is dense in r (reading 9), so the
+  paper's cubic-spline interpolation of a sparse r-grid is not needed;
+* the dynamic exponent z from log t = z log xi + b + b' xi^(-omega), omega = 1.75 (Eq. 5 / D1,
+  PAPER.md:75-81, 223-225), least squares with the error of xi propagated through the
+  derivative of the fitting function, chi^2/dof and the fit quality
+  Q = Gamma(dof/2, chi^2/2) / Gamma(dof/2), errors by the jackknife.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+OMEGA = 1.75          # corrections-to-scaling exponent used by the paper
+
+
+def jackknife(samples: np.ndarray, estimator=None):
+    """samples[run, ...] -> (estimate on the mean of all runs, jackknife error).
+
+    estimator maps the mean over a set of runs to the quantity of interest (default: identity).
+    Leave-one-out means; error^2 = (N-1)/N * sum (theta_i - theta_bar)^2."""
+    x = np.asarray(samples, dtype=np.float64)
+    n = x.shape[0]
+    if n < 2:
+        raise ValueError("the jackknife needs at least two runs")
+    f = (lambda a: a) if estimator is None else estimator
+    total = x.sum(axis=0)
+    full = np.asarray(f(total / n), dtype=np.float64)
+    loo = np.array([np.asarray(f((total - x[i]) / (n - 1)), dtype=np.float64) for i in range(n)])
+    err = np.sqrt((n - 1) / n * ((loo - loo.mean(axis=0)) ** 2).sum(axis=0))
+    return full, err
+
+
+def correlation(Sx, Sy, L: int, Q=None) -> np.ndarray:
+    """C(r) for r = 0..r_max from the axis sums of one run: C(0) = Q / L^2 (1 for Ising),
+    C(r) = (S_x(r) + S_y(r)) / (2 L^2) (reading 10)."""
+    n = float(L) * float(L)
+    c0 = 1.0 if Q is None else float(Q) / n
+    return np.concatenate([[c0], (np.asarray(Sx, np.float64) + np.asarray(Sy, np.float64)) / (2.0 * n)])
+
+
+def _F(r, A, xiF, beta):
+    return A * np.exp(-(r / xiF) ** beta) / np.sqrt(r)
+
+
+def xi_appendix_c(C: np.ndarray, C_err: np.ndarray, details: dict | None = None) -> float:
+    """xi = I_2 / I_1 by the paper's procedure (module docstring); C[r], C_err[r] for r = 0..R."""
+    C = np.asarray(C, np.float64)
+    E = np.asarray(C_err, np.float64)
+    R = C.size - 1
+    r = np.arange(R + 1, dtype=np.float64)
+    # (i) cut-off: the last r before C(r + 1) < 3 err(r + 1)
+    bad = np.nonzero(C[1:] < 3.0 * E[1:])[0]
+    r_cut = int(bad[0]) if bad.size else R                   # bad[0] indexes C[1:], i.e. r = bad[0] + 1
+    if r_cut < 2:
+        raise ValueError("the correlation function is noise from r = 2 on")
+    w = r[: r_cut + 1] ** 2 * C[: r_cut + 1]
+    r_star = int(np.argmax(w))
+    below = lambda frac: next((int(k) for k in range(r_star + 1, r_cut + 1) if w[k] < frac * w[r_star]), None)
+    r_min, r_max = below(0.9), below(1.0 / 3.0)
+    info = {"r_cut": r_cut, "r_star": r_star, "r_min": r_min, "r_max": r_max, "tail_fit": False}
+
+    def trapz(n, upto):
+        y = r[: upto + 1] ** n * C[: upto + 1]
+        return float(np.sum(0.5 * (y[1:] + y[:-1])))
+
+    if r_min is None or r_max is None or r_max - r_min <= 8:
+        I1, I2 = trapz(1, r_cut), trapz(2, r_cut)             # (iii), first branch
+    else:
+        from scipy.optimize import curve_fit
+        rr = r[r_min: r_max + 1]
+        sig = np.maximum(E[r_min: r_max + 1], 1e-300)
+        xi0 = max(float(r_star), 1.0)
+        p0 = (C[r_min] * np.sqrt(rr[0]) * np.e, xi0, 1.5)
+        popt, _ = curve_fit(_F, rr, C[r_min: r_max + 1], p0=p0, sigma=sig, maxfev=20000,
+                            bounds=([0.0, 1e-3, 0.1], [np.inf, np.inf, 10.0]))
+        A, xiF, beta = (float(v) for v in popt)
+        info.update(tail_fit=True, A=A, xi_F=xiF, beta=beta)
+        upper = max(20.0 * xiF, float(r_max) + 1.0)
+        fine = np.linspace(float(r_max), upper, 20001)
+
+        def tail(n):
+            y = fine ** n * _F(fine, A, xiF, beta)
+            return float(np.sum(0.5 * (y[1:] + y[:-1]) * np.diff(fine)))
+
+        I1, I2 = trapz(1, r_max) + tail(1), trapz(2, r_max) + tail(2)
+    if details is not None:
+        details.update(info, I1=I1, I2=I2)
+    return I2 / I1
+
+
+def xi_with_error(C_runs: np.ndarray):
+    """C_runs[run, r] -> (xi, jackknife error): the cut-offs are fixed from the full sample's mean
+    and error, then xi is recomputed on every leave-one-out mean."""
+    C_runs = np.asarray(C_runs, np.float64)
+    n = C_runs.shape[0]
+    err = C_runs.std(axis=0, ddof=1) / np.sqrt(n)
+    xi, xi_err = jackknife(C_runs, lambda m: xi_appendix_c(m, err))
+    return float(xi), float(xi_err)
+
+
+def _fit_z_once(logt, xi, xi_err, omega):
+    """Weighted linear least squares of log t = z log xi + b + b' xi^-omega; the weights use the
+    error of xi propagated through f'(xi), iterated to self-consistency."""
+    X = np.stack([np.log(xi), np.ones_like(xi), xi ** (-omega)], axis=1)
+    sigma = np.maximum(xi_err / xi, 1e-300)                       # start: f' ~ z / xi with z ~ 1
+    for _ in range(20):
+        W = 1.0 / sigma
+        p, *_ = np.linalg.lstsq(X * W[:, None], logt * W, rcond=None)
+        fprime = p[0] / xi - omega * p[2] * xi ** (-omega - 1.0)
+        new = np.maximum(1e-40 + xi_err * np.abs(fprime), 1e-300)  # t_error = 1e-40
+        if np.allclose(new, sigma, rtol=1e-10):
+            sigma = new
+            break
+        sigma = new
+    chi2 = float(np.sum(((X @ p - logt) / sigma) ** 2))
+    return p, chi2
+
+
+def fit_z(t, xi, xi_err, omega: float = OMEGA, t_min: float = 0.0) -> dict:
+    """z from Eq. (5) / (D1) on the points with t >= t_min.  Returns z, b, b', chi2, dof, Q."""
+    from scipy.special import gammaincc
+    t, xi, xi_err = (np.asarray(a, np.float64) for a in (t, xi, xi_err))
+    keep = t >= t_min
+    if keep.sum() < 4:
+        raise ValueError("need at least 4 points for a 3-parameter fit")
+    p, chi2 = _fit_z_once(np.log(t[keep]), xi[keep], xi_err[keep], omega)
+    dof = int(keep.sum()) - 3
+    return {"z": float(p[0]), "b": float(p[1]), "b1": float(p[2]), "chi2": chi2, "dof": dof,
+            "Q": float(gammaincc(dof / 2.0, chi2 / 2.0))}
+
+
+def fit_z_jackknife(t, C_runs_by_time, omega: float = OMEGA, t_min: float = 0.0) -> dict:
+    """C_runs_by_time[time][run, r] -> z with its jackknife error over the runs (App. D):
+    xi(t) is recomputed and the fit repeated on every leave-one-out sample."""
+    t = np.asarray(t, np.float64)
+    stacks = [np.asarray(c, np.float64) for c in C_runs_by_time]
+    n = stacks[0].shape[0]
+    errs = [c.std(axis=0, ddof=1) / np.sqrt(n) for c in stacks]
+    xi_full, xi_err = [], []
+    for c in stacks:
+        x, e = xi_with_error(c)
+        xi_full.append(float(x)); xi_err.append(float(e))
+    xi_full, xi_err = np.array(xi_full), np.array(xi_err)
+    full = fit_z(t, xi_full, xi_err, omega, t_min)
+    zs = []
+    for i in range(n):
+        xi_i = np.array([xi_appendix_c((c.sum(axis=0) - c[i]) / (n - 1), e) for c, e in zip(stacks, errs)])
+        zs.append(fit_z(t, xi_i, xi_err, omega, t_min)["z"])
+    zs = np.array(zs)
+    full["z_err"] = float(np.sqrt((n - 1) / n * np.sum((zs - zs.mean()) ** 2)))
+    full["xi"], full["xi_err"] = xi_full, xi_err
+    return full

@@ -80,6 +80,26 @@ def run(w: workloads.Workload, sweeps: int | None = None, r_max: int | None = No
     return records
 
 
+def replica_correlations(w: workloads.Workload, n_runs: int, sweeps: int, r_max: int, L: int | None = None,
+                         device: str = "cuda:0"):
+    """n_runs independent realisations of workload w (seeds w.seed + 7919 k): returns
+    (times[T], C[T][run, r] for r = 0..r_max, e[T][run]) at the record times 2^k <= sweeps --
+    the input of the estimator layer (analysis.py)."""
+    from . import analysis
+    times = [t for t in w.measure_times(sweeps) if t > 0]
+    C = [np.zeros((n_runs, r_max + 1)) for _ in times]
+    e = [np.zeros(n_runs) for _ in times]
+    for k in range(n_runs):
+        g = lat.Lattice(L or w.L, w.model, w.delta, w.seed + 7919 * k, device=device)
+        for a, t in enumerate(times):
+            g.sweep(w.beta_schedule(t - g.time, g.time))
+            M, Q, Sx, Sy = g.measure(r_max)
+            C[a][k] = analysis.correlation(Sx, Sy, g.L, Q)
+            e[a][k] = lat.energy(Sx, Sy, Q, w.delta, g.L)
+        g.close()
+    return np.array(times, dtype=np.float64), C, e
+
+
 def main(argv=None) -> int:
     ap = argparse.ArgumentParser(description=__doc__.split("\n\n")[0])
     ap.add_argument("--workload", required=True, choices=sorted(workloads.CONFIGS))
@@ -102,3 +122,4 @@ def main(argv=None) -> int:
 
 if __name__ == "__main__":
     raise SystemExit(main())
+

@@ -1,0 +1,87 @@
+"""The estimator layer (paper_2503_14688_b200/analysis.py) on synthetic data with known answers."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2503_14688_b200 import analysis as an
+
+
+def test_jackknife_reduces_to_the_standard_error_for_the_mean():
+    rng = np.random.default_rng(1)
+    x = rng.normal(3.0, 2.0, size=(50, 4))
+    mean, err = an.jackknife(x)
+    assert np.allclose(mean, x.mean(axis=0))
+    assert np.allclose(err, x.std(axis=0, ddof=1) / math.sqrt(50))
+    # a nonlinear estimator: error of the square of the mean ~ 2 |mean| sigma_mean
+    sq, sq_err = an.jackknife(x[:, 0], lambda m: m ** 2)
+    assert abs(sq_err / (2 * abs(x[:, 0].mean()) * x[:, 0].std(ddof=1) / math.sqrt(50)) - 1) < 0.05
+    with pytest.raises(ValueError):
+        an.jackknife(x[:1])
+
+
+def _synthetic_C(xiF, beta, R, A=1.0):
+    r = np.arange(R + 1, dtype=np.float64)
+    C = np.ones(R + 1)
+    C[1:] = A * np.exp(-(r[1:] / xiF) ** beta) / np.sqrt(r[1:])
+    return C
+
+
+@pytest.mark.parametrize("xiF,beta", [(20.0, 1.0), (35.0, 1.4), (12.0, 0.8)])
+def test_xi_appendix_c_recovers_the_tail_function(xiF, beta):
+    """For C(r) = A exp[-(r/xi_F)^beta] / sqrt(r) (Eq. C2), I_n = A xi_F^(n+1/2) Gamma((n+1/2)/beta)/beta,
+    so xi = I_2/I_1 = xi_F Gamma(2.5/beta) / Gamma(1.5/beta)."""
+    R = 2000
+    C = _synthetic_C(xiF, beta, R, A=0.7)
+    err = np.full(R + 1, 1e-9)
+    d = {}
+    xi = an.xi_appendix_c(C, err, d)
+    exact = xiF * math.gamma(2.5 / beta) / math.gamma(1.5 / beta)
+    assert abs(xi / exact - 1) < 0.02, (xi, exact, d)
+    assert d["tail_fit"] and d["r_star"] < d["r_min"] < d["r_max"] < d["r_cut"]
+    assert abs(d["xi_F"] / xiF - 1) < 1e-3 and abs(d["beta"] - beta) < 1e-3
+    # with large errors the cut-off comes early and the data are integrated as they are
+    d2 = {}
+    an.xi_appendix_c(C, np.full(R + 1, 0.05), d2)
+    assert d2["r_cut"] < d["r_cut"] and C[d2["r_cut"] + 1] < 0.15 <= C[d2["r_cut"]]
+
+
+def test_xi_with_error_on_noisy_runs():
+    rng = np.random.default_rng(7)
+    C = _synthetic_C(25.0, 1.2, 800)
+    runs = C[None, :] + rng.normal(0.0, 2e-4, size=(40, C.size))
+    xi, err = an.xi_with_error(runs)
+    exact = 25.0 * math.gamma(2.5 / 1.2) / math.gamma(1.5 / 1.2)
+    assert 0 < err < 0.05 * exact and abs(xi - exact) < max(5 * err, 0.03 * exact)
+
+
+def test_fit_z_recovers_the_exponent_of_eq_5():
+    """Points generated from log t = z log xi + b + b' xi^-omega are fitted back exactly."""
+    z, b, b1 = 2.1676, -0.35, 1.9
+    xi = np.geomspace(5.0, 1100.0, 18)
+    t = np.exp(z * np.log(xi) + b + b1 * xi ** (-an.OMEGA))
+    fit = an.fit_z(t, xi, 1e-3 * xi)
+    assert abs(fit["z"] - z) < 1e-9 and abs(fit["b"] - b) < 1e-8 and abs(fit["b1"] - b1) < 1e-6
+    assert fit["dof"] == 15 and fit["chi2"] < 1e-12 and fit["Q"] > 0.999
+    # t_min drops the early points; too few points is an error
+    assert an.fit_z(t, xi, 1e-3 * xi, t_min=t[10])["dof"] == 5
+    with pytest.raises(ValueError):
+        an.fit_z(t, xi, 1e-3 * xi, t_min=t[-3])
+    # noisy xi: z within a few sigma of chi^2-consistent noise, Q not tiny
+    rng = np.random.default_rng(3)
+    noisy = xi * (1 + 2e-3 * rng.normal(size=xi.size))
+    f2 = an.fit_z(t, noisy, 2e-3 * xi)
+    assert abs(f2["z"] - z) < 0.02 and f2["Q"] > 1e-3
+
+
+def test_fit_z_jackknife_on_synthetic_runs():
+    rng = np.random.default_rng(11)
+    z, b, b1 = 2.1676, 0.1, 1.0
+    xiF = np.geomspace(6.0, 60.0, 8)
+    ratio = math.gamma(2.5 / 1.3) / math.gamma(1.5 / 1.3)
+    xi_true = xiF * ratio
+    t = np.exp(z * np.log(xi_true) + b + b1 * xi_true ** (-an.OMEGA))
+    stacks = [_synthetic_C(x, 1.3, 1200)[None, :] + rng.normal(0, 1e-5, size=(12, 1201)) for x in xiF]
+    fit = an.fit_z_jackknife(t, stacks)
+    assert abs(fit["z"] - z) < 0.05 and 0 <= fit["z_err"] < 0.05
+    assert np.all(np.abs(fit["xi"] / xi_true - 1) < 0.02)
