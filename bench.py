@@ -320,6 +320,23 @@ def main():
     e2e_ms = timed(step_e2e, args.steps, tdone + 1)
     tdone += 1 + args.steps
 
+    # ---- measurement pass, timed separately --------------------------------------------------
+    r_meas = w.r_max if args.measure_rmax < 0 else args.measure_rmax
+    r_meas = max(1, min(r_meas, L // 2))
+    meas = None
+    if rank == 0:
+        # ~3e12 (word, r) pairs/s per axis (profiles/): bound the default run to a few seconds
+        words = L * L // 32
+        if args.measure_rmax < 0 and words * r_meas > 1 << 42:     # an explicit --measure-rmax is honoured
+            r_meas = max(1, (1 << 42) // words)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(g.stream)
+        M, Q, Sx, Sy = g.measure(r_meas)
+        ev1.record(g.stream)
+        torch.cuda.synchronize(dev)
+        xi_v, r_cut = lat.xi(Sx, Sy, Q, L)
+        meas = {"r_max": r_meas, "ms": ev0.elapsed_time(ev1), "t": g.time, "M": M,
+                "e": lat.energy(Sx, Sy, Q, w.delta, L), "xi": xi_v, "r_cut": r_cut}
     # ---- worst-case input: the all-up state (every site has 4 aligned neighbours, so every
     # lane needs a random decision and ties are ~3x more frequent than after the quench) ----------
     worst = None
@@ -332,23 +349,6 @@ def main():
         worst = {"value": updates_per_step * nw / (worst_ms * 1e6), "unit": UNIT, "steps": nw,
                  "input": "all spins up at t0 (SURVEY.md 8(d) worst case), then the same sweeps"}
 
-    # ---- measurement pass, timed separately --------------------------------------------------
-    r_meas = w.r_max if args.measure_rmax < 0 else args.measure_rmax
-    r_meas = max(1, min(r_meas, L // 2))
-    meas = None
-    if rank == 0:
-        # ~3e12 (word, r) pairs/s per axis (profiles/): bound the default run to a few seconds
-        words = L * L // 32
-        if words * r_meas > 1 << 42:
-            r_meas = max(1, (1 << 42) // words)
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        ev0.record(g.stream)
-        M, Q, Sx, Sy = g.measure(r_meas)
-        ev1.record(g.stream)
-        torch.cuda.synchronize(dev)
-        xi_v, r_cut = lat.xi(Sx, Sy, Q, L)
-        meas = {"r_max": r_meas, "ms": ev0.elapsed_time(ev1), "t": g.time, "M": M,
-                "e": lat.energy(Sx, Sy, Q, w.delta, L), "xi": xi_v, "r_cut": r_cut}
     barrier()
 
     if rank != 0:
