@@ -49,3 +49,43 @@ def test_measure_times():
     assert w.measure_times(20) == [0, 1, 2, 4, 8, 16, 20]
     assert w.measure_times()[-1] == 2000 and 1024 in w.measure_times()
     assert math.log2(W.CONFIGS["ising_L2p20"].spins) == 40
+
+
+def _paper_values():
+    import os
+    vals = {}
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_values.txt")
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        f = line.split()
+        nums = []
+        for tok in f[1:]:
+            try:
+                nums.append(float(tok))
+            except ValueError:
+                break
+        vals[f[0]] = nums
+    return vals
+
+
+def test_constants_against_the_numbers_the_paper_prints():
+    """tests/golden/paper_values.txt (each line cites its passage) against the workload constants
+    and the constants of the estimator layer and the physics tests."""
+    from paper_2503_14688_b200 import analysis
+    p = _paper_values()
+    assert abs(1.0 / W.BETA_C_ISING - p["Tc_ising"][0]) < 1e-15            # Onsager, 16 digits
+    assert abs(2.0 / math.log(1.0 + math.sqrt(2.0)) - p["Tc_ising"][0]) < 1e-15
+    assert abs(W.T_BC - p["Tc_blume_capel"][0]) < 2e-4                      # BASELINE config 3 rounds T_c to 1.6934
+    assert p["E_eq_ising"][0] == -math.sqrt(2.0)
+    assert analysis.OMEGA == p["omega"][0]
+    i2, b2 = W.CONFIGS["ising_L2p16_twostep"], W.CONFIGS["bc_L2p16_twostep"]
+    assert 1.0 / i2.beta_1 == p["ising_T1"][0] and abs(1.0 / i2.beta_f - p["ising_T2"][0]) < 1e-15
+    assert i2.t_switch in [int(x) for x in p["ising_t_switch"]] and i2.sweeps == int(p["ising_t_max2"][0])
+    assert abs(1.0 / b2.beta_1 - p["bc_T1"][0]) < 1e-15 and abs(1.0 / b2.beta_f - p["bc_T2"][0]) < 1e-15
+    assert b2.t_switch in [int(x) for x in p["bc_t_switch"]] and b2.sweeps == int(p["bc_t_max2"][0])
+    # T_1 ~ 0.73 T_c for both models (PAPER.md:65-71)
+    assert abs(p["ising_T1"][0] / p["Tc_ising"][0] - 0.73) < 0.005
+    assert abs(p["bc_T1"][0] / p["Tc_blume_capel"][0] - 0.73) < 0.005
+    # the record: 8.7 fs per update = 114 943 updates/ns in aggregate
+    assert abs(1e6 / p["time_per_update_fs"][0] - 114943) < 1
