@@ -264,14 +264,19 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    local %= max(torch.cuda.device_count(), 1)     # more ranks than GPUs only in tests (gloo)
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        if args.dist_backend == "nccl":
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group("gloo")
 
     w = workloads.CONFIGS[args.workload]
     L = args.L or pick_L(w, torch, dev)
-    L = replicas.agree_min(L, dev)              # all replicas use the same size
+    cdev = dev if args.dist_backend == "nccl" else "cpu"   # where the plumbing tensors live
+    L = replicas.agree_min(L, cdev)             # all replicas use the same size
     g = lat.Lattice(L, w.model, w.delta, seed=replicas.replica_seed(w.seed, rank), scheme=args.scheme,
                     device=str(dev))
     updates_per_step = L * L
@@ -288,7 +293,7 @@ def main():
             fn(start_t + k)
         ev1.record(g.stream)
         torch.cuda.synchronize(dev)
-        ms = replicas.max_over_ranks(ev0.elapsed_time(ev1), dev)
+        ms = replicas.max_over_ranks(ev0.elapsed_time(ev1), cdev)
         barrier()
         return ms
 
