@@ -201,20 +201,22 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
             gg[w] = lop3<0xDA>(nz, sg, bw);
             const uint32_t r = lop3<0xC5>(nz, sg, bw);            // (nz & sg) | (~nz & ~b)
             // x + 4 = sum over the 4 neighbours of [sign r] + [not sign -r], bit-sliced
-            const uint32_t a1 = U.nz[w] & ~(U.sg[w] ^ r), n1 = ~(U.nz[w] & (U.sg[w] ^ r));
-            const uint32_t a2 = D.nz[w] & ~(D.sg[w] ^ r), n2 = ~(D.nz[w] & (D.sg[w] ^ r));
-            const uint32_t a3 = C.nz[w] & ~(C.sg[w] ^ r), n3 = ~(C.nz[w] & (C.sg[w] ^ r));
-            const uint32_t a4 = Sn & ~(Ss ^ r), n4 = ~(Sn & (Ss ^ r));
-            const uint32_t s1 = a1 ^ a2 ^ a3, c1 = maj3m(a1, a2, a3);
-            const uint32_t s2 = n1 ^ n2 ^ n3, c2 = maj3m(n1, n2, n3);
-            const uint32_t s3 = s1 ^ s2 ^ a4, c3 = maj3m(s1, s2, a4);
+            // explicit truth tables (inputs nz, sg, r): [sign r] = nz & ~(sg ^ r) = 0x90,
+            // [not sign -r] = ~(nz & (sg ^ r)) = 0x9F; adders: xor3 = 0x96, majority = 0xE8
+            const uint32_t a1 = lop3<0x90>(U.nz[w], U.sg[w], r), n1 = lop3<0x9F>(U.nz[w], U.sg[w], r);
+            const uint32_t a2 = lop3<0x90>(D.nz[w], D.sg[w], r), n2 = lop3<0x9F>(D.nz[w], D.sg[w], r);
+            const uint32_t a3 = lop3<0x90>(C.nz[w], C.sg[w], r), n3 = lop3<0x9F>(C.nz[w], C.sg[w], r);
+            const uint32_t a4 = lop3<0x90>(Sn, Ss, r), n4 = lop3<0x9F>(Sn, Ss, r);
+            const uint32_t s1 = lop3<0x96>(a1, a2, a3), c1 = lop3<0xE8>(a1, a2, a3);
+            const uint32_t s2 = lop3<0x96>(n1, n2, n3), c2 = lop3<0xE8>(n1, n2, n3);
+            const uint32_t s3 = lop3<0x96>(s1, s2, a4), c3 = lop3<0xE8>(s1, s2, a4);
             const uint32_t h0 = s3 ^ n4, c4 = s3 & n4;            // weight 1 done
-            const uint32_t t1 = c1 ^ c2 ^ c3, d1 = maj3m(c1, c2, c3);
+            const uint32_t t1 = lop3<0x96>(c1, c2, c3), d1 = lop3<0xE8>(c1, c2, c3);
             const uint32_t h1 = t1 ^ c4, d2 = t1 & c4;            // weight 2 done
             const uint32_t h2 = d1 ^ d2, h3 = d1 & d2;            // weights 4, 8
             H0[w] = h0;
-            Y1[w] = h3 | (h1 & h0);                               // x >= 3  (x+4 in {7, 8})
-            pos[w] = h3 | (h2 & (h1 | h0));                       // x >= 1  (x+4 >= 5)
+            Y1[w] = lop3<0xF8>(h3, h1, h0);                       // h3 | (h1 & h0): x >= 3  (x+4 in {7, 8})
+            pos[w] = h3 | lop3<0xE0>(h2, h1, h0);                 // h3 | (h2 & (h1 | h0)): x >= 1
         }
     }
     uint32_t alw[4], acc[4], eq[4];
