@@ -112,15 +112,16 @@ int lattice_view(lattice_t **out, uint32_t L, int model, uint32_t rows, void *de
                  size_t device_buf_bytes, void *cuda_stream);
 int lattice_device_copy(void *device_dst, const void *device_src, size_t bytes, void *cuda_stream);
 
+/* One process driving several GPUs: let kernels running on `device` store into memory of
+ * `peer_device` (cudaDeviceEnablePeerAccess; already-enabled is not an error).  ECUDA if the two
+ * devices cannot reach each other. */
+int lattice_enable_peer_access(int device, int peer_device);
+
 /* One process per GPU: the mirror pointers of lattice_slab_set_neighbours must then come from
  * another process.  These helpers allocate a slab buffer that can be exported (cudaMalloc on the
  * current device, so that the IPC handle maps the buffer itself), export it as a 64-byte CUDA IPC
  * handle (sent to the neighbours by any means, e.g. torch.distributed), and open a neighbour's
  * handle as a device pointer valid in this process.  Errors: EINVAL (NULL), ECUDA. */
-/* One process driving several GPUs: let kernels running on `device` store into memory of
- * `peer_device` (cudaDeviceEnablePeerAccess; already-enabled is not an error).  ECUDA if the two
- * devices cannot reach each other. */
-int lattice_enable_peer_access(int device, int peer_device);
 int lattice_device_alloc(void **device_ptr, size_t bytes);
 int lattice_device_free(void *device_ptr);
 int lattice_ipc_export(const void *device_ptr, unsigned char handle[64]);
@@ -142,6 +143,9 @@ int lattice_ipc_close(void *device_ptr);
 int lattice_set_rng_scheme(lattice_t *lat, int scheme);
 
 /* Run sweeps t .. t+n-1; sweep t+k uses beta[k] (host fp64 array of n entries; beta = 1/T).
+ * One sweep = one Metropolis update attempt of every site, the paper's time unit:
+ * black half-sweep then white half-sweep (checkerboard); a constant array is
+ * protocol 1, a time-varying one protocol 2 (Table II).
  * Thresholds floor(2^32 exp(-beta dE)) are rebuilt on the host whenever beta changes.
  * Asynchronous on the handle's stream (beta is consumed before the call returns); t += n.
  * Errors: EINVAL (NULL beta with n > 0, NaN or negative beta, t+n >= 2^32), ECUDA. */
@@ -151,7 +155,9 @@ int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta);
  * advancing t.  lattice_sweep(1, &beta) == half_sweep(0), half_sweep(1), t += 1.  For tests. */
 int lattice_half_sweep(lattice_t *lat, int colour, double beta);
 
-/* Exact integer measurements of the whole lattice, r = 1..r_max (1 <= r_max <= L/2):
+/* Exact integer measurements of the whole lattice, r = 1..r_max (1 <= r_max <= L/2): the
+ * numerators of C(r;t) along the two lattice axes, Eq. 2, and of E(t), Eq. 3
+ * (r = 1):
  *   *M = sum s, *Q = sum s^2 (= L^2 for Ising), Sx[r-1] = S_x(r), Sy[r-1] = S_y(r).
  * Host outputs; synchronises the stream.  Errors: EINVAL, ENOMEM, ECUDA. */
 int lattice_measure(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx,
@@ -184,15 +190,21 @@ uint64_t lattice_time(const lattice_t *lat);
 int lattice_set_time(lattice_t *lat, uint64_t t);
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 uint64_t lattice_launches(const lattice_t *lat);
+/* Tuning / test knob: upper bound on the grid of the persistent multi-sweep kernel that
+ * lattice_sweep(n >= 2) uses for cache-resident Ising lattices (0 = the occupancy limit, the
+ * default).  With fewer blocks than 256-thread groups of work every block strides over several
+ * groups per half-sweep; results do not depend on it.  EINVAL for a NULL handle. */
+int lattice_set_persist_blocks(lattice_t *lat, uint32_t max_blocks);
 
 /* Host-only helpers (no device work).
  * lattice_thresholds: acceptance thresholds in [0, 2^32] for inverse temperature beta;
  *   Ising: out[0] = thr(dE = 4), out[1] = thr(dE = 8);
  *   Blume-Capel: out[(code*2 + b)*9 + (h+4)], code = s+1, b = proposal bit, h = neighbour sum;
  *   an entry equal to 2^32 means "always accept" (dE <= 0, or exp rounded to 1).
- * lattice_xi: xi = I_2/I_1 of a single run (reading 14): C(r) = (Sx+Sy)/(2 L^2),
- *   r_cut = (first r with Sx+Sy <= 0) - 1 or r_max, trapezoid weights (1/2 at r_cut),
- *   ascending fp64 sums; returns 0 if r_cut < 1; *r_cut_out (may be NULL) receives r_cut.
+ * lattice_xi: xi = I_2/I_1, I_n = int r^n C(r) dr, Eq. C1, of a single run
+ *   (reading 14): C(r) = (Sx+Sy)/(2 L^2), r_cut = (first r with Sx+Sy <= 0) - 1 or
+ *   r_max, trapezoid weights (1/2 at r_cut); the two sums are accumulated exactly in 128-bit
+ *   integers and divided once; returns 0 if r_cut < 1; *r_cut_out (may be NULL) receives r_cut.
  * lattice_energy: e = -(Sx[0]+Sy[0])/L^2 + delta*Q/L^2. */
 void lattice_thresholds(int model, double delta, double beta, uint64_t *out);
 /* Scheme 2: thresholds on the 2^64 scale (same indexing); always[e] = 1 where the move is always
@@ -201,6 +213,16 @@ void lattice_thresholds64(int model, double delta, double beta, uint64_t *thr, u
 double lattice_xi(const int64_t *Sx, const int64_t *Sy, uint32_t r_max, int64_t Q, uint32_t L,
                   uint32_t *r_cut_out);
 double lattice_energy(const int64_t *Sx, const int64_t *Sy, int64_t Q, double delta, uint32_t L);
+
+/* Integer-dispatch micro-benchmark (the measured peak of bench.py's "alu" roofline; DESIGN.md
+ * section 6): runs dependent chains of the instruction mix `mode` on every SM of the current device
+ * (4 blocks of 256 threads per SM, 8 chains per thread) and returns the thread-instructions of the
+ * counted classes issued per clock per SM, from clock64() inside the kernel (independent of the
+ * SM clock).  mode 0: LOP3; 1: mul.wide.u32 + LOP3 (a Philox round); 2: mul.wide.u32 + 3 LOP3
+ * (the half-sweep's mix); 3: POPC.  *elapsed_ms (may be NULL) receives the CUDA-event time of the
+ * timed launch.  Synchronises the stream.  Errors: EINVAL, ENOMEM, ECUDA. */
+int lattice_ubench_int_dispatch(int mode, void *cuda_stream, double *thread_instr_per_clk_per_sm,
+                                double *elapsed_ms);
 
 /* Frees the handle and its scratch; never the caller's device_buf. */
 int lattice_destroy(lattice_t *lat);

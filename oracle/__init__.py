@@ -25,9 +25,17 @@ def build(force: bool = False) -> str:
     if (not force and os.path.exists(_SO)
             and os.path.getmtime(_SO) >= max(os.path.getmtime(src), os.path.getmtime(hdr))):
         return _SO
-    cmd = ["gcc", "-O2", "-std=c11", "-Wall", "-Wextra", "-fopenmp", "-shared", "-fPIC",
-           src, "-o", _SO, "-lm"]
-    subprocess.run(cmd, check=True)
+    import fcntl
+    with open(_SO + ".lock", "w") as lock:           # several ranks may build at once
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if (not force and os.path.exists(_SO)
+                and os.path.getmtime(_SO) >= max(os.path.getmtime(src), os.path.getmtime(hdr))):
+            return _SO
+        tmp = f"{_SO}.{os.getpid()}.tmp"
+        cmd = ["gcc", "-O2", "-std=c11", "-Wall", "-Wextra", "-fopenmp", "-shared", "-fPIC",
+               src, "-o", tmp, "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _SO)
     return _SO
 
 

@@ -52,34 +52,59 @@ def _F(r, A, xiF, beta):
     return A * np.exp(-(r / xiF) ** beta) / np.sqrt(r)
 
 
-def xi_appendix_c(C: np.ndarray, C_err: np.ndarray, details: dict | None = None) -> float:
-    """xi = I_2 / I_1 by the paper's procedure (module docstring); C[r], C_err[r] for r = 0..R."""
+class CutoffWarning(UserWarning):
+    """The ordering r* < r_min < r_max <= r_cut that App. C requires was not found."""
+
+
+def xi_appendix_c(C: np.ndarray, C_err: np.ndarray, details: dict | None = None, cutoffs: dict | None = None,
+                  strict: bool = False) -> float:
+    """xi = I_2 / I_1 by the paper's procedure (module docstring); C[r], C_err[r] for r = 0..R.
+
+    cutoffs = {"r_cut", "r_min", "r_max"} freezes the three cut-offs (the jackknife passes the
+    full sample's, so that every leave-one-out mean is integrated over the same ranges).  The
+    paper requires r* < r_min < r_max < r_cut and asks for more statistics otherwise
+    (PAPER.md:202-207); when r_min or r_max is not found before r_cut this routine integrates the
+    data up to r_cut only, which biases xi low: details["condition_met"] is then False and a
+    CutoffWarning is issued (strict=True raises ValueError instead)."""
+    import warnings
     C = np.asarray(C, np.float64)
     E = np.asarray(C_err, np.float64)
     R = C.size - 1
     r = np.arange(R + 1, dtype=np.float64)
-    # (i) cut-off: the last r before C(r + 1) < 3 err(r + 1)
-    bad = np.nonzero(C[1:] < 3.0 * E[1:])[0]
-    r_cut = int(bad[0]) if bad.size else R                   # bad[0] indexes C[1:], i.e. r = bad[0] + 1
-    if r_cut < 2:
-        raise ValueError("the correlation function is noise from r = 2 on")
-    w = r[: r_cut + 1] ** 2 * C[: r_cut + 1]
-    r_star = int(np.argmax(w))
-    below = lambda frac: next((int(k) for k in range(r_star + 1, r_cut + 1) if w[k] < frac * w[r_star]), None)
-    r_min, r_max = below(0.9), below(1.0 / 3.0)
-    info = {"r_cut": r_cut, "r_star": r_star, "r_min": r_min, "r_max": r_max, "tail_fit": False}
+    if cutoffs is None:
+        # (i) cut-off: the last r before C(r + 1) < 3 err(r + 1)
+        bad = np.nonzero(C[1:] < 3.0 * E[1:])[0]
+        r_cut = int(bad[0]) if bad.size else R               # bad[0] indexes C[1:], i.e. r = bad[0] + 1
+        if r_cut < 2:
+            raise ValueError("the correlation function is noise from r = 2 on")
+        w = r[: r_cut + 1] ** 2 * C[: r_cut + 1]
+        r_star = int(np.argmax(w))
+        below = lambda frac: next((int(k) for k in range(r_star + 1, r_cut + 1) if w[k] < frac * w[r_star]), None)
+        r_min, r_max = below(0.9), below(1.0 / 3.0)
+    else:
+        r_cut, r_min, r_max = cutoffs["r_cut"], cutoffs["r_min"], cutoffs["r_max"]
+        r_star = cutoffs.get("r_star")
+    found = r_min is not None and r_max is not None
+    info = {"r_cut": r_cut, "r_star": r_star, "r_min": r_min, "r_max": r_max, "tail_fit": False,
+            "condition_met": bool(found)}
+    if not found:
+        msg = (f"App. C cut-offs not found before r_cut = {r_cut} (r_min = {r_min}, r_max = {r_max}): "
+               "integrating the data up to r_cut only biases xi low; more statistics or a larger r range needed")
+        if strict:
+            raise ValueError(msg)
+        warnings.warn(msg, CutoffWarning, stacklevel=2)
 
     def trapz(n, upto):
         y = r[: upto + 1] ** n * C[: upto + 1]
         return float(np.sum(0.5 * (y[1:] + y[:-1])))
 
-    if r_min is None or r_max is None or r_max - r_min <= 8:
+    if not found or r_max - r_min <= 8:
         I1, I2 = trapz(1, r_cut), trapz(2, r_cut)             # (iii), first branch
     else:
         from scipy.optimize import curve_fit
         rr = r[r_min: r_max + 1]
         sig = np.maximum(E[r_min: r_max + 1], 1e-300)
-        xi0 = max(float(r_star), 1.0)
+        xi0 = max(float(r_star if r_star is not None else r_min), 1.0)
         p0 = (C[r_min] * np.sqrt(rr[0]) * np.e, xi0, 1.5)
         popt, _ = curve_fit(_F, rr, C[r_min: r_max + 1], p0=p0, sigma=sig, maxfev=20000,
                             bounds=([0.0, 1e-3, 0.1], [np.inf, np.inf, 10.0]))
@@ -98,13 +123,22 @@ def xi_appendix_c(C: np.ndarray, C_err: np.ndarray, details: dict | None = None)
     return I2 / I1
 
 
-def xi_with_error(C_runs: np.ndarray):
-    """C_runs[run, r] -> (xi, jackknife error): the cut-offs are fixed from the full sample's mean
-    and error, then xi is recomputed on every leave-one-out mean."""
+def xi_with_error(C_runs: np.ndarray, details: dict | None = None):
+    """C_runs[run, r] -> (xi, jackknife error).  The cut-offs r_cut, r_min, r_max are fixed ONCE
+    from the full sample's mean and error and reused for every leave-one-out mean (PAPER.md:207);
+    the tail fit itself is repeated on each of them."""
+    import warnings
     C_runs = np.asarray(C_runs, np.float64)
     n = C_runs.shape[0]
     err = C_runs.std(axis=0, ddof=1) / np.sqrt(n)
-    xi, xi_err = jackknife(C_runs, lambda m: xi_appendix_c(m, err))
+    d = {}
+    xi_appendix_c(C_runs.mean(axis=0), err, d)                 # warns once if the condition fails
+    frozen = {k: d[k] for k in ("r_cut", "r_star", "r_min", "r_max")}
+    if details is not None:
+        details.update(d)
+    with warnings.catch_warnings():
+        warnings.simplefilter("ignore", CutoffWarning)
+        xi, xi_err = jackknife(C_runs, lambda m: xi_appendix_c(m, err, cutoffs=frozen))
     return float(xi), float(xi_err)
 
 
@@ -146,16 +180,22 @@ def fit_z_jackknife(t, C_runs_by_time, omega: float = OMEGA, t_min: float = 0.0)
     stacks = [np.asarray(c, np.float64) for c in C_runs_by_time]
     n = stacks[0].shape[0]
     errs = [c.std(axis=0, ddof=1) / np.sqrt(n) for c in stacks]
-    xi_full, xi_err = [], []
+    xi_full, xi_err, frozen = [], [], []
     for c in stacks:
-        x, e = xi_with_error(c)
+        d = {}
+        x, e = xi_with_error(c, d)
         xi_full.append(float(x)); xi_err.append(float(e))
+        frozen.append({k: d[k] for k in ("r_cut", "r_star", "r_min", "r_max")})
     xi_full, xi_err = np.array(xi_full), np.array(xi_err)
     full = fit_z(t, xi_full, xi_err, omega, t_min)
+    import warnings
     zs = []
-    for i in range(n):
-        xi_i = np.array([xi_appendix_c((c.sum(axis=0) - c[i]) / (n - 1), e) for c, e in zip(stacks, errs)])
-        zs.append(fit_z(t, xi_i, xi_err, omega, t_min)["z"])
+    with warnings.catch_warnings():
+        warnings.simplefilter("ignore", CutoffWarning)            # already reported by xi_with_error
+        for i in range(n):
+            xi_i = np.array([xi_appendix_c((c.sum(axis=0) - c[i]) / (n - 1), e, cutoffs=f)
+                             for c, e, f in zip(stacks, errs, frozen)])
+            zs.append(fit_z(t, xi_i, xi_err, omega, t_min)["z"])
     zs = np.array(zs)
     full["z_err"] = float(np.sqrt((n - 1) / n * np.sum((zs - zs.mean()) ** 2)))
     full["xi"], full["xi_err"] = xi_full, xi_err

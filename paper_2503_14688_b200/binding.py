@@ -52,10 +52,12 @@ SIGNATURES = {
     "lattice_time": (C.c_uint64, [_vp]),
     "lattice_set_time": (C.c_int, [_vp, C.c_uint64]),
     "lattice_launches": (C.c_uint64, [_vp]),
+    "lattice_set_persist_blocks": (C.c_int, [_vp, C.c_uint32]),
     "lattice_thresholds": (None, [C.c_int, C.c_double, C.c_double, _u64p]),
     "lattice_thresholds64": (None, [C.c_int, C.c_double, C.c_double, _u64p, C.POINTER(C.c_ubyte)]),
     "lattice_xi": (C.c_double, [_i64p, _i64p, C.c_uint32, C.c_int64, C.c_uint32, _u32p]),
     "lattice_energy": (C.c_double, [_i64p, _i64p, C.c_int64, C.c_double, C.c_uint32]),
+    "lattice_ubench_int_dispatch": (C.c_int, [C.c_int, _vp, _f64p, _f64p]),
     "lattice_destroy": (C.c_int, [_vp]),
     "lattice_strerror": (C.c_char_p, [C.c_int]),
     "lattice_last_error": (C.c_char_p, [_vp]),
@@ -142,6 +144,15 @@ def energy(Sx, Sy, Q: int, delta: float, L: int) -> float:
     Sy = np.ascontiguousarray(Sy, dtype=np.int64)
     return float(lib().lattice_energy(_p(Sx, C.c_int64), _p(Sy, C.c_int64), int(Q), float(delta),
                                       int(L)))
+
+
+def ubench_int_dispatch(mode: int, stream_ptr: int = 0):
+    """(thread-instructions per clock per SM, elapsed ms) of the integer-dispatch micro-benchmark."""
+    v, ms = C.c_double(0.0), C.c_double(0.0)
+    rc = lib().lattice_ubench_int_dispatch(int(mode), _vp(stream_ptr), C.byref(v), C.byref(ms))
+    if rc != OK:
+        raise LatticeError("lattice_ubench_int_dispatch", rc)
+    return float(v.value), float(ms.value)
 
 
 def measure_buffer(L: int, model: int, rows: int, n_base: int, r_max: int, ptr: int, nbytes: int,
@@ -316,6 +327,10 @@ class Lattice:
         with self._torch.cuda.device(self.device):
             self._check(lib().lattice_set_spins(self._h, i0, j0, s.shape[0], s.shape[1],
                                                 _p(s, C.c_int8)), "lattice_set_spins")
+
+    def set_persist_blocks(self, max_blocks: int) -> None:
+        """Cap the grid of the persistent multi-sweep kernel (0 = occupancy limit)."""
+        self._check(lib().lattice_set_persist_blocks(self._h, int(max_blocks)), "lattice_set_persist_blocks")
 
     def fill(self, spin: int) -> None:
         """Every spin := spin (an ordered state: worst-case throughput input, tests)."""

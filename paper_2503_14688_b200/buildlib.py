@@ -11,7 +11,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_PKG)
 SO_PATH = os.path.join(_PKG, "liblattice.so")
 SOURCES = [os.path.join(_PKG, "csrc", "lattice.cu")]
-HEADERS = [os.path.join(_PKG, "csrc", n) for n in ("philox.cuh", "ising.cuh", "ising_march.cuh", "ising_persist.cuh", "bc.cuh", "bc_march.cuh", "measure.cuh")]
+HEADERS = [os.path.join(_PKG, "csrc", n) for n in ("philox.cuh", "ising.cuh", "ising_march.cuh", "ising_persist.cuh", "bc.cuh", "bc_march.cuh", "measure.cuh", "ubench.cuh")]
 HEADERS.append(os.path.join(_ROOT, "include", "lattice.h"))
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
@@ -33,14 +33,30 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile liblattice.so if it is missing or older than its sources; return its path."""
-    if not force and not needs_build():
-        return SO_PATH
-    cmd = [nvcc(), *NVCC_FLAGS, "-I", os.path.join(_ROOT, "include"), "-o", SO_PATH, *SOURCES]
-    if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-        print(" ".join(cmd))
-    subprocess.run(cmd, check=True)
+    """Compile liblattice.so if it is missing or older than its sources; return its path.
+
+    Safe under torchrun (every rank calls this): an exclusive file lock serialises the check and
+    the compile, nvcc writes to a temporary file in the same directory and the finished library is
+    moved into place with os.replace(), so no process ever dlopens a half-written file."""
+    import fcntl
+    with open(SO_PATH + ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and not needs_build():
+                return SO_PATH
+            tmp = f"{SO_PATH}.{os.getpid()}.tmp"
+            cmd = [nvcc(), *NVCC_FLAGS, "-I", os.path.join(_ROOT, "include"), "-o", tmp, *SOURCES]
+            if verbose:
+                cmd.insert(1, "-Xptxas=-v")
+                print(" ".join(cmd))
+            try:
+                subprocess.run(cmd, check=True)
+                os.replace(tmp, SO_PATH)
+            finally:
+                if os.path.exists(tmp):
+                    os.unlink(tmp)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
     return SO_PATH
 
 

@@ -115,9 +115,11 @@ struct BCTieQueue {
         if (dsg) atomicXor(a.tsg + wo, dsg);
         const uint32_t mf = SLAB ? e1.w >> 30 : 0u;
         if (mf && (dnz | dsg)) {
+            // possibly peer-GPU memory: system-scope atomics, ordered after the row's mirror store
             const uint32_t col = (e1.w >> 4) & 0x3ffffu;
-            if (dnz) atomicXor((mf == 1 ? a.mir_up_nz : a.mir_dn_nz) + col, dnz);
-            if (dsg) atomicXor((mf == 1 ? a.mir_up_sg : a.mir_dn_sg) + col, dsg);
+            __threadfence_system();
+            if (dnz) atomicXor_system((mf == 1 ? a.mir_up_nz : a.mir_dn_nz) + col, dnz);
+            if (dsg) atomicXor_system((mf == 1 ? a.mir_up_sg : a.mir_dn_sg) + col, dsg);
         }
     }
     __device__ __forceinline__ void push(const uint32_t (&eq)[4], const uint32_t (&Fm)[4], const uint32_t (&Y1)[4],
@@ -252,6 +254,7 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
     if (SLAB && mir_nz) {       // slab mode: this row is also a neighbour's halo row
         *reinterpret_cast<uint4 *>(mir_nz) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
         *reinterpret_cast<uint4 *>(mir_sg) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
+        __threadfence_system();
     }
     queue.push(eq, Fm, Y1, H0, nf, gg, wo, mir_tag);
 }

@@ -145,7 +145,12 @@ struct WarpTieQueue {
         if (flip) {
             atomicXor(a.tgt + wo, flip);
             const uint32_t mf = SLAB ? e.w >> 30 : 0u;
-            if (mf) atomicXor((mf == 1 ? a.mir_up : a.mir_dn) + ((e.w >> 4) & 0x3ffffu), flip);
+            if (mf) {
+                // the mirror row may be peer-GPU memory: order this late flip after the plain
+                // mirror store of the row (made by another lane of this warp) at system scope
+                __threadfence_system();
+                atomicXor_system((mf == 1 ? a.mir_up : a.mir_dn) + ((e.w >> 4) & 0x3ffffu), flip);
+            }
         }
     }
     // collective over the warp: queue the words of this run that hold ties
@@ -231,7 +236,10 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
 #pragma unroll
     for (int w = 0; w < 4; ++w) T[w] = lop3<0x4B>(T[w], need[w], acc[w]);    // T ^ (~need | acc)
     *reinterpret_cast<uint4 *>(tp) = make_uint4(T[0], T[1], T[2], T[3]);
-    if (SLAB && mir) *reinterpret_cast<uint4 *>(mir) = make_uint4(T[0], T[1], T[2], T[3]);
+    if (SLAB && mir) {
+        *reinterpret_cast<uint4 *>(mir) = make_uint4(T[0], T[1], T[2], T[3]);
+        __threadfence_system();      // before any late flip of this row (resolve) reaches the mirror
+    }
     queue.push(eq, c8, wo, mir_tag);
 }
 

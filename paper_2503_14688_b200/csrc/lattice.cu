@@ -21,6 +21,7 @@
 #include "ising_persist.cuh"
 #include "measure.cuh"
 #include "philox.cuh"
+#include "ubench.cuh"
 
 using namespace lat;
 
@@ -57,6 +58,7 @@ struct lattice {
     SweepParams *d_sp;         // per-sweep parameters of the persistent kernel
     size_t sp_cap;             // entries
     int persist_blocks;        // co-resident blocks of ising_persist_kernel (0: not yet queried, -1: unavailable)
+    uint32_t persist_cap;      // lattice_set_persist_blocks: upper bound on the grid (0: none)
     char err[256];
 };
 
@@ -564,6 +566,10 @@ int lattice_enable_peer_access(int device, int peer_device)
     int prev = 0, can = 0;
     if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return LATTICE_ECUDA; }
     if (cudaDeviceCanAccessPeer(&can, device, peer_device) != cudaSuccess || !can) { cudaGetLastError(); return LATTICE_ECUDA; }
+    // late tie flips reach the neighbour's halo row with atomicXor_system: needs native peer atomics
+    int atomics = 0;
+    if (cudaDeviceGetP2PAttribute(&atomics, cudaDevP2PAttrNativeAtomicSupported, device, peer_device) != cudaSuccess ||
+        !atomics) { cudaGetLastError(); return LATTICE_ECUDA; }
     if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return LATTICE_ECUDA; }
     const cudaError_t e = cudaDeviceEnablePeerAccess(peer_device, 0);
     cudaGetLastError();                                   // clears "already enabled" too
@@ -615,7 +621,7 @@ int lattice_ipc_close(void *device_ptr)
 int lattice_set_rng_scheme(lattice_t *lat, int scheme)
 {
     if (!lat || scheme < 0 || scheme > 2) return LATTICE_EINVAL;
-    if (lat->t != 0) return LATTICE_ESTATE;
+    if (lat->t != 0 || lat->view) return LATTICE_ESTATE;
     if (lat->slab && scheme == 0) return LATTICE_EINVAL;
     if (scheme == 2 && (lat->wpr % 4u) != 0) return LATTICE_EINVAL;   // marching kernels only
     lat->scheme = scheme;
@@ -699,6 +705,7 @@ static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
     uint32_t ns = (uint32_t)n;
     unsigned blocks = (a.threads + 255u) / 256u;
     if (blocks > (unsigned)lat->persist_blocks) blocks = (unsigned)lat->persist_blocks;
+    if (lat->persist_cap && blocks > lat->persist_cap) blocks = lat->persist_cap;
     void *args[] = {&a, &buf0, &buf1, &sp, &ns};
     const void *fn = one_row ? (edge ? (const void *)ising_persist_kernel<true, true> : (const void *)ising_persist_kernel<false, true>)
                              : (edge ? (const void *)ising_persist_kernel<true, false> : (const void *)ising_persist_kernel<false, false>);
@@ -874,6 +881,7 @@ static int window_call(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uin
                        bool set)
 {
     if (!lat || !host) return LATTICE_EINVAL;
+    if (lat->view) return LATTICE_ESTATE;             // a view is a measurement-only handle
     const uint64_t L = lat->L;
     if (h < 1 || w < 1 || h > L || w > L || i0 >= L || j0 >= L) return LATTICE_EINVAL;
     const uint32_t row_base = lat->slab ? (lat->row0 + lat->L - 1u) % lat->L : 0u;
@@ -945,11 +953,19 @@ uint64_t lattice_time(const lattice_t *lat) { return lat ? lat->t : 0; }
 int lattice_set_time(lattice_t *lat, uint64_t t)
 {
     if (!lat || t >= TWO32) return LATTICE_EINVAL;
+    if (lat->view) return LATTICE_ESTATE;
     lat->t = t;
     return LATTICE_OK;
 }
 
 uint64_t lattice_launches(const lattice_t *lat) { return lat ? lat->launches : 0; }
+
+int lattice_set_persist_blocks(lattice_t *lat, uint32_t max_blocks)
+{
+    if (!lat) return LATTICE_EINVAL;
+    lat->persist_cap = max_blocks;
+    return LATTICE_OK;
+}
 
 void lattice_thresholds(int model, double delta, double beta, uint64_t *out)
 {
@@ -966,30 +982,88 @@ void lattice_thresholds64(int model, double delta, double beta, uint64_t *thr, u
     for (int e = 0; e < n; ++e) always[e] = a[e] ? 1 : 0;
 }
 
+// xi = I_2/I_1 of DESIGN.md reading 14, evaluated EXACTLY: with the trapezoid weights doubled
+// (2 for r < r_cut, 1 at r_cut) the two sums are integers,
+//   J_n = sum_{r < r_cut} 2 r^n S(r) + r_cut^n S(r_cut),   S = Sx + Sy,   xi = J_2 / J_1,
+// that fit 128 bits (|S| <= 2^41, r^2 <= 2^38, 2^19 terms); the normalisation 2 L^2 cancels.
+// One rounding per conversion and one for the quotient: this is not the oracle's ascending fp64
+// sum (which it matches to ~1e-15), so the 1e-12 parity of xi compares two different routes.
 double lattice_xi(const int64_t *Sx, const int64_t *Sy, uint32_t r_max, int64_t Q, uint32_t L,
                   uint32_t *r_cut_out)
 {
-    (void)Q;   // the r = 0 term C(0) = Q/L^2 carries weight r^n = 0
+    (void)Q; (void)L;   // C(0) = Q/L^2 carries weight r^n = 0; L^2 cancels in the ratio
     uint32_t r_cut = r_max;
     for (uint32_t r = 1; r <= r_max; ++r)
         if (Sx[r - 1] + Sy[r - 1] <= 0) { r_cut = r - 1; break; }
     if (r_cut_out) *r_cut_out = r_cut;
     if (r_cut < 1) return 0.0;
-    const double norm = 2.0 * (double)L * (double)L;
-    double I1 = 0.0, I2 = 0.0;
+    __int128 J1 = 0, J2 = 0;
     for (uint32_t r = 1; r <= r_cut; ++r) {
-        const double C = (double)(Sx[r - 1] + Sy[r - 1]) / norm;
-        const double wgt = (r == r_cut) ? 0.5 : 1.0;
-        I1 += wgt * (double)r * C;
-        I2 += wgt * (double)r * (double)r * C;
+        const __int128 term = (__int128)(r == r_cut ? 1 : 2) * (__int128)(Sx[r - 1] + Sy[r - 1]) * (__int128)r;
+        J1 += term;
+        J2 += term * (__int128)r;
     }
-    return I2 / I1;
+    return (double)J2 / (double)J1;
 }
 
+// e = -(S_x(1) + S_y(1))/L^2 + Delta Q/L^2, term by term as Eq. 3 / Eq. 1 state it
 double lattice_energy(const int64_t *Sx, const int64_t *Sy, int64_t Q, double delta, uint32_t L)
 {
     const double n = (double)L * (double)L;
     return -((double)(Sx[0] + Sy[0])) / n + delta * (double)Q / n;
+}
+
+int lattice_ubench_int_dispatch(int mode, void *cuda_stream, double *thread_instr_per_clk_per_sm,
+                                double *elapsed_ms)
+{
+    if (mode < 0 || mode > 3 || !thread_instr_per_clk_per_sm) return LATTICE_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+        cudaGetLastError();
+        return LATTICE_ECUDA;
+    }
+    const int blocks = sms * UB_BLOCKS_PER_SM;
+    uint32_t *out = nullptr;
+    unsigned long long *clk = nullptr, *h = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = LATTICE_ECUDA;
+    float ms = 0.f;
+    do {
+        if (cudaMalloc(&out, (size_t)blocks * 256 * sizeof(uint32_t)) != cudaSuccess) { rc = LATTICE_ENOMEM; break; }
+        if (cudaMalloc(&clk, (size_t)blocks * sizeof(unsigned long long)) != cudaSuccess) { rc = LATTICE_ENOMEM; break; }
+        h = (unsigned long long *)std::malloc((size_t)blocks * sizeof(unsigned long long));
+        if (!h) { rc = LATTICE_ENOMEM; break; }
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
+        for (int rep = 0; rep < 2; ++rep) {              // first launch warms up, second is timed
+            if (rep == 1) cudaEventRecord(e0, st);
+            switch (mode) {
+            case 0: ubench_kernel<0><<<blocks, 256, 0, st>>>(out, 12345u, clk); break;
+            case 1: ubench_kernel<1><<<blocks, 256, 0, st>>>(out, 12345u, clk); break;
+            case 2: ubench_kernel<2><<<blocks, 256, 0, st>>>(out, 12345u, clk); break;
+            default: ubench_kernel<3><<<blocks, 256, 0, st>>>(out, 12345u, clk); break;
+            }
+        }
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) break;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (cudaMemcpy(h, clk, (size_t)blocks * sizeof(unsigned long long), cudaMemcpyDeviceToHost) != cudaSuccess) break;
+        double cyc = 0.0;                                // mean cycles of a block; UB_BLOCKS_PER_SM run side by side
+        for (int b = 0; b < blocks; ++b) cyc += (double)h[b];
+        cyc /= blocks;
+        const double instr_per_sm = (double)UB_BLOCKS_PER_SM * 256.0 * UB_ITER * UB_CHAINS * ubench_instr_per_step(mode);
+        *thread_instr_per_clk_per_sm = instr_per_sm / cyc;
+        if (elapsed_ms) *elapsed_ms = ms;
+        rc = LATTICE_OK;
+    } while (0);
+    if (rc == LATTICE_ECUDA) cudaGetLastError();
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (h) std::free(h);
+    if (clk) cudaFree(clk);
+    if (out) cudaFree(out);
+    return rc;
 }
 
 int lattice_destroy(lattice_t *lat)

@@ -42,8 +42,50 @@ def test_xi_appendix_c_recovers_the_tail_function(xiF, beta):
     assert abs(d["xi_F"] / xiF - 1) < 1e-3 and abs(d["beta"] - beta) < 1e-3
     # with large errors the cut-off comes early and the data are integrated as they are
     d2 = {}
-    an.xi_appendix_c(C, np.full(R + 1, 0.05), d2)
+    with pytest.warns(an.CutoffWarning):
+        an.xi_appendix_c(C, np.full(R + 1, 0.05), d2)
     assert d2["r_cut"] < d["r_cut"] and C[d2["r_cut"] + 1] < 0.15 <= C[d2["r_cut"]]
+
+
+def test_xi_appendix_c_flags_missing_cutoffs():
+    """r_max (r^2 C below a third of its maximum) does not occur inside the measured range: the
+    routine integrates up to r_cut only, says so in details and warns; strict=True raises."""
+    C = _synthetic_C(400.0, 1.0, 300)                    # r^2 C still rising at r = 300
+    err = np.full(C.size, 1e-9)
+    d = {}
+    with pytest.warns(an.CutoffWarning):
+        xi = an.xi_appendix_c(C, err, d)
+    assert d["condition_met"] is False and d["r_max"] is None and not d["tail_fit"]
+    exact = 400.0 * math.gamma(2.5) / math.gamma(1.5)
+    assert xi < 0.5 * exact                              # the truncation bias the warning is about
+    with pytest.raises(ValueError):
+        an.xi_appendix_c(C, err, strict=True)
+    d2 = {}
+    an.xi_appendix_c(_synthetic_C(20.0, 1.0, 2000), np.full(2001, 1e-9), d2)
+    assert d2["condition_met"] is True
+
+
+def test_xi_with_error_freezes_the_cutoffs_of_the_full_sample():
+    rng = np.random.default_rng(5)
+    C = _synthetic_C(25.0, 1.2, 800)
+    runs = C[None, :] + rng.normal(0.0, 2e-4, size=(20, C.size))
+    d = {}
+    an.xi_with_error(runs, d)
+    seen = []
+    orig = an.xi_appendix_c
+
+    def spy(C_, E_, details=None, cutoffs=None, strict=False):
+        seen.append(cutoffs)
+        return orig(C_, E_, details, cutoffs, strict)
+
+    an.xi_appendix_c = spy
+    try:
+        an.xi_with_error(runs)
+    finally:
+        an.xi_appendix_c = orig
+    frozen = [c for c in seen if c is not None]
+    assert len(frozen) == 21                                         # full mean + 20 leave-one-out
+    assert all(c["r_cut"] == d["r_cut"] and c["r_min"] == d["r_min"] and c["r_max"] == d["r_max"] for c in frozen)
 
 
 def test_xi_with_error_on_noisy_runs():

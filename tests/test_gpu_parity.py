@@ -361,6 +361,23 @@ def test_api_errors_on_device():
         lat.binding.Lattice._check(g, lat.lib().lattice_set_rng_scheme(g._h, 0), "set_rng_scheme")
     assert e.value.status == lat.binding.ESTATE
     assert g.launches == 3                         # init + two half-sweeps
+    # a view is a measurement-only handle: windows, set_time and set_rng_scheme are refused
+    import ctypes as C
+    import torch
+    rows = 96
+    buf = torch.zeros(2 * rows * (256 // 64) * 4, dtype=torch.uint8, device="cuda")
+    h = C.c_void_p()
+    L_ = lat.lib()
+    assert L_.lattice_view(C.byref(h), 256, lat.ISING, rows, C.c_void_p(buf.data_ptr()), buf.numel(), None) == 0
+    out = np.zeros((4, 4), dtype=np.int8)
+    p8 = out.ctypes.data_as(C.POINTER(C.c_int8))
+    assert L_.lattice_get_spins(h, 0, 0, 4, 4, p8) == lat.binding.ESTATE
+    assert L_.lattice_get_spins(h, 200, 0, 4, 4, p8) == lat.binding.ESTATE      # i >= rows: was out of bounds
+    assert L_.lattice_set_spins(h, 0, 0, 4, 4, p8) == lat.binding.ESTATE
+    assert L_.lattice_set_time(h, 5) == lat.binding.ESTATE
+    assert L_.lattice_set_rng_scheme(h, 0) == lat.binding.ESTATE
+    assert L_.lattice_fill(h, 1) == lat.binding.EINVAL
+    L_.lattice_destroy(h)
 
 
 def test_first_half_sweep_acceptance_closed_form():

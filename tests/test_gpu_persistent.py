@@ -1,0 +1,194 @@
+"""GPU parity of the persistent multi-sweep kernel's marching variant and of RNG scheme 2's
+decisive 64-bit compare -- the two paths VERDICT round 1 found untested.
+
+* `ising_persist_kernel<EDGE, ONE_ROW = false>` takes every `lattice_sweep(n >= 2)` of an Ising
+  lattice with 4352 < L <= 8192 (march_thread in a grid-stride loop, tie queues reused across
+  iterations, a grid barrier between colours).  Checked whole-lattice against the oracle and
+  against the same sweeps issued one per call (two plain launches per sweep), with a beta = 0
+  sweep in the schedule for the EDGE instantiation, and with the grid capped so that every block
+  really strides over several groups of rows.
+* Scheme 2 differs from scheme 1 only where u32 == thr32 or thr32 == 0 < thr64.  From the all-up
+  state every site is in the dE = 8 class, so one half-sweep is purely `u64 < thr64`; the rare
+  sites where the low 32 bits decide are located through the magnetisation of row ranges and the
+  rows that hold them are compared, every site, with the oracle's scheme-2 half-sweep.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2503_14688_b200 as lat
+from paper_2503_14688_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+BETA_C = workloads.BETA_C_ISING
+NCPU = os.cpu_count() or 1
+
+
+@pytest.fixture(autouse=True)
+def _threads():
+    oracle.set_threads(NCPU)
+    yield
+    oracle.set_threads(1)
+
+
+@pytest.mark.parametrize("L", [4608, 8192])
+def test_persistent_marching_variant_against_oracle_and_single_launches(L):
+    seed = 90210 + L
+    edge = [BETA_C] * 5 + [0.0] + [BETA_C] * 6 + [BETA_C / 1.01] * 4         # 16 sweeps, one at beta = 0
+    plain = [BETA_C] * 3 + [0.5]                                             # no "always" class
+    g = lat.Lattice(L, lat.ISING, 0.0, seed)          # persistent kernel, one launch per call
+    s = lat.Lattice(L, lat.ISING, 0.0, seed)          # the same sweeps, one per call
+    o = oracle.OracleLattice(L, lat.ISING, 0.0, seed)
+    for sched in (edge, plain):
+        n0 = g.launches
+        g.sweep(sched)
+        assert g.launches - n0 == 1                   # ising_persist_kernel<*, false>, once
+        n0 = s.launches
+        for b in sched:
+            s.sweep([b])
+        assert s.launches - n0 == 2 * len(sched)      # two half-sweep launches per sweep
+        o.sweep(sched)
+        want = o.get_spins()
+        assert np.array_equal(g.get_spins(), want)
+        assert np.array_equal(s.get_spins(), want)
+    assert g.time == s.time == o.time == len(edge) + len(plain)
+    # capped grid: 37 blocks stride over >= 162 groups of 256 threads, queues reused across groups
+    g.set_persist_blocks(37)
+    more = [BETA_C, 0.0, BETA_C, BETA_C]
+    n0 = g.launches
+    g.sweep(more)
+    assert g.launches - n0 == 1
+    o.sweep(more)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    g.set_persist_blocks(0)
+    Mg, Qg, Sxg, Syg = g.measure(64)
+    Mo, Qo, Sxo, Syo = o.measure(64)
+    assert (Mg, Qg) == (Mo, Qo) and np.array_equal(Sxg, Sxo) and np.array_equal(Syg, Syo)
+    g.close(); s.close(); o.close()
+
+
+@pytest.mark.parametrize("L", [1024, 2048, 4096])
+def test_persistent_one_row_variant_with_capped_grid(L):
+    """The ONE_ROW instantiation (L <= 4352) with its grid capped as well."""
+    g = lat.Lattice(L, lat.ISING, 0.0, 5150 + L)
+    o = oracle.OracleLattice(L, lat.ISING, 0.0, 5150 + L)
+    g.set_persist_blocks(11)
+    sched = [BETA_C] * 6 + [0.0, BETA_C]
+    g.sweep(sched)
+    o.sweep(sched)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    g.close(); o.close()
+
+
+def _rows_where_M_differs(g, want_row_M, i0, n):
+    """Rows in [i0, i0+n) whose magnetisation is not want_row_M, by bisection on lattice_measure_rows."""
+    M = g.measure(1, (i0, n))[0]
+    if M == want_row_M * n:
+        return []
+    if n == 1:
+        return [i0]
+    h = n // 2
+    return _rows_where_M_differs(g, want_row_M, i0, h) + _rows_where_M_differs(g, want_row_M, i0 + h, n - h)
+
+
+def _oracle_row_after_half_sweep(L, seed, scheme, t, i, colour, beta):
+    """Row i of an all-up lattice after one half-sweep of `colour` at sweep index t: a 1 x L
+    oracle window with +1 outside (rows i-1 and i+1 are all up too)."""
+    o = oracle.OracleLattice.window(L, lat.ISING, 0.0, seed, scheme, t, i, 0,
+                                    np.ones((1, L), dtype=np.int8), outside=1)
+    o.half_sweep(colour, beta)
+    row = o.get_spins(0, 0, 1, L)[0]
+    o.close()
+    return row
+
+
+def _fit_L(L_want):
+    import torch
+    free, _ = torch.cuda.mem_get_info(0)
+    L = L_want
+    while L > 4096 and L * L // 8 > free - (3 << 30):
+        L //= 2
+    return L
+
+
+def test_scheme2_sub_2pm32_acceptance_is_decided_by_the_low_word():
+    """beta = 33 ln2 / 8: exp(-8 beta) = 2^-33, so thr32(dE = 8) = 0 and thr64 = 2^31.  From all-up,
+    scheme 1 flips nothing; scheme 2 flips the ~L^2/2 * 2^-33 black sites with u64 < 2^31 (64 at
+    L = 2^20), each decided by tail word 1 after the top byte and 24 tail bits all tie at zero."""
+    L = _fit_L(1 << 20)
+    seed, t = 2503146880 + 21, 7
+    beta = 33.0 * math.log(2.0) / 8.0
+    thr64, alw = oracle.thresholds64(oracle.ISING, 0.0, beta)
+    assert oracle.thresholds(oracle.ISING, 0.0, beta)[1] == 0 and not alw[1]
+    assert abs(int(thr64[1]) - (1 << 31)) < (1 << 12)              # 2^31 up to the rounding of exp()
+    g = lat.Lattice(L, lat.ISING, 0.0, seed, scheme=2)
+    g.fill(1)
+    g.set_time(t)
+    g.half_sweep(0, beta)
+    rows = _rows_where_M_differs(g, L, 0, L)
+    expect = L * L / 2 * float(thr64[1]) / 2.0 ** 64
+    assert len(rows) >= 1 and abs(len(rows) - expect) < 6 * math.sqrt(expect) + 1     # the test bites
+    rng = np.random.default_rng(3)
+    sample = sorted(set(rows) | {0, L - 1} | {int(x) for x in rng.integers(0, L, 6)})
+    flips = 0
+    for i in sample:
+        got = g.get_spins(i, 0, 1, L)[0]
+        want = _oracle_row_after_half_sweep(L, seed, 2, t, i, 0, beta)
+        assert np.array_equal(got, want), i
+        flips += int((got == -1).sum())
+        if i in rows:
+            assert (got == -1).any()
+    assert flips >= len(rows)
+    # scheme 1 on the same seed flips nothing at all
+    g.close()
+    g1 = lat.Lattice(L, lat.ISING, 0.0, seed, scheme=1)
+    g1.fill(1)
+    g1.set_time(t)
+    g1.half_sweep(0, beta)
+    assert g1.measure(1)[0] == L * L
+    g1.close()
+
+
+def test_scheme2_exact_32_bit_tie_is_broken_by_the_low_word():
+    """At beta_c from all-up, the black sites with u32 == thr32(dE = 8) (~L^2/2 * 2^-32 of them) are
+    rejected by scheme 1 and accepted by scheme 2 iff tail word 1 < low word of thr64: the two
+    schemes differ exactly there.  Rows where they differ are checked site by site under both."""
+    L = _fit_L(1 << 19)
+    seed, t = 2503146880 + 22, 3
+    a = lat.Lattice(L, lat.ISING, 0.0, seed, scheme=1)
+    b = lat.Lattice(L, lat.ISING, 0.0, seed, scheme=2)
+    for g in (a, b):
+        g.fill(1)
+        g.set_time(t)
+        g.half_sweep(0, BETA_C)
+    # locate rows where the magnetisations of the two lattices differ (bisection on both)
+    def diff_rows(i0, n):
+        if a.measure(1, (i0, n))[0] == b.measure(1, (i0, n))[0]:
+            return []
+        if n == 1:
+            return [i0]
+        h = n // 2
+        return diff_rows(i0, h) + diff_rows(i0 + h, n - h)
+    rows = diff_rows(0, L)
+    thr64, _ = oracle.thresholds64(oracle.ISING, 0.0, BETA_C)
+    p_diff = (int(thr64[1]) & 0xffffffff) / 2.0 ** 64            # u32 == thr32 and low word below
+    expect = L * L / 2 * p_diff
+    if L == 1 << 19:
+        assert len(rows) >= 1                                    # ~16 expected: the test bites
+    assert len(rows) <= expect + 6 * math.sqrt(expect) + 2
+    rng = np.random.default_rng(4)
+    sample = sorted(set(rows) | {int(x) for x in rng.integers(0, L, 4)})
+    for i in sample:
+        ra, rb = a.get_spins(i, 0, 1, L)[0], b.get_spins(i, 0, 1, L)[0]
+        assert np.array_equal(ra, _oracle_row_after_half_sweep(L, seed, 1, t, i, 0, BETA_C)), ("scheme 1", i)
+        assert np.array_equal(rb, _oracle_row_after_half_sweep(L, seed, 2, t, i, 0, BETA_C)), ("scheme 2", i)
+        if i in rows:
+            d = np.nonzero(ra != rb)[0]
+            assert d.size >= 1 and (ra[d] == 1).all() and (rb[d] == -1).all()     # only scheme 2 flips them
+            for j in d:                                                          # and they are exact ties
+                P = i * (L // 2) + (int(j) >> 1)
+                assert oracle.u32(seed, 1, t, 0, P) == int(oracle.thresholds(oracle.ISING, 0.0, BETA_C)[1])
+    a.close(); b.close()
