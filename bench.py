@@ -6,20 +6,33 @@
 A "step" is one full-lattice Metropolis sweep (black half-sweep + white half-sweep, thresholds
 rebuilt from the step's beta on the host) of BASELINE.json's throughput configuration:
 2D Ising, L = 2^20 (128 GiB at 1 bit/spin), disordered start, beta_c.  If the device cannot
-hold 128 GiB the largest power-of-two L that fits is used and named in config.workload.
+hold 128 GiB the largest power-of-two L that fits is used and named in config.workload.  For
+workloads whose sweep takes less than ~2 s / K a step is `sweeps_per_step` sweeps issued as ONE
+lattice_sweep(n) call (the persistent multi-sweep path where it applies), chosen so that the K
+timed steps last at least --min-seconds (default 2 s): every quoted number then has clock
+samples (config.sweeps_per_step says how many).
 
 One JSON line is printed by rank 0:
   value     whole-job spin updates/ns, device-timed (CUDA events), lattice resident in HBM
   e2e       the same metric through the C-ABI with host buffers every step: the step's beta goes
             in as a host fp64 array and the step's result (M, Q, S_x(1), S_y(1) -> e, m) comes
             back to host memory (lattice_sweep + lattice_measure), all inside the timed region
-  roofline  the binding roofline of the dominant kernel (the half-sweep): "bound": "alu" -- thread-
-            instructions of the 16-lane integer dispatch class per launch / mean launch time,
-            against 148 SM x 64 lanes x the sampled SM clock
+  roofline  the binding roofline of the dominant kernel (the half-sweep): "bound": "alu" --
+            ALGORITHMIC thread-instructions of the half-rate dispatch class per launch (hand
+            count) / mean launch time measured here, against a peak MEASURED
+            in this run: lattice_ubench_int_dispatch lanes/clk/SM x SMs x the sampled SM clock.
+            `executed_frac` and `traffic` use constants from the committed ncu capture named in
+            `profile` (not from this run; `stale_profile` says whether the kernel sources changed
+            since that capture)
   roofline_hbm  the HBM roofline BASELINE.json's metric asks for: algorithmic bytes (0.375
             B/update Ising, 0.75 BC: read both colours once, write one) / mean launch time,
             against the measured copy bandwidth in MEASURED_PEAKS.json
-  cpu_baseline  the oracle, as it stands, on the host cores over a bounded sample
+  blume_capel   (default invocation, 1 GPU) the same measurements for Blume-Capel at the paper's
+            size (L = 2^19) and for BASELINE config 5b (L = 2^15, beta ramp), each
+            with its own value, e2e, roofline, roofline_hbm and clocks
+  cpu_baseline  the oracle, as it stands, on the host cores over bounded samples: `value` is the
+            all-cores figure for the timed model and RNG scheme; `matrix` holds 1 thread and all
+            cores x schemes 0/1 x both models, `cpu_model` the CPU
   measure   the measurement pass (M, Q, C(r) on both axes) timed separately after the sweeps
 
 N > 1 (torchrun): the path is specified for one GPU with no collectives (BASELINE.json
@@ -36,6 +49,7 @@ import os
 import subprocess
 import sys
 import tempfile
+import threading
 import time
 
 import numpy as np
@@ -44,24 +58,13 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_2503_14688_b200 import profile_constants as pc  # noqa: E402
 from paper_2503_14688_b200 import workloads  # noqa: E402
 
 METRIC = "spin updates/ns per B200 (Ising & Blume-Capel) and % of HBM roofline"
 UNIT = "spin updates/ns"
-BYTES_PER_UPDATE = {workloads.ISING: 0.375, workloads.BLUME_CAPEL: 0.75}
-# Integer-pipe roofline of the dominant kernel: thread-instructions of the
-# half-rate class (ALU pipe: LOP3/SHF/SEL/ISETP..., plus IMAD.WIDE/IMAD.HI, which block the same
-# 16-lane dispatch for two cycles) per spin update.
-#   ALGORITHMIC: the floor of the method under the RNG contract (folded Philox planes, 2 LOP3 per
-#   word per plane of compare, class logic, 2^-8 tails), the analogue of algorithmic bytes;
-#   EXECUTED: from the committed ncu captures under profiles/ (sm__inst_executed_pipe_alu +
-#   IMAD.WIDE/HI counts / updates per launch).
-ALG_HALF_RATE_INSTR_PER_UPDATE = {workloads.ISING: 2.98, workloads.BLUME_CAPEL: 4.46}
-EXE_HALF_RATE_INSTR_PER_UPDATE = {workloads.ISING: 3.39, workloads.BLUME_CAPEL: 5.30}
-#: DRAM bytes per update measured by ncu (dram__bytes_read.sum + dram__bytes_write.sum) / updates
-DRAM_BYTES_PER_UPDATE_NCU = {workloads.ISING: 0.383, workloads.BLUME_CAPEL: 0.667}
-SM_COUNT, HALF_RATE_LANES_PER_CLK_PER_SM = 148, 64
 KERNEL = {workloads.ISING: "ising_march_kernel", workloads.BLUME_CAPEL: "bc_march_kernel"}
+MODEL_NAME = ["ising", "blume-capel"]
 
 
 def measured_peaks():
@@ -73,71 +76,170 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
 
 
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 class ClockSampler:
-    """nvidia-smi clock/throttle samples during the timed region (profiling recipe's line)."""
-    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
-              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons of one GPU during a timed region.
 
-    def __init__(self, index: int):
-        self.index, self.proc, self.path = index, None, None
+    In-process through NVML (pynvml): one sample when the region starts, one every 20 ms from a
+    thread, one when it ends -- so even a region of a few milliseconds has >= 2 samples.  If
+    NVML cannot be loaded the profiling recipe's `nvidia-smi -lms` line is used instead."""
+    BAD = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+           0x80: "hw_power_brake_slowdown"}
+    NOTE = {0x4: "sw_power_cap"}
+    SMI_FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+                  "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                  "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def start(self):
+    def __init__(self, torch, dev):
+        self.nv, self.h, self.index = None, None, dev.index or 0
+        self.sm, self.reasons, self.power = [], set(), []
+        self.sm_max = None
+        self._stop, self._thr, self._smi, self._smi_path = threading.Event(), None, None, None
         try:
-            fd, self.path = tempfile.mkstemp(suffix=".csv")
-            os.close(fd)
-            self.proc = subprocess.Popen(
-                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
-                 "--format=csv,noheader,nounits", "-lms", "100"],
-                stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+            import pynvml
+            pynvml.nvmlInit()
+            uuid = getattr(torch.cuda.get_device_properties(dev), "uuid", None)
+            h = None
+            if uuid is not None:
+                for cand in (f"GPU-{uuid}", str(uuid)):
+                    try:
+                        h = pynvml.nvmlDeviceGetHandleByUUID(cand.encode() if isinstance(cand, str) else cand)
+                        break
+                    except Exception:
+                        h = None
+            if h is None:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+                ids = [v for v in vis.split(",") if v.strip().isdigit()]
+                phys = int(ids[self.index]) if self.index < len(ids) else self.index
+                h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.nv, self.h = pynvml, h
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
         except Exception:
-            self.proc = None
+            self.nv = None
 
-    def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.proc is None:
-            return out
-        self.proc.terminate()
+    def _sample(self):
+        nv = self.nv
         try:
-            self.proc.wait(timeout=5)
-        except Exception:
-            self.proc.kill()
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        try:
-            for line in open(self.path):
-                f = [x.strip() for x in line.split(",")]
-                if len(f) < 9:
-                    continue
-                try:
-                    sm.append(float(f[1])); mx.append(float(f[2]))
-                except ValueError:
-                    continue
-                for name, v in zip(names, f[5:9]):
-                    if v.lower().startswith("active"):
-                        reasons.add(name)
-            os.unlink(self.path)
+            self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+            try:
+                mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+            except Exception:
+                mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            for bit, name in {**self.BAD, **self.NOTE}.items():
+                if mask & bit:
+                    self.reasons.add(name)
+            self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
         except Exception:
             pass
-        if sm:
-            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
-        out["reasons"] = sorted(reasons)
+
+    def _loop(self):
+        while not self._stop.wait(0.02):
+            self._sample()
+
+    def start(self):
+        self.sm, self.reasons, self.power = [], set(), []
+        self._stop.clear()
+        if self.nv is not None:
+            self._sample()
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+            return
+        try:
+            fd, self._smi_path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self._smi = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.SMI_FIELDS}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=open(self._smi_path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self._smi = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": 0, "source": "none"}
+        if self.nv is not None:
+            self._stop.set()
+            if self._thr is not None:
+                self._thr.join(timeout=2)
+            self._sample()
+            out["source"] = "nvml in-process, 20 ms"
+        elif self._smi is not None:
+            self._smi.terminate()
+            try:
+                self._smi.wait(timeout=5)
+            except Exception:
+                self._smi.kill()
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            mx = []
+            try:
+                for line in open(self._smi_path):
+                    f = [x.strip() for x in line.split(",")]
+                    if len(f) < 9:
+                        continue
+                    try:
+                        self.sm.append(float(f[1])); mx.append(float(f[2]))
+                    except ValueError:
+                        continue
+                    for name, v in zip(names, f[5:9]):
+                        if v.lower().startswith("active"):
+                            self.reasons.add(name)
+                os.unlink(self._smi_path)
+            except Exception:
+                pass
+            if mx:
+                out["sm_max_mhz"] = float(max(mx))
+            out["source"] = "nvidia-smi -lms 100"
+        if self.sm:
+            out.update(sm_mhz=float(np.median(self.sm)), sm_min_mhz=float(min(self.sm)), samples=len(self.sm))
+        if self.power:
+            out["power_w_max"] = float(max(self.power))
+        out["reasons"] = sorted(self.reasons)
         return out
 
 
-def oracle_rate(w, L, sweeps, scheme=1):
-    """Updates/ns of the CPU oracle (all host cores) on `sweeps` sweeps of an L x L sample."""
+def oracle_rate(model, delta, seed, beta, L, sweeps, scheme=1, threads=None):
+    """Updates/ns of the CPU oracle on `sweeps` sweeps of an L x L sample; (rate, seconds, threads)."""
     import oracle
     oracle.build()
-    cores = os.cpu_count() or 1
-    oracle.set_threads(cores)
-    o = oracle.OracleLattice(L, w.model, w.delta, w.seed, scheme)
-    beta = w.beta_schedule(sweeps)
+    oracle.set_threads(threads or os.cpu_count() or 1)
+    used = oracle.get_threads()
+    o = oracle.OracleLattice(L, model, delta, seed, scheme)
+    b = np.full(sweeps, beta, dtype=np.float64)
     t0 = time.perf_counter()
-    o.sweep(beta)
+    o.sweep(b)
     dt = time.perf_counter() - t0
     o.close()
-    return L * L * sweeps / dt / 1e9, dt, oracle.get_threads()
+    return L * L * sweeps / dt / 1e9, dt, used
+
+
+def cpu_baseline_matrix(w, scheme):
+    """BASELINE.md section 3 / SURVEY.md section 8(d): the oracle as it stands, 1 thread and all host cores,
+    RNG schemes 0 and 1, both models, on bounded samples (~2 s each, ~20 s in total)."""
+    cores = os.cpu_count() or 1
+    rows = []
+    for model, delta, beta in ((workloads.ISING, 0.0, workloads.BETA_C_ISING),
+                               (workloads.BLUME_CAPEL, 0.0, workloads.BETA_BC)):
+        for sch in (0, 1):
+            for thr, L, ns in ((1, 1024, 8), (cores, 4096, 8)):
+                rate, dt, used = oracle_rate(model, delta, w.seed, beta, L, ns, sch, thr)
+                rows.append({"model": MODEL_NAME[model], "rng_scheme": sch, "threads": used, "value": rate,
+                             "unit": UNIT, "sample": f"{ns} sweeps of {L}x{L}", "seconds": round(dt, 2)})
+    beta0 = float(w.beta_schedule(1)[0])
+    Ls, ns = min(w.L, 4096), 48
+    rate, dt, used = oracle_rate(w.model, w.delta, w.seed, beta0, Ls, ns, scheme, cores)
+    return {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle", "cpu_model": cpu_model(),
+            "sample": f"{ns} sweeps of a {Ls}x{Ls} lattice of the timed model ({MODEL_NAME[w.model]}), "
+                      f"beta and RNG scheme {scheme} ({dt:.1f} s); matrix: 8 sweeps of 1024^2 (1 thread) / "
+                      f"4096^2 (all cores)",
+            "matrix": rows}
 
 
 def run_reference(args):
@@ -147,10 +249,11 @@ def run_reference(args):
         return
     w = workloads.CONFIGS[args.workload]
     Ls, ns = min(w.L, 4096), 8                   # one step = 8 sweeps of a 4096 x 4096 sample (~1 s)
+    beta0 = float(w.beta_schedule(1)[0])
     for _ in range(args.warmup):
-        oracle_rate(w, 256, 1)
+        oracle_rate(w.model, w.delta, w.seed, beta0, 256, 1)
     t0 = time.perf_counter()
-    rates = [oracle_rate(w, Ls, ns) for _ in range(args.steps)]
+    rates = [oracle_rate(w.model, w.delta, w.seed, beta0, Ls, ns) for _ in range(args.steps)]
     wall = time.perf_counter() - t0
     value = Ls * Ls * ns * args.steps / sum(r[1] for r in rates) / 1e9
     sample = (f"{args.steps} steps, each {ns} sweeps of a {Ls}x{Ls} {w.name}-shaped lattice "
@@ -161,7 +264,7 @@ def run_reference(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32",
         "data": "synthetic", "config": {"workload": w.name, "L": w.L, "sample_L": Ls},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": rates[0][2] if rates else 0,
-                         "kind": "oracle", "sample": sample},
+                         "kind": "oracle", "sample": sample, "cpu_model": cpu_model()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line))
@@ -232,6 +335,192 @@ def pick_L(w, torch, dev):
     return L
 
 
+_UBENCH = {}
+
+
+def dispatch_peak(lat, torch, dev, stream_ptr):
+    """Measured integer-dispatch rates (thread-instr/clk/SM) from the library's micro-benchmark,
+    once per process: {"lop3", "mulwide_lop3", "mulwide_3lop3", "popc"}."""
+    if not _UBENCH:
+        with torch.cuda.device(dev):
+            for mode, name in enumerate(("lop3", "mulwide_lop3", "mulwide_3lop3", "popc")):
+                v, _ = lat.binding.ubench_int_dispatch(mode, stream_ptr)
+                _UBENCH[name] = v
+    return dict(_UBENCH)
+
+
+def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, measure_pass, worst_case):
+    """Time workload w (device-resident and end to end); returns the pieces of the JSON line."""
+    L = args.L or pick_L(w, torch, dev)
+    L = replicas.agree_min(L, cdev)             # all replicas use the same size
+    g = lat.Lattice(L, w.model, w.delta, seed=replicas.replica_seed(w.seed, rank), scheme=args.scheme,
+                    device=str(dev))
+    updates_per_sweep = L * L
+    K, W = args.steps, args.warmup
+
+    def barrier():
+        replicas.barrier()
+        torch.cuda.synchronize(dev)
+
+    def timed(fn, steps, start_t, sps):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        ev0.record(g.stream)
+        for k in range(steps):
+            fn(start_t + k * sps, sps)
+        ev1.record(g.stream)
+        torch.cuda.synchronize(dev)
+        ms = replicas.max_over_ranks(ev0.elapsed_time(ev1), cdev)
+        barrier()
+        return ms
+
+    def sched(t, n):
+        return w.beta_schedule(n, t)
+
+    def step_device(t, n):
+        g.sweep(sched(t, n))
+
+    e2e_out = {}
+
+    def step_e2e(t, n):
+        g.sweep(sched(t, n))                    # host fp64 beta in
+        e2e_out["r"] = g.measure(1)             # host int64 counts out (synchronises)
+
+    peaks = dispatch_peak(lat, torch, dev, g.stream.cuda_stream)
+
+    # ---- warm-up (W steps of one sweep), then size the step so that K steps last >= min_seconds ----
+    t_now = 0
+    for _ in range(max(W - 1, 0)):
+        step_device(t_now, 1)
+        t_now += 1
+    est_ms = timed(step_device, 1, t_now, 1) if W >= 1 else 1.0
+    t_now += 1 if W >= 1 else 0
+    sps = 1
+    if args.min_seconds > 0 and K * est_ms < args.min_seconds * 1e3:
+        want_ms = args.min_seconds * 1e3 / K
+        sps = int(min(max(1, np.ceil(want_ms / max(est_ms, 1e-3))), 65536))
+        # second calibration at the real step size: several sweeps per call run faster than one
+        # (persistent kernel, no launch gaps), so the first guess is usually too small
+        for _ in range(2):
+            ms1 = timed(step_device, 1, t_now, sps)
+            t_now += sps
+            if ms1 >= want_ms or sps >= 65536:
+                break
+            sps = int(min(np.ceil(sps * want_ms / max(ms1, 1e-3) * 1.05), 65536))
+        sps = -int(replicas.agree_min(-sps, cdev)) if world > 1 else sps     # the largest over ranks
+        step_device(t_now, sps)                 # one untimed step of the final size
+        t_now += sps
+
+    # ---- device-resident timing ------------------------------------------------------------
+    n0 = g.launches
+    sampler = ClockSampler(torch, dev)
+    if rank == 0:
+        sampler.start()
+    ms = timed(step_device, K, t_now, sps)
+    clocks = sampler.stop() if rank == 0 else {}
+    launches = g.launches - n0
+    t_now += K * sps
+
+    # ---- end-to-end timing (host buffers in and out every step) ------------------------------
+    step_e2e(t_now, sps)
+    t_now += sps
+    if rank == 0:
+        sampler.start()
+    e2e_ms = timed(step_e2e, K, t_now, sps)
+    e2e_clocks = sampler.stop() if rank == 0 else {}
+    t_now += K * sps
+
+    # ---- measurement pass, timed separately --------------------------------------------------
+    meas = None
+    if measure_pass and rank == 0:
+        r_meas = w.r_max if args.measure_rmax < 0 else args.measure_rmax
+        r_meas = max(1, min(r_meas, L // 2))
+        # ~3e12 (word, r) pairs/s per axis (profiles/): bound the default run to a few seconds
+        words = L * L // 32
+        if args.measure_rmax < 0 and words * r_meas > 1 << 42:     # an explicit --measure-rmax is honoured
+            r_meas = max(1, (1 << 42) // words)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(g.stream)
+        M, Q, Sx, Sy = g.measure(r_meas)
+        ev1.record(g.stream)
+        torch.cuda.synchronize(dev)
+        xi_v, r_cut = lat.xi(Sx, Sy, Q, L)
+        meas = {"r_max": r_meas, "ms": ev0.elapsed_time(ev1), "t": g.time, "M": M,
+                "e": lat.energy(Sx, Sy, Q, w.delta, L), "xi": xi_v, "r_cut": r_cut}
+    # ---- worst-case input: the all-up state (every site has 4 aligned neighbours, so every
+    # lane needs a random decision and ties are ~3x more frequent than after the quench) ----------
+    worst = None
+    if worst_case and world == 1:
+        g.fill(1)
+        nw = max(2, min(4, K))
+        step_device(t_now, sps)
+        t_now += sps
+        worst_ms = timed(step_device, nw, t_now, sps)
+        t_now += nw * sps
+        worst = {"value": updates_per_sweep * nw * sps / (worst_ms * 1e6), "unit": UNIT, "steps": nw,
+                 "input": "all spins up at t0 (SURVEY.md 8(d) worst case), then the same sweeps"}
+    barrier()
+    state_bytes = lat.state_bytes(L, w.model)
+    g.close()
+    del g
+    torch.cuda.empty_cache()
+
+    # ---- rooflines ---------------------------------------------------------------------------
+    updates = updates_per_sweep * sps * K
+    value = replicas.job_rate(updates, world, ms)
+    e2e_value = replicas.job_rate(updates, world, e2e_ms)
+    peak, peak_src, sm_max = measured_peaks()
+    cap = pc.captured(w.model)
+    bpu = pc.ALGORITHMIC_BYTES_PER_UPDATE[w.model]
+    half_sweeps = 2 * sps * K
+    hs_ms = ms / half_sweeps                    # mean duration of one half-sweep (one launch, or one
+    upl = updates_per_sweep / 2                 # colour pass inside the persistent kernel)
+    achieved = bpu * upl / (hs_ms * 1e-3) / 1e9
+    in_l2 = state_bytes <= (126 << 20)
+    roofline_hbm = {"bound": "hbm", "kernel": KERNEL[w.model], "achieved": achieved, "peak": peak,
+                    "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                    "bytes_per_update": bpu, "half_sweep_ms": hs_ms, "l2_resident": in_l2}
+    mhz = clocks.get("sm_mhz") or sm_max
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    lanes = peaks["mulwide_3lop3"]
+    ipu = pc.ALGORITHMIC_HALF_RATE_INSTR_PER_UPDATE[w.model]
+    ipu_exe = cap["executed_half_rate_instr_per_update"]
+    peak_alu = sms * lanes * mhz * 1e6 / 1e12
+    ach_alu = ipu * upl / (hs_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": KERNEL[w.model], "achieved": ach_alu, "peak": peak_alu,
+                "unit": "T thread-instr/s", "frac": ach_alu / peak_alu,
+                "frac_is": "model: algorithmic instruction count (DESIGN.md section 6) x updates / launch time "
+                           "measured in this run, over the dispatch peak measured in this run",
+                "traffic": cap["dram_bytes_per_update"] * upl,
+                "traffic_source": f"constant from {cap['profile']} (ncu dram__bytes_read+write per update at commit "
+                                  f"{cap['commit']}) x updates per launch; NOT measured in this run",
+                "instr_per_update_algorithmic": ipu,
+                "instr_per_update_executed": ipu_exe,
+                "executed_source": f"constant from {cap['profile']} (commit {cap['commit']}); not this run",
+                "executed_frac": ach_alu / peak_alu * ipu_exe / ipu,
+                "stale_profile": cap["stale_profile"],
+                "sm_mhz": mhz, "half_sweep_ms": hs_ms,
+                "peak_lanes_per_clk_per_sm": lanes, "sm_count": sms,
+                "peak_source": "measured in this run: lattice_ubench_int_dispatch (1 mul.wide.u32 + 3 LOP3 chains, "
+                               "clock64) x SM count x sampled SM clock",
+                "ubench_thread_instr_per_clk_per_sm": peaks,
+                "hbm_frac": achieved / peak, "hbm_achieved_GBs": achieved, "hbm_peak_GBs": peak}
+    return {
+        "value": value, "ms_per_step": ms / K, "L": L,
+        "config": {"workload": w.name if L == w.L else f"{w.name}@L={L}", "model": MODEL_NAME[w.model],
+                   "L": L, "spins": L * L, "state_bytes": state_bytes,
+                   "beta": float(w.beta_schedule(1)[0]), "rng_scheme": args.scheme, "seed": w.seed,
+                   "sweeps_per_step": sps, "timed_seconds": ms / 1e3,
+                   "l2": "inputs_larger_than_l2" if not in_l2 else "l2_resident_by_design",
+                   "parallelism": "replicas" if world > 1 else "single"},
+        "clocks": clocks, "gpu_launches": int(launches),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * sps,
+                "d2h_bytes_per_step": 8 * (2 + 4 * 1), "ms_per_step": e2e_ms / K, "clocks": e2e_clocks,
+                "what": f"lattice_sweep({sps}, host beta[{sps}]) + lattice_measure(r_max=1) -> host int64, per step"},
+        "roofline": roofline, "roofline_hbm": roofline_hbm, "worst_case": worst, "measure": meas,
+    }
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -241,7 +530,11 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--scheme", type=int, default=1)
     ap.add_argument("--L", type=int, default=0, help="override the lattice side (debugging)")
+    ap.add_argument("--min-seconds", type=float, default=2.0,
+                    help="lower bound on the timed region: a step becomes several sweeps per call if needed")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-blume-capel", action="store_true",
+                    help="skip the Blume-Capel workloads the default invocation also times")
     ap.add_argument("--measure-rmax", type=int, default=-1,
                     help="r_max of the separately timed measurement pass (-1: the workload's)")
     ap.add_argument("--sharded", action="store_true",
@@ -272,144 +565,39 @@ def main():
             dist.init_process_group("nccl", device_id=dev)
         else:
             dist.init_process_group("gloo")
+    cdev = dev if args.dist_backend == "nccl" else "cpu"   # where the plumbing tensors live
 
     w = workloads.CONFIGS[args.workload]
-    L = args.L or pick_L(w, torch, dev)
-    cdev = dev if args.dist_backend == "nccl" else "cpu"   # where the plumbing tensors live
-    L = replicas.agree_min(L, cdev)             # all replicas use the same size
-    g = lat.Lattice(L, w.model, w.delta, seed=replicas.replica_seed(w.seed, rank), scheme=args.scheme,
-                    device=str(dev))
-    updates_per_step = L * L
+    res = bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, measure_pass=True, worst_case=True)
 
-    def barrier():
-        replicas.barrier()
-        torch.cuda.synchronize(dev)
-
-    def timed(fn, steps, start_t):
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        barrier()
-        ev0.record(g.stream)
-        for k in range(steps):
-            fn(start_t + k)
-        ev1.record(g.stream)
-        torch.cuda.synchronize(dev)
-        ms = replicas.max_over_ranks(ev0.elapsed_time(ev1), cdev)
-        barrier()
-        return ms
-
-    sched = w.beta_schedule(2 * (args.warmup + args.steps) + 16)
-
-    def step_device(t):
-        g.sweep(sched[t:t + 1])
-
-    e2e_out = {}
-
-    def step_e2e(t):
-        g.sweep(sched[t:t + 1])                 # host fp64 beta in
-        e2e_out["r"] = g.measure(1)             # host int64 counts out (synchronises)
-
-    # ---- device-resident timing ------------------------------------------------------------
-    for k in range(args.warmup):
-        step_device(k)
-    n0 = g.launches
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    ms = timed(step_device, args.steps, args.warmup)
-    clocks = sampler.stop() if rank == 0 else {}
-    launches = g.launches - n0
-    tdone = args.warmup + args.steps
-
-    # ---- end-to-end timing (host buffers in and out every step) ------------------------------
-    step_e2e(tdone)
-    e2e_ms = timed(step_e2e, args.steps, tdone + 1)
-    tdone += 1 + args.steps
-
-    # ---- measurement pass, timed separately --------------------------------------------------
-    r_meas = w.r_max if args.measure_rmax < 0 else args.measure_rmax
-    r_meas = max(1, min(r_meas, L // 2))
-    meas = None
-    if rank == 0:
-        # ~3e12 (word, r) pairs/s per axis (profiles/): bound the default run to a few seconds
-        words = L * L // 32
-        if args.measure_rmax < 0 and words * r_meas > 1 << 42:     # an explicit --measure-rmax is honoured
-            r_meas = max(1, (1 << 42) // words)
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        ev0.record(g.stream)
-        M, Q, Sx, Sy = g.measure(r_meas)
-        ev1.record(g.stream)
-        torch.cuda.synchronize(dev)
-        xi_v, r_cut = lat.xi(Sx, Sy, Q, L)
-        meas = {"r_max": r_meas, "ms": ev0.elapsed_time(ev1), "t": g.time, "M": M,
-                "e": lat.energy(Sx, Sy, Q, w.delta, L), "xi": xi_v, "r_cut": r_cut}
-    # ---- worst-case input: the all-up state (every site has 4 aligned neighbours, so every
-    # lane needs a random decision and ties are ~3x more frequent than after the quench) ----------
-    worst = None
-    if world == 1:
-        g.fill(1)
-        nw = max(2, min(4, args.steps))
-        g.sweep(sched[tdone:tdone + 1])
-        worst_ms = timed(step_device, nw, tdone + 1)
-        tdone += 1 + nw
-        worst = {"value": updates_per_step * nw / (worst_ms * 1e6), "unit": UNIT, "steps": nw,
-                 "input": "all spins up at t0 (SURVEY.md 8(d) worst case), then the same sweeps"}
-
-    barrier()
+    # the metric's second half: Blume-Capel at the paper's size and BASELINE config 5b, same process
+    extra = {}
+    if world == 1 and not args.no_blume_capel and args.workload == "ising_L2p20" and not args.L:
+        for name in ("bc_L2p19", "bc_L2p15_ramp"):
+            r = bench_workload(workloads.CONFIGS[name], args, lat, torch, dev, rank, world, cdev, replicas,
+                               measure_pass=False, worst_case=True)
+            extra[name] = {"value": r["value"], "unit": UNIT, "steps": args.steps, "ms_per_step": r["ms_per_step"],
+                           "config": r["config"], "clocks": r["clocks"], "gpu_launches": r["gpu_launches"],
+                           "e2e": r["e2e"], "roofline": r["roofline"], "roofline_hbm": r["roofline_hbm"],
+                           "worst_case": r["worst_case"]}
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    value = replicas.job_rate(updates_per_step * args.steps, world, ms)
-    e2e_value = replicas.job_rate(updates_per_step * args.steps, world, e2e_ms)
-    peak, peak_src, sm_max = measured_peaks()
-    bpu = BYTES_PER_UPDATE[w.model]
-    launch_ms = ms / max(launches, 1)
-    alg_bytes = bpu * updates_per_step / 2          # per half-sweep launch
-    achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
-    in_l2 = lat.state_bytes(L, w.model) <= (126 << 20)
-    roofline_hbm = {"bound": "hbm", "kernel": KERNEL[w.model], "achieved": achieved, "peak": peak,
-                    "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                    "bytes_per_update": bpu, "launch_ms": launch_ms, "l2_resident": in_l2}
-    # the binding roofline: the 16-lane integer dispatch (ALU pipe + IMAD.WIDE), DESIGN.md section 6
-    mhz = clocks.get("sm_mhz") or sm_max
-    ipu, ipu_exe = ALG_HALF_RATE_INSTR_PER_UPDATE[w.model], EXE_HALF_RATE_INSTR_PER_UPDATE[w.model]
-    peak_alu = SM_COUNT * HALF_RATE_LANES_PER_CLK_PER_SM * mhz * 1e6 / 1e12
-    ach_alu = ipu * (updates_per_step / 2) / (launch_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": KERNEL[w.model], "achieved": ach_alu, "peak": peak_alu,
-                "unit": "T thread-instr/s", "frac": ach_alu / peak_alu,
-                "traffic": DRAM_BYTES_PER_UPDATE_NCU[w.model] * updates_per_step / 2,
-                "traffic_source": "ncu dram bytes per update (profiles/) x updates per launch",
-                "instr_per_update": ipu, "executed_instr_per_update": ipu_exe,
-                "executed_frac": ach_alu / peak_alu * ipu_exe / ipu,
-                "sm_mhz": mhz, "launch_ms": launch_ms,
-                "peak_source": "148 SM x 64 lanes/clk (ALU + IMAD.WIDE dispatch) x sampled SM clock",
-                "hbm_frac": achieved / peak, "hbm_achieved_GBs": achieved, "hbm_peak_GBs": peak}
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-        "config": {"workload": w.name if L == w.L else f"{w.name}@L={L}", "model": ["ising", "blume-capel"][w.model],
-                   "L": L, "spins": L * L, "state_bytes": lat.state_bytes(L, w.model),
-                   "beta": float(sched[0]), "rng_scheme": args.scheme, "seed": w.seed,
-                   "l2": "inputs_larger_than_l2" if not in_l2 else "l2_resident_by_design",
-                   "parallelism": "replicas" if world > 1 else "single"},
-        "clocks": clocks, "gpu_launches": int(launches),
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8,
-                "d2h_bytes_per_step": 8 * (2 + 4 * 1), "ms_per_step": e2e_ms / args.steps,
-                "what": "lattice_sweep(1, host beta) + lattice_measure(r_max=1) -> host int64"},
-        "roofline": roofline,
-        "roofline_hbm": roofline_hbm,
-        "worst_case": worst,
-        "measure": meas,
+        "config": res["config"], "clocks": res["clocks"], "gpu_launches": res["gpu_launches"],
+        "e2e": res["e2e"], "roofline": res["roofline"], "roofline_hbm": res["roofline_hbm"],
+        "worst_case": res["worst_case"], "measure": res["measure"],
     }
-    if not args.no_cpu_baseline:
-        Ls, ns = min(L, 4096), 96
-        rate, dt, cores = oracle_rate(w, Ls, ns, args.scheme)
-        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": f"{ns} sweeps of a {Ls}x{Ls} lattice of the same model, "
-                                          f"beta and RNG scheme ({dt:.1f} s)"}
+    if extra:
+        line["blume_capel"] = extra
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline_matrix(w, args.scheme)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -250,12 +250,13 @@ class Lattice:
 
     def close(self) -> None:
         if getattr(self, "_h", None):
+            self.synchronize()
             lib().lattice_destroy(self._h)
             self._h = None
             if self._own_ptr is not None:
-                self.synchronize()
                 lib().lattice_device_free(_vp(self._own_ptr))
                 self._own_ptr = None
+            self.buf = None                          # hand the device memory back to torch
 
     def __del__(self):
         try:

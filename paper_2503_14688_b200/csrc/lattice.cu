@@ -1030,13 +1030,17 @@ int lattice_ubench_int_dispatch(int mode, void *cuda_stream, double *thread_inst
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     int rc = LATTICE_ECUDA;
     float ms = 0.f;
+    const size_t clk_bytes = (size_t)3 * UB_MAX_SM * sizeof(unsigned long long);
     do {
         if (cudaMalloc(&out, (size_t)blocks * 256 * sizeof(uint32_t)) != cudaSuccess) { rc = LATTICE_ENOMEM; break; }
-        if (cudaMalloc(&clk, (size_t)blocks * sizeof(unsigned long long)) != cudaSuccess) { rc = LATTICE_ENOMEM; break; }
-        h = (unsigned long long *)std::malloc((size_t)blocks * sizeof(unsigned long long));
+        if (cudaMalloc(&clk, clk_bytes) != cudaSuccess) { rc = LATTICE_ENOMEM; break; }
+        h = (unsigned long long *)std::malloc(clk_bytes);
         if (!h) { rc = LATTICE_ENOMEM; break; }
         if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
         for (int rep = 0; rep < 2; ++rep) {              // first launch warms up, second is timed
+            for (int k = 0; k < UB_MAX_SM; ++k) { h[3 * k] = ~0ull; h[3 * k + 1] = 0; h[3 * k + 2] = 0; }
+            if (cudaMemcpyAsync(clk, h, clk_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) break;
+            if (cudaStreamSynchronize(st) != cudaSuccess) break;     // h is reused by the next rep
             if (rep == 1) cudaEventRecord(e0, st);
             switch (mode) {
             case 0: ubench_kernel<0><<<blocks, 256, 0, st>>>(out, 12345u, clk); break;
@@ -1048,12 +1052,18 @@ int lattice_ubench_int_dispatch(int mode, void *cuda_stream, double *thread_inst
         cudaEventRecord(e1, st);
         if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) break;
         cudaEventElapsedTime(&ms, e0, e1);
-        if (cudaMemcpy(h, clk, (size_t)blocks * sizeof(unsigned long long), cudaMemcpyDeviceToHost) != cudaSuccess) break;
-        double cyc = 0.0;                                // mean cycles of a block; UB_BLOCKS_PER_SM run side by side
-        for (int b = 0; b < blocks; ++b) cyc += (double)h[b];
-        cyc /= blocks;
-        const double instr_per_sm = (double)UB_BLOCKS_PER_SM * 256.0 * UB_ITER * UB_CHAINS * ubench_instr_per_step(mode);
-        *thread_instr_per_clk_per_sm = instr_per_sm / cyc;
+        if (cudaMemcpy(h, clk, clk_bytes, cudaMemcpyDeviceToHost) != cudaSuccess) break;
+        // per SM: instructions of the blocks that ran there / (latest end - earliest start); mean over SMs
+        const double per_block = 256.0 * UB_ITER * UB_CHAINS * ubench_instr_per_step(mode);
+        double sum = 0.0;
+        int used = 0;
+        for (int k = 0; k < UB_MAX_SM; ++k) {
+            if (h[3 * k + 2] == 0 || h[3 * k + 1] <= h[3 * k]) continue;
+            sum += per_block * (double)h[3 * k + 2] / (double)(h[3 * k + 1] - h[3 * k]);
+            ++used;
+        }
+        if (!used) break;
+        *thread_instr_per_clk_per_sm = sum / used;
         if (elapsed_ms) *elapsed_ms = ms;
         rc = LATTICE_OK;
     } while (0);

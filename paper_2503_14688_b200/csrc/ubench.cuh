@@ -4,7 +4,10 @@
 // instructions (ALU pipe) and the 32x32->64 multiplies of Philox (IMAD.WIDE / IMAD.HI) share
 // (DESIGN.md section 6).  Instead of quoting a nominal 64 lanes/clk/SM, bench.py runs this kernel
 // in the same process and uses the MEASURED thread-instructions per clock per SM as the peak.
-// Cycles come from clock64() inside the kernel, so the figure does not depend on the SM clock.
+// Cycles come from clock64() inside the kernel, so the figure does not depend on the SM clock:
+// per SM, the span from the earliest start to the latest end over ALL warps that ran on it (the
+// warp schedulers favour old warps, so one warp's own span understates the time), and the
+// instructions of the blocks that actually landed on that SM.
 //   mode 0: independent LOP3 chains                       (the ALU pipe alone)
 //   mode 1: 1 mul.wide.u32 + 1 LOP3 per step              (the Philox round mix, 1 : 1)
 //   mode 2: 1 mul.wide.u32 + 3 LOP3 per step              (the half-sweep's overall mix, ~1 : 3)
@@ -14,11 +17,14 @@
 
 namespace lat {
 
-constexpr int UB_ITER = 4096, UB_CHAINS = 8, UB_BLOCKS_PER_SM = 4;
+constexpr int UB_ITER = 4096, UB_CHAINS = 8, UB_BLOCKS_PER_SM = 4, UB_MAX_SM = 512;
 
 template <int MODE>
 __global__ void __launch_bounds__(256) ubench_kernel(uint32_t *out, uint32_t seed, unsigned long long *clk)
 {
+    // clk[3 * smid + {0, 1, 2}] = earliest start, latest end, number of blocks on that SM
+    uint32_t smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
     uint32_t x[UB_CHAINS], y[UB_CHAINS];
 #pragma unroll
     for (int i = 0; i < UB_CHAINS; ++i) { x[i] = seed + threadIdx.x * 7u + i; y[i] = seed ^ (i * 0x9E3779B9u); }
@@ -49,7 +55,11 @@ __global__ void __launch_bounds__(256) ubench_kernel(uint32_t *out, uint32_t see
 #pragma unroll
     for (int i = 0; i < UB_CHAINS; ++i) s ^= x[i] ^ y[i];
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
-    if (threadIdx.x == 0) clk[blockIdx.x] = t1 - t0;
+    if ((threadIdx.x & 31u) == 0 && smid < UB_MAX_SM) {
+        atomicMin(clk + 3 * smid, t0);
+        atomicMax(clk + 3 * smid + 1, t1);
+        if (threadIdx.x == 0) atomicAdd(clk + 3 * smid + 2, 1ull);
+    }
 }
 
 // thread-instructions of the counted classes per step of one chain

@@ -86,6 +86,10 @@ CONFIGS: dict[str, Workload] = {
                                  1024, protocol=2, beta_f=BETA_C_ISING / 1.01),
     "bc_L2p15_ramp": Workload("bc_L2p15_ramp", BLUME_CAPEL, 1 << 15, 0.0, SEED_BASE + 6, 20000,
                               1024, protocol=2, beta_f=BETA_BC / 1.01),
+    # Blume-Capel at the paper's own size and temperature (Table I: L = 2^19,
+    # T_c = 1.69355839821214427017, t_max = 524288): 64 GiB at 2 bits/spin -- bench.py's BC line
+    "bc_L2p19": Workload("bc_L2p19", BLUME_CAPEL, 1 << 19, 0.0, SEED_BASE + 9, 524288, 4096,
+                         beta_f=1.0 / 1.69355839821214427017),
     # the paper's own two-step schedules (Table II, PAPER.md:142-153;
     # the middle t_switch of each model).  Same API, a different beta array.
     "ising_L2p16_twostep": Workload("ising_L2p16_twostep", ISING, 1 << 16, 0.0, SEED_BASE + 7,
