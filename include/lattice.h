@@ -75,6 +75,35 @@ size_t lattice_state_bytes(uint32_t L, int model);
 int lattice_create(lattice_t **out, uint32_t L, int model, double delta, uint64_t seed,
                    void *device_buf, size_t device_buf_bytes, void *cuda_stream);
 
+/* ---- Batches of independent replicas ----------------------------------------------------------
+ * The paper's error bars come from 40-4000 independent runs per point (Tables I-II,
+ * PAPER.md:126-153; jackknife over realisations).  A batch handle evolves
+ * n_replicas lattices of the same L, model and Delta under the same beta schedule, replica k keyed
+ * by seeds[k]: every replica is bit for bit the stand-alone lattice lattice_create(L, model, Delta,
+ * seeds[k]) would give.  Layout of the buffer: [replica][<single-lattice layout>], i.e.
+ * lattice_batch_bytes = n_replicas * lattice_state_bytes.  What fills the GPU at cache-resident
+ * sizes: Ising lattices with L a multiple of 256 update all replicas in one launch per half-sweep
+ * (replica = blockIdx.y, its Philox round keys from a table in the kernel parameters); Ising
+ * L = 64 and 128 keep each replica in the registers of a (half-)warp and run ALL n sweeps of a
+ * lattice_sweep call in one launch; other shapes fall back to one launch per replica.
+ *   lattice_sweep / lattice_half_sweep / lattice_set_rng_scheme / lattice_set_time / lattice_fill /
+ *   lattice_time / lattice_launches act on all replicas; lattice_measure_batch returns the counts
+ *   of every replica: M[k], Q[k], Sx[k * r_max + r - 1], Sy[k * r_max + r - 1].
+ *   lattice_replica lends the handle of replica k (owned by the batch, valid until the batch is
+ *   destroyed, not to be destroyed itself): lattice_get_spins / lattice_set_spins /
+ *   lattice_measure / lattice_measure_rows / lattice_fill work on it; sweeps, set_time and
+ *   set_rng_scheme return ESTATE.  On the batch handle itself the per-lattice calls
+ *   (get/set_spins, measure, measure_rows) return ESTATE.
+ * Errors: EINVAL (as lattice_create; n_replicas == 0 or > 2^20; NULL seeds), ENOMEM, ECUDA. */
+size_t lattice_batch_bytes(uint32_t n_replicas, uint32_t L, int model);       /* 0 if invalid */
+int lattice_create_batch(lattice_t **out, uint32_t n_replicas, uint32_t L, int model, double delta,
+                         const uint64_t *seeds, void *device_buf, size_t device_buf_bytes,
+                         void *cuda_stream);
+uint32_t lattice_replicas(const lattice_t *lat);       /* 1 for a plain lattice, 0 for NULL */
+int lattice_replica(lattice_t *batch, uint32_t k, lattice_t **out);
+int lattice_measure_batch(lattice_t *batch, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx,
+                          int64_t *Sy);
+
 /* ---- Row-slab domain decomposition (the paper's third level of parallelism, PAPER.md:32-34;
  * SURVEY.md section 8(f) NEXT-1) -------------------------------------------
  * A slab owns global rows row0 .. row0+n_rows-1 of a periodic L x L lattice and keeps one halo

@@ -28,6 +28,12 @@ SIGNATURES = {
     "lattice_state_bytes": (C.c_size_t, [C.c_uint32, C.c_int]),
     "lattice_create": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_double, C.c_uint64,
                                  _vp, C.c_size_t, _vp]),
+    "lattice_batch_bytes": (C.c_size_t, [C.c_uint32, C.c_uint32, C.c_int]),
+    "lattice_create_batch": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_uint32, C.c_int, C.c_double, _u64p,
+                                       _vp, C.c_size_t, _vp]),
+    "lattice_replicas": (C.c_uint32, [_vp]),
+    "lattice_replica": (C.c_int, [_vp, C.c_uint32, C.POINTER(_vp)]),
+    "lattice_measure_batch": (C.c_int, [_vp, C.c_uint32, _i64p, _i64p, _i64p, _i64p]),
     "lattice_slab_bytes": (C.c_size_t, [C.c_uint32, C.c_int, C.c_uint32]),
     "lattice_create_slab": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_double, C.c_uint64,
                                       C.c_uint32, C.c_uint32, _vp, C.c_size_t, _vp]),
@@ -337,6 +343,126 @@ class Lattice:
         """Every spin := spin (an ordered state: worst-case throughput input, tests)."""
         with self._torch.cuda.device(self.device):
             self._check(lib().lattice_fill(self._h, int(spin)), "lattice_fill")
+
+    def synchronize(self) -> None:
+        self.stream.synchronize()
+
+
+class LatticeBatch:
+    """n independent replicas of one lattice shape in a single device buffer (include/lattice.h,
+    "Batches of independent replicas"): replica k is bit-identical to Lattice(L, model, delta,
+    seeds[k]).  sweep() advances all of them; measure() returns per-replica counts."""
+
+    def __init__(self, L: int, seeds, model: int = ISING, delta: float = 0.0, scheme: int = 1,
+                 device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2503_14688_b200 needs a CUDA device; there is no CPU path")
+        self.seeds = np.ascontiguousarray(np.asarray(seeds, dtype=np.uint64))
+        self.n = int(self.seeds.size)
+        self.L, self.model, self.delta = int(L), int(model), float(delta)
+        nbytes = int(lib().lattice_batch_bytes(self.n, self.L, self.model))
+        if nbytes == 0:
+            raise LatticeError("lattice_batch_bytes", EINVAL, f"n={self.n} L={L} model={model}")
+        self._torch = torch
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            self.buf = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = _vp()
+            rc = lib().lattice_create_batch(C.byref(h), self.n, self.L, self.model, self.delta,
+                                            _p(self.seeds, C.c_uint64), _vp(self.buf.data_ptr()), nbytes,
+                                            _vp(self.stream.cuda_stream))
+        if rc != OK:
+            raise LatticeError("lattice_create_batch", rc)
+        self._h = h
+        self.scheme = int(scheme)
+        if scheme != 1:
+            self._check(lib().lattice_set_rng_scheme(self._h, int(scheme)), "lattice_set_rng_scheme")
+
+    def _check(self, rc: int, what: str) -> None:
+        if rc != OK:
+            detail = lib().lattice_last_error(self._h).decode() if rc == ECUDA else ""
+            raise LatticeError(what, rc, detail)
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            self.stream.synchronize()
+            lib().lattice_destroy(self._h)
+            self._h = None
+            self.buf = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def time(self) -> int:
+        return int(lib().lattice_time(self._h))
+
+    @property
+    def launches(self) -> int:
+        return int(lib().lattice_launches(self._h))
+
+    def set_time(self, t: int) -> None:
+        self._check(lib().lattice_set_time(self._h, int(t)), "lattice_set_time")
+
+    def sweep(self, beta) -> None:
+        b = np.ascontiguousarray(np.atleast_1d(beta), dtype=np.float64)
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_sweep(self._h, b.size, _p(b, C.c_double)), "lattice_sweep")
+
+    def half_sweep(self, colour: int, beta: float) -> None:
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_half_sweep(self._h, int(colour), float(beta)), "lattice_half_sweep")
+
+    def fill(self, spin: int) -> None:
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_fill(self._h, int(spin)), "lattice_fill")
+
+    def measure(self, r_max: int):
+        """(M[n], Q[n], Sx[n, r_max], Sy[n, r_max]) as exact integers."""
+        M = np.zeros(self.n, dtype=np.int64)
+        Q = np.zeros(self.n, dtype=np.int64)
+        Sx = np.zeros((self.n, r_max), dtype=np.int64)
+        Sy = np.zeros((self.n, r_max), dtype=np.int64)
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_measure_batch(self._h, r_max, _p(M, C.c_int64), _p(Q, C.c_int64),
+                                                    _p(Sx, C.c_int64), _p(Sy, C.c_int64)),
+                        "lattice_measure_batch")
+        return M, Q, Sx, Sy
+
+    def _replica(self, k: int):
+        h = _vp()
+        self._check(lib().lattice_replica(self._h, int(k), C.byref(h)), "lattice_replica")
+        return h
+
+    def get_spins(self, k: int, i0: int = 0, j0: int = 0, h: int | None = None, w: int | None = None):
+        h = self.L if h is None else h
+        w = self.L if w is None else w
+        out = np.zeros((h, w), dtype=np.int8)
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_get_spins(self._replica(k), i0, j0, h, w, _p(out, C.c_int8)),
+                        "lattice_get_spins")
+        return out
+
+    def set_spins(self, k: int, spins, i0: int = 0, j0: int = 0) -> None:
+        s = np.ascontiguousarray(spins, dtype=np.int8)
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_set_spins(self._replica(k), i0, j0, s.shape[0], s.shape[1],
+                                                _p(s, C.c_int8)), "lattice_set_spins")
+
+    def measure_replica(self, k: int, r_max: int, rows=None):
+        Sx = np.zeros(r_max, dtype=np.int64)
+        Sy = np.zeros(r_max, dtype=np.int64)
+        M, Q = C.c_int64(0), C.c_int64(0)
+        i0, n = (0, self.L) if rows is None else rows
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_measure_rows(self._replica(k), i0, n, r_max, C.byref(M), C.byref(Q),
+                                                   _p(Sx, C.c_int64), _p(Sy, C.c_int64)), "lattice_measure_rows")
+        return int(M.value), int(Q.value), Sx, Sy
 
     def synchronize(self) -> None:
         self.stream.synchronize()

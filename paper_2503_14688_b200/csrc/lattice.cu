@@ -19,6 +19,7 @@
 #include "ising.cuh"
 #include "ising_march.cuh"
 #include "ising_persist.cuh"
+#include "ising_batch.cuh"
 #include "measure.cuh"
 #include "philox.cuh"
 #include "ubench.cuh"
@@ -59,6 +60,15 @@ struct lattice {
     size_t sp_cap;             // entries
     int persist_blocks;        // co-resident blocks of ising_persist_kernel (0: not yet queried, -1: unavailable)
     uint32_t persist_cap;      // lattice_set_persist_blocks: upper bound on the grid (0: none)
+    // batch of independent replicas (lattice_create_batch): the batch handle owns one child handle
+    // per replica (buf offset, own seed / round keys); a child has parent != nullptr
+    uint32_t n_rep;            // 0 for a plain lattice or a child
+    size_t rep_words;          // 32-bit words per replica
+    lattice **kids;            // [n_rep]
+    lattice *parent;
+    RoundKeys *h_keys;         // [n_rep] host copy of the replicas' round keys
+    RoundKeys *d_keys;         // [n_rep] device copy (ising_tiny_kernel)
+    BatchKeys *bk;             // staging of one chunk's keys for the batched marching launch
     char err[256];
 };
 
@@ -300,7 +310,7 @@ int launch_bc_march(lattice *lat, int colour)
 
 int launch_half_sweep(lattice *lat, int colour)
 {
-    if (lat->view) return LATTICE_ESTATE;
+    if (lat->view || lat->n_rep) return LATTICE_ESTATE;
     if (lat->slab) {
         if (!lat->have_nbr) return LATTICE_ESTATE;
         if (lat->model == LATTICE_ISING) return launch_ising_march(lat, colour);
@@ -463,6 +473,90 @@ int lattice_create(lattice_t **out, uint32_t L, int model, double delta, uint64_
     return LATTICE_OK;
 }
 
+size_t lattice_batch_bytes(uint32_t n_replicas, uint32_t L, int model)
+{
+    const size_t one = lattice_state_bytes(L, model);
+    if (one == 0 || n_replicas == 0 || n_replicas > (1u << 20)) return 0;
+    if (one > ((size_t)1 << 46) / n_replicas) return 0;
+    return one * n_replicas;
+}
+
+static void free_handle(lattice *lat)
+{
+    if (!lat) return;
+    if (lat->kids) {
+        for (uint32_t r = 0; r < lat->n_rep; ++r) free_handle(lat->kids[r]);
+        std::free(lat->kids);
+    }
+    if (lat->d_cnt) cudaFree(lat->d_cnt);
+    if (lat->d_win) cudaFree(lat->d_win);
+    if (lat->d_sp) cudaFree(lat->d_sp);
+    if (lat->d_keys) cudaFree(lat->d_keys);
+    if (lat->h_keys) std::free(lat->h_keys);
+    if (lat->bk) std::free(lat->bk);
+    delete lat;
+}
+
+int lattice_create_batch(lattice_t **out, uint32_t n_replicas, uint32_t L, int model, double delta,
+                         const uint64_t *seeds, void *device_buf, size_t device_buf_bytes, void *cuda_stream)
+{
+    if (!out || !seeds) return LATTICE_EINVAL;
+    const size_t need = lattice_batch_bytes(n_replicas, L, model);
+    if (need == 0 || !std::isfinite(delta) || !device_buf || device_buf_bytes < need ||
+        ((uintptr_t)device_buf & 15u) != 0)
+        return LATTICE_EINVAL;
+    lattice *lat = new (std::nothrow) lattice();
+    if (!lat) return LATTICE_ENOMEM;
+    std::memset(lat, 0, sizeof *lat);
+    lat->L = L; lat->wpr = L / 64u; lat->model = model; lat->delta = delta; lat->seed = seeds[0];
+    lat->rows = L; lat->n_own = L; lat->scheme = 1;
+    lat->buf = (uint32_t *)device_buf;
+    lat->stream = (cudaStream_t)cuda_stream;
+    lat->n_rep = n_replicas;
+    lat->rep_words = lattice_state_bytes(L, model) / sizeof(uint32_t);
+    lat->kids = (lattice **)std::calloc(n_replicas, sizeof(lattice *));
+    lat->h_keys = (RoundKeys *)std::malloc((size_t)n_replicas * sizeof(RoundKeys));
+    lat->bk = (BatchKeys *)std::calloc(1, sizeof(BatchKeys));
+    if (!lat->kids || !lat->h_keys || !lat->bk) { free_handle(lat); return LATTICE_ENOMEM; }
+    for (uint32_t r = 0; r < n_replicas; ++r) {
+        // every replica is a stand-alone lattice in its own stretch of the buffer: lattice_create
+        // fills it with the disordered start of ITS seed (asynchronous on the stream)
+        lattice *kid = nullptr;
+        const int rc = lattice_create(&kid, L, model, delta, seeds[r], lat->buf + (size_t)r * lat->rep_words,
+                                      lat->rep_words * sizeof(uint32_t), cuda_stream);
+        if (rc != LATTICE_OK) { free_handle(lat); return rc; }
+        kid->parent = lat;
+        lat->kids[r] = kid;
+        lat->h_keys[r] = kid->K;
+    }
+    lat->K = lat->h_keys[0];
+    if (cudaMalloc(&lat->d_keys, (size_t)n_replicas * sizeof(RoundKeys)) != cudaSuccess) {
+        cudaGetLastError();
+        free_handle(lat);
+        return LATTICE_ENOMEM;
+    }
+    // pageable source: staged before the call returns
+    if (cudaMemcpyAsync(lat->d_keys, lat->h_keys, (size_t)n_replicas * sizeof(RoundKeys), cudaMemcpyHostToDevice,
+                        lat->stream) != cudaSuccess) {
+        cudaGetLastError();
+        free_handle(lat);
+        return LATTICE_ECUDA;
+    }
+    *out = lat;
+    return LATTICE_OK;
+}
+
+uint32_t lattice_replicas(const lattice_t *lat) { return lat ? (lat->n_rep ? lat->n_rep : 1u) : 0u; }
+
+int lattice_replica(lattice_t *batch, uint32_t k, lattice_t **out)
+{
+    if (!batch || !out || batch->n_rep == 0 || k >= batch->n_rep) return LATTICE_EINVAL;
+    lattice *kid = batch->kids[k];
+    kid->t = batch->t;                                    // a borrowed view of replica k as it is now
+    *out = kid;
+    return LATTICE_OK;
+}
+
 size_t lattice_slab_bytes(uint32_t L, int model, uint32_t n_rows)
 {
     if (lattice_state_bytes(L, model) == 0 || (L % 256u) != 0) return 0;
@@ -621,27 +715,65 @@ int lattice_ipc_close(void *device_ptr)
 int lattice_set_rng_scheme(lattice_t *lat, int scheme)
 {
     if (!lat || scheme < 0 || scheme > 2) return LATTICE_EINVAL;
-    if (lat->t != 0 || lat->view) return LATTICE_ESTATE;
+    if (lat->t != 0 || lat->view || lat->parent) return LATTICE_ESTATE;
     if (lat->slab && scheme == 0) return LATTICE_EINVAL;
     if (scheme == 2 && (lat->wpr % 4u) != 0) return LATTICE_EINVAL;   // marching kernels only
     lat->scheme = scheme;
     lat->have_beta = false;                                           // thresholds depend on the scheme
+    for (uint32_t r = 0; r < lat->n_rep; ++r) { lat->kids[r]->scheme = scheme; lat->kids[r]->have_beta = false; }
     return LATTICE_OK;
 }
+
+static int launch_half_sweep_batch(lattice *lat, int colour);
 
 int lattice_half_sweep(lattice_t *lat, int colour, double beta)
 {
     if (!lat || (colour != 0 && colour != 1) || std::isnan(beta) || beta < 0.0) return LATTICE_EINVAL;
     if (lat->t >= 0xffffffffull) return LATTICE_EINVAL;
+    if (lat->parent) return LATTICE_ESTATE;
     refresh_thresholds(lat, beta);
+    if (lat->n_rep) return launch_half_sweep_batch(lat, colour);
     return launch_half_sweep(lat, colour);
+}
+
+// Per-sweep parameters of the in-kernel sweep loops (ising_persist_kernel, ising_tiny_kernel): the
+// thresholds of beta[0..n) on the device, in lat->d_sp.  *edge: some sweep has an "always" class.
+static int upload_sweep_params(lattice *lat, uint64_t n, const double *beta, bool *edge)
+{
+    if (lat->sp_cap < n) {
+        if (lat->d_sp) cudaFree(lat->d_sp);
+        lat->d_sp = nullptr; lat->sp_cap = 0;
+        const size_t cap = n < 1024 ? 1024 : n;
+        if (cudaMalloc(&lat->d_sp, cap * sizeof(SweepParams)) != cudaSuccess) { cudaGetLastError(); return LATTICE_ENOMEM; }
+        lat->sp_cap = cap;
+    }
+    SweepParams *h = (SweepParams *)std::malloc(n * sizeof(SweepParams));
+    if (!h) return LATTICE_ENOMEM;
+    *edge = false;
+    for (uint64_t k = 0; k < n; ++k) {
+        refresh_thresholds(lat, beta[k]);
+        const bool always4 = lat->alwT[0], always8 = lat->alwT[1];
+        SweepParams &p = h[k];
+        p.thr4 = lat->thrT[0];
+        p.thr8 = lat->thrT[1];
+        p.mask4 = always4 ? 0u : 0xffffffffu;
+        p.mask8 = always8 ? 0u : 0xffffffffu;
+        for (int q = 0; q < 8; ++q)
+            p.pcase[q] = (uint32_t)((p.thr4 >> (63 - q)) & 1u) | ((uint32_t)((p.thr8 >> (63 - q)) & 1u) << 1);
+        *edge = *edge || always4 || always8;
+    }
+    // pageable source: the copy is staged before the call returns, so h can be freed right away
+    const cudaError_t ce = cudaMemcpyAsync(lat->d_sp, h, n * sizeof(SweepParams), cudaMemcpyHostToDevice, lat->stream);
+    std::free(h);
+    if (ce != cudaSuccess) return cuda_fail(lat, ce, "sweep parameter upload");
+    return LATTICE_OK;
 }
 
 // Cache-resident Ising lattices: all n sweeps in one cooperative launch (ising_persist.cuh).
 // Returns 1 if the path does not apply (the caller then launches the half-sweeps one by one).
 static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
 {
-    if (lat->model != LATTICE_ISING || lat->scheme < 1 || lat->slab || lat->view || (lat->wpr % 4u) != 0 ||
+    if (lat->model != LATTICE_ISING || lat->scheme < 1 || lat->slab || lat->view || lat->n_rep || (lat->wpr % 4u) != 0 ||
         lat->L > 8192u || n < 2 || lat->persist_blocks < 0)
         return 1;
     if (lat->persist_blocks == 0) {
@@ -666,32 +798,9 @@ static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
     }
     const uint32_t L = lat->L, wpr = lat->wpr, nq = wpr / 4u;
     const size_t pw = (size_t)L * wpr;
-    if (lat->sp_cap < n) {
-        if (lat->d_sp) cudaFree(lat->d_sp);
-        lat->d_sp = nullptr; lat->sp_cap = 0;
-        const size_t cap = n < 1024 ? 1024 : n;
-        if (cudaMalloc(&lat->d_sp, cap * sizeof(SweepParams)) != cudaSuccess) { cudaGetLastError(); return LATTICE_ENOMEM; }
-        lat->sp_cap = cap;
-    }
-    SweepParams *h = (SweepParams *)std::malloc(n * sizeof(SweepParams));
-    if (!h) return LATTICE_ENOMEM;
     bool edge = false;
-    for (uint64_t k = 0; k < n; ++k) {
-        refresh_thresholds(lat, beta[k]);
-        const bool always4 = lat->alwT[0], always8 = lat->alwT[1];
-        SweepParams &p = h[k];
-        p.thr4 = lat->thrT[0];
-        p.thr8 = lat->thrT[1];
-        p.mask4 = always4 ? 0u : 0xffffffffu;
-        p.mask8 = always8 ? 0u : 0xffffffffu;
-        for (int q = 0; q < 8; ++q)
-            p.pcase[q] = (uint32_t)((p.thr4 >> (63 - q)) & 1u) | ((uint32_t)((p.thr8 >> (63 - q)) & 1u) << 1);
-        edge = edge || always4 || always8;
-    }
-    // pageable source: the copy is staged before the call returns, so h can be freed right away
-    const cudaError_t ce = cudaMemcpyAsync(lat->d_sp, h, n * sizeof(SweepParams), cudaMemcpyHostToDevice, lat->stream);
-    std::free(h);
-    if (ce != cudaSuccess) return cuda_fail(lat, ce, "sweep parameter upload");
+    const int urc = upload_sweep_params(lat, n, beta, &edge);
+    if (urc != LATTICE_OK) return urc;
 
     IsingMarchArgs a;
     std::memset(&a, 0, sizeof a);
@@ -716,12 +825,146 @@ static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
     return LATTICE_OK;
 }
 
+// ---- batch of replicas (lattice_create_batch) -----------------------------------------------------
+// One half-sweep of every replica.  Ising lattices whose rows are whole 128-bit runs go through the
+// batched marching kernel (all replicas of a chunk in one launch); everything else falls back to one
+// launch per replica through the replica's own handle.
+static int launch_half_sweep_batch(lattice *lat, int colour)
+{
+    if (lat->model == LATTICE_ISING && lat->scheme >= 1 && (lat->wpr % 4u) == 0) {
+        const uint32_t wpr = lat->wpr, nq = wpr / 4u, L = lat->L;
+        const size_t pw = (size_t)L * wpr;
+        IsingMarchArgs a;
+        std::memset(&a, 0, sizeof a);
+        a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t; a.colour = (uint32_t)colour;
+        const bool always4 = lat->alwT[0], always8 = lat->alwT[1];
+        a.thr4 = lat->thrT[0];
+        a.thr8 = lat->thrT[1];
+        a.mask4 = always4 ? 0u : 0xffffffffu;
+        a.mask8 = always8 ? 0u : 0xffffffffu;
+        for (int p = 0; p < 8; ++p)
+            a.pcase[p] = (uint32_t)((a.thr4 >> (63 - p)) & 1u) | ((uint32_t)((a.thr8 >> (63 - p)) & 1u) << 1);
+        // rows per thread: as for one lattice, but the batch as a whole has to fill the GPU
+        uint32_t R = 2;
+        for (uint32_t cand = 32; cand > 2; cand >>= 1) {
+            if (L % cand) continue;
+            const unsigned long long threads = (unsigned long long)nq * (L / cand);
+            if ((threads % 32u) == 0 && threads * lat->n_rep >= (1ull << 19)) { R = cand; break; }
+        }
+        const bool one_row = (unsigned long long)nq * (L / 2u) * lat->n_rep < 148ull * 256ull * 4ull;
+        a.R = one_row ? 1u : R;
+        a.threads = nq * (L / a.R);
+        const unsigned bx = (a.threads + 255u) / 256u;
+        const bool edge = always4 || always8;
+        BatchKeys &bk = *lat->bk;                         // 10 KiB: filled per chunk, copied at launch
+        for (uint32_t r0 = 0; r0 < lat->n_rep; r0 += BATCH_CHUNK) {
+            const uint32_t nr = lat->n_rep - r0 < (uint32_t)BATCH_CHUNK ? lat->n_rep - r0 : (uint32_t)BATCH_CHUNK;
+            std::memcpy(bk.K, lat->h_keys + r0, nr * sizeof(RoundKeys));
+            a.tgt = lat->buf + (size_t)r0 * lat->rep_words + (size_t)colour * pw;
+            a.opp = lat->buf + (size_t)r0 * lat->rep_words + (size_t)(1 - colour) * pw;
+            const dim3 grid(bx, nr);
+            const unsigned long long stride = lat->rep_words;
+#define LAT_LAUNCH_BATCH(C, E, O) ising_march_batch_kernel<C, E, O><<<grid, 256, 0, lat->stream>>>(a, bk, stride)
+            if (one_row) {
+                if (colour == 0) { if (edge) LAT_LAUNCH_BATCH(0, true, true); else LAT_LAUNCH_BATCH(0, false, true); }
+                else { if (edge) LAT_LAUNCH_BATCH(1, true, true); else LAT_LAUNCH_BATCH(1, false, true); }
+            } else {
+                if (colour == 0) { if (edge) LAT_LAUNCH_BATCH(0, true, false); else LAT_LAUNCH_BATCH(0, false, false); }
+                else { if (edge) LAT_LAUNCH_BATCH(1, true, false); else LAT_LAUNCH_BATCH(1, false, false); }
+            }
+#undef LAT_LAUNCH_BATCH
+            lat->launches += 1;
+            CU(lat, cudaGetLastError());
+        }
+        return LATTICE_OK;
+    }
+    for (uint32_t r = 0; r < lat->n_rep; ++r) {
+        lattice *kid = lat->kids[r];
+        kid->t = lat->t;
+        kid->scheme = lat->scheme;
+        kid->have_beta = true;
+        kid->beta = lat->beta;
+        std::memcpy(kid->thr64, lat->thr64, sizeof lat->thr64);
+        std::memcpy(kid->thrT, lat->thrT, sizeof lat->thrT);
+        std::memcpy(kid->alwT, lat->alwT, sizeof lat->alwT);
+        const int rc = launch_half_sweep(kid, colour);
+        if (rc) return rc;
+    }
+    return LATTICE_OK;
+}
+
+// n sweeps of every replica.  L = 64, 128 (Ising, bit-plane schemes): the whole call is ONE launch of
+// ising_tiny_kernel, replicas resident in registers.  Otherwise two (chunked) launches per sweep.
+static int sweep_batch(lattice *lat, uint64_t n, const double *beta)
+{
+    if (lat->model == LATTICE_ISING && lat->scheme >= 1 && lat->wpr <= 2u) {
+        for (uint64_t done = 0; done < n;) {
+            const uint64_t chunk = n - done < 65536 ? n - done : 65536;
+            bool edge = false;
+            const int rc = upload_sweep_params(lat, chunk, beta + done, &edge);
+            if (rc) return rc;
+            const uint32_t lanes = 16u * lat->wpr;
+            const unsigned long long threads = (unsigned long long)lat->n_rep * lanes;
+            const unsigned blocks = (unsigned)((threads + 127u) / 128u);
+            if (lat->wpr == 1u)
+                ising_tiny_kernel<1><<<blocks, 128, 0, lat->stream>>>(lat->buf, lat->d_keys, lat->d_sp, lat->n_rep,
+                                                                       (uint32_t)lat->t, (uint32_t)chunk);
+            else
+                ising_tiny_kernel<2><<<blocks, 128, 0, lat->stream>>>(lat->buf, lat->d_keys, lat->d_sp, lat->n_rep,
+                                                                       (uint32_t)lat->t, (uint32_t)chunk);
+            lat->launches += 1;
+            CU(lat, cudaGetLastError());
+            lat->t += chunk;
+            done += chunk;
+        }
+        return LATTICE_OK;
+    }
+    if (lat->model == LATTICE_ISING && lat->scheme >= 1 && (lat->wpr % 4u) == 0 && lat->L <= 1024u && n >= 2) {
+        // one block per replica, all sweeps of the chunk in one launch (ising_block_kernel)
+        for (uint64_t done = 0; done < n;) {
+            const uint64_t chunk = n - done < 65536 ? n - done : 65536;
+            bool edge = false;
+            const int rc = upload_sweep_params(lat, chunk, beta + done, &edge);
+            if (rc) return rc;
+            IsingMarchArgs a;
+            std::memset(&a, 0, sizeof a);
+            a.L = lat->L; a.wpr = lat->wpr; a.t = (uint32_t)lat->t;
+            a.R = 1u;
+            a.threads = (lat->wpr / 4u) * lat->L;                     // one row of one run per thread
+            const unsigned bs = a.threads < (unsigned)BLOCK_KERNEL_THREADS ? a.threads : (unsigned)BLOCK_KERNEL_THREADS;
+            const unsigned long long stride = lat->rep_words;
+            if (edge)
+                ising_block_kernel<true><<<lat->n_rep, bs, 0, lat->stream>>>(a, lat->buf, lat->d_keys, lat->d_sp,
+                                                                            (uint32_t)chunk, stride);
+            else
+                ising_block_kernel<false><<<lat->n_rep, bs, 0, lat->stream>>>(a, lat->buf, lat->d_keys, lat->d_sp,
+                                                                             (uint32_t)chunk, stride);
+            lat->launches += 1;
+            CU(lat, cudaGetLastError());
+            lat->t += chunk;
+            done += chunk;
+        }
+        return LATTICE_OK;
+    }
+    for (uint64_t k = 0; k < n; ++k) {
+        refresh_thresholds(lat, beta[k]);
+        int rc = launch_half_sweep_batch(lat, 0);
+        if (rc) return rc;
+        rc = launch_half_sweep_batch(lat, 1);
+        if (rc) return rc;
+        lat->t += 1;
+    }
+    return LATTICE_OK;
+}
+
 int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta)
 {
     if (!lat || (n && !beta)) return LATTICE_EINVAL;
+    if (lat->parent) return LATTICE_ESTATE;               // replicas are swept through their batch handle
     if (lat->t + n >= TWO32) return LATTICE_EINVAL;
     for (uint64_t k = 0; k < n; ++k)
         if (std::isnan(beta[k]) || beta[k] < 0.0) return LATTICE_EINVAL;
+    if (lat->n_rep) return sweep_batch(lat, n, beta);
     for (uint64_t done = 0; done < n;) {
         // cache-resident Ising lattices: up to 65536 sweeps per cooperative launch
         const uint64_t chunk = n - done < 65536 ? n - done : 65536;
@@ -741,19 +984,47 @@ int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta)
     return LATTICE_OK;
 }
 
-// device counters -> the signed sums of the ABI (synchronises the stream)
-static int finish_measure(lattice *lat, uint64_t n_rows, uint32_t r_max, size_t entries, int64_t *M,
-                          int64_t *Q, int64_t *Sx, int64_t *Sy)
+// Generic measurement kernels over n_rep buffers `buf + k * rep_words` (counters at cnt + k *
+// cnt_stride): M, Q if mq; then naxes axes starting at axis0 (0 = x, 1 = y), base rows gi0 .. gi0+gn-1.
+static int enqueue_generic(lattice *lat, const uint32_t *buf, unsigned long long *cnt, uint32_t n_rep,
+                           size_t rep_words, size_t cnt_stride, uint32_t gi0, uint32_t gn, uint32_t r_max,
+                           bool mq, uint32_t axis0, uint32_t naxes)
 {
-    const uint64_t L = lat->L;
-    unsigned long long *h = (unsigned long long *)std::malloc(entries * sizeof(unsigned long long));
-    if (!h) return LATTICE_ENOMEM;
-    cudaError_t e = cudaMemcpyAsync(h, lat->d_cnt, entries * sizeof(unsigned long long),
-                                    cudaMemcpyDeviceToHost, lat->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(lat->stream);
-    if (e != cudaSuccess) { std::free(h); return cuda_fail(lat, e, "measure copy/sync"); }
-    const int64_t N = (int64_t)(n_rows * L);
-    if (lat->model == LATTICE_ISING) {
+    MeasArgs a;
+    a.buf = buf; a.L = lat->rows; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
+    a.r_max = r_max; a.r0 = 0; a.axis0 = axis0; a.cnt = cnt;
+    a.i0 = gi0; a.n_rows = gn;
+    a.rep_words = rep_words; a.cnt_stride = cnt_stride;
+    const unsigned long long words = 2ull * gn * lat->wpr;
+    const unsigned bx = (unsigned)((words + 255) / 256);
+    if (mq) {
+        unsigned gx = bx > 148u * 16u ? 148u * 16u : bx;
+        if (n_rep > 1 && gx > 8u) gx = 8u;
+        a.bpr = gx;
+        measure_mq_kernel<<<gx * n_rep, 256, 0, lat->stream>>>(a);
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+    }
+    unsigned gx = bx;
+    const unsigned long long cap = (148ull * 32ull + 2ull * r_max * n_rep - 1) / (2ull * r_max * n_rep);
+    if (gx > cap) gx = (unsigned)(cap ? cap : 1);
+    if (gx < 1) gx = 1;
+    a.bpr = gx;
+    for (uint32_t r0 = 0; r0 < r_max; r0 += 65535u) {         // at most 65535 r values in grid.y
+        const uint32_t nr = (r_max - r0 < 65535u) ? r_max - r0 : 65535u;
+        a.r0 = r0;
+        measure_corr_kernel<<<dim3(gx * n_rep, nr, naxes), 256, 0, lat->stream>>>(a);
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+    }
+    return LATTICE_OK;
+}
+
+// device counters (MeasArgs::cnt layout, `entries` of them) -> the signed sums of the ABI
+static void convert_counts(int model, int64_t N, uint32_t r_max, const unsigned long long *h, int64_t *M,
+                           int64_t *Q, int64_t *Sx, int64_t *Sy)
+{
+    if (model == LATTICE_ISING) {
         *M = 2 * (int64_t)h[0] - N;
         *Q = N;
         for (uint32_t r = 0; r < r_max; ++r) {
@@ -768,38 +1039,33 @@ static int finish_measure(lattice *lat, uint64_t n_rows, uint32_t r_max, size_t 
             Sy[r] = (int64_t)h[2 + 2 * ((size_t)r_max + r)] - 2 * (int64_t)h[3 + 2 * ((size_t)r_max + r)];
         }
     }
-    std::free(h);
+}
+
+// copies `entries` counters from `src` (device) to the host and synchronises the stream
+static int fetch_counts(lattice *lat, const unsigned long long *src, size_t entries, unsigned long long **out)
+{
+    unsigned long long *h = (unsigned long long *)std::malloc(entries * sizeof(unsigned long long));
+    if (!h) return LATTICE_ENOMEM;
+    cudaError_t e = cudaMemcpyAsync(h, src, entries * sizeof(unsigned long long), cudaMemcpyDeviceToHost, lat->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(lat->stream);
+    if (e != cudaSuccess) { std::free(h); return cuda_fail(lat, e, "measure copy/sync"); }
+    *out = h;
     return LATTICE_OK;
 }
 
-int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t r_max, int64_t *M,
-                         int64_t *Q, int64_t *Sx, int64_t *Sy)
+// Launches (no synchronisation) that add the counts of base rows i0 .. i0+n_rows-1 of lat's buffer,
+// r = 1..r_max, to the zeroed counters at cnt.  Row-blocked kernels: the y axis (and M, Q) over the
+// whole 16-row blocks of the slab, the x axis over every row when a row is a whole number of 16-word
+// segments; whatever they do not cover (ragged rows, narrow lattices) goes through the generic ones.
+static int enqueue_measure(lattice *lat, unsigned long long *cnt, uint64_t i0, uint64_t n_rows, uint32_t r_max)
 {
-    if (!lat || !M || !Q || !Sx || !Sy) return LATTICE_EINVAL;
-    const uint64_t L = lat->L;
-    const uint64_t R = lat->view ? lat->rows : L;                 // rows that can be base rows
-    if (r_max < 1 || r_max > L / 2 || i0 >= R || n_rows < 1 || n_rows > R || i0 + n_rows > R)
-        return LATTICE_EINVAL;
-    // a row slab measures its own rows only, and only r = 1 (row i+1 of the last own row is the
-    // lower halo); larger r along y would need r_max halo rows
-    if (lat->slab && (r_max != 1 || i0 < lat->row0 || i0 + n_rows > (uint64_t)lat->row0 + lat->n_own))
-        return LATTICE_EINVAL;
-    // a view is not periodic along y: the partner rows i + r must lie inside the buffer
-    if (lat->view && i0 + n_rows + r_max > lat->rows) return LATTICE_EINVAL;
-    const size_t entries = 2 + 4 * (size_t)r_max;
-    int rc = ensure_cnt(lat, entries);
-    if (rc) return rc;
-    CU(lat, cudaMemsetAsync(lat->d_cnt, 0, entries * sizeof(unsigned long long), lat->stream));
-    // Row-blocked kernels: the y axis (and M, Q) over the whole 16-row blocks of the slab, the
-    // x axis over every row when a row is a whole number of 16-word segments.  Whatever they do
-    // not cover (ragged rows, narrow lattices) goes through the generic kernels.
     if (r_max == 1 && (lat->wpr % 4u) == 0) {
         // the per-step record (e, m, q): one pass over the slab
         MeasE1Args e1;
         e1.buf = lat->buf; e1.rows = lat->rows; e1.wpr = lat->wpr;
         e1.i0 = lat->slab ? (uint32_t)(i0 - lat->row0) + 1u : (uint32_t)i0;      // local row index
         e1.par_off = lat->slab ? ((lat->row0 + 1u) & 1u) : 0u;
-        e1.n_rows = (uint32_t)n_rows; e1.cnt = lat->d_cnt;
+        e1.n_rows = (uint32_t)n_rows; e1.cnt = cnt;
         const unsigned long long threads =
             (unsigned long long)(lat->wpr / 4u) * ((n_rows + MEAS_E1_ROWS - 1) / MEAS_E1_ROWS);
         const unsigned grid = (unsigned)((threads + 127) / 128);
@@ -807,7 +1073,7 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
         else measure_e1_kernel<1><<<grid, 128, 0, lat->stream>>>(e1);
         lat->launches += 1;
         CU(lat, cudaGetLastError());
-        return finish_measure(lat, n_rows, r_max, entries, M, Q, Sx, Sy);
+        return LATTICE_OK;
     }
     const uint32_t nblk = (uint32_t)(n_rows / MEAS_NB);
     const uint32_t rows_blk = nblk * MEAS_NB;
@@ -815,7 +1081,7 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
     const unsigned chunks = (r_max + MEAS_RC - 1) / MEAS_RC;
     MeasBlkArgs b;
     // the kernels' "L" is the number of rows per plane (plane stride, y wrap): rows == L for a lattice
-    b.buf = lat->buf; b.L = lat->rows; b.wpr = lat->wpr; b.i0 = (uint32_t)i0; b.r_max = r_max; b.cnt = lat->d_cnt;
+    b.buf = lat->buf; b.L = lat->rows; b.wpr = lat->wpr; b.i0 = (uint32_t)i0; b.r_max = r_max; b.cnt = cnt;
     if (nblk) {
         b.n = nblk;
         const unsigned long long threads = 2ull * nblk * lat->wpr;
@@ -834,41 +1100,75 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
         lat->launches += 1;
         CU(lat, cudaGetLastError());
     }
-    MeasArgs a;
-    a.buf = lat->buf; a.L = lat->rows; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
-    a.r_max = r_max; a.r0 = 0; a.axis0 = 0; a.cnt = lat->d_cnt;
-    auto generic = [&](uint32_t gi0, uint32_t gn, bool mq, uint32_t axis0, uint32_t naxes) -> int {
-        a.i0 = gi0; a.n_rows = gn; a.axis0 = axis0;
-        const unsigned long long words = 2ull * gn * lat->wpr;
-        const unsigned bx = (unsigned)((words + 255) / 256);
-        if (mq) {
-            const unsigned gx = bx > 148u * 16u ? 148u * 16u : bx;
-            measure_mq_kernel<<<gx, 256, 0, lat->stream>>>(a);
-            lat->launches += 1;
-            CU(lat, cudaGetLastError());
-        }
-        unsigned gx = bx;
-        const unsigned long long cap = (148ull * 32ull + 2ull * r_max - 1) / (2ull * r_max);
-        if (gx > cap) gx = (unsigned)(cap ? cap : 1);
-        if (gx < 1) gx = 1;
-        for (uint32_t r0 = 0; r0 < r_max; r0 += 65535u) {     // at most 65535 r values in grid.y
-            const uint32_t nr = (r_max - r0 < 65535u) ? r_max - r0 : 65535u;
-            a.r0 = r0;
-            measure_corr_kernel<<<dim3(gx, nr, naxes), 256, 0, lat->stream>>>(a);
-            lat->launches += 1;
-            CU(lat, cudaGetLastError());
-        }
-        return LATTICE_OK;
-    };
-    if (rows_blk < n_rows) {            // ragged rows: M, Q, y axis (and x axis if not done above)
-        rc = generic((uint32_t)i0 + rows_blk, (uint32_t)n_rows - rows_blk, true, x_blk ? 1u : 0u, x_blk ? 1u : 2u);
+    int rc = LATTICE_OK;
+    if (rows_blk < n_rows)              // ragged rows: M, Q, y axis (and x axis if not done above)
+        rc = enqueue_generic(lat, lat->buf, cnt, 1, 0, 0, (uint32_t)i0 + rows_blk, (uint32_t)n_rows - rows_blk,
+                             r_max, true, x_blk ? 1u : 0u, x_blk ? 1u : 2u);
+    if (rc == LATTICE_OK && !x_blk && rows_blk)     // narrow lattice: x axis of the blocked rows
+        rc = enqueue_generic(lat, lat->buf, cnt, 1, 0, 0, (uint32_t)i0, rows_blk, r_max, false, 0u, 1u);
+    return rc;
+}
+
+int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t r_max, int64_t *M,
+                         int64_t *Q, int64_t *Sx, int64_t *Sy)
+{
+    if (!lat || !M || !Q || !Sx || !Sy) return LATTICE_EINVAL;
+    if (lat->n_rep) return LATTICE_ESTATE;                        // lattice_measure_batch / lattice_replica
+    const uint64_t L = lat->L;
+    const uint64_t R = lat->view ? lat->rows : L;                 // rows that can be base rows
+    if (r_max < 1 || r_max > L / 2 || i0 >= R || n_rows < 1 || n_rows > R || i0 + n_rows > R)
+        return LATTICE_EINVAL;
+    // a row slab measures its own rows only, and only r = 1 (row i+1 of the last own row is the
+    // lower halo); larger r along y would need r_max halo rows
+    if (lat->slab && (r_max != 1 || i0 < lat->row0 || i0 + n_rows > (uint64_t)lat->row0 + lat->n_own))
+        return LATTICE_EINVAL;
+    // a view is not periodic along y: the partner rows i + r must lie inside the buffer
+    if (lat->view && i0 + n_rows + r_max > lat->rows) return LATTICE_EINVAL;
+    const size_t entries = 2 + 4 * (size_t)r_max;
+    int rc = ensure_cnt(lat, entries);
+    if (rc) return rc;
+    CU(lat, cudaMemsetAsync(lat->d_cnt, 0, entries * sizeof(unsigned long long), lat->stream));
+    rc = enqueue_measure(lat, lat->d_cnt, i0, n_rows, r_max);
+    if (rc) return rc;
+    unsigned long long *h = nullptr;
+    rc = fetch_counts(lat, lat->d_cnt, entries, &h);
+    if (rc) return rc;
+    convert_counts(lat->model, (int64_t)(n_rows * L), r_max, h, M, Q, Sx, Sy);
+    std::free(h);
+    return LATTICE_OK;
+}
+
+// Whole-lattice counts of every replica of a batch: M[k], Q[k], Sx[k * r_max + r-1], Sy[...].
+// Narrow replicas (L < 1024) are measured by ONE set of launches of the generic kernels over all
+// replicas; wider ones replica by replica with the row-blocked kernels, without synchronising in
+// between.  One copy and one synchronisation at the end.
+int lattice_measure_batch(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy)
+{
+    if (!lat || !M || !Q || !Sx || !Sy || lat->n_rep == 0) return LATTICE_EINVAL;
+    const uint64_t L = lat->L;
+    if (r_max < 1 || r_max > L / 2) return LATTICE_EINVAL;
+    const size_t entries = 2 + 4 * (size_t)r_max, total = entries * lat->n_rep;
+    int rc = ensure_cnt(lat, total);
+    if (rc) return rc;
+    CU(lat, cudaMemsetAsync(lat->d_cnt, 0, total * sizeof(unsigned long long), lat->stream));
+    if (L < 1024u) {
+        rc = enqueue_generic(lat, lat->buf, lat->d_cnt, lat->n_rep, lat->rep_words, entries, 0u, (uint32_t)L, r_max,
+                             true, 0u, 2u);
         if (rc) return rc;
+    } else {
+        for (uint32_t k = 0; k < lat->n_rep; ++k) {
+            rc = enqueue_measure(lat->kids[k], lat->d_cnt + (size_t)k * entries, 0, L, r_max);
+            if (rc) return rc;
+        }
     }
-    if (!x_blk && rows_blk) {           // narrow lattice: x axis of the blocked rows
-        rc = generic((uint32_t)i0, rows_blk, false, 0u, 1u);
-        if (rc) return rc;
-    }
-    return finish_measure(lat, n_rows, r_max, entries, M, Q, Sx, Sy);
+    unsigned long long *h = nullptr;
+    rc = fetch_counts(lat, lat->d_cnt, total, &h);
+    if (rc) return rc;
+    for (uint32_t k = 0; k < lat->n_rep; ++k)
+        convert_counts(lat->model, (int64_t)(L * L), r_max, h + (size_t)k * entries, M + k, Q + k,
+                       Sx + (size_t)k * r_max, Sy + (size_t)k * r_max);
+    std::free(h);
+    return LATTICE_OK;
 }
 
 int lattice_measure(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy)
@@ -881,7 +1181,8 @@ static int window_call(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uin
                        bool set)
 {
     if (!lat || !host) return LATTICE_EINVAL;
-    if (lat->view) return LATTICE_ESTATE;             // a view is a measurement-only handle
+    if (lat->view || lat->n_rep) return LATTICE_ESTATE;   // a view is measurement-only; a batch hands out
+                                                          // its replicas through lattice_replica
     const uint64_t L = lat->L;
     if (h < 1 || w < 1 || h > L || w > L || i0 >= L || j0 >= L) return LATTICE_EINVAL;
     const uint32_t row_base = lat->slab ? (lat->row0 + lat->L - 1u) % lat->L : 0u;
@@ -935,6 +1236,13 @@ int lattice_fill(lattice_t *lat, int spin)
 {
     if (!lat || lat->view || spin < -1 || spin > 1 || (lat->model == LATTICE_ISING && spin == 0))
         return LATTICE_EINVAL;
+    if (lat->n_rep) {
+        for (uint32_t r = 0; r < lat->n_rep; ++r) {
+            const int rc = lattice_fill(lat->kids[r], spin);
+            if (rc) return rc;
+        }
+        return LATTICE_OK;
+    }
     const size_t plane = (size_t)lat->rows * lat->wpr * sizeof(uint32_t);
     if (lat->model == LATTICE_ISING) {
         CU(lat, cudaMemsetAsync(lat->buf, spin > 0 ? 0xFF : 0x00, 2 * plane, lat->stream));
@@ -953,12 +1261,18 @@ uint64_t lattice_time(const lattice_t *lat) { return lat ? lat->t : 0; }
 int lattice_set_time(lattice_t *lat, uint64_t t)
 {
     if (!lat || t >= TWO32) return LATTICE_EINVAL;
-    if (lat->view) return LATTICE_ESTATE;
+    if (lat->view || lat->parent) return LATTICE_ESTATE;
     lat->t = t;
     return LATTICE_OK;
 }
 
-uint64_t lattice_launches(const lattice_t *lat) { return lat ? lat->launches : 0; }
+uint64_t lattice_launches(const lattice_t *lat)
+{
+    if (!lat) return 0;
+    uint64_t n = lat->launches;
+    for (uint32_t r = 0; r < lat->n_rep; ++r) n += lat->kids[r]->launches;
+    return n;
+}
 
 int lattice_set_persist_blocks(lattice_t *lat, uint32_t max_blocks)
 {
@@ -1079,10 +1393,8 @@ int lattice_ubench_int_dispatch(int mode, void *cuda_stream, double *thread_inst
 int lattice_destroy(lattice_t *lat)
 {
     if (!lat) return LATTICE_EINVAL;
-    if (lat->d_cnt) cudaFree(lat->d_cnt);
-    if (lat->d_win) cudaFree(lat->d_win);
-    if (lat->d_sp) cudaFree(lat->d_sp);
-    delete lat;
+    if (lat->parent) return LATTICE_ESTATE;               // replicas are owned by their batch handle
+    free_handle(lat);
     return LATTICE_OK;
 }
 

@@ -28,6 +28,10 @@ struct MeasArgs {
     uint32_t r0;                     // this launch covers r = r0+1 .. r0+gridDim.y
     uint32_t axis0;                  // axis of blockIdx.z == 0 (0 = x, 1 = y)
     unsigned long long *cnt;
+    // batch of replicas: blockIdx.x = replica * bpr + block; replica k reads buf + k * rep_words
+    // and adds to cnt + k * cnt_stride (bpr = gridDim.x, strides 0 for a single lattice)
+    uint32_t bpr;
+    unsigned long long rep_words, cnt_stride;
 };
 
 __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v)
@@ -55,43 +59,48 @@ __device__ __forceinline__ void block_add2(unsigned long long a, unsigned long l
     }
 }
 
-// word k of (colour, plane) in row i
-__device__ __forceinline__ const uint32_t *plane_ptr(const MeasArgs &a, uint32_t colour, uint32_t plane)
+// word k of (colour, plane) in row i of the lattice that starts at buf
+__device__ __forceinline__ const uint32_t *plane_ptr(const MeasArgs &a, const uint32_t *buf, uint32_t colour,
+                                                     uint32_t plane)
 {
     const size_t pw = (size_t)a.L * a.wpr;
-    return a.model == 0 ? a.buf + (size_t)colour * pw : a.buf + (size_t)(2 * colour + plane) * pw;
+    return a.model == 0 ? buf + (size_t)colour * pw : buf + (size_t)(2 * colour + plane) * pw;
 }
 
 __global__ void __launch_bounds__(256) measure_mq_kernel(const MeasArgs a)
 {
+    const uint32_t rep = blockIdx.x / a.bpr, bx = blockIdx.x - rep * a.bpr;
+    const uint32_t *buf = a.buf + rep * a.rep_words;
     const unsigned long long total = 2ull * a.n_rows * a.wpr;
     unsigned long long c0 = 0, c1 = 0;
-    for (unsigned long long g = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; g < total;
-         g += (unsigned long long)gridDim.x * blockDim.x) {
+    for (unsigned long long g = (unsigned long long)bx * blockDim.x + threadIdx.x; g < total;
+         g += (unsigned long long)a.bpr * blockDim.x) {
         const uint32_t colour = (uint32_t)(g / ((unsigned long long)a.n_rows * a.wpr));
         const unsigned long long rem = g % ((unsigned long long)a.n_rows * a.wpr);
         const size_t off = ((size_t)a.i0 * a.wpr) + rem;
         if (a.model == 0) {
-            c0 += __popc(plane_ptr(a, colour, 0)[off]);
+            c0 += __popc(plane_ptr(a, buf, colour, 0)[off]);
         } else {
-            const uint32_t nz = plane_ptr(a, colour, 0)[off], sg = plane_ptr(a, colour, 1)[off];
+            const uint32_t nz = plane_ptr(a, buf, colour, 0)[off], sg = plane_ptr(a, buf, colour, 1)[off];
             c0 += __popc(nz & ~sg);
             c1 += __popc(nz & sg);
         }
     }
-    block_add2(c0, c1, a.cnt);
+    block_add2(c0, c1, a.cnt + rep * a.cnt_stride);
 }
 
-// grid = (blocks_x, n_r, n_axes): r = r0 + blockIdx.y + 1, axis = axis0 + blockIdx.z (0 = x, 1 = y)
+// grid = (replicas * bpr, n_r, n_axes): r = r0 + blockIdx.y + 1, axis = axis0 + blockIdx.z (0 = x, 1 = y)
 __global__ void __launch_bounds__(256) measure_corr_kernel(const MeasArgs a)
 {
+    const uint32_t rep = blockIdx.x / a.bpr, bx = blockIdx.x - rep * a.bpr;
+    const uint32_t *buf = a.buf + rep * a.rep_words;
     const uint32_t r = a.r0 + blockIdx.y + 1, axis = a.axis0 + blockIdx.z;
     const uint32_t L = a.L, wpr = a.wpr;
     const unsigned long long per_colour = (unsigned long long)a.n_rows * wpr;
     const unsigned long long total = 2ull * per_colour;
     unsigned long long c0 = 0, c1 = 0;
-    for (unsigned long long g = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; g < total;
-         g += (unsigned long long)gridDim.x * blockDim.x) {
+    for (unsigned long long g = (unsigned long long)bx * blockDim.x + threadIdx.x; g < total;
+         g += (unsigned long long)a.bpr * blockDim.x) {
         const uint32_t colour = (uint32_t)(g / per_colour);
         const unsigned long long rem = g % per_colour;
         const uint32_t i = a.i0 + (uint32_t)(rem / wpr), k = (uint32_t)(rem % wpr);
@@ -110,12 +119,12 @@ __global__ void __launch_bounds__(256) measure_corr_kernel(const MeasArgs a)
         }
         const size_t o0 = (size_t)i * wpr + k, o1 = (size_t)i2 * wpr + k1, o2 = (size_t)i2 * wpr + k2;
         if (a.model == 0) {
-            const uint32_t *w0 = plane_ptr(a, colour, 0), *w1 = plane_ptr(a, c2, 0);
+            const uint32_t *w0 = plane_ptr(a, buf, colour, 0), *w1 = plane_ptr(a, buf, c2, 0);
             const uint32_t partner = __funnelshift_r(w1[o1], w1[o2], bo);
             c0 += __popc(w0[o0] ^ partner);
         } else {
-            const uint32_t *n0 = plane_ptr(a, colour, 0), *s0 = plane_ptr(a, colour, 1);
-            const uint32_t *n1 = plane_ptr(a, c2, 0), *s1 = plane_ptr(a, c2, 1);
+            const uint32_t *n0 = plane_ptr(a, buf, colour, 0), *s0 = plane_ptr(a, buf, colour, 1);
+            const uint32_t *n1 = plane_ptr(a, buf, c2, 0), *s1 = plane_ptr(a, buf, c2, 1);
             const uint32_t pn = __funnelshift_r(n1[o1], n1[o2], bo);
             const uint32_t ps = __funnelshift_r(s1[o1], s1[o2], bo);
             const uint32_t both = n0[o0] & pn;
@@ -123,7 +132,7 @@ __global__ void __launch_bounds__(256) measure_corr_kernel(const MeasArgs a)
             c1 += __popc(both & (s0[o0] ^ ps));
         }
     }
-    block_add2(c0, c1, a.cnt + 2 + 2 * ((size_t)axis * a.r_max + (r - 1)));
+    block_add2(c0, c1, a.cnt + rep * a.cnt_stride + 2 + 2 * ((size_t)axis * a.r_max + (r - 1)));
 }
 
 // ---- row-blocked kernels (the production measurement path) ----------------------------------
