@@ -30,6 +30,9 @@ One JSON line is printed by rank 0:
   blume_capel   (default invocation, 1 GPU) the same measurements for Blume-Capel at the paper's
             size (L = 2^19) and for BASELINE config 5b (L = 2^15, beta ramp), each
             with its own value, e2e, roofline, roofline_hbm and clocks
+  batched_replicas  (default invocation, 1 GPU) aggregate updates/ns of 64 replicas of L = 4096 and
+            4096 replicas of L = 64 in one batch handle each (lattice_create_batch): the shapes of
+            BASELINE configs 2 and 1, which fill the GPU only as batches
   cpu_baseline  the oracle, as it stands, on the host cores over bounded samples: `value` is the
             all-cores figure for the timed model and RNG scheme; `matrix` holds 1 thread and all
             cores x schemes 0/1 x both models, `cpu_model` the CPU
@@ -521,6 +524,65 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
     }
 
 
+def bench_batch(name, L, n_rep, args, lat, torch, dev):
+    """Aggregate updates/ns of n_rep independent Ising replicas of side L in one batch handle
+    (lattice_create_batch) at beta_c: K steps of `sps` sweeps per lattice_sweep call, sized to
+    --min-seconds, clock-sampled; e2e adds lattice_measure_batch(r_max = 1) per step."""
+    seeds = np.arange(n_rep, dtype=np.uint64) * 1000 + np.uint64(workloads.SEED_BASE + 31)
+    b = lat.LatticeBatch(L, seeds, lat.ISING, 0.0, args.scheme, device=str(dev))
+    K = args.steps
+    beta = workloads.BETA_C_ISING
+
+    def timed(fn, steps, sps):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(dev)
+        ev0.record(b.stream)
+        for _ in range(steps):
+            fn(sps)
+        ev1.record(b.stream)
+        torch.cuda.synchronize(dev)
+        return ev0.elapsed_time(ev1)
+
+    def step_device(n):
+        b.sweep(np.full(n, beta))
+
+    def step_e2e(n):
+        b.sweep(np.full(n, beta))
+        b.measure(1)
+
+    for _ in range(max(args.warmup, 1)):
+        step_device(4)
+    sps, want_ms = 4, args.min_seconds * 1e3 / K
+    for _ in range(3):
+        ms1 = timed(step_device, 1, sps)
+        if ms1 >= want_ms or sps >= 65536:
+            break
+        sps = int(min(np.ceil(sps * want_ms / max(ms1, 1e-3) * 1.05), 65536))
+    n0 = b.launches
+    sampler = ClockSampler(torch, dev)
+    sampler.start()
+    ms = timed(step_device, K, sps)
+    clocks = sampler.stop()
+    launches = b.launches - n0
+    step_e2e(sps)
+    sampler.start()
+    e2e_ms = timed(step_e2e, K, sps)
+    e2e_clocks = sampler.stop()
+    b.close()
+    del b
+    torch.cuda.empty_cache()
+    updates = L * L * n_rep * sps * K
+    return {"value": updates / (ms * 1e6), "unit": UNIT, "steps": K, "ms_per_step": ms / K,
+            "config": {"workload": name, "model": "ising", "L": L, "replicas": n_rep, "spins": L * L * n_rep,
+                       "state_bytes": L * L // 8 * n_rep, "beta": beta, "rng_scheme": args.scheme,
+                       "sweeps_per_step": sps, "timed_seconds": ms / 1e3,
+                       "l2": "l2_resident_by_design" if L * L // 8 * n_rep <= (126 << 20) else "inputs_larger_than_l2"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "e2e": {"value": updates / (e2e_ms * 1e6), "unit": UNIT, "h2d_bytes_per_step": 8 * sps,
+                    "d2h_bytes_per_step": 8 * 6 * n_rep, "ms_per_step": e2e_ms / K, "clocks": e2e_clocks,
+                    "what": f"lattice_sweep({sps}) on the batch + lattice_measure_batch(r_max=1) -> host int64 per replica"}}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -535,6 +597,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-blume-capel", action="store_true",
                     help="skip the Blume-Capel workloads the default invocation also times")
+    ap.add_argument("--no-batches", action="store_true",
+                    help="skip the batched-replica workloads the default invocation also times")
     ap.add_argument("--measure-rmax", type=int, default=-1,
                     help="r_max of the separately timed measurement pass (-1: the workload's)")
     ap.add_argument("--sharded", action="store_true",
@@ -581,6 +645,12 @@ def main():
                            "e2e": r["e2e"], "roofline": r["roofline"], "roofline_hbm": r["roofline_hbm"],
                            "worst_case": r["worst_case"]}
 
+    # cache-resident sizes fill the GPU only as batches of replicas (BASELINE configs 1 and 2's shapes)
+    batches = {}
+    if world == 1 and not args.no_batches and args.workload == "ising_L2p20" and not args.L:
+        for name, Lb, nb in (("ising_L4096_x64", 4096, 64), ("ising_L64_x4096", 64, 4096)):
+            batches[name] = bench_batch(name, Lb, nb, args, lat, torch, dev)
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -596,6 +666,8 @@ def main():
     }
     if extra:
         line["blume_capel"] = extra
+    if batches:
+        line["batched_replicas"] = batches
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline_matrix(w, args.scheme)
     print(json.dumps(line))

@@ -198,6 +198,15 @@ int lattice_measure(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int6
 int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t r_max,
                          int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy);
 
+/* The same sums for a sparse list of separations -- the paper samples C(r;t) sparsely in r
+ * (PAPER.md:207): Sx[q] = S_x(r[q]), Sy[q] = S_y(r[q]), q = 0..n_r-1, over base rows
+ * i0 .. i0+n_rows-1 (the whole lattice: 0, L).  r is a host array; each entry in [1, L/2], any
+ * order, repeats allowed; n_r <= 2^20.  Cost: one partner read per (word, r[q]) instead of one
+ * per (word, r <= r_max).  Host outputs; synchronises the stream.  On a slab only r = 1 is
+ * available (as for lattice_measure_rows).  Errors: EINVAL, ESTATE (batch handle), ENOMEM, ECUDA. */
+int lattice_measure_list(lattice_t *lat, uint64_t i0, uint64_t n_rows, const uint32_t *r, uint32_t n_r,
+                         int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy);
+
 /* Unpacked -1/0/+1 windows, row-major h x w, global origin (i0, j0), periodic wrap.
  * h, w <= L.  set_spins rejects values outside the model's alphabet (EINVAL).  Both
  * synchronise the stream.  For tests, windowed replay and checkpoints. */
@@ -219,6 +228,15 @@ uint64_t lattice_time(const lattice_t *lat);
 int lattice_set_time(lattice_t *lat, uint64_t t);
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 uint64_t lattice_launches(const lattice_t *lat);
+/* Launch-time specialisation of the Ising half-sweep: how many of the handle's launches ran a
+ * kernel instantiated for the plane cases of their beta (the LOP3 truth tables of the bit-serial
+ * threshold compare as compile-time constants, no per-plane dispatch), and whether such an
+ * instantiation exists for (model, delta, beta) -- it does for beta_c = ln(1 + sqrt 2)/2
+ * (PAPER.md:40), for T_1 = 1.66 and T_2 = 2.27414861561203 of the two-step protocol (Table II,
+ * PAPER.md:144-146) and for any beta whose thresholds share their top bytes with one of these.
+ * Results never depend on which kernel runs. */
+uint64_t lattice_specialised_launches(const lattice_t *lat);
+int lattice_plane_case_specialised(int model, double delta, double beta);
 /* Tuning / test knob: upper bound on the grid of the persistent multi-sweep kernel that
  * lattice_sweep(n >= 2) uses for cache-resident Ising lattices (0 = the occupancy limit, the
  * default).  With fewer blocks than 256-thread groups of work every block strides over several

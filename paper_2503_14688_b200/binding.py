@@ -52,6 +52,7 @@ SIGNATURES = {
     "lattice_measure": (C.c_int, [_vp, C.c_uint32, _i64p, _i64p, _i64p, _i64p]),
     "lattice_measure_rows": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint32, _i64p, _i64p,
                                        _i64p, _i64p]),
+    "lattice_measure_list": (C.c_int, [_vp, C.c_uint64, C.c_uint64, _u32p, C.c_uint32, _i64p, _i64p, _i64p, _i64p]),
     "lattice_get_spins": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _i8p]),
     "lattice_set_spins": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _i8p]),
     "lattice_fill": (C.c_int, [_vp, C.c_int]),
@@ -59,6 +60,8 @@ SIGNATURES = {
     "lattice_set_time": (C.c_int, [_vp, C.c_uint64]),
     "lattice_launches": (C.c_uint64, [_vp]),
     "lattice_set_persist_blocks": (C.c_int, [_vp, C.c_uint32]),
+    "lattice_specialised_launches": (C.c_uint64, [_vp]),
+    "lattice_plane_case_specialised": (C.c_int, [C.c_int, C.c_double, C.c_double]),
     "lattice_thresholds": (None, [C.c_int, C.c_double, C.c_double, _u64p]),
     "lattice_thresholds64": (None, [C.c_int, C.c_double, C.c_double, _u64p, C.POINTER(C.c_ubyte)]),
     "lattice_xi": (C.c_double, [_i64p, _i64p, C.c_uint32, C.c_int64, C.c_uint32, _u32p]),
@@ -279,6 +282,10 @@ class Lattice:
     def launches(self) -> int:
         return int(lib().lattice_launches(self._h))
 
+    @property
+    def specialised_launches(self) -> int:
+        return int(lib().lattice_specialised_launches(self._h))
+
     def set_neighbours(self, up: "Lattice", down: "Lattice") -> None:
         """Row-slab mode: the slabs owning the rows above / below (self twice for a single slab)."""
         self.set_neighbour_ptrs(up.data_ptr, up.slab[1], down.data_ptr, down.slab[1])
@@ -316,6 +323,20 @@ class Lattice:
                 rc = lib().lattice_measure_rows(self._h, rows[0], rows[1], r_max, C.byref(M),
                                                 C.byref(Q), _p(Sx, C.c_int64), _p(Sy, C.c_int64))
         self._check(rc, "lattice_measure")
+        return int(M.value), int(Q.value), Sx, Sy
+
+    def measure_list(self, r_list, rows=None):
+        """(M, Q, Sx[len(r_list)], Sy[len(r_list)]) for a sparse list of separations r."""
+        r = np.ascontiguousarray(np.asarray(r_list, dtype=np.uint32))
+        Sx = np.zeros(r.size, dtype=np.int64)
+        Sy = np.zeros(r.size, dtype=np.int64)
+        M, Q = C.c_int64(0), C.c_int64(0)
+        if rows is None:
+            rows = self.slab if self.slab is not None else (0, self.L)
+        with self._torch.cuda.device(self.device):
+            rc = lib().lattice_measure_list(self._h, rows[0], rows[1], _p(r, C.c_uint32), r.size, C.byref(M),
+                                            C.byref(Q), _p(Sx, C.c_int64), _p(Sy, C.c_int64))
+        self._check(rc, "lattice_measure_list")
         return int(M.value), int(Q.value), Sx, Sy
 
     def get_spins(self, i0: int = 0, j0: int = 0, h: int | None = None, w: int | None = None):

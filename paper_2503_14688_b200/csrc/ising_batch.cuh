@@ -33,7 +33,7 @@ struct BatchKeys {                           // 10 KiB of kernel parameters
 };
 
 #ifdef __CUDACC__
-template <int COLOUR, bool EDGE, bool ONE_ROW>
+template <int COLOUR, bool EDGE, bool ONE_ROW, int PC = -1>
 __global__ void __launch_bounds__(256) ising_march_batch_kernel(const IsingMarchArgs a0,
                                                                 const __grid_constant__ BatchKeys bk,
                                                                 unsigned long long rep_stride)
@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(256) ising_march_batch_kernel(const IsingMarch
     build_plane_fold(a.K, a.t, a.colour, TAG_ACC_PLANE, a.F);
     WarpTieQueue<false> queue{a, s_q[warp], lane, 0u};
     if (ONE_ROW) row_thread<COLOUR, EDGE>(a, g, queue);
-    else march_thread<COLOUR, EDGE, false>(a, g, queue);
+    else march_thread<COLOUR, EDGE, false, PC>(a, g, queue);
     queue.drain();
 }
 

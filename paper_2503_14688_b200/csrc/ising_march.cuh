@@ -111,6 +111,40 @@ __device__ __forceinline__ void plane_compare(uint32_t pcase, const uint32_t (&c
 }
 #undef LAT_PL
 
+// Launch-time specialisation: the plane cases depend only on the top bytes of the two thresholds,
+// i.e. on beta.  For the inverse temperatures the workloads actually run at (constant-beta runs are
+// all of Table I; the two-step protocol has two values) the host picks a kernel
+// instantiated with the packed cases PC = sum_k pcase[k] << 2k, where every LOP3 immediate is a
+// compile-time constant and the eight brx.idx dispatches are gone.  PC < 0: the generic path above.
+template <int PCASE>
+__device__ __forceinline__ void plane_compare_fixed(const uint32_t (&c8)[4], const uint4 &b, uint32_t (&acc)[4],
+                                                    uint32_t (&eq)[4])
+{
+    constexpr int TA = PCASE == 0 ? 0x22 : PCASE == 1 ? 0x2B : PCASE == 2 ? 0xB2 : 0xBB;
+    constexpr int TE = PCASE == 0 ? 0x30 : PCASE == 1 ? 0x60 : PCASE == 2 ? 0x90 : 0xC0;
+    const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        acc[w] = lop3<TA>(c8[w], bw[w], acc[w]);
+        eq[w] = lop3<TE>(eq[w], bw[w], c8[w]);
+    }
+}
+
+// planes K, K-1, ..., 0 (least significant plane first) of unit ps
+template <int PC, int K>
+struct PlaneLoop {
+    template <class Args>
+    static __device__ __forceinline__ void run(const Args &a, const PlaneShared &ps, const uint32_t (&c8)[4],
+                                               uint32_t (&acc)[4], uint32_t (&eq)[4])
+    {
+        // fb[k] = fb[0] ^ (k << 16): the plane index enters as an immediate of the first XOR
+        const uint4 b4 = plane_block(ps, a.F.fb[0] ^ ((uint32_t)K << 16), a.F, a.K);
+        if constexpr (PC >= 0) plane_compare_fixed<(PC >> (2 * K)) & 3>(c8, b4, acc, eq);
+        else plane_compare(a.pcase[K], c8, b4, acc, eq);
+        if constexpr (K > 0) PlaneLoop<PC, K - 1>::run(a, ps, c8, acc, eq);
+    }
+};
+
 // Per-warp queue of words that contain tied lanes.  One 128-bit entry per word:
 //   x = the tied lanes of the word, y = which of them are class dE = 8, (z, w) = word offset.
 // Pushing is loop-free (one ballot per word of the run); the bits of a word are only
@@ -191,7 +225,7 @@ struct WarpTieQueue {
 // and queues the ties.  EDGE: some class has threshold 2^32 (beta = 0): mask it out of `need`.
 // mir / mir_tag: slab mode only -- where this row is mirrored (null: nowhere) and the queue tag
 // (column word << 4 | flag << 30) that lets a late flip reach the mirror too.
-template <int PAR, bool EDGE, bool SLAB>
+template <int PAR, bool EDGE, bool SLAB, int PC = -1>
 __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, unsigned long long wo, uint32_t *tp,
                                           const uint4 &U4, const uint4 &C4, const uint4 &D4, uint32_t E,
                                           WarpTieQueue<SLAB> &queue, uint32_t *mir = nullptr, uint32_t mir_tag = 0)
@@ -226,12 +260,7 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
     // top byte of u32(site) against the top byte of the lane's threshold, least significant
     // plane first
     const PlaneShared ps = plane_shared(G, a.F);
-#pragma unroll
-    for (int k = 7; k >= 0; --k) {
-        // fb[k] = fb[0] ^ (k << 16): the plane index enters as an immediate of the first XOR
-        const uint4 b4 = plane_block(ps, a.F.fb[0] ^ ((uint32_t)k << 16), a.F, a.K);
-        plane_compare(a.pcase[k], c8, b4, acc, eq);
-    }
+    PlaneLoop<PC, 7>::run(a, ps, c8, acc, eq);
     // lanes outside need flip unconditionally (dE <= 0); a tied lane has acc = 0 and stays put
 #pragma unroll
     for (int w = 0; w < 4; ++w) T[w] = lop3<0x4B>(T[w], need[w], acc[w]);    // T ^ (~need | acc)
@@ -245,7 +274,7 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
 
 // The march of one thread: rows i0 .. i0+R-1 of run q, g = s * (wpr/4) + q (ties are queued, not
 // drained).
-template <int COLOUR, bool EDGE, bool SLAB>
+template <int COLOUR, bool EDGE, bool SLAB, int PC = -1>
 __device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g, WarpTieQueue<SLAB> &queue)
 {
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
@@ -276,9 +305,9 @@ __device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g
             const uint4 D = *reinterpret_cast<const uint4 *>(dn + kw);
             const uint32_t E = op[COLOUR == 0 ? ke0 : ke1];
             if (SLAB && top && r == 0)
-                march_row<COLOUR, EDGE, SLAB>(a, G, wo, tp, U, C, D, E, queue, a.mir_up + kw, (kw << 4) | (1u << 30));
+                march_row<COLOUR, EDGE, SLAB, PC>(a, G, wo, tp, U, C, D, E, queue, a.mir_up + kw, (kw << 4) | (1u << 30));
             else
-                march_row<COLOUR, EDGE, SLAB>(a, G, wo, tp, U, C, D, E, queue);
+                march_row<COLOUR, EDGE, SLAB, PC>(a, G, wo, tp, U, C, D, E, queue);
             U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
         {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
@@ -287,9 +316,9 @@ __device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g
             const uint4 D = *reinterpret_cast<const uint4 *>(dn + kw);
             const uint32_t E = op[COLOUR == 0 ? ke1 : ke0];
             if (SLAB && bot && r + 2 == a.R)
-                march_row<COLOUR ^ 1, EDGE, SLAB>(a, G, wo, tp, U, C, D, E, queue, a.mir_dn + kw, (kw << 4) | (2u << 30));
+                march_row<COLOUR ^ 1, EDGE, SLAB, PC>(a, G, wo, tp, U, C, D, E, queue, a.mir_dn + kw, (kw << 4) | (2u << 30));
             else
-                march_row<COLOUR ^ 1, EDGE, SLAB>(a, G, wo, tp, U, C, D, E, queue);
+                march_row<COLOUR ^ 1, EDGE, SLAB, PC>(a, G, wo, tp, U, C, D, E, queue);
             U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
     }
@@ -334,7 +363,13 @@ __global__ void __launch_bounds__(256) ising_row_kernel(const IsingMarchArgs a)
     queue.drain();
 }
 
-template <int COLOUR, bool EDGE, bool SLAB>
+// The plane-case values with a specialised instantiation (host side: ising_pc_index):
+//   0xF910  beta_c = ln(1 + sqrt 2)/2: thr4 = 0x2B......, thr8 = 0x07......  (BASELINE configs 1, 2, 4)
+//   0x7440  T_1 = 1.66 of the paper's two-step protocol (Table II)
+//   0xAD10  T_2 = 2.27414861561203 of the same protocol, and beta_c/1.01 (plateau of config 5a)
+#define LAT_ISING_PC_LIST(X) X(0xF910) X(0x7440) X(0xAD10)
+
+template <int COLOUR, bool EDGE, bool SLAB, int PC = -1>
 __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a)
 {
     __shared__ uint4 s_q[8][TIE_Q_SLOTS];
@@ -342,7 +377,7 @@ __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;
     if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
     WarpTieQueue<SLAB> queue{a, s_q[warp], lane, 0u};
-    march_thread<COLOUR, EDGE, SLAB>(a, g, queue);
+    march_thread<COLOUR, EDGE, SLAB, PC>(a, g, queue);
     queue.drain();
 }
 #endif

@@ -44,6 +44,7 @@ struct lattice {
     uint32_t *buf;             // caller-owned device memory
     cudaStream_t stream;
     uint64_t launches;
+    uint64_t spec_launches;    // launches of plane-case specialised kernels (lattice_specialised_launches)
     RoundKeys K;
     // cached thresholds
     bool have_beta;
@@ -55,6 +56,8 @@ struct lattice {
     unsigned long long *d_cnt;
     size_t cnt_cap;            // entries
     int8_t *d_win;
+    uint32_t *d_rlist;         // lattice_measure_list: the list of r on the device
+    size_t rlist_cap;          // entries
     size_t win_cap;            // bytes
     SweepParams *d_sp;         // per-sweep parameters of the persistent kernel
     size_t sp_cap;             // entries
@@ -193,6 +196,14 @@ bool ising_one_row(const lattice *lat)
     return !lat->slab && marching < 148ull * 256ull;      // measured: helps up to L = 4096
 }
 
+// packed plane cases of the current thresholds: sum_k pcase[k] << 2k (ising_march.cuh)
+static int ising_packed_pc(const uint32_t (&pcase)[8])
+{
+    int pc = 0;
+    for (int k = 0; k < 8; ++k) pc |= (int)(pcase[k] & 3u) << (2 * k);
+    return pc;
+}
+
 int launch_ising_march(lattice *lat, int colour)
 {
     const uint32_t wpr = lat->wpr, nq = wpr / 4u;
@@ -230,8 +241,27 @@ int launch_ising_march(lattice *lat, int colour)
         if (colour == 0) { if (edge) ising_row_kernel<0, true><<<rb, 256, 0, lat->stream>>>(a); else ising_row_kernel<0, false><<<rb, 256, 0, lat->stream>>>(a); }
         else { if (edge) ising_row_kernel<1, true><<<rb, 256, 0, lat->stream>>>(a); else ising_row_kernel<1, false><<<rb, 256, 0, lat->stream>>>(a); }
     } else {
-        if (colour == 0) { if (edge) LAT_LAUNCH_MARCH(0, true, false); else LAT_LAUNCH_MARCH(0, false, false); }
-        else { if (edge) LAT_LAUNCH_MARCH(1, true, false); else LAT_LAUNCH_MARCH(1, false, false); }
+        bool done = false;
+        if (!edge) {
+            // launch-time specialisation: an instantiation with these plane cases compiled in
+            const int pc = ising_packed_pc(a.pcase);
+            switch (pc) {
+#define LAT_PC_CASE(V)                                                                                   \
+            case V:                                                                                      \
+                if (colour == 0) ising_march_kernel<0, false, false, V><<<blocks, 256, 0, lat->stream>>>(a); \
+                else ising_march_kernel<1, false, false, V><<<blocks, 256, 0, lat->stream>>>(a);             \
+                done = true;                                                                             \
+                break;
+            LAT_ISING_PC_LIST(LAT_PC_CASE)
+#undef LAT_PC_CASE
+            default: break;
+            }
+            if (done) lat->spec_launches += 1;
+        }
+        if (!done) {
+            if (colour == 0) { if (edge) LAT_LAUNCH_MARCH(0, true, false); else LAT_LAUNCH_MARCH(0, false, false); }
+            else { if (edge) LAT_LAUNCH_MARCH(1, true, false); else LAT_LAUNCH_MARCH(1, false, false); }
+        }
     }
 #undef LAT_LAUNCH_MARCH
     lat->launches += 1;
@@ -490,6 +520,7 @@ static void free_handle(lattice *lat)
     }
     if (lat->d_cnt) cudaFree(lat->d_cnt);
     if (lat->d_win) cudaFree(lat->d_win);
+    if (lat->d_rlist) cudaFree(lat->d_rlist);
     if (lat->d_sp) cudaFree(lat->d_sp);
     if (lat->d_keys) cudaFree(lat->d_keys);
     if (lat->h_keys) std::free(lat->h_keys);
@@ -865,7 +896,23 @@ static int launch_half_sweep_batch(lattice *lat, int colour)
             const dim3 grid(bx, nr);
             const unsigned long long stride = lat->rep_words;
 #define LAT_LAUNCH_BATCH(C, E, O) ising_march_batch_kernel<C, E, O><<<grid, 256, 0, lat->stream>>>(a, bk, stride)
-            if (one_row) {
+            bool done = false;
+            if (!one_row && !edge) {
+                switch (ising_packed_pc(a.pcase)) {
+#define LAT_PC_CASE(V)                                                                                              \
+                case V:                                                                                             \
+                    if (colour == 0) ising_march_batch_kernel<0, false, false, V><<<grid, 256, 0, lat->stream>>>(a, bk, stride); \
+                    else ising_march_batch_kernel<1, false, false, V><<<grid, 256, 0, lat->stream>>>(a, bk, stride);             \
+                    done = true;                                                                                    \
+                    break;
+                LAT_ISING_PC_LIST(LAT_PC_CASE)
+#undef LAT_PC_CASE
+                default: break;
+                }
+                if (done) lat->spec_launches += 1;
+            }
+            if (done) {
+            } else if (one_row) {
                 if (colour == 0) { if (edge) LAT_LAUNCH_BATCH(0, true, true); else LAT_LAUNCH_BATCH(0, false, true); }
                 else { if (edge) LAT_LAUNCH_BATCH(1, true, true); else LAT_LAUNCH_BATCH(1, false, true); }
             } else {
@@ -988,13 +1035,14 @@ int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta)
 // cnt_stride): M, Q if mq; then naxes axes starting at axis0 (0 = x, 1 = y), base rows gi0 .. gi0+gn-1.
 static int enqueue_generic(lattice *lat, const uint32_t *buf, unsigned long long *cnt, uint32_t n_rep,
                            size_t rep_words, size_t cnt_stride, uint32_t gi0, uint32_t gn, uint32_t r_max,
-                           bool mq, uint32_t axis0, uint32_t naxes)
+                           bool mq, uint32_t axis0, uint32_t naxes, const uint32_t *rlist = nullptr)
 {
     MeasArgs a;
     a.buf = buf; a.L = lat->rows; a.wpr = lat->wpr; a.model = (uint32_t)lat->model;
     a.r_max = r_max; a.r0 = 0; a.axis0 = axis0; a.cnt = cnt;
     a.i0 = gi0; a.n_rows = gn;
     a.rep_words = rep_words; a.cnt_stride = cnt_stride;
+    a.rlist = rlist;
     const unsigned long long words = 2ull * gn * lat->wpr;
     const unsigned bx = (unsigned)((words + 255) / 256);
     if (mq) {
@@ -1138,6 +1186,70 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
     return LATTICE_OK;
 }
 
+// Sparse list of separations (the paper's own choice): Sx[q] = S_x(r[q]), Sy[q] =
+// S_y(r[q]) over base rows i0 .. i0+n_rows-1.  The row-blocked list kernel over the whole 16-row
+// blocks, the generic kernel for the remaining rows.
+int lattice_measure_list(lattice_t *lat, uint64_t i0, uint64_t n_rows, const uint32_t *r, uint32_t n_r,
+                         int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy)
+{
+    if (!lat || !r || !M || !Q || !Sx || !Sy) return LATTICE_EINVAL;
+    if (lat->n_rep) return LATTICE_ESTATE;
+    const uint64_t L = lat->L;
+    const uint64_t R = lat->view ? lat->rows : L;
+    if (n_r < 1 || n_r > (1u << 20) || i0 >= R || n_rows < 1 || n_rows > R || i0 + n_rows > R) return LATTICE_EINVAL;
+    uint32_t r_hi = 0;
+    for (uint32_t q = 0; q < n_r; ++q) {
+        if (r[q] < 1 || r[q] > L / 2) return LATTICE_EINVAL;
+        if (r[q] > r_hi) r_hi = r[q];
+    }
+    if (lat->slab && (r_hi != 1 || i0 < lat->row0 || i0 + n_rows > (uint64_t)lat->row0 + lat->n_own))
+        return LATTICE_EINVAL;
+    if (lat->view && i0 + n_rows + r_hi > lat->rows) return LATTICE_EINVAL;
+    if (lat->slab) {
+        // a slab only has r = 1: the dense one-pass kernel, replicated over the list
+        int64_t sx = 0, sy = 0;
+        const int rc1 = lattice_measure_rows(lat, i0, n_rows, 1, M, Q, &sx, &sy);
+        if (rc1) return rc1;
+        for (uint32_t q = 0; q < n_r; ++q) { Sx[q] = sx; Sy[q] = sy; }
+        return LATTICE_OK;
+    }
+    const size_t entries = 2 + 4 * (size_t)n_r;
+    int rc = ensure_cnt(lat, entries);
+    if (rc) return rc;
+    if (lat->rlist_cap < n_r) {
+        if (lat->d_rlist) cudaFree(lat->d_rlist);
+        lat->d_rlist = nullptr; lat->rlist_cap = 0;
+        const size_t cap = n_r < 256 ? 256 : n_r;
+        if (cudaMalloc(&lat->d_rlist, cap * sizeof(uint32_t)) != cudaSuccess) { cudaGetLastError(); return LATTICE_ENOMEM; }
+        lat->rlist_cap = cap;
+    }
+    CU(lat, cudaMemcpyAsync(lat->d_rlist, r, n_r * sizeof(uint32_t), cudaMemcpyHostToDevice, lat->stream));
+    CU(lat, cudaMemsetAsync(lat->d_cnt, 0, entries * sizeof(unsigned long long), lat->stream));
+    const uint32_t nblk = (uint32_t)(n_rows / MEAS_NB), rows_blk = nblk * MEAS_NB;
+    const unsigned chunks = (n_r + MEAS_LIST_CHUNK - 1) / MEAS_LIST_CHUNK;
+    if (nblk) {
+        MeasListArgs b;
+        b.buf = lat->buf; b.L = lat->rows; b.wpr = lat->wpr; b.i0 = (uint32_t)i0; b.rlist = lat->d_rlist; b.n_r = n_r;
+        b.mq = 1u; b.cnt = lat->d_cnt; b.n = nblk;
+        const unsigned long long threads = 2ull * nblk * lat->wpr;
+        const dim3 grid((unsigned)((threads + 127) / 128), chunks);
+        if (lat->model == LATTICE_ISING) measure_list_kernel<0><<<grid, 128, 0, lat->stream>>>(b);
+        else measure_list_kernel<1><<<grid, 128, 0, lat->stream>>>(b);
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+    }
+    if (rows_blk < n_rows)              // ragged rows: M, Q and both axes through the generic kernel
+        rc = enqueue_generic(lat, lat->buf, lat->d_cnt, 1, 0, 0, (uint32_t)i0 + rows_blk, (uint32_t)n_rows - rows_blk,
+                             n_r, true, 0u, 2u, lat->d_rlist);
+    if (rc) return rc;
+    unsigned long long *h = nullptr;
+    rc = fetch_counts(lat, lat->d_cnt, entries, &h);
+    if (rc) return rc;
+    convert_counts(lat->model, (int64_t)(n_rows * L), n_r, h, M, Q, Sx, Sy);
+    std::free(h);
+    return LATTICE_OK;
+}
+
 // Whole-lattice counts of every replica of a batch: M[k], Q[k], Sx[k * r_max + r-1], Sy[...].
 // Narrow replicas (L < 1024) are measured by ONE set of launches of the generic kernels over all
 // replicas; wider ones replica by replica with the row-blocked kernels, without synchronising in
@@ -1272,6 +1384,26 @@ uint64_t lattice_launches(const lattice_t *lat)
     uint64_t n = lat->launches;
     for (uint32_t r = 0; r < lat->n_rep; ++r) n += lat->kids[r]->launches;
     return n;
+}
+
+uint64_t lattice_specialised_launches(const lattice_t *lat) { return lat ? lat->spec_launches : 0; }
+
+int lattice_plane_case_specialised(int model, double delta, double beta)
+{
+    if (model != LATTICE_ISING || std::isnan(beta) || beta < 0.0) return 0;
+    (void)delta;
+    uint64_t thr[2];
+    build_thresholds(LATTICE_ISING, 0.0, beta, thr);
+    if (thr[0] >= TWO32 || thr[1] >= TWO32) return 0;
+    uint32_t pcase[8];
+    for (int k = 0; k < 8; ++k)
+        pcase[k] = (uint32_t)((thr[0] >> (31 - k)) & 1u) | ((uint32_t)((thr[1] >> (31 - k)) & 1u) << 1);
+    switch (ising_packed_pc(pcase)) {
+#define LAT_PC_CASE(V) case V: return 1;
+    LAT_ISING_PC_LIST(LAT_PC_CASE)
+#undef LAT_PC_CASE
+    default: return 0;
+    }
 }
 
 int lattice_set_persist_blocks(lattice_t *lat, uint32_t max_blocks)

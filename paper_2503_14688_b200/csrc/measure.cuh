@@ -32,6 +32,9 @@ struct MeasArgs {
     // and adds to cnt + k * cnt_stride (bpr = gridDim.x, strides 0 for a single lattice)
     uint32_t bpr;
     unsigned long long rep_words, cnt_stride;
+    // sparse list of r (lattice_measure_list): when non-null, blockIdx.y indexes rlist (device) and
+    // the counters, r_max being the length of the list
+    const uint32_t *rlist;
 };
 
 __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v)
@@ -94,7 +97,8 @@ __global__ void __launch_bounds__(256) measure_corr_kernel(const MeasArgs a)
 {
     const uint32_t rep = blockIdx.x / a.bpr, bx = blockIdx.x - rep * a.bpr;
     const uint32_t *buf = a.buf + rep * a.rep_words;
-    const uint32_t r = a.r0 + blockIdx.y + 1, axis = a.axis0 + blockIdx.z;
+    const uint32_t ridx = a.r0 + blockIdx.y, axis = a.axis0 + blockIdx.z;
+    const uint32_t r = a.rlist ? a.rlist[ridx] : ridx + 1;
     const uint32_t L = a.L, wpr = a.wpr;
     const unsigned long long per_colour = (unsigned long long)a.n_rows * wpr;
     const unsigned long long total = 2ull * per_colour;
@@ -132,7 +136,7 @@ __global__ void __launch_bounds__(256) measure_corr_kernel(const MeasArgs a)
             c1 += __popc(both & (s0[o0] ^ ps));
         }
     }
-    block_add2(c0, c1, a.cnt + rep * a.cnt_stride + 2 + 2 * ((size_t)axis * a.r_max + (r - 1)));
+    block_add2(c0, c1, a.cnt + rep * a.cnt_stride + 2 + 2 * ((size_t)axis * a.r_max + ridx));
 }
 
 // ---- row-blocked kernels (the production measurement path) ----------------------------------
@@ -195,8 +199,8 @@ struct MeasBlkArgs {
     unsigned long long *cnt;         // same layout as MeasArgs::cnt
 };
 
-template <int MODEL>
-__device__ __forceinline__ const uint32_t *blk_plane(const MeasBlkArgs &a, uint32_t colour, uint32_t plane)
+template <int MODEL, class Args>
+__device__ __forceinline__ const uint32_t *blk_plane(const Args &a, uint32_t colour, uint32_t plane)
 {
     const size_t pw = (size_t)a.L * a.wpr;
     return MODEL == 0 ? a.buf + (size_t)colour * pw : a.buf + (size_t)(2 * colour + plane) * pw;
@@ -415,6 +419,131 @@ __global__ void __launch_bounds__(128) measure_x_kernel(const MeasBlkArgs a)
     }
 }
 
+// ---- sparse lists of r (lattice_measure_list) --------------------------------------------------
+//
+// The paper samples C(r;t) sparsely in r.  Same thread layout and carry-save
+// reduction as the dense kernels, but the partner words of each listed r are loaded afresh: one
+// partner read per (word, r, axis) instead of a sliding window.  blockIdx.y selects a chunk of
+// MEAS_LIST_CHUNK list entries; counters as in the dense kernels with r - 1 replaced by the index
+// in the list and r_max by its length n_r.
+constexpr int MEAS_LIST_CHUNK = 32;
+
+struct MeasListArgs {
+    const uint32_t *buf;
+    uint32_t L, wpr;                 // rows per plane, words per row
+    uint32_t i0, n;                  // first base row, number of 16-row blocks
+    const uint32_t *rlist;           // device, n_r entries, each in [1, L/2]
+    uint32_t n_r;
+    uint32_t mq;                     // also count M, Q (chunk 0)
+    unsigned long long *cnt;
+};
+
+// Both axes in one kernel: thread = (colour c, 16-row block, word column k) keeps its 16 base words
+// (one per row) in registers; for every listed r it loads, coalesced along k,
+//   y axis: the 16 words of rows i + r at the same k (colour c if r is even, else 1 - c),
+//   x axis: per row the two words k + (s >> 5), + 1 of the partner colour, funnel-shifted by
+//           s & 31, with s = r/2 (+ the row's parity (i + c) & 1 for odd r).
+template <int MODEL>
+__global__ void __launch_bounds__(128) measure_list_kernel(const MeasListArgs a)
+{
+    __shared__ unsigned int s_cnt[2][MEAS_LIST_CHUNK][2];          // [axis][entry][count]
+    __shared__ unsigned long long s_mq[2];
+    for (uint32_t t = threadIdx.x; t < 2 * MEAS_LIST_CHUNK * 2; t += blockDim.x) (&s_cnt[0][0][0])[t] = 0;
+    if (threadIdx.x < 2) s_mq[threadIdx.x] = 0;
+    __syncthreads();
+    const uint32_t q0 = blockIdx.y * MEAS_LIST_CHUNK;
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t per_colour = a.n * a.wpr;
+    const bool live = g < 2u * per_colour;
+    const uint32_t mask = __ballot_sync(0xffffffffu, live);
+    const uint32_t lane = threadIdx.x & 31u;
+    if (live) {
+        const uint32_t leader = __ffs(mask) - 1;
+        const uint32_t c = g >= per_colour ? 1u : 0u;
+        const uint32_t rem = g - c * per_colour;
+        const uint32_t rb = rem / a.wpr, k = rem - rb * a.wpr;
+        const uint32_t ib0 = a.i0 + MEAS_NB * rb;
+        const uint32_t par0 = (ib0 + c) & 1u;                         // (i + c) & 1 of the block's first row
+        const uint32_t *bp0 = blk_plane<MODEL>(a, c, 0), *bp1 = blk_plane<MODEL>(a, c, 1);
+        const uint32_t *op0 = blk_plane<MODEL>(a, c ^ 1u, 0), *op1 = blk_plane<MODEL>(a, c ^ 1u, 1);
+        const unsigned long long plane_words = (unsigned long long)a.L * a.wpr;
+        const unsigned long long ob = (unsigned long long)ib0 * a.wpr;
+        uint32_t B0[MEAS_NB], B1[MEAS_NB];
+#pragma unroll
+        for (int j = 0; j < MEAS_NB; ++j) {
+            B0[j] = bp0[ob + (unsigned long long)j * a.wpr + k];
+            B1[j] = MODEL ? bp1[ob + (unsigned long long)j * a.wpr + k] : 0u;
+        }
+        if (blockIdx.y == 0 && a.mq) {
+            uint32_t m0 = 0, m1 = 0;
+#pragma unroll
+            for (int j = 0; j < MEAS_NB; ++j) {
+                if (MODEL == 0) m0 += __popc(B0[j]);
+                else { m0 += __popc(B0[j] & ~B1[j]); m1 += __popc(B0[j] & B1[j]); }
+            }
+            const uint32_t v0 = __reduce_add_sync(mask, m0);
+            const uint32_t v1 = MODEL ? __reduce_add_sync(mask, m1) : 0u;
+            if (lane == leader) {
+                atomicAdd(&s_mq[0], (unsigned long long)v0);
+                if (MODEL) atomicAdd(&s_mq[1], (unsigned long long)v1);
+            }
+        }
+        const uint32_t q1 = min(q0 + (uint32_t)MEAS_LIST_CHUNK, a.n_r);
+        for (uint32_t q = q0; q < q1; ++q) {
+            const uint32_t r = a.rlist[q];
+            const uint32_t *p0 = (r & 1u) ? op0 : bp0, *p1 = (r & 1u) ? op1 : bp1;
+            uint32_t X[MEAS_NB], Y[MEAS_NB];
+            {   // y axis
+                uint32_t row = ib0 + r;                                // < 2 L
+                if (row >= a.L) row -= a.L;
+                unsigned long long o = (unsigned long long)row * a.wpr + k;
+#pragma unroll
+                for (int j = 0; j < MEAS_NB; ++j) {
+                    const uint32_t w0 = p0[o];
+                    if (MODEL == 0) X[j] = B0[j] ^ w0;
+                    else { X[j] = B0[j] & w0; Y[j] = X[j] & (B1[j] ^ p1[o]); }
+                    o += a.wpr; if (o >= plane_words) o -= plane_words;
+                }
+                const uint32_t c0 = weighted_popc16(X);
+                const uint32_t c1 = MODEL ? weighted_popc16(Y) : 0u;
+                add_r(s_cnt[1], q - q0, mask, leader, lane, c0, c1, MODEL != 0);
+            }
+            {   // x axis: rows j and j+1 have parities par0 and par0 ^ 1
+                const uint32_t sA = (r >> 1) + ((r & 1u) ? par0 : 0u), sB = (r >> 1) + ((r & 1u) ? (par0 ^ 1u) : 0u);
+                uint32_t kA = k + (sA >> 5), kB = k + (sB >> 5);     // s >> 5 <= wpr / 2
+                if (kA >= a.wpr) kA -= a.wpr;
+                if (kB >= a.wpr) kB -= a.wpr;
+                const uint32_t kA1 = (kA + 1 == a.wpr) ? 0 : kA + 1, kB1 = (kB + 1 == a.wpr) ? 0 : kB + 1;
+                const uint32_t bA = sA & 31u, bB = sB & 31u;
+                unsigned long long o = ob;
+#pragma unroll
+                for (int j = 0; j < MEAS_NB; ++j) {
+                    const uint32_t ka = (j & 1) ? kB : kA, ka1 = (j & 1) ? kB1 : kA1, bs = (j & 1) ? bB : bA;
+                    const uint32_t w0 = __funnelshift_r(p0[o + ka], p0[o + ka1], bs);
+                    if (MODEL == 0) X[j] = B0[j] ^ w0;
+                    else {
+                        const uint32_t w1 = __funnelshift_r(p1[o + ka], p1[o + ka1], bs);
+                        X[j] = B0[j] & w0; Y[j] = X[j] & (B1[j] ^ w1);
+                    }
+                    o += a.wpr;
+                }
+                const uint32_t c0 = weighted_popc16(X);
+                const uint32_t c1 = MODEL ? weighted_popc16(Y) : 0u;
+                add_r(s_cnt[0], q - q0, mask, leader, lane, c0, c1, MODEL != 0);
+            }
+        }
+    }
+    __syncthreads();
+    for (uint32_t t = threadIdx.x; t < 2 * MEAS_LIST_CHUNK * 2; t += blockDim.x) {
+        const uint32_t axis = t / (MEAS_LIST_CHUNK * 2), e = t % (MEAS_LIST_CHUNK * 2);
+        const uint32_t q = q0 + (e >> 1);
+        const unsigned int v = (&s_cnt[0][0][0])[t];
+        if (q < a.n_r && v)
+            atomicAdd(a.cnt + 2 + 2 * ((size_t)axis * a.n_r + q) + (e & 1u), (unsigned long long)v);
+    }
+    if (threadIdx.x < 2 && s_mq[threadIdx.x]) atomicAdd(a.cnt + threadIdx.x, s_mq[threadIdx.x]);
+}
+
 // ---- r_max == 1: M, Q and the nearest-neighbour sums (the energy) in one pass ---------------
 //
 // The per-step record of a run (e, m, q) needs only r = 1.  One thread owns one 128-bit run of
@@ -438,26 +567,109 @@ template <int MODEL>
 struct E1Row {                       // one 128-bit run of both colours (+ planes) of one row
     uint32_t a0[4], a1[4];           // colour 0: spins (Ising) or nz, sg (BC)
     uint32_t b0[4], b1[4];           // colour 1
+    uint32_t e0, e1;                 // the word after the run of the colour whose bits pair shifted
 };
 
-template <int MODEL>
-__device__ __forceinline__ void e1_load(const MeasE1Args &a, unsigned long long off, E1Row<MODEL> &r)
+// Row `row` (local index; == a.rows wraps to 0) of run kw; ODD = parity of the GLOBAL row: the colour
+// c with (i + c) odd pairs along x with colour 1-c shifted down by one bit, i.e. it needs the word
+// after the run (kn) of colour ODD.
+template <int MODEL, int ODD>
+__device__ __forceinline__ void e1_load(const MeasE1Args &a, uint32_t row, uint32_t kw, uint32_t kn, E1Row<MODEL> &r)
 {
     const size_t pw = (size_t)a.rows * a.wpr;
-    const uint4 x = *reinterpret_cast<const uint4 *>(a.buf + off);
+    const unsigned long long ro = (row == a.rows) ? 0ull : (unsigned long long)row * a.wpr;
+    const uint32_t *p = a.buf + ro + kw;
+    const uint4 x = *reinterpret_cast<const uint4 *>(p);
     r.a0[0] = x.x; r.a0[1] = x.y; r.a0[2] = x.z; r.a0[3] = x.w;
     if (MODEL == 0) {
-        const uint4 y = *reinterpret_cast<const uint4 *>(a.buf + pw + off);
+        const uint4 y = *reinterpret_cast<const uint4 *>(p + pw);
         r.b0[0] = y.x; r.b0[1] = y.y; r.b0[2] = y.z; r.b0[3] = y.w;
 #pragma unroll
         for (int w = 0; w < 4; ++w) { r.a1[w] = 0; r.b1[w] = 0; }
+        r.e0 = a.buf[(size_t)ODD * pw + ro + kn];
+        r.e1 = 0;
     } else {
-        const uint4 xs = *reinterpret_cast<const uint4 *>(a.buf + pw + off);
-        const uint4 y = *reinterpret_cast<const uint4 *>(a.buf + 2 * pw + off);
-        const uint4 ys = *reinterpret_cast<const uint4 *>(a.buf + 3 * pw + off);
+        const uint4 xs = *reinterpret_cast<const uint4 *>(p + pw);
+        const uint4 y = *reinterpret_cast<const uint4 *>(p + 2 * pw);
+        const uint4 ys = *reinterpret_cast<const uint4 *>(p + 3 * pw);
         r.a1[0] = xs.x; r.a1[1] = xs.y; r.a1[2] = xs.z; r.a1[3] = xs.w;
         r.b0[0] = y.x; r.b0[1] = y.y; r.b0[2] = y.z; r.b0[3] = y.w;
         r.b1[0] = ys.x; r.b1[1] = ys.y; r.b1[2] = ys.z; r.b1[3] = ys.w;
+        r.e0 = a.buf[(size_t)(2 * ODD) * pw + ro + kn];
+        r.e1 = a.buf[(size_t)(2 * ODD + 1) * pw + ro + kn];
+    }
+}
+
+// The 8 words per tree that base row `cur` (global parity ODD) contributes, at tree slots o..o+7:
+// XM / XN: +1 / -1 sites; XX (XXo): x-axis pairs (and those of opposite sign); XY (XYo): y axis.
+template <int MODEL, int ODD>
+__device__ __forceinline__ void e1_row(const E1Row<MODEL> &cur, const E1Row<MODEL> &nxt, int o, uint32_t (&XM)[16],
+                                       uint32_t (&XN)[16], uint32_t (&XX)[16], uint32_t (&XXo)[16], uint32_t (&XY)[16],
+                                       uint32_t (&XYo)[16])
+{
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        // partner-colour words shifted by one bit: colour ODD is the shifted partner of colour 1-ODD
+        const uint32_t p0lo = ODD ? cur.b0[w] : cur.a0[w];
+        const uint32_t p0hi = w < 3 ? (ODD ? cur.b0[w < 3 ? w + 1 : 0] : cur.a0[w < 3 ? w + 1 : 0]) : cur.e0;
+        const uint32_t sh0 = __funnelshift_r(p0lo, p0hi, 1);
+        const uint32_t t0 = ODD ? cur.a0[w] : cur.b0[w];              // the shifted pairing's base colour
+        if (MODEL == 0) {
+            XM[o + w] = cur.a0[w]; XM[o + w + 4] = cur.b0[w];
+            XX[o + w] = cur.a0[w] ^ cur.b0[w];                        // in-place pairing
+            XX[o + w + 4] = t0 ^ sh0;
+            XY[o + w] = cur.a0[w] ^ nxt.b0[w];
+            XY[o + w + 4] = cur.b0[w] ^ nxt.a0[w];
+        } else {
+            const uint32_t p1lo = ODD ? cur.b1[w] : cur.a1[w];
+            const uint32_t p1hi = w < 3 ? (ODD ? cur.b1[w < 3 ? w + 1 : 0] : cur.a1[w < 3 ? w + 1 : 0]) : cur.e1;
+            const uint32_t sh1 = __funnelshift_r(p1lo, p1hi, 1);
+            const uint32_t t1 = ODD ? cur.a1[w] : cur.b1[w];
+            XM[o + w] = cur.a0[w] & ~cur.a1[w]; XM[o + w + 4] = cur.b0[w] & ~cur.b1[w];
+            XN[o + w] = cur.a0[w] & cur.a1[w]; XN[o + w + 4] = cur.b0[w] & cur.b1[w];
+            XX[o + w] = cur.a0[w] & cur.b0[w];
+            XXo[o + w] = XX[o + w] & (cur.a1[w] ^ cur.b1[w]);
+            XX[o + w + 4] = t0 & sh0;
+            XXo[o + w + 4] = XX[o + w + 4] & (t1 ^ sh1);
+            XY[o + w] = cur.a0[w] & nxt.b0[w];
+            XYo[o + w] = XY[o + w] & (cur.a1[w] ^ nxt.b1[w]);
+            XY[o + w + 4] = cur.b0[w] & nxt.a0[w];
+            XYo[o + w + 4] = XY[o + w + 4] & (cur.b1[w] ^ nxt.a1[w]);
+        }
+    }
+}
+
+// The march of one thread over base rows ia .. ia+nr-1 (local indices), two rows per step, with the
+// two rows of the NEXT step already in flight while the current pair is reduced (the kernel is
+// bound by HBM latency x bytes in flight, not by arithmetic).  P0 = global parity of row ia.
+template <int MODEL, int P0>
+__device__ __forceinline__ void e1_march(const MeasE1Args &a, uint32_t kw, uint32_t kn, uint32_t ia, uint32_t nr,
+                                         uint32_t (&acc)[6])
+{
+    E1Row<MODEL> r0, r1, r2, r3, r4;                 // rows ia+rr .. ia+rr+4 of the current step
+    e1_load<MODEL, P0>(a, ia, kw, kn, r0);
+    e1_load<MODEL, P0 ^ 1>(a, ia + 1, kw, kn, r1);   // nr >= 1: row ia+1 is at least a partner row
+    if (nr >= 2) e1_load<MODEL, P0>(a, ia + 2, kw, kn, r2);
+    for (uint32_t rr = 0; rr < nr; rr += 2) {
+        if (rr + 3 <= nr) e1_load<MODEL, P0 ^ 1>(a, ia + rr + 3, kw, kn, r3);
+        if (rr + 4 <= nr) e1_load<MODEL, P0>(a, ia + rr + 4, kw, kn, r4);
+        uint32_t XM[16], XN[16], XX[16], XXo[16], XY[16], XYo[16];
+        e1_row<MODEL, P0>(r0, r1, 0, XM, XN, XX, XXo, XY, XYo);
+        if (rr + 1 < nr) {
+            e1_row<MODEL, P0 ^ 1>(r1, r2, 8, XM, XN, XX, XXo, XY, XYo);
+        } else {
+#pragma unroll
+            for (int o = 8; o < 16; ++o) { XM[o] = XN[o] = XX[o] = XXo[o] = XY[o] = XYo[o] = 0; }
+        }
+        acc[0] += weighted_popc16(XM);
+        acc[2] += weighted_popc16(XX);
+        acc[4] += weighted_popc16(XY);
+        if (MODEL) {
+            acc[1] += weighted_popc16(XN);
+            acc[3] += weighted_popc16(XXo);
+            acc[5] += weighted_popc16(XYo);
+        }
+        r0 = r2; r1 = r3; r2 = r4;
     }
 }
 
@@ -474,73 +686,8 @@ __global__ void __launch_bounds__(128) measure_e1_kernel(const MeasE1Args a)
         const uint32_t kn = (kw + 4 == a.wpr) ? 0 : kw + 4;       // word after the run (periodic)
         const uint32_t ia = a.i0 + sl * MEAS_E1_ROWS;
         const uint32_t nr = min((uint32_t)MEAS_E1_ROWS, a.i0 + a.n_rows - ia);
-        const size_t pw = (size_t)a.rows * a.wpr;
-        unsigned long long ro = (unsigned long long)ia * a.wpr;
-        E1Row<MODEL> cur, nxt;
-        e1_load<MODEL>(a, ro + kw, cur);
-        for (uint32_t rr = 0; rr < nr; rr += 2) {
-            uint32_t XM[16], XN[16], XX[16], XXo[16], XY[16], XYo[16];
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                if (rr + h < nr) {
-                    const uint32_t i = ia + rr + h;
-                    const unsigned long long rd = (i + 1 == a.rows) ? 0ull : ro + a.wpr;
-                    e1_load<MODEL>(a, rd + kw, nxt);
-                    // x axis: colour (i&1) pairs in place; the other colour sees its partner
-                    // colour shifted down by one bit (partner at p+1)
-                    const uint32_t odd = (i + a.par_off) & 1u;      // parity of the global row
-                    // colour whose partner is shifted: c with (i+c)&1 == 1, i.e. c = 1 - odd;
-                    // its partner colour is `odd`: side word of colour `odd` (planes 0, 1)
-                    const uint32_t *sp = a.buf + (MODEL == 0 ? (size_t)odd * pw : (size_t)(2 * odd) * pw) + ro + kn;
-                    const uint32_t e0 = sp[0];
-                    const uint32_t e1 = MODEL ? sp[pw] : 0u;
-#pragma unroll
-                    for (int w = 0; w < 4; ++w) {
-                        const int o = 8 * h + w;
-                        // partner-colour words shifted by one bit
-                        const uint32_t p0lo = odd ? cur.b0[w] : cur.a0[w];
-                        const uint32_t p0hi = w < 3 ? (odd ? cur.b0[w < 3 ? w + 1 : 0] : cur.a0[w < 3 ? w + 1 : 0]) : e0;
-                        const uint32_t sh0 = __funnelshift_r(p0lo, p0hi, 1);
-                        const uint32_t t0 = odd ? cur.a0[w] : cur.b0[w];      // the shifted pairing's base colour
-                        if (MODEL == 0) {
-                            XM[o] = cur.a0[w]; XM[o + 4] = cur.b0[w];
-                            XX[o] = cur.a0[w] ^ cur.b0[w];                    // in-place pairing
-                            XX[o + 4] = t0 ^ sh0;
-                            XY[o] = cur.a0[w] ^ nxt.b0[w];
-                            XY[o + 4] = cur.b0[w] ^ nxt.a0[w];
-                        } else {
-                            const uint32_t p1lo = odd ? cur.b1[w] : cur.a1[w];
-                            const uint32_t p1hi = w < 3 ? (odd ? cur.b1[w < 3 ? w + 1 : 0] : cur.a1[w < 3 ? w + 1 : 0]) : e1;
-                            const uint32_t sh1 = __funnelshift_r(p1lo, p1hi, 1);
-                            const uint32_t t1 = odd ? cur.a1[w] : cur.b1[w];
-                            XM[o] = cur.a0[w] & ~cur.a1[w]; XM[o + 4] = cur.b0[w] & ~cur.b1[w];
-                            XN[o] = cur.a0[w] & cur.a1[w]; XN[o + 4] = cur.b0[w] & cur.b1[w];
-                            XX[o] = cur.a0[w] & cur.b0[w];
-                            XXo[o] = XX[o] & (cur.a1[w] ^ cur.b1[w]);
-                            XX[o + 4] = t0 & sh0;
-                            XXo[o + 4] = XX[o + 4] & (t1 ^ sh1);
-                            XY[o] = cur.a0[w] & nxt.b0[w];
-                            XYo[o] = XY[o] & (cur.a1[w] ^ nxt.b1[w]);
-                            XY[o + 4] = cur.b0[w] & nxt.a0[w];
-                            XYo[o + 4] = XY[o + 4] & (cur.b1[w] ^ nxt.a1[w]);
-                        }
-                    }
-                    cur = nxt;
-                    ro = rd;
-                } else {
-#pragma unroll
-                    for (int o = 8; o < 16; ++o) { XM[o] = XN[o] = XX[o] = XXo[o] = XY[o] = XYo[o] = 0; }
-                }
-            }
-            acc[0] += weighted_popc16(XM);
-            acc[2] += weighted_popc16(XX);
-            acc[4] += weighted_popc16(XY);
-            if (MODEL) {
-                acc[1] += weighted_popc16(XN);
-                acc[3] += weighted_popc16(XXo);
-                acc[5] += weighted_popc16(XYo);
-            }
-        }
+        if ((ia + a.par_off) & 1u) e1_march<MODEL, 1>(a, kw, kn, ia, nr, acc);
+        else e1_march<MODEL, 0>(a, kw, kn, ia, nr, acc);
     }
     __shared__ unsigned long long sh[6];
     if (threadIdx.x < 6) sh[threadIdx.x] = 0;

@@ -81,21 +81,31 @@ def run(w: workloads.Workload, sweeps: int | None = None, r_max: int | None = No
 
 
 def replica_correlations(w: workloads.Workload, n_runs: int, sweeps: int, r_max: int, L: int | None = None,
-                         device: str = "cuda:0"):
+                         device: str = "cuda:0", batch: int | None = None):
     """n_runs independent realisations of workload w (seeds w.seed + 7919 k): returns
     (times[T], C[T][run, r] for r = 0..r_max, e[T][run]) at the record times 2^k <= sweeps --
-    the input of the estimator layer (analysis.py)."""
+    the input of the estimator layer (analysis.py).  The realisations run as batches of replicas
+    (lattice_create_batch): `batch` per handle, by default as many as fit in 1/4 of the free
+    device memory, so that small lattices fill the GPU."""
+    import torch
     from . import analysis
+    L = L or w.L
     times = [t for t in w.measure_times(sweeps) if t > 0]
     C = [np.zeros((n_runs, r_max + 1)) for _ in times]
     e = [np.zeros(n_runs) for _ in times]
-    for k in range(n_runs):
-        g = lat.Lattice(L or w.L, w.model, w.delta, w.seed + 7919 * k, device=device)
+    if batch is None:
+        free, _ = torch.cuda.mem_get_info(torch.device(device))
+        batch = max(1, min(n_runs, (free // 4) // lat.state_bytes(L, w.model)))
+    for k0 in range(0, n_runs, batch):
+        nb = min(batch, n_runs - k0)
+        seeds = np.array([w.seed + 7919 * (k0 + k) for k in range(nb)], dtype=np.uint64)
+        g = lat.LatticeBatch(L, seeds, w.model, w.delta, device=device)
         for a, t in enumerate(times):
             g.sweep(w.beta_schedule(t - g.time, g.time))
             M, Q, Sx, Sy = g.measure(r_max)
-            C[a][k] = analysis.correlation(Sx, Sy, g.L, Q)
-            e[a][k] = lat.energy(Sx, Sy, Q, w.delta, g.L)
+            for k in range(nb):
+                C[a][k0 + k] = analysis.correlation(Sx[k], Sy[k], L, Q[k])
+                e[a][k0 + k] = lat.energy(Sx[k], Sy[k], Q[k], w.delta, L)
         g.close()
     return np.array(times, dtype=np.float64), C, e
 

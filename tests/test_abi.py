@@ -177,3 +177,17 @@ def test_thresholds64_equal_oracle(model, delta):
         tg, ag = lat.thresholds64(model, delta, beta)
         to, ao = oracle.thresholds64(model, delta, beta)
         assert np.array_equal(tg, to) and np.array_equal(ag, ao), beta
+
+
+def test_plane_case_specialisations_match_the_config_betas():
+    """The hard-coded plane-case constants of ising_march.cuh are the ones the thresholds of the
+    workloads' betas give (host-only: the library derives the cases from lattice_thresholds)."""
+    f = lat.lib().lattice_plane_case_specialised
+    for name in ("ising_L64", "ising_L4096", "ising_L2p20"):
+        w = workloads.CONFIGS[name]
+        assert f(w.model, w.delta, float(w.beta_schedule(1)[0])) == 1, name
+    w = workloads.CONFIGS["ising_L2p16_twostep"]
+    assert f(w.model, 0.0, w.beta_1) == 1 and f(w.model, 0.0, w.beta_f) == 1
+    w = workloads.CONFIGS["ising_L2p16_ramp"]
+    assert f(w.model, 0.0, w.beta_f) == 1                       # the plateau after the ramp
+    assert f(lat.ISING, 0.0, 0.2) == 0 and f(lat.BLUME_CAPEL, 0.0, workloads.BETA_BC) == 0

@@ -96,6 +96,11 @@ def _check_slab(g, w, i0, n, r_max):
     for r in rs:
         assert Sx[r - 1] == Sxo[r], ("Sx", r)
         assert Sy[r - 1] == Syo[r], ("Sy", r)
+    # the sparse-list call on the same slab: the same separations, handed over unsorted
+    rl = rs[::-1]
+    Ml, Ql, Sxl, Syl = g.measure_list(rl, (i0, n))
+    assert (Ml, Ql) == (Mo, Qo)
+    assert Sxl.tolist() == [Sxo[r] for r in rl] and Syl.tolist() == [Syo[r] for r in rl]
 
 
 @pytest.mark.parametrize("name,t_late,r_slab", [("ising_L2p20", 0, 4096), ("ising_L2p16_ramp", 990, 1024),
@@ -120,6 +125,8 @@ def test_full_size_windowed_replay_and_slab_measurements(name, t_late, r_slab):
     if t_late > g.time:                          # later in the run (domains have formed; for the
         g.sweep(w.beta_schedule(t_late - g.time, g.time))   # ramp: the thresholds change per sweep)
     _replay(g, w, g.time, 3)
+    if name == "ising_L2p20":                    # constant beta_c: the plane-case specialised kernel ran
+        assert g.specialised_launches == 2 * 6
     # a sweep counter with the high bit set keys correctly too
     g.set_time(3_000_000_000)
     _replay(g, w, 3_000_000_000, 2)

@@ -109,6 +109,46 @@ def test_half_sweeps_and_extreme_temperatures(model, scheme):
         assert np.array_equal(g.get_spins(), o.get_spins()), beta
 
 
+def test_plane_case_specialised_kernels_are_bit_identical():
+    """Launch-time specialisation (compile-time LOP3 truth tables for the betas the workloads run at):
+    the specialised instantiations run -- the launch-kind counter says so -- and give the oracle's
+    trajectory; a beta without an instantiation takes the generic brx.idx kernel in between."""
+    L = 4608                                          # large enough for the marching kernel (not one row per thread)
+    specials = [BETA_C, 1.0 / 1.66, 1.0 / 2.27414861561203, BETA_C / 1.01]
+    for b in specials:
+        assert lat.lib().lattice_plane_case_specialised(lat.ISING, 0.0, b) == 1
+    assert lat.lib().lattice_plane_case_specialised(lat.ISING, 0.0, 0.3) == 0
+    assert lat.lib().lattice_plane_case_specialised(lat.ISING, 0.0, 0.35) == 0
+    assert lat.lib().lattice_plane_case_specialised(lat.ISING, 0.0, 0.0) == 0
+    g = lat.Lattice(L, lat.ISING, 0.0, 60606)
+    o = oracle.OracleLattice(L, lat.ISING, 0.0, 60606)
+    sched = [BETA_C, BETA_C, 0.3, 1.0 / 1.66, 1.0 / 1.66, 0.0, 1.0 / 2.27414861561203, BETA_C / 1.01, 0.35, BETA_C]
+    for b in sched:                                   # one sweep per call: two plain launches each
+        g.sweep([b])
+    o.sweep(sched)
+    assert g.specialised_launches == 2 * sum(1 for b in sched if b in specials)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    # from the all-up state: every lane needs a decision, ties are most frequent
+    g.fill(1)
+    o.set_spins(np.ones((L, L), dtype=np.int8))
+    for b in (BETA_C, 1.0 / 1.66, 1.0 / 2.27414861561203):
+        g.sweep([b]); o.sweep([b])
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    g.close(); o.close()
+    # the batched marching kernel has the same instantiations
+    seeds = np.array([1, 2, 3, 4], dtype=np.uint64)
+    bt = lat.LatticeBatch(L, seeds)
+    for b in (BETA_C, 0.3, BETA_C / 1.01):
+        bt.sweep([b])
+    for k in (0, 3):
+        o = oracle.OracleLattice(L, lat.ISING, 0.0, int(seeds[k]))
+        o.sweep([BETA_C, 0.3, BETA_C / 1.01])
+        assert np.array_equal(bt.get_spins(k), o.get_spins())
+        o.close()
+    assert int(lat.lib().lattice_specialised_launches(bt._h)) == 4
+    bt.close()
+
+
 def test_ising_infinite_temperature_flips_every_spin():
     g = lat.Lattice(512, lat.ISING, 0.0, 3)
     s0 = g.get_spins()
@@ -231,6 +271,41 @@ def test_measure_blocked_kernels_all_r_and_ragged_slabs(L, r_max, model):
     _same_measure(g, o, r_max, L)
     for i0, n in ((0, 16), (3, 45), (L - 33, 33), (500, 7)):
         _same_measure(g, o, min(r_max, 70), L, rows=(i0, n))
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+@pytest.mark.parametrize("L", [64, 192, 1024, 1536, 2048])
+def test_measure_list_sparse_r(L, model):
+    """lattice_measure_list (the paper's sparse sampling in r): every listed r equals
+    the oracle's dense count at that r -- log-spaced lists, unsorted lists with repeats, r = 1 and
+    r = L/2, whole lattice and ragged row ranges (list kernels + generic remainder)."""
+    g = lat.Lattice(L, model, 0.0, 4321 + L)
+    o = oracle.OracleLattice(L, model, 0.0, 4321 + L)
+    beta = BETA_C if model == lat.ISING else workloads.BETA_BC
+    g.sweep([beta] * 12)
+    o.sweep([beta] * 12)
+    half = L // 2
+    Mo, Qo, Sxo, Syo = o.measure(half)
+    lists = [sorted({max(1, int(round(half ** (k / 40)))) for k in range(41)}),
+             [half, 1, 2, 1, half - 1, 33, 33, 17][: 8 if half > 33 else 5],
+             [3], list(range(1, min(half, 70) + 1))]
+    for rl in lists:
+        rl = [r for r in rl if 1 <= r <= half]
+        M, Q, Sx, Sy = g.measure_list(rl)
+        assert (M, Q) == (Mo, Qo)
+        assert Sx.tolist() == [int(Sxo[r - 1]) for r in rl], rl
+        assert Sy.tolist() == [int(Syo[r - 1]) for r in rl], rl
+    for i0, n in ((0, 16), (3, 45), (L - 33, 33), (L // 2, 7), (1, 1)):
+        rl = [1, 2, 5, half // 2, half]
+        Ms, Qs, Sxs, Sys = o.measure(half, (i0, n))
+        M, Q, Sx, Sy = g.measure_list(rl, (i0, n))
+        assert (M, Q) == (Ms, Qs)
+        assert Sx.tolist() == [int(Sxs[r - 1]) for r in rl] and Sy.tolist() == [int(Sys[r - 1]) for r in rl]
+    with pytest.raises(lat.LatticeError):
+        g.measure_list([0])
+    with pytest.raises(lat.LatticeError):
+        g.measure_list([half + 1])
+    g.close(); o.close()
 
 
 @pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
