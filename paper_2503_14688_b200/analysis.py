@@ -200,3 +200,195 @@ def fit_z_jackknife(t, C_runs_by_time, omega: float = OMEGA, t_min: float = 0.0)
     full["z_err"] = float(np.sqrt((n - 1) / n * np.sum((zs - zs.mean()) ** 2)))
     full["xi"], full["xi_err"] = xi_full, xi_err
     return full
+
+
+# ---- sparse r-grids: cubic-spline interpolation of C(r) ---------------------------
+def densify(r, C, C_err=None):
+    """C sampled at the sorted separations r (r[0] may be 0) -> (C_dense, err_dense) on r = 0..r[-1].
+
+    The paper measures C(r;t) on a sparse grid of r and integrates with cubic splines (PAPER.md:207,
+    ref. [62]); `lattice_measure_list` returns exactly such samples.  The spline goes through
+    (0, C(0) = 1 or the given value) and the samples; errors are interpolated linearly."""
+    from scipy.interpolate import CubicSpline
+    r = np.asarray(r, np.float64)
+    C = np.asarray(C, np.float64)
+    if r[0] != 0.0:
+        r = np.concatenate([[0.0], r])
+        C = np.concatenate([[1.0], C])
+        if C_err is not None:
+            C_err = np.concatenate([[0.0], np.asarray(C_err, np.float64)])
+    if np.any(np.diff(r) <= 0):
+        raise ValueError("r must be strictly increasing")
+    grid = np.arange(int(r[-1]) + 1, dtype=np.float64)
+    dense = CubicSpline(r, C)(grid)
+    err = None if C_err is None else np.interp(grid, r, np.asarray(C_err, np.float64))
+    return dense, err
+
+
+def xi_sparse(r, C, C_err, details: dict | None = None, **kw) -> float:
+    """xi = I_2 / I_1 (App. C) from C(r) on a sparse r-grid: spline to the integers, then xi_appendix_c."""
+    dense, err = densify(r, C, C_err)
+    return xi_appendix_c(dense, err, details, **kw)
+
+
+# ---- z from the energy, Eq. (6) / (D2), and the joint fit of Fig. 3 ------------------------------
+E_EQ_ISING = -np.sqrt(2.0)     # Onsager: E_eq(T_c) = -sqrt 2 (PAPER.md:81)
+NU_ISING = 1.0                 # D - 1/nu = 1 in two dimensions (PAPER.md:58)
+
+
+def _energy_design(t, z, omega, nu):
+    """columns t^(-1/z), t^(-2/z), t^(-(omega + 1/nu)/z) of Eq. (6)."""
+    lt = np.log(t)
+    return np.stack([np.exp(-lt / z), np.exp(-2.0 * lt / z), np.exp(-(omega + 1.0 / nu) * lt / z)], axis=1)
+
+
+def _wlsq(X, y, sigma):
+    W = 1.0 / sigma
+    p, *_ = np.linalg.lstsq(X * W[:, None], y * W, rcond=None)
+    return p, float(np.sum(((X @ p - y) * W) ** 2))
+
+
+def _minimise_over_z(chi2_of_z, bracket=(1.2, 4.0)):
+    """The fits are linear in everything but z: minimise the profiled chi^2(z) in one dimension."""
+    from scipy.optimize import minimize_scalar
+    zs = np.linspace(bracket[0], bracket[1], 57)
+    vals = np.array([chi2_of_z(z) for z in zs])
+    k = int(np.argmin(vals))
+    lo, hi = zs[max(k - 1, 0)], zs[min(k + 1, zs.size - 1)]
+    res = minimize_scalar(chi2_of_z, bounds=(lo, hi), method="bounded", options={"xatol": 1e-12})
+    return float(res.x)
+
+
+def fit_z_energy(t, E, E_err, E_eq: float = E_EQ_ISING, omega: float = OMEGA, nu: float = NU_ISING,
+                 t_min: float = 0.0) -> dict:
+    """z from the local observable: E(t) - E_eq = b t^(-1/z) + b' t^(-2/z) + b'' t^(-(omega+1/nu)/z)
+    (Eq. 6 / D2) on the points with t >= t_min.  Only meaningful where E_eq
+    is known exactly (Ising: -sqrt 2).  Returns z, b, b1, b2, chi2, dof, Q."""
+    from scipy.special import gammaincc
+    t, E, E_err = (np.asarray(a, np.float64) for a in (t, E, E_err))
+    keep = t >= t_min
+    if keep.sum() < 5:
+        raise ValueError("need at least 5 points for a 4-parameter fit")
+    tt, y, s = t[keep], E[keep] - E_eq, np.maximum(E_err[keep], 1e-300)
+
+    def chi2_of_z(z):
+        return _wlsq(_energy_design(tt, z, omega, nu), y, s)[1]
+
+    z = _minimise_over_z(chi2_of_z)
+    p, chi2 = _wlsq(_energy_design(tt, z, omega, nu), y, s)
+    dof = int(keep.sum()) - 4
+    return {"z": z, "b": float(p[0]), "b1": float(p[1]), "b2": float(p[2]), "chi2": chi2, "dof": dof,
+            "Q": float(gammaincc(dof / 2.0, chi2 / 2.0))}
+
+
+def fit_z_joint(datasets, omega: float = OMEGA, nu: float = NU_ISING, t_min: float = 0.0) -> dict:
+    """One z for several data sets (the main panel of Fig. 3; "a piecewise function
+    that depends on the respective data set").  Each data set is a dict
+      {"kind": "xi", "t": ..., "xi": ..., "xi_err": ...}               fitted with Eq. (5) / (D1)
+      {"kind": "E",  "t": ..., "E": ..., "E_err": ..., "E_eq": ...}    fitted with Eq. (6) / (D2)
+    with its own non-universal amplitudes (b, b' [, b'']); chi^2 is the sum over the sets, the weights
+    of the xi sets use the error of xi propagated through f'(xi), iterated."""
+    from scipy.special import gammaincc
+    sets = []
+    for d in datasets:
+        t = np.asarray(d["t"], np.float64)
+        keep = t >= t_min
+        if d["kind"] == "xi":
+            xi, xe = np.asarray(d["xi"], np.float64)[keep], np.asarray(d["xi_err"], np.float64)[keep]
+            sets.append({"kind": "xi", "logt": np.log(t[keep]), "xi": xi, "xe": xe, "sigma": np.maximum(xe / xi, 1e-300),
+                         "npar": 2})
+        elif d["kind"] == "E":
+            sets.append({"kind": "E", "t": t[keep], "y": np.asarray(d["E"], np.float64)[keep] - d.get("E_eq", E_EQ_ISING),
+                         "sigma": np.maximum(np.asarray(d["E_err"], np.float64)[keep], 1e-300), "npar": 3})
+        else:
+            raise ValueError("kind must be 'xi' or 'E'")
+    n_pts = sum(len(s["sigma"]) for s in sets)
+    n_par = 1 + sum(s["npar"] for s in sets)
+    if n_pts <= n_par:
+        raise ValueError("not enough points for the joint fit")
+
+    def solve(z):
+        total, pars = 0.0, []
+        for s in sets:
+            if s["kind"] == "xi":
+                X = np.stack([np.ones_like(s["xi"]), s["xi"] ** (-omega)], axis=1)
+                p, c2 = _wlsq(X, s["logt"] - z * np.log(s["xi"]), s["sigma"])
+            else:
+                p, c2 = _wlsq(_energy_design(s["t"], z, omega, nu), s["y"], s["sigma"])
+            total += c2
+            pars.append(p)
+        return total, pars
+
+    z = 2.0
+    for _ in range(20):
+        z = _minimise_over_z(lambda zz: solve(zz)[0])
+        chi2, pars = solve(z)
+        changed = False
+        for s, p in zip(sets, pars):
+            if s["kind"] != "xi":
+                continue
+            fprime = z / s["xi"] - omega * p[1] * s["xi"] ** (-omega - 1.0)
+            new = np.maximum(1e-40 + s["xe"] * np.abs(fprime), 1e-300)       # t_error = 1e-40 (PAPER.md:235)
+            changed = changed or not np.allclose(new, s["sigma"], rtol=1e-10)
+            s["sigma"] = new
+        if not changed:
+            break
+    chi2, pars = solve(z)
+    dof = n_pts - n_par
+    return {"z": z, "amplitudes": [p.tolist() for p in pars], "chi2": chi2, "dof": dof,
+            "Q": float(gammaincc(dof / 2.0, chi2 / 2.0))}
+
+
+def fit_z_energy_jackknife(t, E_runs_by_time, **kw) -> dict:
+    """E_runs_by_time[time][run] -> the Eq. (6) fit with jackknife errors over the runs (App. D)."""
+    t = np.asarray(t, np.float64)
+    stacks = np.array([np.asarray(e, np.float64) for e in E_runs_by_time])      # [time, run]
+    n = stacks.shape[1]
+    mean, err = stacks.mean(axis=1), stacks.std(axis=1, ddof=1) / np.sqrt(n)
+    full = fit_z_energy(t, mean, err, **kw)
+    zs = np.array([fit_z_energy(t, (stacks.sum(axis=1) - stacks[:, i]) / (n - 1), err, **kw)["z"] for i in range(n)])
+    full["z_err"] = float(np.sqrt((n - 1) / n * np.sum((zs - zs.mean()) ** 2)))
+    full["E"], full["E_err"] = mean, err
+    return full
+
+
+# ---- late approach to equilibrium in the two-step protocol, Eq. (8) --------------------------------
+def fit_exponential_approach(curves, E_eq: float | None = E_EQ_ISING, t_min: float = 0.0) -> dict:
+    """Joint fit of E(t; f) = E_eq + b(f) exp(-t / tau) over several protocols f with one f-independent
+    tau (Eq. 8, PAPER.md:104-108).  curves = [{"f": ..., "t": ..., "E": ..., "E_err": ...}, ...].
+    E_eq fixed (Ising: -sqrt 2) or, if None, an additional f-independent parameter (Blume-Capel).
+    Linear in b(f) (and E_eq) at fixed tau: the profiled chi^2 is minimised over tau alone."""
+    from scipy.optimize import minimize_scalar
+    from scipy.special import gammaincc
+    cs = []
+    for c in curves:
+        t = np.asarray(c["t"], np.float64)
+        keep = t >= t_min
+        cs.append((t[keep], np.asarray(c["E"], np.float64)[keep], np.maximum(np.asarray(c["E_err"], np.float64)[keep], 1e-300)))
+    nf = len(cs)
+    n_pts = sum(len(c[0]) for c in cs)
+
+    def solve(tau):
+        rows, ys, ss = [], [], []
+        for k, (t, E, s) in enumerate(cs):
+            X = np.zeros((t.size, nf + (1 if E_eq is None else 0)))
+            X[:, k] = np.exp(-t / tau)
+            if E_eq is None:
+                X[:, nf] = 1.0
+            rows.append(X); ys.append(E - (0.0 if E_eq is None else E_eq)); ss.append(s)
+        p, c2 = _wlsq(np.concatenate(rows), np.concatenate(ys), np.concatenate(ss))
+        return c2, p
+
+    t_all = np.concatenate([c[0] for c in cs])
+    span = float(t_all.max() - t_all.min()) or 1.0
+    taus = np.geomspace(span / 200.0, span * 20.0, 80)
+    vals = np.array([solve(x)[0] for x in taus])
+    k = int(np.argmin(vals))
+    res = minimize_scalar(lambda x: solve(x)[0], bounds=(taus[max(k - 1, 0)], taus[min(k + 1, taus.size - 1)]),
+                          method="bounded", options={"xatol": 1e-10 * span})
+    tau = float(res.x)
+    chi2, p = solve(tau)
+    dof = n_pts - (nf + 1 + (1 if E_eq is None else 0))
+    return {"tau": tau, "b": {float(c["f"]): float(p[k]) for k, c in enumerate(curves)},
+            "E_eq": float(p[nf]) if E_eq is None else float(E_eq), "chi2": chi2, "dof": dof,
+            "Q": float(gammaincc(max(dof, 1) / 2.0, chi2 / 2.0))}

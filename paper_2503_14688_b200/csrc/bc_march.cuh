@@ -42,6 +42,16 @@ struct BCMarchArgs {
     uint32_t lut_always;            // truth table of "threshold == 2^32" over (F, Y1, H0)
     unsigned long long thr[8];      // threshold of class (F<<2 | Y1<<1 | H0) on the 2^64 scale (scheme 1:
                                     // thr32 << 32); the low 56 bits are compared with the 56 tail bits
+    // general crystal field (GEN kernels; Delta != 0): per move type an 8-entry table indexed by
+    // idx = (hA << 2 | h1 << 1 | h0) of the lane's x + 4 (hA = h3 for flips, h2 otherwise; see
+    // bc_march_row_gen): truth tables of threshold bit (63-k) and of "always", thresholds for ties
+    // Table A serves the flips (idx 1..4) and the one of vacate / occupy whose x <= 0 entries are all
+    // "always" (idx 5, 6, 7, 0 for x = 1..4): vacate for Delta >= 0 (share_v = 1), occupy otherwise;
+    // table B serves the other type (all eight idx).
+    uint32_t lutA[8], lutB[8];
+    uint32_t lutA_always, lutB_always;
+    uint32_t share_v;
+    unsigned long long thrG[24];    // [type 0 flip, 1 vacate, 2 occupy][idx]
     uint32_t fbp;                   // folded counter word of the PROP plane
     PlaneFold F;                    // folded ACC_PLANE stream of (t, colour)
     RoundKeys K;
@@ -259,14 +269,207 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
     queue.push(eq, Fm, Y1, H0, nf, gg, wo, mir_tag);
 }
 
-template <int COLOUR, bool SLAB>
-__global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
+// ---- any crystal field Delta (|Delta| <= 4) -------------------------------------------------------
+//
+// For Delta != 0 vacate (dE = x - Delta) and occupy (dE = x + Delta) no longer share thresholds and
+// x <= 0 is no longer "always" for them (Eq. 1), so a deciding lane is in one of up
+// to 4 + 8 + 8 classes.  Per move type the threshold bit of plane k is still a function of three
+// bits of the bit-sliced x + 4 = (h3 h2 h1 h0):
+//   flip   : only x = 1..4 can need a decision; (h3, h1, h0) tells 5, 6, 7, 8 apart;
+//   vacate / occupy : x = -3..4 <-> (x + 4) & 7 = (h2, h1, h0), with x = 4 on index 0 -- legal when
+//            x = -4 is "always" for both (true for |Delta| <= 4; the host checks the table and
+//            falls back to the generic kernel otherwise).
+// With hA = flip ? h3 : h2 every table takes the same inputs (hA, h1, h0).  Two tables suffice: for
+// Delta >= 0 a vacate with x <= 0 is always accepted (dE = x - Delta <= 0), so its deciding entries
+// x = 1..4 sit on idx 5, 6, 7, 0 and share table A with the flips (idx 1..4), while occupy owns table
+// B; for Delta < 0 vacate and occupy swap roles.  Per word per plane: two dispatched LOP3, one select
+// by table, then the same two-LOP3 compare as before.
+template <bool SLAB>
+struct BCTieQueueGen {
+    const BCMarchArgs &a;
+    uint4 *q;                   // [3 * TIE_Q_SLOTS] this warp's slice
+    uint32_t lane, pending;
+
+    // [0] = (tied lanes, F, V, hA)   [1] = (h1, h0, nz-toggle mask, sg-toggle mask)
+    // [2] = (word offset lo, bits 32..35 | column word << 4 | mirror flag << 30, -, -)
+    __device__ __forceinline__ void resolve(uint32_t idx)
+    {
+        const uint4 e0 = q[3 * idx], e1 = q[3 * idx + 1], e2 = q[3 * idx + 2];
+        const unsigned long long wo = ((unsigned long long)(e2.y & 0xFu) << 32) | e2.x;
+        uint32_t ties = e0.x, hit = 0;
+        while (ties) {
+            const uint32_t bit = __ffs(ties) - 1;
+            ties &= ties - 1;
+            const uint32_t type = ((e0.y >> bit) & 1u) ? 0u : ((e0.z >> bit) & 1u) ? 1u : 2u;
+            const uint32_t i3 = (((e0.w >> bit) & 1u) << 2) | (((e1.x >> bit) & 1u) << 1) | ((e1.y >> bit) & 1u);
+            const unsigned long long P = ((SLAB ? wo + a.p_off : wo) << 5) + bit;
+            const uint4 blk = philox4x32_10((uint32_t)P, (uint32_t)(P >> 32), a.t,
+                                            a.colour | (TAG_ACC_TAIL << 8), a.K);
+            const unsigned long long u56 = ((unsigned long long)(blk.x >> 8) << 32) | blk.y;
+            if (u56 < (a.thrG[type * 8u + i3] & 0x00ffffffffffffffull)) hit |= 1u << bit;
+        }
+        const uint32_t dnz = hit & e1.z, dsg = hit & e1.w;
+        if (dnz) atomicXor(a.tnz + wo, dnz);
+        if (dsg) atomicXor(a.tsg + wo, dsg);
+        const uint32_t mf = SLAB ? e2.y >> 30 : 0u;
+        if (mf && (dnz | dsg)) {
+            const uint32_t col = (e2.y >> 4) & 0x3ffffu;
+            __threadfence_system();
+            if (dnz) atomicXor_system((mf == 1 ? a.mir_up_nz : a.mir_dn_nz) + col, dnz);
+            if (dsg) atomicXor_system((mf == 1 ? a.mir_up_sg : a.mir_dn_sg) + col, dsg);
+        }
+    }
+    __device__ __forceinline__ void push(const uint32_t (&eq)[4], const uint32_t (&Fm)[4], const uint32_t (&Vm)[4],
+                                         const uint32_t (&hA)[4], const uint32_t (&H1)[4], const uint32_t (&H0)[4],
+                                         const uint32_t (&nf)[4], const uint32_t (&gg)[4], unsigned long long wo,
+                                         uint32_t mir_tag)
+    {
+        const uint32_t below = (1u << lane) - 1u;
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const bool has = eq[w] != 0;
+            const uint32_t m = __ballot_sync(0xffffffffu, has);
+            if (has) {
+                const unsigned long long o = wo + (unsigned)w;
+                const uint32_t slot = pending + __popc(m & below);
+                q[3 * slot] = make_uint4(eq[w], Fm[w], Vm[w], hA[w]);
+                q[3 * slot + 1] = make_uint4(H1[w], H0[w], nf[w], gg[w]);
+                q[3 * slot + 2] = make_uint4((uint32_t)o, SLAB ? (uint32_t)(o >> 32) | (mir_tag + ((unsigned)w << 4))
+                                                               : (uint32_t)(o >> 32), 0u, 0u);
+            }
+            pending += __popc(m);
+        }
+        __syncwarp();
+        while (pending >= 32) {
+            pending -= 32;
+            resolve(pending + lane);
+            __syncwarp();
+        }
+    }
+    __device__ __forceinline__ void drain()
+    {
+        __syncwarp();
+        if (lane < pending) resolve(lane);
+        pending = 0;
+    }
+};
+
+template <int PAR, bool SLAB>
+__device__ __forceinline__ void bc_march_row_gen(const BCMarchArgs &a, uint32_t G, unsigned long long wo,
+                                                 uint32_t *tn, uint32_t *ts,
+                                                 const BCRow &U, const BCRow &C, const BCRow &D,
+                                                 uint32_t En, uint32_t Es, BCTieQueueGen<SLAB> &queue,
+                                                 uint32_t *mir_nz = nullptr, uint32_t *mir_sg = nullptr,
+                                                 uint32_t mir_tag = 0)
 {
-    __shared__ uint4 s_q[8][2 * TIE_Q_SLOTS];
+    BCRow T;
+    bcm_load(tn, ts, 0, T);
+    const PlaneShared ps = plane_shared(G, a.F);
+    uint32_t Fm[4], Vm[4], hA[4], H1[4], H0[4], pos[4], z4[4], nf[4], gg[4];
+    {
+        const uint4 pb = plane_block(ps, a.fbp, a.F, a.K);        // proposal bits
+        const uint32_t b[4] = {pb.x, pb.y, pb.z, pb.w};
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            uint32_t Sn, Ss;
+            if (PAR == 0) {
+                Sn = fsl1(w == 0 ? En : C.nz[w > 0 ? w - 1 : 0], C.nz[w]);
+                Ss = fsl1(w == 0 ? Es : C.sg[w > 0 ? w - 1 : 0], C.sg[w]);
+            } else {
+                Sn = fsr1(C.nz[w], w == 3 ? En : C.nz[w < 3 ? w + 1 : 0]);
+                Ss = fsr1(C.sg[w], w == 3 ? Es : C.sg[w < 3 ? w + 1 : 0]);
+            }
+            const uint32_t nz = T.nz[w], sg = T.sg[w], bw = b[w];
+            Fm[w] = lop3<0x90>(nz, sg, bw);                       // flip: nz & ~(sg ^ b)
+            Vm[w] = nz & ~Fm[w];                                  // vacate; occupy = ~nz
+            nf[w] = ~Fm[w];
+            gg[w] = lop3<0xDA>(nz, sg, bw);
+            const uint32_t r = lop3<0xC5>(nz, sg, bw);            // reference sign (bc_march_row)
+            const uint32_t a1 = lop3<0x90>(U.nz[w], U.sg[w], r), n1 = lop3<0x9F>(U.nz[w], U.sg[w], r);
+            const uint32_t a2 = lop3<0x90>(D.nz[w], D.sg[w], r), n2 = lop3<0x9F>(D.nz[w], D.sg[w], r);
+            const uint32_t a3 = lop3<0x90>(C.nz[w], C.sg[w], r), n3 = lop3<0x9F>(C.nz[w], C.sg[w], r);
+            const uint32_t a4 = lop3<0x90>(Sn, Ss, r), n4 = lop3<0x9F>(Sn, Ss, r);
+            const uint32_t s1 = lop3<0x96>(a1, a2, a3), c1 = lop3<0xE8>(a1, a2, a3);
+            const uint32_t s2 = lop3<0x96>(n1, n2, n3), c2 = lop3<0xE8>(n1, n2, n3);
+            const uint32_t s3 = lop3<0x96>(s1, s2, a4), c3 = lop3<0xE8>(s1, s2, a4);
+            const uint32_t h0 = s3 ^ n4, c4 = s3 & n4;
+            const uint32_t t1 = lop3<0x96>(c1, c2, c3), d1 = lop3<0xE8>(c1, c2, c3);
+            const uint32_t h1 = t1 ^ c4, d2 = t1 & c4;
+            const uint32_t h2 = d1 ^ d2, h3 = d1 & d2;
+            H0[w] = h0; H1[w] = h1;
+            hA[w] = lop3<0xCA>(Fm[w], h3, h2);                    // flip ? h3 : h2
+            pos[w] = h3 | lop3<0xE0>(h2, h1, h0);                 // x >= 1
+            z4[w] = ~(h3 | h2 | h1 | h0);                         // x == -4
+        }
+    }
+    uint32_t aA[4], aB[4], selA[4], need[4], acc[4], eq[4];
+    lut3_dispatch(a.lutA_always, hA, H1, H0, aA);
+    lut3_dispatch(a.lutB_always, hA, H1, H0, aB);
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        // lanes of table A: flips and the sharing type (nz lanes if vacate shares, else flip | ~nz)
+        selA[w] = a.share_v ? (Fm[w] | Vm[w]) : ~Vm[w];
+        // table A lanes decide only for x >= 1; table B lanes unless "always" (x = -4 always is)
+        need[w] = lop3<0xCA>(selA[w], pos[w] & ~aA[w], ~(aB[w] | z4[w]));
+        eq[w] = need[w];
+        acc[w] = 0;
+    }
+#pragma unroll 1                     // two 256-entry dispatch tables per iteration: keep one copy
+    for (int k = 7; k >= 0; --k) {
+        const uint4 b4 = plane_block(ps, a.F.fb[0] ^ ((uint32_t)k << 16), a.F, a.K);
+        const uint32_t b[4] = {b4.x, b4.y, b4.z, b4.w};
+        uint32_t gA[4], gB[4];
+        lut3_dispatch(a.lutA[k], hA, H1, H0, gA);
+        lut3_dispatch(a.lutB[k], hA, H1, H0, gB);
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const uint32_t tau = lop3<0xCA>(selA[w], gA[w], gB[w]);
+            acc[w] = maj3m(tau, ~b[w], acc[w]);
+            eq[w] &= ~(b[w] ^ tau);
+        }
+    }
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t ok = ~need[w] | acc[w];                    // a tied lane has acc = 0
+        T.nz[w] ^= ok & nf[w];
+        T.sg[w] ^= ok & gg[w];
+    }
+    *reinterpret_cast<uint4 *>(tn) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
+    *reinterpret_cast<uint4 *>(ts) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
+    if (SLAB && mir_nz) {
+        *reinterpret_cast<uint4 *>(mir_nz) = make_uint4(T.nz[0], T.nz[1], T.nz[2], T.nz[3]);
+        *reinterpret_cast<uint4 *>(mir_sg) = make_uint4(T.sg[0], T.sg[1], T.sg[2], T.sg[3]);
+        __threadfence_system();
+    }
+    queue.push(eq, Fm, Vm, hA, H1, H0, nf, gg, wo, mir_tag);
+}
+
+// GEN = false: the integer-dE (Delta = 0 type) rows above; GEN = true: bc_march_row_gen
+template <bool GEN, int PAR, bool SLAB, class Queue>
+__device__ __forceinline__ void bc_row(const BCMarchArgs &a, uint32_t G, unsigned long long wo, uint32_t *tn,
+                                       uint32_t *ts, const BCRow &U, const BCRow &C, const BCRow &D, uint32_t En,
+                                       uint32_t Es, Queue &queue, uint32_t *mir_nz = nullptr,
+                                       uint32_t *mir_sg = nullptr, uint32_t mir_tag = 0)
+{
+    if constexpr (GEN) bc_march_row_gen<PAR, SLAB>(a, G, wo, tn, ts, U, C, D, En, Es, queue, mir_nz, mir_sg, mir_tag);
+    else bc_march_row<PAR, SLAB>(a, G, wo, tn, ts, U, C, D, En, Es, queue, mir_nz, mir_sg, mir_tag);
+}
+
+template <bool GEN, bool SLAB>
+struct BCQueueOf { using type = BCTieQueue<SLAB>; };
+template <bool SLAB>
+struct BCQueueOf<true, SLAB> { using type = BCTieQueueGen<SLAB>; };
+
+template <int COLOUR, bool SLAB, bool GEN = false>
+__global__ void __launch_bounds__(256, GEN ? 2 : 3) bc_march_kernel(const BCMarchArgs a)
+{
+    // the general queue (3 x 16 bytes per entry, 60 KiB per block) exceeds the static limit: dynamic
+    extern __shared__ uint4 s_dyn[];
+    __shared__ uint4 s_fix[GEN ? 1 : 8][GEN ? 1 : 2 * TIE_Q_SLOTS];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;
     if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
-    BCTieQueue<SLAB> queue{a, s_q[warp], lane, 0u};
+    typename BCQueueOf<GEN, SLAB>::type queue{a, GEN ? s_dyn + warp * (3 * TIE_Q_SLOTS) : s_fix[GEN ? 0 : warp], lane, 0u};
 
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
     const uint32_t q = g % nq, s = g / nq;
@@ -294,10 +497,10 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
             bcm_load(dn, dn + pw, kw, D);
             const uint32_t ke = COLOUR == 0 ? ke0 : ke1;
             if (SLAB && top && r == 0)
-                bc_march_row<COLOUR, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
+                bc_row<GEN, COLOUR, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
                                      a.mir_up_nz + kw, a.mir_up_sg + kw, (kw << 4) | (1u << 30));
             else
-                bc_march_row<COLOUR, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+                bc_row<GEN, COLOUR, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
             U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
         {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
@@ -306,10 +509,10 @@ __global__ void __launch_bounds__(256, 3) bc_march_kernel(const BCMarchArgs a)
             bcm_load(dn, dn + pw, kw, D);
             const uint32_t ke = COLOUR == 0 ? ke1 : ke0;
             if (SLAB && bot && r + 2 == a.R)
-                bc_march_row<COLOUR ^ 1, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
+                bc_row<GEN, COLOUR ^ 1, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
                                          a.mir_dn_nz + kw, a.mir_dn_sg + kw, (kw << 4) | (2u << 30));
             else
-                bc_march_row<COLOUR ^ 1, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+                bc_row<GEN, COLOUR ^ 1, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
             U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
     }

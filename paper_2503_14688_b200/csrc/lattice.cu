@@ -292,7 +292,23 @@ bool bc_table_is_integer_dE(const lattice *lat)
     return true;
 }
 
-int launch_bc_march(lattice *lat, int colour)
+// bc_march_row_gen applies when x = -4 is "always" for vacate and occupy (|Delta| <= 4) and every
+// flip with x <= 0 is (dE = 2x <= 0: any Delta)
+bool bc_table_is_general_ok(const lattice *lat)
+{
+    if (!lat->alwT[bc_entry(BC_VACATE, -4)] || !lat->alwT[bc_entry(BC_OCCUPY, -4)]) return false;
+    for (int x = -4; x <= 0; ++x)
+        if (!lat->alwT[bc_entry(BC_FLIP, x)]) return false;
+    // one of vacate / occupy must be "always" for every x <= 0 (it shares table A with the flips)
+    bool v = true, o = true;
+    for (int x = -4; x <= 0; ++x) {
+        v = v && lat->alwT[bc_entry(BC_VACATE, x)];
+        o = o && lat->alwT[bc_entry(BC_OCCUPY, x)];
+    }
+    return v || o;
+}
+
+int launch_bc_march(lattice *lat, int colour, bool gen = false)
 {
     const uint32_t wpr = lat->wpr, nq = wpr / 4u;
     const size_t pw = (size_t)lat->rows * wpr;
@@ -322,17 +338,55 @@ int launch_bc_march(lattice *lat, int colour)
             for (int k = 0; k < 8; ++k)
                 if ((lat->thrT[e] >> (63 - k)) & 1u) a.lut[k] |= 1u << cls;
         }
+    // general crystal field: per move type an 8-entry table indexed by (hA, h1, h0) (bc_march.cuh)
+    for (int k = 0; k < 8; ++k) a.lutA[k] = a.lutB[k] = 0;
+    a.lutA_always = a.lutB_always = 0;
+    a.share_v = 1;
+    for (int e = 0; e < 24; ++e) a.thrG[e] = 0;
+    if (gen) {
+        bool v_ok = true;                                 // vacate "always" for every x <= 0 (Delta >= 0)
+        for (int x = -4; x <= 0; ++x) v_ok = v_ok && lat->alwT[bc_entry(BC_VACATE, x)];
+        a.share_v = v_ok ? 1u : 0u;
+        const int sharer = v_ok ? BC_VACATE : BC_OCCUPY;
+        for (int type = 0; type < 3; ++type) {
+            const bool inA = type == BC_FLIP || type == sharer;
+            uint32_t *lut = inA ? a.lutA : a.lutB;
+            uint32_t &always = inA ? a.lutA_always : a.lutB_always;
+            for (int x = (inA ? 1 : -3); x <= 4; ++x) {
+                // flip: x + 4 = 5, 6, 7, 8 -> (h3, h1, h0) = 1, 2, 3, 4; otherwise (x + 4) & 7
+                const uint32_t idx = type == BC_FLIP ? (x == 4 ? 4u : (uint32_t)x) : (uint32_t)((x + 4) & 7);
+                const int e = bc_entry(type, x);
+                a.thrG[type * 8 + (int)idx] = lat->thrT[e];
+                if (lat->alwT[e]) { always |= 1u << idx; continue; }
+                for (int k = 0; k < 8; ++k)
+                    if ((lat->thrT[e] >> (63 - k)) & 1u) lut[k] |= 1u << idx;
+            }
+        }
+    }
     a.K = lat->K;
     build_plane_fold(lat->K, a.t, a.colour, TAG_ACC_PLANE, a.F);
     a.fbp = (a.colour | (TAG_PROP_PLANE << 8)) ^ lat->K.k1[0];
     const unsigned blocks = (a.threads + 255u) / 256u;
-    if (lat->slab) {
-        if (colour == 0) bc_march_kernel<0, true><<<blocks, 256, 0, lat->stream>>>(a);
-        else bc_march_kernel<1, true><<<blocks, 256, 0, lat->stream>>>(a);
-    } else {
-        if (colour == 0) bc_march_kernel<0, false><<<blocks, 256, 0, lat->stream>>>(a);
-        else bc_march_kernel<1, false><<<blocks, 256, 0, lat->stream>>>(a);
+    const size_t dyn = gen ? (size_t)8 * 3 * TIE_Q_SLOTS * sizeof(uint4) : 0;       // the general tie queue
+    if (gen) {
+        static bool opted = false;                       // > 48 KiB of dynamic shared memory: opt in once
+        if (!opted) {
+            cudaFuncSetAttribute(bc_march_kernel<0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+            cudaFuncSetAttribute(bc_march_kernel<1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+            cudaFuncSetAttribute(bc_march_kernel<0, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+            cudaFuncSetAttribute(bc_march_kernel<1, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+            opted = true;
+        }
     }
+#define LAT_LAUNCH_BC(C, S, G) bc_march_kernel<C, S, G><<<blocks, 256, dyn, lat->stream>>>(a)
+    if (lat->slab) {
+        if (gen) { if (colour == 0) LAT_LAUNCH_BC(0, true, true); else LAT_LAUNCH_BC(1, true, true); }
+        else { if (colour == 0) LAT_LAUNCH_BC(0, true, false); else LAT_LAUNCH_BC(1, true, false); }
+    } else {
+        if (gen) { if (colour == 0) LAT_LAUNCH_BC(0, false, true); else LAT_LAUNCH_BC(1, false, true); }
+        else { if (colour == 0) LAT_LAUNCH_BC(0, false, false); else LAT_LAUNCH_BC(1, false, false); }
+    }
+#undef LAT_LAUNCH_BC
     lat->launches += 1;
     CU(lat, cudaGetLastError());
     return LATTICE_OK;
@@ -344,14 +398,16 @@ int launch_half_sweep(lattice *lat, int colour)
     if (lat->slab) {
         if (!lat->have_nbr) return LATTICE_ESTATE;
         if (lat->model == LATTICE_ISING) return launch_ising_march(lat, colour);
-        // Blume-Capel slabs run only the marching kernel: tables without the Delta = 0 structure
-        // (bc_march.cuh) are not supported in slab mode
-        if (!bc_table_is_integer_dE(lat)) return LATTICE_EINVAL;
-        return launch_bc_march(lat, colour);
+        // Blume-Capel slabs run only the marching kernels: the Delta = 0 type table, or any table
+        // with |Delta| <= 4 (bc_march.cuh)
+        if (bc_table_is_integer_dE(lat)) return launch_bc_march(lat, colour);
+        if (bc_table_is_general_ok(lat)) return launch_bc_march(lat, colour, true);
+        return LATTICE_EINVAL;
     }
-    if (lat->model == LATTICE_BLUME_CAPEL && lat->scheme >= 1 && (lat->wpr % 4u) == 0 &&
-        bc_table_is_integer_dE(lat))
-        return launch_bc_march(lat, colour);
+    if (lat->model == LATTICE_BLUME_CAPEL && lat->scheme >= 1 && (lat->wpr % 4u) == 0) {
+        if (bc_table_is_integer_dE(lat)) return launch_bc_march(lat, colour);
+        if (bc_table_is_general_ok(lat)) return launch_bc_march(lat, colour, true);
+    }
     if (lat->model == LATTICE_ISING && lat->scheme >= 1 && (lat->wpr % 4u) == 0)
         return launch_ising_march(lat, colour);
     if (lat->scheme == 2) return LATTICE_EINVAL;      // the generic kernels compare 32 bits only

@@ -127,3 +127,77 @@ def test_fit_z_jackknife_on_synthetic_runs():
     fit = an.fit_z_jackknife(t, stacks)
     assert abs(fit["z"] - z) < 0.05 and 0 <= fit["z_err"] < 0.05
     assert np.all(np.abs(fit["xi"] / xi_true - 1) < 0.02)
+
+
+def test_fit_z_energy_recovers_eq_6():
+    """Points generated from Eq. (6) / (D2) are fitted back: z and the three amplitudes."""
+    z, b, b1, b2 = 2.1676, 0.31, -0.12, 0.4
+    t = np.geomspace(16, 524288, 40)
+    E = an.E_EQ_ISING + b * t ** (-1 / z) + b1 * t ** (-2 / z) + b2 * t ** (-(an.OMEGA + 1.0) / z)
+    fit = an.fit_z_energy(t, E, np.full(t.size, 1e-9))
+    assert abs(fit["z"] - z) < 1e-6 and abs(fit["b"] - b) < 1e-5 and fit["dof"] == 36 and fit["chi2"] < 1.0
+    assert an.fit_z_energy(t, E, np.full(t.size, 1e-9), t_min=1000.0)["dof"] < 36
+    rng = np.random.default_rng(2)
+    noisy = E + 2e-6 * rng.normal(size=t.size)
+    f2 = an.fit_z_energy(t, noisy, np.full(t.size, 2e-6))
+    assert abs(f2["z"] - z) < 0.02 and f2["Q"] > 1e-3
+    with pytest.raises(ValueError):
+        an.fit_z_energy(t[:4], E[:4], np.full(4, 1e-9))
+    # a wrong E_eq is not absorbed: the fit quality collapses (why the paper uses it for Ising only)
+    bad = an.fit_z_energy(t, noisy, np.full(t.size, 2e-6), E_eq=an.E_EQ_ISING + 1e-3)
+    assert bad["chi2"] > 10 * f2["chi2"]
+
+
+def test_fit_z_joint_shares_one_exponent_across_data_sets():
+    """xi (Eq. 5) of two 'models' with different amplitudes + E (Eq. 6): one z for all (Fig. 3)."""
+    z = 2.1676
+    rng = np.random.default_rng(4)
+    sets = []
+    for b, b1 in ((-0.35, 1.9), (0.4, -0.8)):
+        xi = np.geomspace(6.0, 1100.0, 16)
+        t = np.exp(z * np.log(xi) + b + b1 * xi ** (-an.OMEGA))
+        sets.append({"kind": "xi", "t": t, "xi": xi * (1 + 1e-4 * rng.normal(size=xi.size)), "xi_err": 1e-4 * xi})
+    tE = np.geomspace(32, 524288, 24)
+    E = an.E_EQ_ISING + 0.3 * tE ** (-1 / z) - 0.1 * tE ** (-2 / z) + 0.2 * tE ** (-(an.OMEGA + 1.0) / z)
+    sets.append({"kind": "E", "t": tE, "E": E + 1e-7 * rng.normal(size=tE.size), "E_err": np.full(tE.size, 1e-7)})
+    fit = an.fit_z_joint(sets)
+    assert abs(fit["z"] - z) < 2e-3 and fit["dof"] == 16 + 16 + 24 - (1 + 2 + 2 + 3)
+    assert fit["Q"] > 1e-3 and len(fit["amplitudes"]) == 3
+    assert abs(fit["amplitudes"][0][0] + 0.35) < 0.02 and abs(fit["amplitudes"][2][0] - 0.3) < 0.01
+    single = an.fit_z_joint(sets[:1])                     # one xi set: the same answer as fit_z
+    ref = an.fit_z(sets[0]["t"], sets[0]["xi"], sets[0]["xi_err"])
+    assert abs(single["z"] - ref["z"]) < 1e-6
+
+
+def test_fit_z_energy_jackknife_and_exponential_approach():
+    rng = np.random.default_rng(9)
+    z = 2.17
+    t = np.geomspace(64, 262144, 20)
+    E = an.E_EQ_ISING + 0.3 * t ** (-1 / z) - 0.05 * t ** (-2 / z)
+    runs = [E[k] + 3e-6 * rng.normal(size=24) for k in range(t.size)]
+    fit = an.fit_z_energy_jackknife(t, runs)
+    assert abs(fit["z"] - z) < 0.05 and 0 < fit["z_err"] < 0.05
+    # Eq. (8): one tau for all f, b(f) changes sign around f = 0.59
+    tau = 3.0e4
+    tt = np.linspace(4e4, 3e5, 30)
+    curves = [{"f": f, "t": tt, "E": an.E_EQ_ISING + b * np.exp(-tt / tau) + 1e-8 * rng.normal(size=tt.size),
+               "E_err": np.full(tt.size, 1e-8)} for f, b in ((0.54, 1.5e-4), (0.59, 0.0), (0.64, -2.4e-4))]
+    res = an.fit_exponential_approach(curves)
+    assert abs(res["tau"] / tau - 1) < 0.01
+    assert abs(res["b"][0.54] - 1.5e-4) < 2e-6 and abs(res["b"][0.59]) < 2e-6 and res["b"][0.64] < -2e-4
+    free = an.fit_exponential_approach(curves, E_eq=None)            # Blume-Capel: E_eq is a parameter
+    assert abs(free["E_eq"] - an.E_EQ_ISING) < 1e-7 and abs(free["tau"] / tau - 1) < 0.02
+
+
+def test_sparse_r_grid_spline_reproduces_the_dense_estimate():
+    """C(r) sampled on a log-spaced r-grid and splined gives the dense-grid xi."""
+    C = _synthetic_C(30.0, 1.3, 1500, A=0.8)
+    err = np.full(C.size, 1e-9)
+    dense = an.xi_appendix_c(C, err)
+    r = np.unique(np.round(np.geomspace(1, 1500, 90)).astype(int))
+    sparse = an.xi_sparse(r, C[r], err[r])
+    assert abs(sparse / dense - 1) < 5e-3
+    d, e = an.densify(r, C[r], err[r])
+    assert d.size == 1501 and np.allclose(d[r], C[r]) and e.size == 1501
+    with pytest.raises(ValueError):
+        an.densify([3, 2], [0.1, 0.2])

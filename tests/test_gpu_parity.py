@@ -372,10 +372,37 @@ def test_scheme2_64_bit_thresholds(L, model):
 def test_scheme2_needs_marching_kernels():
     with pytest.raises(lat.LatticeError):
         lat.Lattice(64, lat.ISING, 0.0, 1, scheme=2)                 # L not a multiple of 256
-    b = lat.Lattice(256, lat.BLUME_CAPEL, 0.5, 1, scheme=2)          # Delta != 0: generic table
+    b = lat.Lattice(256, lat.BLUME_CAPEL, 5.5, 1, scheme=2)          # |Delta| > 4: only the generic kernel
     with pytest.raises(lat.LatticeError):
         b.sweep([0.5])
     b.close()
+
+
+@pytest.mark.parametrize("scheme", [1, 2])
+@pytest.mark.parametrize("L,delta,T", [(256, 0.7, 1.2), (512, -1.3, 2.0), (1024, 1.965, 0.6), (2048, 1.965, 0.9),
+                                       (256, 3.5, 1.0), (512, -4.0, 1.5), (256, 4.0, 0.8), (768, -0.25, 1.7)])
+def test_blume_capel_marching_kernel_with_crystal_field(L, delta, T, scheme):
+    """Delta != 0 on the marching path (bc_march_row_gen): vacate and occupy have their own
+    thresholds and x <= 0 is not "always" for them (Eq. 1, PAPER.md:38-40).  Spins and counts
+    against the oracle, including sweeps at beta = 0, at very low temperature and from ordered
+    states (every lane deciding, ties most frequent)."""
+    g = lat.Lattice(L, lat.BLUME_CAPEL, delta, 8800 + L, scheme)
+    o = oracle.OracleLattice(L, lat.BLUME_CAPEL, delta, 8800 + L, scheme)
+    sched = [1.0 / T] * 8 + [0.0, 0.05, 4.0, math.inf, 1.0 / T]
+    n0 = g.launches
+    g.sweep(sched[:3])
+    g.sweep(sched[3:])
+    assert g.launches - n0 == 2 * len(sched)
+    o.sweep(sched)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    _same_measure(g, o, min(L // 2, 48), L, delta)
+    for spin in (1, 0, -1):
+        g.fill(spin)
+        o.set_spins(np.full((L, L), spin, dtype=np.int8))
+        g.sweep([1.0 / T] * 3)
+        o.sweep([1.0 / T] * 3)
+        assert np.array_equal(g.get_spins(), o.get_spins()), spin
+    g.close(); o.close()
 
 
 def test_randomised_parity_sweep_of_parameters():

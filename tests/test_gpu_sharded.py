@@ -63,13 +63,28 @@ def test_sharded_many_sweeps_many_ties_across_boundaries(model):
     sh.close(); g.close()
 
 
+@pytest.mark.parametrize("delta,T", [(0.7, 1.2), (-1.3, 2.0), (1.965, 0.6)])
+def test_sharded_blume_capel_with_crystal_field(delta, T):
+    """Slab mode for Delta != 0 (the general marching kernel mirrors halos and late tie flips too)."""
+    L, n_slabs, seed = 512, 4, 2718
+    sh = ShardedLattice(L, n_slabs, seed, model=lat.BLUME_CAPEL, delta=delta)
+    o = oracle.OracleLattice(L, lat.BLUME_CAPEL, delta, seed)
+    beta = [1.0 / T] * 30 + [0.0, 3.0] + [1.0 / T] * 8
+    sh.sweep(beta)
+    o.sweep(beta)
+    assert np.array_equal(sh.get_spins(), o.get_spins())
+    M, Q, Sx, Sy = o.measure(1)
+    assert sh.measure() == (M, Q, int(Sx[0]), int(Sy[0]))
+    sh.close(); o.close()
+
+
 def test_slab_api_errors():
     L = 256
     with pytest.raises(lat.LatticeError):
         lat.Lattice(L, lat.ISING, 0.0, 1, slab=(0, 100))             # n_rows not a multiple of 64
     with pytest.raises(lat.LatticeError):
         lat.Lattice(L, lat.ISING, 0.0, 1, slab=(32, 64))             # row0 not a multiple of 64
-    b = lat.Lattice(L, lat.BLUME_CAPEL, 0.7, 1, slab=(0, 256))      # Delta != 0: no marching table
+    b = lat.Lattice(L, lat.BLUME_CAPEL, 4.7, 1, slab=(0, 256))      # |Delta| > 4: no marching table
     b.set_neighbours(b, b)
     with pytest.raises(lat.LatticeError):
         b.half_sweep(0, 0.5)
