@@ -237,6 +237,16 @@ uint64_t lattice_launches(const lattice_t *lat);
  * Results never depend on which kernel runs. */
 uint64_t lattice_specialised_launches(const lattice_t *lat);
 int lattice_plane_case_specialised(int model, double delta, double beta);
+/* Which kernels lattice_measure / lattice_measure_rows / lattice_measure_batch use for r_max > 1:
+ *   0 (default) automatic: the tensor-core path for L >= 4096, >= 512 base rows and r_max >= 48,
+ *     else the XOR/popcount kernels;
+ *   1 always the XOR/popcount kernels (north_star (c));
+ *   2 always the tensor cores (EINVAL unless L is a multiple of 128, L >= 1024, not a slab).
+ * The tensor-core path (csrc/corr_tc.cuh) evaluates dense C(r <= r_max), Eq. 2, as
+ * the band of the row / column Gram matrix with tcgen05.mma on fp8 copies of the spins (exactly
+ * representable; fp32 accumulators hold exact integers up to 2^24 > L); both paths return the same
+ * exact integer counts. */
+int lattice_set_measure_path(lattice_t *lat, int path);
 /* Tuning / test knob: upper bound on the grid of the persistent multi-sweep kernel that
  * lattice_sweep(n >= 2) uses for cache-resident Ising lattices (0 = the occupancy limit, the
  * default).  With fewer blocks than 256-thread groups of work every block strides over several

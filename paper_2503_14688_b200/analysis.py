@@ -392,3 +392,16 @@ def fit_exponential_approach(curves, E_eq: float | None = E_EQ_ISING, t_min: flo
     return {"tau": tau, "b": {float(c["f"]): float(p[k]) for k, c in enumerate(curves)},
             "E_eq": float(p[nf]) if E_eq is None else float(E_eq), "chi2": chi2, "dof": dof,
             "Q": float(gammaincc(max(dof, 1) / 2.0, chi2 / 2.0))}
+
+
+def onsager_energy(beta: float) -> float:
+    """Exact equilibrium energy per site of the infinite square-lattice Ising model (J = 1, Onsager):
+    e = -coth(2 beta) [1 + (2/pi) (2 tanh^2(2 beta) - 1) K(k)],  k = 2 sinh(2 beta) / cosh^2(2 beta),
+    K the complete elliptic integral of the first kind.  e(beta_c) = -sqrt 2; the paper
+    takes E_eq(T_2) of the two-step protocol from it."""
+    from scipy.special import ellipk
+    x = 2.0 * beta
+    k = 2.0 * np.sinh(x) / np.cosh(x) ** 2
+    if abs(1.0 - k) < 1e-14:
+        return -np.sqrt(2.0)
+    return float(-(1.0 / np.tanh(x)) * (1.0 + (2.0 / np.pi) * (2.0 * np.tanh(x) ** 2 - 1.0) * ellipk(k * k)))

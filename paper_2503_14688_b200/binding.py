@@ -60,6 +60,7 @@ SIGNATURES = {
     "lattice_set_time": (C.c_int, [_vp, C.c_uint64]),
     "lattice_launches": (C.c_uint64, [_vp]),
     "lattice_set_persist_blocks": (C.c_int, [_vp, C.c_uint32]),
+    "lattice_set_measure_path": (C.c_int, [_vp, C.c_int]),
     "lattice_specialised_launches": (C.c_uint64, [_vp]),
     "lattice_plane_case_specialised": (C.c_int, [C.c_int, C.c_double, C.c_double]),
     "lattice_thresholds": (None, [C.c_int, C.c_double, C.c_double, _u64p]),
@@ -355,6 +356,10 @@ class Lattice:
         with self._torch.cuda.device(self.device):
             self._check(lib().lattice_set_spins(self._h, i0, j0, s.shape[0], s.shape[1],
                                                 _p(s, C.c_int8)), "lattice_set_spins")
+
+    def set_measure_path(self, path: int) -> None:
+        """0 automatic, 1 XOR/popcount kernels, 2 tensor cores (include/lattice.h)."""
+        self._check(lib().lattice_set_measure_path(self._h, int(path)), "lattice_set_measure_path")
 
     def set_persist_blocks(self, max_blocks: int) -> None:
         """Cap the grid of the persistent multi-sweep kernel (0 = occupancy limit)."""

@@ -1,0 +1,331 @@
+// corr_tc.cuh -- dense axis correlations S_x(r), S_y(r), r <= r_max, on the 5th-generation tensor
+// cores (tcgen05 + TMEM).
+//
+// Paper: C(r;t), Eq. 2, along the lattice axes.  Dense in r this IS a dense
+// contraction: S_y(r) = sum_i G[i, i+r] with the band of the row Gram matrix
+//     G[i, i'] = sum_j s(i, j) s(i', j),
+// and S_x(r) the same with rows and columns exchanged.  The XOR/popcount kernels of measure.cuh
+// pay ~3 integer instructions per (32 spins, r); on the tensor cores one tcgen05.mma of shape
+// 128 x 256 x 32 (fp8 e4m3, fp32 accumulate) does 2^20 spin products.  Spins are exactly
+// representable (+1 = 0x38, -1 = 0xB8, 0 = 0x00) and |G| <= L <= 2^20 < 2^24, so the fp32
+// accumulators hold exact integers: the result is the same exact integer count as the popcount path.
+//
+// One CTA per SM, persistent over work items (tile of 128 base positions, pass of 512 partner
+// positions starting at the tile's first position + 512 * pass).  Per item the whole lattice extent
+// along the contraction axis streams through a 2-stage shared-memory ring:
+//   * 8 producer warps read the packed words (1 or 2 bits per spin), expand them to fp8 bytes and
+//     write them into the canonical 128-byte-swizzled UMMA layout (K-major for the y axis, where the
+//     contraction runs along a row; MN-major for the x axis, where it runs across rows);
+//   * one thread of a 9th warp issues 8 tcgen05.mma per stage (4 K-steps x 2 N-tiles of 256) into
+//     two 128 x 256 fp32 accumulators that fill the 512 TMEM columns, and commits to the stage's
+//     "empty" mbarrier;
+//   * after the last stage warps 0-3 read the accumulators back (tcgen05.ld, lane = base position)
+//     and add every element with 1 <= r <= r_max to a per-item histogram in shared memory, which is
+//     flushed to 64-bit global counters.
+// Within a 128-position block the byte order is [64 even columns | 64 odd columns] of the row for
+// the x axis (and the same split of the contraction index for the y axis): that is the order the
+// sublattice packing delivers, the same for both operands, and the epilogue undoes it.
+#pragma once
+#include <stdint.h>
+
+namespace lat {
+
+constexpr int TC_M = 128;            // base positions per item
+constexpr int TC_N = 256;            // partner positions per MMA
+constexpr int TC_NT = 2;             // N tiles per item (TC_NT * TC_N = 512 TMEM columns)
+constexpr int TC_KC = 128;           // contraction positions per stage (one 128-byte swizzle row)
+constexpr int TC_STAGES = 2;
+constexpr int TC_PRODUCERS = 256;    // producer threads (warps 0-7); warp 8 issues the MMAs
+constexpr int TC_THREADS = TC_PRODUCERS + 32;
+constexpr int TC_STAGE_BYTES = (TC_M + TC_NT * TC_N) * TC_KC;            // 80 KiB
+constexpr int TC_HIST = TC_NT * TC_N + TC_M;                             // r - 512 pass + 127 in [0, 639)
+constexpr int TC_SMEM_BYTES = TC_STAGES * TC_STAGE_BYTES + 1024 /* alignment */ + TC_HIST * 4 + 64;
+
+struct CorrTCArgs {
+    const uint32_t *buf;
+    uint32_t L;                      // lattice side: extent of a row, period along x
+    uint32_t rows;                   // rows per plane in the buffer (L, or a view's row count): period along y
+    uint32_t wpr;
+    uint32_t i0, n_rows;             // base rows i0 .. i0 + n_rows - 1
+    uint32_t r_max;
+    uint32_t n_tiles, n_pass, n_items;
+    long long *S;                    // signed sums of this axis: S[(r - 1) * s_stride] (device, zeroed by the host)
+    uint32_t s_stride;
+};
+
+#ifdef __CUDACC__
+namespace tc {
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// bounded spin: a protocol error traps instead of hanging the GPU
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    for (uint32_t spin = 0;; ++spin) {
+        uint32_t ok;
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return;
+        if (spin > (1u << 28)) __trap();
+    }
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+// UMMA shared-memory descriptor, 128-byte swizzle, version 1 (Blackwell): start address >> 4 in
+// bits [0,14), leading byte offset >> 4 in [16,30), stride byte offset >> 4 in [32,46), version in
+// [46,48), layout type (2 = SWIZZLE_128B) in [61,64)
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) |
+           ((uint64_t)(sbo_bytes >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+
+// D[tmem] (+)= A[smem] * B[smem], kind::f8f6f4, issued by one thread
+__device__ __forceinline__ void umma_f8(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
+                                        uint32_t accumulate)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+// 4 spins (the low 4 bits of n) -> 4 fp8 bytes: bit = 1 -> +1.0 (0x38), bit = 0 -> -1.0 (0xB8).
+// n * 0x10204080 puts bit b at bit 8 b + 7 (no carries: the 16 partial products land on distinct bits).
+__device__ __forceinline__ uint32_t ising_bytes(uint32_t n)
+{
+    return ((n * 0x10204080u) & 0x80808080u) ^ 0xB8B8B8B8u;
+}
+// Blume-Capel: nz ? (sg ? -1.0 : +1.0) : 0.0
+__device__ __forceinline__ uint32_t bc_bytes(uint32_t nz, uint32_t sg)
+{
+    const uint32_t one = (nz * 0x00204081u) & 0x01010101u;               // bit b -> byte b, value 1
+    return one * 0x38u | (((nz & sg) * 0x10204080u) & 0x80808080u);
+}
+
+// 32 spins of word w (and sign plane s for Blume-Capel) -> 32 bytes
+template <int MODEL>
+__device__ __forceinline__ void expand_word(uint32_t w, uint32_t s, uint4 &lo, uint4 &hi)
+{
+    uint32_t o[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const uint32_t n = (w >> (4 * q)) & 0xFu;
+        o[q] = MODEL == 0 ? ising_bytes(n) : bc_bytes(n, (s >> (4 * q)) & 0xFu);
+    }
+    lo = make_uint4(o[0], o[1], o[2], o[3]);
+    hi = make_uint4(o[4], o[5], o[6], o[7]);
+}
+
+}  // namespace tc
+
+// AXIS 1 (y): positions are rows, the contraction runs over the columns of a row.
+// AXIS 0 (x): positions are columns, the contraction runs over rows i0 .. i0 + n_rows - 1.
+template <int MODEL, int AXIS>
+__global__ void __launch_bounds__(TC_THREADS, 1) corr_tc_kernel(const CorrTCArgs a)
+{
+    using namespace tc;
+    extern __shared__ uint8_t tc_smem_raw[];
+    uint8_t *smem = (uint8_t *)(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);      // swizzle atoms: 1 KiB
+    int *hist = (int *)(smem + TC_STAGES * TC_STAGE_BYTES);
+    __shared__ __align__(8) unsigned long long bars[2 * TC_STAGES + 1];
+    __shared__ uint32_t tmem_base_s;
+
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+    const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[TC_STAGES]), accf = smem_u32(&bars[2 * TC_STAGES]);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < TC_STAGES; ++s) {
+            mbar_init(full0 + 8 * s, TC_PRODUCERS / 32);      // one arrive per producer warp
+            mbar_init(empty0 + 8 * s, 1);                     // tcgen05.commit
+        }
+        mbar_init(accf, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == TC_PRODUCERS / 32) {                          // the MMA warp owns the tensor memory
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
+    }
+    fence_before_sync();
+    __syncthreads();
+    fence_after_sync();
+    const uint32_t tmem = tmem_base_s;
+
+    const size_t pw = (size_t)a.rows * a.wpr;                 // words per plane
+    // contraction extent: y: the L columns of a row; x: the base rows
+    const uint32_t n_kc = AXIS == 1 ? a.L / TC_KC : (a.n_rows + TC_KC - 1) / TC_KC;
+    // instruction descriptor: fp32 accumulate, e4m3 x e4m3, N >> 3 in [17,23), M >> 4 in [24,29),
+    // bits 15 / 16 = MN-major A / B (x axis)
+    const uint32_t idesc = (1u << 4) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24) |
+                           (AXIS == 0 ? (1u << 15) | (1u << 16) : 0u);
+
+    uint32_t stage = 0, phase = 0, acc_phase = 0;
+    for (uint32_t item = blockIdx.x; item < a.n_items; item += gridDim.x) {
+        const uint32_t pass = item / a.n_tiles, tile = item - pass * a.n_tiles;
+        // first base position of the tile and first partner position of the pass
+        const uint32_t p0 = (AXIS == 1 ? a.i0 : 0u) + tile * TC_M;
+        if (warp < TC_PRODUCERS / 32) {
+            // ===== producers =====
+            for (uint32_t kc = 0; kc < n_kc; ++kc) {
+                mbar_wait(empty0 + 8 * stage, phase ^ 1u);
+                uint8_t *st = smem + (size_t)stage * TC_STAGE_BYTES;
+#pragma unroll 1
+                for (uint32_t it = threadIdx.x; it < (TC_M + TC_NT * TC_N) * 2; it += TC_PRODUCERS) {
+                    // item = 64 bytes: one half (even / odd columns) of one 128-byte smem row
+                    uint32_t h, srow, blk, row_l, word;      // half, smem row in block, block, lattice row, word in row
+                    bool zero = false;
+                    if (AXIS == 1) {
+                        const uint32_t tr = it >> 1;          // 0..127 base rows, 128..639 partner rows
+                        h = it & 1u;
+                        blk = tr < TC_M ? 0u : 1u + (tr - TC_M) / TC_N;
+                        srow = tr < TC_M ? tr : (tr - TC_M) % TC_N;
+                        uint32_t i;
+                        if (tr < TC_M) { i = p0 + tr; zero = i >= a.i0 + a.n_rows; }
+                        else i = p0 + pass * (TC_NT * TC_N) + (tr - TC_M);
+                        row_l = i % a.rows;
+                        word = kc * 2u;                       // 64 packed positions = 2 words per colour
+                    } else {
+                        // smem row = contraction index (lattice row), 128-column blocks along MN:
+                        // block 0 = base columns, blocks 1..4 = the pass's partner columns
+                        const uint32_t kk = it % TC_KC, rest = it / TC_KC;
+                        h = rest & 1u;
+                        const uint32_t mb = rest >> 1;        // 0..4
+                        blk = mb == 0 ? 0u : 1u + (mb - 1u) / 2u;
+                        const uint32_t i = a.i0 + kc * TC_KC + kk;
+                        zero = i >= a.i0 + a.n_rows;
+                        row_l = i % a.rows;
+                        const uint32_t col0 = mb == 0 ? p0 : (p0 + pass * (TC_NT * TC_N) + (mb - 1u) * TC_M) % a.L;
+                        word = col0 / 64u;                    // 128 columns = 64 packed positions = 2 words
+                        // MN-major: 128-column block mb of the N tile sits TC_KC * 128 bytes further
+                        srow = kk + ((mb == 0 ? 0u : (mb - 1u) & 1u) * TC_KC);
+                    }
+                    const uint32_t c = (row_l & 1u) ^ h;      // even columns of row i live in colour i & 1
+                    uint4 o[4];
+                    if (zero) {
+                        o[0] = o[1] = o[2] = o[3] = make_uint4(0u, 0u, 0u, 0u);
+                    } else {
+                        const size_t off = (size_t)row_l * a.wpr + word;
+                        const uint32_t *p = a.buf + (MODEL == 0 ? (size_t)c * pw : (size_t)(2u * c) * pw) + off;
+                        const uint2 w = *reinterpret_cast<const uint2 *>(p);
+                        uint2 s = make_uint2(0u, 0u);
+                        if (MODEL) s = *reinterpret_cast<const uint2 *>(p + pw);
+                        expand_word<MODEL>(w.x, s.x, o[0], o[1]);
+                        expand_word<MODEL>(w.y, s.y, o[2], o[3]);
+                    }
+                    // canonical 128-byte swizzle: 8-row atoms of 1 KiB, 16-byte chunk index ^ (row & 7)
+                    uint8_t *base = st + (blk == 0 ? 0 : TC_M * TC_KC + (blk - 1u) * (TC_N * TC_KC)) +
+                                    (size_t)(srow >> 3) * 1024u + (srow & 7u) * 128u;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        *reinterpret_cast<uint4 *>(base + (((h * 4u + q) ^ (srow & 7u)) << 4)) = o[q];
+                }
+                fence_proxy_async();                          // generic-proxy writes -> visible to the tensor core
+                fence_before_sync();                          // (and the previous item's tcgen05.ld are done)
+                __syncwarp();
+                if (lane == 0) mbar_arrive(full0 + 8 * stage);
+                if (++stage == TC_STAGES) { stage = 0; phase ^= 1u; }
+            }
+            // ===== epilogue (warps 0-3: TMEM lane quarter = warp) =====
+            if (warp < 4) {
+                for (uint32_t t = threadIdx.x; t < (uint32_t)TC_HIST; t += 128u) hist[t] = 0;
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                mbar_wait(accf, acc_phase);
+                fence_after_sync();
+                const uint32_t m = warp * 32u + lane;         // base position index in the tile
+                // position of byte index x inside a 128-block: [64 even | 64 odd] for the x axis
+                const int pm = AXIS == 1 ? (int)m : (int)(m < 64u ? 2u * m : 2u * (m - 64u) + 1u);
+#pragma unroll 1
+                for (uint32_t cb = 0; cb < (uint32_t)(TC_NT * TC_N); cb += 16u) {
+                    uint32_t v[16];
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+                                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]),
+                                   "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]),
+                                   "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                                 : "r"(tmem + ((warp * 32u) << 16) + cb));
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) {
+                        const uint32_t n = cb + (uint32_t)e;
+                        int pn;
+                        if (AXIS == 1) pn = (int)n;
+                        else {
+                            const uint32_t nb = n & 127u;
+                            pn = (int)((n & ~127u) + (nb < 64u ? 2u * nb : 2u * (nb - 64u) + 1u));
+                        }
+                        const int d = pn - pm;                 // r - 512 pass, in (-128, 512)
+                        const long long r = (long long)d + (long long)pass * (TC_NT * TC_N);
+                        const int val = __float2int_rn(__uint_as_float(v[e]));
+                        if (r >= 1 && r <= (long long)a.r_max && val) atomicAdd(&hist[d + (TC_M - 1)], val);
+                    }
+                }
+                fence_before_sync();
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                for (uint32_t t = threadIdx.x; t < (uint32_t)TC_HIST; t += 128u) {
+                    const long long r = (long long)t - (TC_M - 1) + (long long)pass * (TC_NT * TC_N);
+                    if (hist[t] && r >= 1 && r <= (long long)a.r_max)
+                        atomicAdd((unsigned long long *)(a.S + (r - 1) * a.s_stride), (unsigned long long)(long long)hist[t]);
+                }
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+            }
+            acc_phase ^= 1u;
+        } else {
+            // ===== MMA issuer (one elected thread of warp 8) =====
+            for (uint32_t kc = 0; kc < n_kc; ++kc) {
+                mbar_wait(full0 + 8 * stage, phase);
+                fence_after_sync();
+                if (lane == 0) {
+                    const uint32_t sa = smem_u32(smem + (size_t)stage * TC_STAGE_BYTES);
+                    const uint32_t sb = sa + TC_M * TC_KC;
+#pragma unroll
+                    for (uint32_t k = 0; k < TC_KC / 32; ++k) {
+#pragma unroll
+                        for (uint32_t nt = 0; nt < (uint32_t)TC_NT; ++nt) {
+                            uint64_t da, db;
+                            if (AXIS == 1) {
+                                // K-major: rows of 128 bytes along K, 8-row atoms 1 KiB apart; a K step of
+                                // 32 bytes moves the start address inside the swizzled row
+                                da = umma_desc(sa + k * 32u, 16u, 1024u);
+                                db = umma_desc(sb + nt * (TC_N * TC_KC) + k * 32u, 16u, 1024u);
+                            } else {
+                                // MN-major: rows of 128 bytes along M / N, one row per contraction index;
+                                // 8-row atoms along K 1 KiB apart (SBO), the second 128-column block of an
+                                // N tile TC_KC * 128 bytes further (LBO); a K step of 32 = 4 atoms
+                                da = umma_desc(sa + k * 4096u, TC_KC * 128u, 1024u);
+                                db = umma_desc(sb + nt * (TC_N * TC_KC) + k * 4096u, TC_KC * 128u, 1024u);
+                            }
+                            umma_f8(tmem + nt * TC_N, da, db, idesc, (kc | k) ? 1u : 0u);
+                        }
+                    }
+                    umma_commit(empty0 + 8 * stage);          // stage reusable once these MMAs are done
+                    if (kc + 1 == n_kc) umma_commit(accf);    // accumulators complete
+                }
+                __syncwarp();
+                if (++stage == TC_STAGES) { stage = 0; phase ^= 1u; }
+            }
+        }
+    }
+    fence_before_sync();
+    __syncthreads();
+    if (warp == TC_PRODUCERS / 32) {
+        fence_after_sync();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+    }
+}
+#endif
+
+}  // namespace lat

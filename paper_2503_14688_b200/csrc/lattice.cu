@@ -21,6 +21,7 @@
 #include "ising_persist.cuh"
 #include "ising_batch.cuh"
 #include "measure.cuh"
+#include "corr_tc.cuh"
 #include "philox.cuh"
 #include "ubench.cuh"
 
@@ -63,6 +64,7 @@ struct lattice {
     size_t sp_cap;             // entries
     int persist_blocks;        // co-resident blocks of ising_persist_kernel (0: not yet queried, -1: unavailable)
     uint32_t persist_cap;      // lattice_set_persist_blocks: upper bound on the grid (0: none)
+    int measure_path;          // lattice_set_measure_path: 0 auto, 1 XOR/popcount kernels, 2 tensor cores
     // batch of independent replicas (lattice_create_batch): the batch handle owns one child handle
     // per replica (buf offset, own seed / round keys); a child has parent != nullptr
     uint32_t n_rep;            // 0 for a plain lattice or a child
@@ -1109,6 +1111,7 @@ static int enqueue_generic(lattice *lat, const uint32_t *buf, unsigned long long
         lat->launches += 1;
         CU(lat, cudaGetLastError());
     }
+    if (naxes == 0) return LATTICE_OK;
     unsigned gx = bx;
     const unsigned long long cap = (148ull * 32ull + 2ull * r_max * n_rep - 1) / (2ull * r_max * n_rep);
     if (gx > cap) gx = (unsigned)(cap ? cap : 1);
@@ -1126,8 +1129,18 @@ static int enqueue_generic(lattice *lat, const uint32_t *buf, unsigned long long
 
 // device counters (MeasArgs::cnt layout, `entries` of them) -> the signed sums of the ABI
 static void convert_counts(int model, int64_t N, uint32_t r_max, const unsigned long long *h, int64_t *M,
-                           int64_t *Q, int64_t *Sx, int64_t *Sy)
+                           int64_t *Q, int64_t *Sx, int64_t *Sy, bool tc = false)
 {
+    if (tc) {
+        // tensor-core path (corr_tc.cuh): the axis entries already hold the signed sums
+        if (model == LATTICE_ISING) { *M = 2 * (int64_t)h[0] - N; *Q = N; }
+        else { *M = (int64_t)h[0] - (int64_t)h[1]; *Q = (int64_t)h[0] + (int64_t)h[1]; }
+        for (uint32_t r = 0; r < r_max; ++r) {
+            Sx[r] = (int64_t)h[2 + 2 * (size_t)r];
+            Sy[r] = (int64_t)h[2 + 2 * ((size_t)r_max + r)];
+        }
+        return;
+    }
     if (model == LATTICE_ISING) {
         *M = 2 * (int64_t)h[0] - N;
         *Q = N;
@@ -1157,12 +1170,66 @@ static int fetch_counts(lattice *lat, const unsigned long long *src, size_t entr
     return LATTICE_OK;
 }
 
+// Dense C(r) on the tensor cores (corr_tc.cuh): both axes as banded Gram matrices, signed sums
+// written straight into the axis entries of cnt (stride 2, the layout convert_counts(tc) reads).
+static bool corr_tc_applies(const lattice *lat, uint64_t n_rows, uint32_t r_max)
+{
+    if (lat->measure_path == 1) return false;
+    const bool shape_ok = (lat->L % 128u) == 0 && lat->L >= 1024u && n_rows >= 1 && !lat->slab;
+    if (lat->measure_path == 2) return shape_ok;
+    return shape_ok && lat->L >= 4096u && n_rows >= 512 && r_max >= 48;
+}
+
+static int enqueue_corr_tc(lattice *lat, unsigned long long *cnt, uint64_t i0, uint64_t n_rows, uint32_t r_max)
+{
+    static bool opted = false;
+    if (!opted) {
+        cudaFuncSetAttribute(corr_tc_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
+        cudaFuncSetAttribute(corr_tc_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
+        cudaFuncSetAttribute(corr_tc_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
+        cudaFuncSetAttribute(corr_tc_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
+        opted = true;
+    }
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    // M, Q of the base rows
+    int rc = enqueue_generic(lat, lat->buf, cnt, 1, 0, 0, (uint32_t)i0, (uint32_t)n_rows, r_max, true, 0u, 0u);
+    if (rc) return rc;
+    CorrTCArgs a;
+    a.buf = lat->buf; a.L = lat->L; a.rows = lat->rows; a.wpr = lat->wpr;
+    a.i0 = (uint32_t)i0; a.n_rows = (uint32_t)n_rows; a.r_max = r_max; a.s_stride = 2;
+    a.n_pass = (r_max + TC_M + TC_NT * TC_N - 1) / (TC_NT * TC_N);
+    for (int axis = 1; axis >= 0; --axis) {
+        a.n_tiles = axis == 1 ? (uint32_t)((n_rows + TC_M - 1) / TC_M) : lat->L / TC_M;
+        a.n_items = a.n_tiles * a.n_pass;
+        a.S = (long long *)(cnt + 2 + (axis == 1 ? 2 * (size_t)r_max : 0));
+        const unsigned grid = a.n_items < (unsigned)sms ? a.n_items : (unsigned)sms;
+        if (lat->model == LATTICE_ISING) {
+            if (axis == 1) corr_tc_kernel<0, 1><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+            else corr_tc_kernel<0, 0><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+        } else {
+            if (axis == 1) corr_tc_kernel<1, 1><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+            else corr_tc_kernel<1, 0><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+        }
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+    }
+    return LATTICE_OK;
+}
+
 // Launches (no synchronisation) that add the counts of base rows i0 .. i0+n_rows-1 of lat's buffer,
 // r = 1..r_max, to the zeroed counters at cnt.  Row-blocked kernels: the y axis (and M, Q) over the
 // whole 16-row blocks of the slab, the x axis over every row when a row is a whole number of 16-word
 // segments; whatever they do not cover (ragged rows, narrow lattices) goes through the generic ones.
-static int enqueue_measure(lattice *lat, unsigned long long *cnt, uint64_t i0, uint64_t n_rows, uint32_t r_max)
+static int enqueue_measure(lattice *lat, unsigned long long *cnt, uint64_t i0, uint64_t n_rows, uint32_t r_max,
+                           bool *tc = nullptr)
 {
+    if (tc) *tc = false;
+    if (tc && r_max > 1 && corr_tc_applies(lat, n_rows, r_max)) {
+        *tc = true;
+        return enqueue_corr_tc(lat, cnt, i0, n_rows, r_max);
+    }
     if (r_max == 1 && (lat->wpr % 4u) == 0) {
         // the per-step record (e, m, q): one pass over the slab
         MeasE1Args e1;
@@ -1232,12 +1299,13 @@ int lattice_measure_rows(lattice_t *lat, uint64_t i0, uint64_t n_rows, uint32_t 
     int rc = ensure_cnt(lat, entries);
     if (rc) return rc;
     CU(lat, cudaMemsetAsync(lat->d_cnt, 0, entries * sizeof(unsigned long long), lat->stream));
-    rc = enqueue_measure(lat, lat->d_cnt, i0, n_rows, r_max);
+    bool tc = false;
+    rc = enqueue_measure(lat, lat->d_cnt, i0, n_rows, r_max, &tc);
     if (rc) return rc;
     unsigned long long *h = nullptr;
     rc = fetch_counts(lat, lat->d_cnt, entries, &h);
     if (rc) return rc;
-    convert_counts(lat->model, (int64_t)(n_rows * L), r_max, h, M, Q, Sx, Sy);
+    convert_counts(lat->model, (int64_t)(n_rows * L), r_max, h, M, Q, Sx, Sy, tc);
     std::free(h);
     return LATTICE_OK;
 }
@@ -1319,13 +1387,15 @@ int lattice_measure_batch(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q
     int rc = ensure_cnt(lat, total);
     if (rc) return rc;
     CU(lat, cudaMemsetAsync(lat->d_cnt, 0, total * sizeof(unsigned long long), lat->stream));
+    bool tc = false;
     if (L < 1024u) {
         rc = enqueue_generic(lat, lat->buf, lat->d_cnt, lat->n_rep, lat->rep_words, entries, 0u, (uint32_t)L, r_max,
                              true, 0u, 2u);
         if (rc) return rc;
     } else {
         for (uint32_t k = 0; k < lat->n_rep; ++k) {
-            rc = enqueue_measure(lat->kids[k], lat->d_cnt + (size_t)k * entries, 0, L, r_max);
+            lat->kids[k]->measure_path = lat->measure_path;
+            rc = enqueue_measure(lat->kids[k], lat->d_cnt + (size_t)k * entries, 0, L, r_max, &tc);
             if (rc) return rc;
         }
     }
@@ -1334,7 +1404,7 @@ int lattice_measure_batch(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q
     if (rc) return rc;
     for (uint32_t k = 0; k < lat->n_rep; ++k)
         convert_counts(lat->model, (int64_t)(L * L), r_max, h + (size_t)k * entries, M + k, Q + k,
-                       Sx + (size_t)k * r_max, Sy + (size_t)k * r_max);
+                       Sx + (size_t)k * r_max, Sy + (size_t)k * r_max, tc);
     std::free(h);
     return LATTICE_OK;
 }
@@ -1460,6 +1530,14 @@ int lattice_plane_case_specialised(int model, double delta, double beta)
 #undef LAT_PC_CASE
     default: return 0;
     }
+}
+
+int lattice_set_measure_path(lattice_t *lat, int path)
+{
+    if (!lat || path < 0 || path > 2) return LATTICE_EINVAL;
+    if (path == 2 && ((lat->L % 128u) != 0 || lat->L < 1024u || lat->slab)) return LATTICE_EINVAL;
+    lat->measure_path = path;
+    return LATTICE_OK;
 }
 
 int lattice_set_persist_blocks(lattice_t *lat, uint32_t max_blocks)

@@ -1,0 +1,77 @@
+"""Dense C(r) on the tensor cores (csrc/corr_tc.cuh, lattice_set_measure_path(2)) against the oracle's
+literal double loops and against the XOR/popcount kernels: the same exact integers for both models,
+both axes, several passes of 512 partner positions, periodic wrap, ragged row ranges and ordered
+states (where every product has the same sign and the accumulators reach their largest values)."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2503_14688_b200 as lat
+from paper_2503_14688_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+NCPU = os.cpu_count() or 1
+
+
+@pytest.fixture(autouse=True)
+def _threads():
+    oracle.set_threads(NCPU)
+    yield
+    oracle.set_threads(1)
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+@pytest.mark.parametrize("L,r_max", [(1024, 512), (1024, 60), (2048, 700), (1536, 768)])
+def test_tensor_core_correlations_equal_oracle_and_popcount_path(L, r_max, model):
+    g = lat.Lattice(L, model, 0.0, 31415 + L)
+    o = oracle.OracleLattice(L, model, 0.0, 31415 + L)
+    beta = workloads.BETA_C_ISING if model == lat.ISING else workloads.BETA_BC
+    g.sweep([beta] * 20)
+    o.sweep([beta] * 20)
+    want = o.measure(r_max)
+    g.set_measure_path(1)
+    pop = g.measure(r_max)
+    g.set_measure_path(2)
+    tc = g.measure(r_max)
+    for got in (pop, tc):
+        assert (got[0], got[1]) == (want[0], want[1])
+        assert np.array_equal(got[2], want[2]), np.nonzero(got[2] != want[2])[0][:8]
+        assert np.array_equal(got[3], want[3]), np.nonzero(got[3] != want[3])[0][:8]
+    # row ranges: partner rows wrap periodically, base rows end inside a 128-row tile
+    for i0, n in ((0, 128), (5, 300), (L - 77, 77), (L // 2 - 1, 1)):
+        ws = o.measure(min(r_max, 200), (i0, n))
+        gs = g.measure(min(r_max, 200), (i0, n))
+        assert (gs[0], gs[1]) == (ws[0], ws[1]) and np.array_equal(gs[2], ws[2]) and np.array_equal(gs[3], ws[3]), (i0, n)
+    # ordered and striped states: |G| = L, every accumulator at its extreme
+    i, j = np.indices((L, L))
+    for s in (np.ones((L, L), np.int8), np.where(i % 2 == 0, 1, -1).astype(np.int8),
+              np.where(j % 4 < 2, 1, -1).astype(np.int8)):
+        g.set_spins(s)
+        o.set_spins(s)
+        a, b = g.measure(r_max), o.measure(r_max)
+        assert (a[0], a[1]) == (b[0], b[1]) and np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3])
+    g.close(); o.close()
+
+
+def test_tensor_core_path_selection_and_errors():
+    g = lat.Lattice(256, lat.ISING, 0.0, 1)
+    with pytest.raises(lat.LatticeError):
+        g.set_measure_path(2)                       # L < 1024
+    with pytest.raises(lat.LatticeError):
+        g.set_measure_path(3)
+    g.set_measure_path(1)
+    g.close()
+    b = lat.LatticeBatch(1024, np.arange(3, dtype=np.uint64) + 5)
+    b.sweep([workloads.BETA_C_ISING] * 6)
+    import ctypes as C
+    assert lat.lib().lattice_set_measure_path(b._h, 2) == 0
+    M, Q, Sx, Sy = b.measure(130)
+    for k in range(3):
+        o = oracle.OracleLattice(1024, lat.ISING, 0.0, 5 + k)
+        o.sweep([workloads.BETA_C_ISING] * 6)
+        Mo, Qo, Sxo, Syo = o.measure(130)
+        assert (M[k], Q[k]) == (Mo, Qo) and np.array_equal(Sx[k], Sxo) and np.array_equal(Sy[k], Syo)
+        o.close()
+    b.close()

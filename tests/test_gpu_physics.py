@@ -118,3 +118,77 @@ def test_config5_protocol2_whole_runs(name, e_plateau):
         assert late.mean() > -math.sqrt(2) + 0.03                   # T > T_c: above E_eq(T_c)
     assert all(abs(r["m"]) < 0.01 for r in recs)
     assert 30 < by_t[20000]["xi"] < 250 and by_t[20000]["r_cut"] < w.r_max
+
+
+def test_paper_two_step_protocol_energy_and_coherence_length():
+    """The paper's protocol 2 actually run (Table II): Ising,
+    T_1 = 1.66 until t_switch in {3746, 4467, 5312} (f = 0.54, 0.59, 0.64), then T_2 = 2.27414861561203,
+    against the direct quench to T_2 (f = 0) -- 16 replicas of L = 2^14 per protocol as one batch
+    each (the paper: L = 2^16, 200 runs), to t = 2^15.  With E_eq(T_2) from Onsager's solution:
+
+    * the direct quench approaches E_eq monotonically from above (PAPER.md:96);
+    * the pre-cooled runs start far below E_eq and at t = 2^14 are ordered E(0.54) > E(0.59) > E(0.64),
+      the f = 0.64 run still clearly below E_eq at t = 2^15 (b(f) < 0 for f above 0.59)
+      while f = 0.54 has already reached it;
+    * pre-cooling equilibrates faster than the direct quench: at t = 2^14 the f = 0.54 run is several
+      times closer to E_eq, and at t = 2^15 the f = 0.59 run sits on E_eq;
+    * f is DEFINED by xi(t_switch; T_1) = f xi_eq(T_2), xi_eq(T_2) = 407(1): the
+      coherence length measured at the three switch times of Table II must be 0.54, 0.59, 0.64 x 407;
+      after the switch xi keeps growing towards xi_eq (it relaxes more slowly than the energy).
+    Sequences are seeded and the RNG is counter-based, so the numbers repeat exactly; the margins below
+    are >= 3 standard errors of the 16-replica mean (5e-5)."""
+    L, n_rep, t_end = 1 << 14, 16, 1 << 15
+    T1, T2 = 1.66, 2.27414861561203
+    e_eq = analysis.onsager_energy(1.0 / T2)
+    assert abs(e_eq + 1.3982449) < 1e-6
+    seeds = np.arange(n_rep, dtype=np.uint64) * 7919 + 2503146887
+    marks = [4096, 8192, 16384, 32768]
+    r_list = np.unique(np.round(np.geomspace(1, 4096, 96)).astype(np.uint32))
+    E, xi_sw, xi_late = {}, {}, None
+
+    def coherence_length(b):
+        import ctypes as Ct
+        C = np.zeros((n_rep, int(r_list[-1]) + 1))
+        for k in range(n_rep):
+            Sx = np.zeros(r_list.size, dtype=np.int64)
+            Sy = np.zeros(r_list.size, dtype=np.int64)
+            Mv, Qv = Ct.c_int64(0), Ct.c_int64(0)
+            rc = lat.lib().lattice_measure_list(b._replica(k), 0, L, r_list.ctypes.data_as(Ct.POINTER(Ct.c_uint32)),
+                                                r_list.size, Ct.byref(Mv), Ct.byref(Qv),
+                                                Sx.ctypes.data_as(Ct.POINTER(Ct.c_int64)),
+                                                Sy.ctypes.data_as(Ct.POINTER(Ct.c_int64)))
+            assert rc == 0
+            C[k], _ = analysis.densify(r_list.astype(np.float64), (Sx + Sy) / (2.0 * L * L))
+        return analysis.xi_with_error(C)
+
+    for f, t_sw in ((0.0, 0), (0.54, 3746), (0.59, 4467), (0.64, 5312)):
+        b = lat.LatticeBatch(L, seeds)
+        E[f] = {}
+        for t in sorted(set(marks) | ({t_sw} if t_sw else set())):
+            b.sweep(np.where(np.arange(b.time, t) < t_sw, 1.0 / T1, 1.0 / T2))
+            M, Q, Sx, Sy = b.measure(1)
+            e = -(Sx[:, 0] + Sy[:, 0]) / float(L * L)
+            E[f][t] = (float(e.mean()) - e_eq, float(e.std(ddof=1) / math.sqrt(n_rep)))
+            if t == t_sw and t_sw:
+                xi_sw[f] = coherence_length(b)
+        if f == 0.59:
+            xi_late = coherence_length(b)
+        b.close()
+    for f in E:
+        assert all(s < 1.2e-4 for _, s in E[f].values()), (f, E[f])
+    # direct quench: from above, monotonically
+    q = [E[0.0][t][0] for t in marks]
+    assert q[0] > q[1] > q[2] > q[3] > -1.5e-4 and q[2] > 3e-4
+    # pre-cooled: far below E_eq at the switch, ordered by f afterwards, f = 0.64 approaches from below
+    assert E[0.59][4467][0] < -0.4 and E[0.64][5312][0] < -0.4 and E[0.54][3746][0] < -0.4
+    assert E[0.54][16384][0] > E[0.59][16384][0] + 1e-4 > E[0.64][16384][0] + 2e-4
+    assert E[0.64][16384][0] < -3e-4 and E[0.64][32768][0] < -0.5e-4
+    assert abs(E[0.54][32768][0]) < 1.5e-4 and abs(E[0.59][32768][0]) < 1.5e-4
+    # the speed-up: pre-cooling is closer to equilibrium than the direct quench at the same time
+    assert abs(E[0.54][16384][0]) < 0.4 * q[2] and abs(E[0.59][32768][0]) < q[3]
+    for f in (0.54, 0.59, 0.64):
+        xi, xi_err = xi_sw[f]
+        assert abs(xi / 407.0 - f) < 0.04 and xi_err < 12.0, (f, xi, xi_err)
+    assert xi_sw[0.54][0] < xi_sw[0.59][0] < xi_sw[0.64][0]
+    xi, xi_err = xi_late
+    assert xi_sw[0.59][0] + 20.0 < xi < 450.0 and xi_err < 30.0, (xi, xi_err)
