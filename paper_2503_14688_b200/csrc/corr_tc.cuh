@@ -13,10 +13,10 @@
 // One CTA per SM, persistent over work items (tile of 128 base positions, pass of 512 partner
 // positions starting at the tile's first position + 512 * pass).  Per item the whole lattice extent
 // along the contraction axis streams through a 2-stage shared-memory ring:
-//   * 8 producer warps read the packed words (1 or 2 bits per spin), expand them to fp8 bytes and
+//   * 20 producer warps read the packed words (1 or 2 bits per spin), expand them to fp8 bytes and
 //     write them into the canonical 128-byte-swizzled UMMA layout (K-major for the y axis, where the
 //     contraction runs along a row; MN-major for the x axis, where it runs across rows);
-//   * one thread of a 9th warp issues 8 tcgen05.mma per stage (4 K-steps x 2 N-tiles of 256) into
+//   * one thread of a 21st warp issues 8 tcgen05.mma per stage (4 K-steps x 2 N-tiles of 256) into
 //     two 128 x 256 fp32 accumulators that fill the 512 TMEM columns, and commits to the stage's
 //     "empty" mbarrier;
 //   * after the last stage warps 0-3 read the accumulators back (tcgen05.ld, lane = base position)
@@ -35,7 +35,7 @@ constexpr int TC_N = 256;            // partner positions per MMA
 constexpr int TC_NT = 2;             // N tiles per item (TC_NT * TC_N = 512 TMEM columns)
 constexpr int TC_KC = 128;           // contraction positions per stage (one 128-byte swizzle row)
 constexpr int TC_STAGES = 2;
-constexpr int TC_PRODUCERS = 256;    // producer threads (warps 0-7); warp 8 issues the MMAs
+constexpr int TC_PRODUCERS = 640;    // producer threads (warps 0-19: 2 chunks of 64 bytes each per stage); warp 20 issues the MMAs
 constexpr int TC_THREADS = TC_PRODUCERS + 32;
 constexpr int TC_STAGE_BYTES = (TC_M + TC_NT * TC_N) * TC_KC;            // 80 KiB
 constexpr int TC_HIST = TC_NT * TC_N + TC_M;                             // r - 512 pass + 127 in [0, 639)
@@ -180,64 +180,96 @@ __global__ void __launch_bounds__(TC_THREADS, 1) corr_tc_kernel(const CorrTCArgs
         const uint32_t p0 = (AXIS == 1 ? a.i0 : 0u) + tile * TC_M;
         if (warp < TC_PRODUCERS / 32) {
             // ===== producers =====
+            // A stage is (128 + 512) x 2 chunks of 64 bytes; thread t owns chunks t, t + 256, ...
+            // (TC_PER_THREAD of them) for the whole item: source pointer, shared-memory offset and
+            // the contraction step at which its lattice row leaves the base rows are fixed per item.
+            constexpr int TC_PER_THREAD = (TC_M + TC_NT * TC_N) * 2 / TC_PRODUCERS;      // 5
+            const uint32_t *src[TC_PER_THREAD];
+            uint32_t dst[TC_PER_THREAD], xr[TC_PER_THREAD], kc_zero[TC_PER_THREAD];
+#pragma unroll
+            for (int q = 0; q < TC_PER_THREAD; ++q) {
+                const uint32_t it = threadIdx.x + (uint32_t)q * TC_PRODUCERS;
+                uint32_t h, srow, blk, row_l, word;          // half, smem row, block, lattice row, word in row
+                kc_zero[q] = 0xffffffffu;                    // first contraction step that is all zeros
+                if (AXIS == 1) {
+                    const uint32_t tr = it >> 1;              // 0..127 base rows, 128..639 partner rows
+                    h = it & 1u;
+                    blk = tr < TC_M ? 0u : 1u + (tr - TC_M) / TC_N;
+                    srow = tr < TC_M ? tr : (tr - TC_M) % TC_N;
+                    uint32_t i;
+                    if (tr < TC_M) { i = p0 + tr; if (i >= a.i0 + a.n_rows) kc_zero[q] = 0u; }
+                    else i = p0 + pass * (TC_NT * TC_N) + (tr - TC_M);
+                    row_l = i % a.rows;
+                    word = 0u;                                // + 2 words (64 packed positions) per step
+                } else {
+                    // smem row = contraction index (lattice row), 128-column blocks along MN:
+                    // block 0 = base columns, blocks 1..4 = the pass's partner columns; the second
+                    // 128-column block of an N tile sits TC_KC rows (16 KiB) further (MN-major LBO)
+                    const uint32_t kk = it % TC_KC, rest = it / TC_KC;
+                    h = rest & 1u;
+                    const uint32_t mb = rest >> 1;            // 0..4
+                    blk = mb == 0 ? 0u : 1u + (mb - 1u) / 2u;
+                    srow = kk + ((mb == 0 ? 0u : (mb - 1u) & 1u) * TC_KC);
+                    row_l = a.i0 + kk;                        // + TC_KC rows per step; never wraps
+                    kc_zero[q] = kk < a.n_rows ? (a.n_rows - kk + TC_KC - 1) / TC_KC : 0u;
+                    const uint32_t col0 = mb == 0 ? p0 : (p0 + pass * (TC_NT * TC_N) + (mb - 1u) * TC_M) % a.L;
+                    word = col0 / 64u;                        // 128 columns = 64 packed positions = 2 words
+                }
+                const uint32_t c = (row_l & 1u) ^ h;          // even columns of row i live in colour i & 1
+                src[q] = a.buf + (MODEL == 0 ? (size_t)c * pw : (size_t)(2u * c) * pw) + (size_t)row_l * a.wpr + word;
+                // canonical 128-byte swizzle: 8-row atoms of 1 KiB, 16-byte chunk index ^ (row & 7)
+                dst[q] = (blk == 0 ? 0u : TC_M * TC_KC + (blk - 1u) * (TC_N * TC_KC)) + (srow >> 3) * 1024u + (srow & 7u) * 128u;
+                xr[q] = (srow & 7u) | (h << 2 << 8);          // low byte: row & 7, bits 8..: first chunk h * 4
+            }
+            const size_t step = AXIS == 1 ? 2u : (size_t)TC_KC * a.wpr;      // words per contraction step
+            // words of step kc (w) and kc + 1 (wn) in registers; the loads of step kc + 2 are issued at
+            // the END of step kc, after the proxy fence (which would otherwise wait for them), and are
+            // in flight during all of step kc + 1
+            uint2 w[TC_PER_THREAD], sgn[TC_PER_THREAD], wn[TC_PER_THREAD], sn[TC_PER_THREAD];
+#pragma unroll
+            for (int q = 0; q < TC_PER_THREAD; ++q) {
+                w[q] = sgn[q] = wn[q] = sn[q] = make_uint2(0u, 0u);
+                if (kc_zero[q] > 0u) {
+                    w[q] = *reinterpret_cast<const uint2 *>(src[q]);
+                    if (MODEL) sgn[q] = *reinterpret_cast<const uint2 *>(src[q] + pw);
+                }
+                if (n_kc > 1u && kc_zero[q] > 1u) {
+                    wn[q] = *reinterpret_cast<const uint2 *>(src[q] + step);
+                    if (MODEL) sn[q] = *reinterpret_cast<const uint2 *>(src[q] + step + pw);
+                }
+            }
             for (uint32_t kc = 0; kc < n_kc; ++kc) {
                 mbar_wait(empty0 + 8 * stage, phase ^ 1u);
-                uint8_t *st = smem + (size_t)stage * TC_STAGE_BYTES;
-#pragma unroll 1
-                for (uint32_t it = threadIdx.x; it < (TC_M + TC_NT * TC_N) * 2; it += TC_PRODUCERS) {
-                    // item = 64 bytes: one half (even / odd columns) of one 128-byte smem row
-                    uint32_t h, srow, blk, row_l, word;      // half, smem row in block, block, lattice row, word in row
-                    bool zero = false;
-                    if (AXIS == 1) {
-                        const uint32_t tr = it >> 1;          // 0..127 base rows, 128..639 partner rows
-                        h = it & 1u;
-                        blk = tr < TC_M ? 0u : 1u + (tr - TC_M) / TC_N;
-                        srow = tr < TC_M ? tr : (tr - TC_M) % TC_N;
-                        uint32_t i;
-                        if (tr < TC_M) { i = p0 + tr; zero = i >= a.i0 + a.n_rows; }
-                        else i = p0 + pass * (TC_NT * TC_N) + (tr - TC_M);
-                        row_l = i % a.rows;
-                        word = kc * 2u;                       // 64 packed positions = 2 words per colour
-                    } else {
-                        // smem row = contraction index (lattice row), 128-column blocks along MN:
-                        // block 0 = base columns, blocks 1..4 = the pass's partner columns
-                        const uint32_t kk = it % TC_KC, rest = it / TC_KC;
-                        h = rest & 1u;
-                        const uint32_t mb = rest >> 1;        // 0..4
-                        blk = mb == 0 ? 0u : 1u + (mb - 1u) / 2u;
-                        const uint32_t i = a.i0 + kc * TC_KC + kk;
-                        zero = i >= a.i0 + a.n_rows;
-                        row_l = i % a.rows;
-                        const uint32_t col0 = mb == 0 ? p0 : (p0 + pass * (TC_NT * TC_N) + (mb - 1u) * TC_M) % a.L;
-                        word = col0 / 64u;                    // 128 columns = 64 packed positions = 2 words
-                        // MN-major: 128-column block mb of the N tile sits TC_KC * 128 bytes further
-                        srow = kk + ((mb == 0 ? 0u : (mb - 1u) & 1u) * TC_KC);
-                    }
-                    const uint32_t c = (row_l & 1u) ^ h;      // even columns of row i live in colour i & 1
+                const uint32_t st = smem_u32(smem) + stage * TC_STAGE_BYTES;
+#pragma unroll
+                for (int q = 0; q < TC_PER_THREAD; ++q) {
                     uint4 o[4];
-                    if (zero) {
+                    if (kc >= kc_zero[q]) {
                         o[0] = o[1] = o[2] = o[3] = make_uint4(0u, 0u, 0u, 0u);
                     } else {
-                        const size_t off = (size_t)row_l * a.wpr + word;
-                        const uint32_t *p = a.buf + (MODEL == 0 ? (size_t)c * pw : (size_t)(2u * c) * pw) + off;
-                        const uint2 w = *reinterpret_cast<const uint2 *>(p);
-                        uint2 s = make_uint2(0u, 0u);
-                        if (MODEL) s = *reinterpret_cast<const uint2 *>(p + pw);
-                        expand_word<MODEL>(w.x, s.x, o[0], o[1]);
-                        expand_word<MODEL>(w.y, s.y, o[2], o[3]);
+                        expand_word<MODEL>(w[q].x, sgn[q].x, o[0], o[1]);
+                        expand_word<MODEL>(w[q].y, sgn[q].y, o[2], o[3]);
                     }
-                    // canonical 128-byte swizzle: 8-row atoms of 1 KiB, 16-byte chunk index ^ (row & 7)
-                    uint8_t *base = st + (blk == 0 ? 0 : TC_M * TC_KC + (blk - 1u) * (TC_N * TC_KC)) +
-                                    (size_t)(srow >> 3) * 1024u + (srow & 7u) * 128u;
+                    const uint32_t r7 = xr[q] & 7u, c0 = xr[q] >> 8;
 #pragma unroll
-                    for (int q = 0; q < 4; ++q)
-                        *reinterpret_cast<uint4 *>(base + (((h * 4u + q) ^ (srow & 7u)) << 4)) = o[q];
+                    for (int e = 0; e < 4; ++e)
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + dst[q] + (((c0 + (uint32_t)e) ^ r7) << 4)),
+                                     "r"(o[e].x), "r"(o[e].y), "r"(o[e].z), "r"(o[e].w) : "memory");
                 }
                 fence_proxy_async();                          // generic-proxy writes -> visible to the tensor core
-                fence_before_sync();                          // (and the previous item's tcgen05.ld are done)
                 __syncwarp();
                 if (lane == 0) mbar_arrive(full0 + 8 * stage);
                 if (++stage == TC_STAGES) { stage = 0; phase ^= 1u; }
+#pragma unroll
+                for (int q = 0; q < TC_PER_THREAD; ++q) {
+                    w[q] = wn[q];
+                    sgn[q] = sn[q];
+                    wn[q] = sn[q] = make_uint2(0u, 0u);
+                    if (kc + 2 < n_kc && kc + 2 < kc_zero[q]) {
+                        wn[q] = *reinterpret_cast<const uint2 *>(src[q] + (size_t)(kc + 2) * step);
+                        if (MODEL) sn[q] = *reinterpret_cast<const uint2 *>(src[q] + (size_t)(kc + 2) * step + pw);
+                    }
+                }
             }
             // ===== epilogue (warps 0-3: TMEM lane quarter = warp) =====
             if (warp < 4) {
