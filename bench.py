@@ -438,9 +438,11 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
     if measure_pass and rank == 0:
         r_meas = w.r_max if args.measure_rmax < 0 else args.measure_rmax
         r_meas = max(1, min(r_meas, L // 2))
-        # ~3e12 (word, r) pairs/s per axis (profiles/): bound the default run to a few seconds
+        # the tensor-core path (csrc/corr_tc.cuh) does C(r <= 4096) at L = 2^20 in ~12 s: the default run
+        # measures the workload's full r_max; only where that path does not apply (L < 4096) and the
+        # XOR/popcount kernels would take long is r_max bounded (an explicit --measure-rmax is honoured)
         words = L * L // 32
-        if args.measure_rmax < 0 and words * r_meas > 1 << 42:     # an explicit --measure-rmax is honoured
+        if args.measure_rmax < 0 and L < 4096 and words * r_meas > 1 << 42:
             r_meas = max(1, (1 << 42) // words)
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record(g.stream)
@@ -448,8 +450,21 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
         ev1.record(g.stream)
         torch.cuda.synchronize(dev)
         xi_v, r_cut = lat.xi(Sx, Sy, Q, L)
+        sparse = None
+        if args.measure_list > 0:
+            # the paper's sparse sampling in r: log-spaced separations up to r_meas
+            rl = sorted({max(1, int(round(r_meas ** (k / max(args.measure_list - 1, 1))))) for k in range(args.measure_list)})
+            ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ev2.record(g.stream)
+            Ml, Ql, Sxl, Syl = g.measure_list(rl)
+            ev3.record(g.stream)
+            torch.cuda.synchronize(dev)
+            same = all(int(Sxl[k]) == int(Sx[r - 1]) and int(Syl[k]) == int(Sy[r - 1]) for k, r in enumerate(rl))
+            sparse = {"points": len(rl), "r_last": rl[-1], "ms": ev2.elapsed_time(ev3), "equals_dense": bool(same and Ml == M)}
         meas = {"r_max": r_meas, "ms": ev0.elapsed_time(ev1), "t": g.time, "M": M,
-                "e": lat.energy(Sx, Sy, Q, w.delta, L), "xi": xi_v, "r_cut": r_cut}
+                "path": "tensor cores (tcgen05 banded Gram, csrc/corr_tc.cuh)" if (L >= 4096 and r_meas >= 48)
+                        else "XOR/popcount kernels (csrc/measure.cuh)",
+                "e": lat.energy(Sx, Sy, Q, w.delta, L), "xi": xi_v, "r_cut": r_cut, "sparse_list": sparse}
     # ---- worst-case input: the all-up state (every site has 4 aligned neighbours, so every
     # lane needs a random decision and ties are ~3x more frequent than after the quench) ----------
     worst = None
@@ -601,6 +616,8 @@ def main():
                     help="skip the batched-replica workloads the default invocation also times")
     ap.add_argument("--measure-rmax", type=int, default=-1,
                     help="r_max of the separately timed measurement pass (-1: the workload's)")
+    ap.add_argument("--measure-list", type=int, default=64,
+                    help="also time lattice_measure_list on this many log-spaced separations (0: skip)")
     ap.add_argument("--sharded", action="store_true",
                     help="N > 1: ONE lattice in row slabs over the ranks (strong scaling, fused halo "
                          "mirroring over peer memory) instead of independent replicas")
