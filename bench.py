@@ -614,6 +614,8 @@ def main():
                     help="skip the Blume-Capel workloads the default invocation also times")
     ap.add_argument("--no-batches", action="store_true",
                     help="skip the batched-replica workloads the default invocation also times")
+    ap.add_argument("--batches-only", action="store_true",
+                    help="time only the batched-replica workloads (profiling aid: prints their JSON object)")
     ap.add_argument("--measure-rmax", type=int, default=-1,
                     help="r_max of the separately timed measurement pass (-1: the workload's)")
     ap.add_argument("--measure-list", type=int, default=64,
@@ -647,6 +649,12 @@ def main():
         else:
             dist.init_process_group("gloo")
     cdev = dev if args.dist_backend == "nccl" else "cpu"   # where the plumbing tensors live
+
+    if args.batches_only:
+        out = {name: bench_batch(name, Lb, nb, args, lat, torch, dev)
+               for name, Lb, nb in (("ising_L4096_x64", 4096, 64), ("ising_L64_x4096", 64, 4096))}
+        print(json.dumps({"batched_replicas": out}))
+        return
 
     w = workloads.CONFIGS[args.workload]
     res = bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, measure_pass=True, worst_case=True)
