@@ -358,6 +358,8 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
     L = replicas.agree_min(L, cdev)             # all replicas use the same size
     g = lat.Lattice(L, w.model, w.delta, seed=replicas.replica_seed(w.seed, rank), scheme=args.scheme,
                     device=str(dev))
+    if args.no_persistent:
+        g.set_persist_blocks(0xffffffff)
     updates_per_sweep = L * L
     K, W = args.steps, args.warmup
 
@@ -528,7 +530,7 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
         "config": {"workload": w.name if L == w.L else f"{w.name}@L={L}", "model": MODEL_NAME[w.model],
                    "L": L, "spins": L * L, "state_bytes": state_bytes,
                    "beta": float(w.beta_schedule(1)[0]), "rng_scheme": args.scheme, "seed": w.seed,
-                   "sweeps_per_step": sps, "timed_seconds": ms / 1e3,
+                   "sweeps_per_step": sps, "timed_seconds": ms / 1e3, "persistent_kernel_allowed": not args.no_persistent,
                    "l2": "inputs_larger_than_l2" if not in_l2 else "l2_resident_by_design",
                    "parallelism": "replicas" if world > 1 else "single"},
         "clocks": clocks, "gpu_launches": int(launches),
@@ -614,6 +616,8 @@ def main():
                     help="skip the Blume-Capel workloads the default invocation also times")
     ap.add_argument("--no-batches", action="store_true",
                     help="skip the batched-replica workloads the default invocation also times")
+    ap.add_argument("--no-persistent", action="store_true",
+                    help="cache-resident lattices: two launches per sweep instead of the persistent multi-sweep kernel (A/B)")
     ap.add_argument("--batches-only", action="store_true",
                     help="time only the batched-replica workloads (profiling aid: prints their JSON object)")
     ap.add_argument("--measure-rmax", type=int, default=-1,

@@ -247,10 +247,16 @@ int lattice_plane_case_specialised(int model, double delta, double beta);
  * representable; fp32 accumulators hold exact integers up to 2^24 > L); both paths return the same
  * exact integer counts. */
 int lattice_set_measure_path(lattice_t *lat, int path);
-/* Tuning / test knob: upper bound on the grid of the persistent multi-sweep kernel that
- * lattice_sweep(n >= 2) uses for cache-resident Ising lattices (0 = the occupancy limit, the
- * default).  With fewer blocks than 256-thread groups of work every block strides over several
- * groups per half-sweep; results do not depend on it.  EINVAL for a NULL handle. */
+/* The persistent multi-sweep kernels: lattice_sweep(n >= 2) on a
+ * cache-resident lattice can run all n sweeps in ONE cooperative launch with a grid barrier per
+ * half-sweep.  max_blocks selects when:
+ *   0 (default)   automatic: only where it is measured faster than two launches per sweep, i.e. Ising
+ *                 lattices with L <= 4352;
+ *   1..2^32-2     on request, for any Ising lattice with L <= 16384 and any Blume-Capel lattice with
+ *                 L <= 16384 and Delta = 0 type threshold tables, with at most max_blocks blocks (fewer
+ *                 blocks than 256-thread groups of work: every block strides over several groups);
+ *   UINT32_MAX    never (two launches per sweep, as for n == 1).
+ * Results do not depend on it.  EINVAL for a NULL handle. */
 int lattice_set_persist_blocks(lattice_t *lat, uint32_t max_blocks);
 
 /* Host-only helpers (no device work).

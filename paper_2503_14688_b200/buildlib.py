@@ -11,7 +11,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_PKG)
 SO_PATH = os.path.join(_PKG, "liblattice.so")
 SOURCES = [os.path.join(_PKG, "csrc", "lattice.cu")]
-HEADERS = [os.path.join(_PKG, "csrc", n) for n in ("philox.cuh", "ising.cuh", "ising_march.cuh", "ising_persist.cuh", "ising_batch.cuh", "bc.cuh", "bc_march.cuh", "measure.cuh", "corr_tc.cuh", "ubench.cuh")]
+HEADERS = sorted(os.path.join(_PKG, "csrc", n) for n in os.listdir(os.path.join(_PKG, "csrc")) if n.endswith(".cuh"))
 HEADERS.append(os.path.join(_ROOT, "include", "lattice.h"))
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",

@@ -55,6 +55,11 @@ struct BCMarchArgs {
     uint32_t fbp;                   // folded counter word of the PROP plane
     PlaneFold F;                    // folded ACC_PLANE stream of (t, colour)
     RoundKeys K;
+#ifdef __CUDACC__
+    // truth table of plane k (a runtime index: a kernel parameter is read from the constant bank;
+    // bc_persist.cuh overrides this with a shared-memory read)
+    __device__ __forceinline__ uint32_t lut_k(int k) const { return lut[k]; }
+#endif
 };
 
 // out[w] = f(a[w], b[w], c[w]), w = 0..3, with f given by the runtime truth table `lut` (LOP3
@@ -181,8 +186,8 @@ __device__ __forceinline__ void bcm_load(const uint32_t *nzp, const uint32_t *sg
 // One row of one 128-bit run.  PAR == 0: side neighbour at p-1 (En, Es = word before the run),
 // PAR == 1: at p+1 (word after it).  Stores the updated words (ties treated as rejections) and
 // queues the ties.
-template <int PAR, bool SLAB>
-__device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, unsigned long long wo,
+template <int PAR, bool SLAB, class Args>
+__device__ __forceinline__ void bc_march_row(const Args &a, uint32_t G, unsigned long long wo,
                                              uint32_t *tn, uint32_t *ts,
                                              const BCRow &U, const BCRow &C, const BCRow &D,
                                              uint32_t En, uint32_t Es, BCTieQueue<SLAB> &queue,
@@ -246,7 +251,7 @@ __device__ __forceinline__ void bc_march_row(const BCMarchArgs &a, uint32_t G, u
         const uint4 b4 = plane_block(ps, a.F.fb[0] ^ ((uint32_t)k << 16), a.F, a.K);
         const uint32_t b[4] = {b4.x, b4.y, b4.z, b4.w};
         uint32_t tau[4];
-        lut3_dispatch(a.lut[k], Fm, Y1, H0, tau);
+        lut3_dispatch(a.lut_k(k), Fm, Y1, H0, tau);
 #pragma unroll
         for (int w = 0; w < 4; ++w) {
             acc[w] = maj3m(tau[w], ~b[w], acc[w]);
@@ -445,8 +450,8 @@ __device__ __forceinline__ void bc_march_row_gen(const BCMarchArgs &a, uint32_t 
 }
 
 // GEN = false: the integer-dE (Delta = 0 type) rows above; GEN = true: bc_march_row_gen
-template <bool GEN, int PAR, bool SLAB, class Queue>
-__device__ __forceinline__ void bc_row(const BCMarchArgs &a, uint32_t G, unsigned long long wo, uint32_t *tn,
+template <bool GEN, int PAR, bool SLAB, class Args, class Queue>
+__device__ __forceinline__ void bc_row(const Args &a, uint32_t G, unsigned long long wo, uint32_t *tn,
                                        uint32_t *ts, const BCRow &U, const BCRow &C, const BCRow &D, uint32_t En,
                                        uint32_t Es, Queue &queue, uint32_t *mir_nz = nullptr,
                                        uint32_t *mir_sg = nullptr, uint32_t mir_tag = 0)
@@ -460,17 +465,11 @@ struct BCQueueOf { using type = BCTieQueue<SLAB>; };
 template <bool SLAB>
 struct BCQueueOf<true, SLAB> { using type = BCTieQueueGen<SLAB>; };
 
-template <int COLOUR, bool SLAB, bool GEN = false>
-__global__ void __launch_bounds__(256, GEN ? 2 : 3) bc_march_kernel(const BCMarchArgs a)
+// The march of one thread: rows i0 .. i0+R-1 of run q, g = s * (wpr/4) + q (ties are queued, not
+// drained) -- shared by bc_march_kernel and bc_persist_kernel (bc_persist.cuh).
+template <int COLOUR, bool SLAB, bool GEN, class Args, class Queue>
+__device__ __forceinline__ void bc_march_thread(const Args &a, uint32_t g, Queue &queue)
 {
-    // the general queue (3 x 16 bytes per entry, 60 KiB per block) exceeds the static limit: dynamic
-    extern __shared__ uint4 s_dyn[];
-    __shared__ uint4 s_fix[GEN ? 1 : 8][GEN ? 1 : 2 * TIE_Q_SLOTS];
-    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t g = blockIdx.x * 256u + threadIdx.x;
-    if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
-    typename BCQueueOf<GEN, SLAB>::type queue{a, GEN ? s_dyn + warp * (3 * TIE_Q_SLOTS) : s_fix[GEN ? 0 : warp], lane, 0u};
-
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
     const uint32_t q = g % nq, s = g / nq;
     const uint32_t kw = q << 2;
@@ -516,6 +515,19 @@ __global__ void __launch_bounds__(256, GEN ? 2 : 3) bc_march_kernel(const BCMarc
             U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
     }
+}
+
+template <int COLOUR, bool SLAB, bool GEN = false>
+__global__ void __launch_bounds__(256, GEN ? 2 : 3) bc_march_kernel(const BCMarchArgs a)
+{
+    // the general queue (3 x 16 bytes per entry, 60 KiB per block) exceeds the static limit: dynamic
+    extern __shared__ uint4 s_dyn[];
+    __shared__ uint4 s_fix[GEN ? 1 : 8][GEN ? 1 : 2 * TIE_Q_SLOTS];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t g = blockIdx.x * 256u + threadIdx.x;
+    if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
+    typename BCQueueOf<GEN, SLAB>::type queue{a, GEN ? s_dyn + warp * (3 * TIE_Q_SLOTS) : s_fix[GEN ? 0 : warp], lane, 0u};
+    bc_march_thread<COLOUR, SLAB, GEN>(a, g, queue);
     queue.drain();
 }
 

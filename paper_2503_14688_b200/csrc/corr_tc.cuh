@@ -23,8 +23,9 @@
 //     and add every element with 1 <= r <= r_max to a per-item histogram in shared memory, which is
 //     flushed to 64-bit global counters.
 // Within a 128-position block the byte order is [64 even columns | 64 odd columns] of the row for
-// the x axis (and the same split of the contraction index for the y axis): that is the order the
-// sublattice packing delivers, the same for both operands, and the epilogue undoes it.
+// the x axis (and the same split of the contraction index for the y axis), and within each 32-spin
+// word the order expand_word produces: that is the order the sublattice packing and the cheapest
+// bit -> byte expansion deliver, the same for both operands, and the epilogue undoes it.
 #pragma once
 #include <stdint.h>
 
@@ -104,28 +105,35 @@ __device__ __forceinline__ void umma_commit(uint32_t bar)
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
 
-// 4 spins (the low 4 bits of n) -> 4 fp8 bytes: bit = 1 -> +1.0 (0x38), bit = 0 -> -1.0 (0xB8).
-// n * 0x10204080 puts bit b at bit 8 b + 7 (no carries: the 16 partial products land on distinct bits).
-__device__ __forceinline__ uint32_t ising_bytes(uint32_t n)
+// 32 spins of word w (and sign plane s for Blume-Capel) -> 32 fp8 bytes, in the order
+//     byte 4 k + b  <->  bit 8 b + 7 - k of the word        (k = 0..7, b = 0..3)
+// (tc_spin_of_byte below): shifting the word left by k puts bits 7-k, 15-k, 23-k, 31-k at the top of
+// its four bytes, and one PRMT with the sign-replicating selector 0xBA98 spreads each of them over a
+// byte (0x00 / 0xFF).  Ising: +1.0 = 0x38 for a set bit, -1.0 = 0xB8 otherwise, i.e. 0xB8 ^ (m & 0x80):
+// per 4 bytes one shift (an IMAD on the FMA pipe), one PRMT and one LOP3.  Blume-Capel: nz ? (sg ? -1.0
+// : +1.0) : 0.0 = m_nz & (0x38 | (m_sg & 0x80)).  The order of the bytes within a word is the same for
+// both operands of the MMA, so a contraction along it is unaffected (y axis) and the epilogue undoes it
+// where the bytes are matrix rows / columns (x axis).
+__device__ __forceinline__ uint32_t sign_bytes(uint32_t x)
 {
-    return ((n * 0x10204080u) & 0x80808080u) ^ 0xB8B8B8B8u;
+    uint32_t m;
+    asm("prmt.b32 %0, %1, %1, 0xBA98;" : "=r"(m) : "r"(x));
+    return m;
 }
-// Blume-Capel: nz ? (sg ? -1.0 : +1.0) : 0.0
-__device__ __forceinline__ uint32_t bc_bytes(uint32_t nz, uint32_t sg)
+__host__ __device__ __forceinline__ uint32_t tc_spin_of_byte(uint32_t y)      // y = 0..31 -> bit of the word
 {
-    const uint32_t one = (nz * 0x00204081u) & 0x01010101u;               // bit b -> byte b, value 1
-    return one * 0x38u | (((nz & sg) * 0x10204080u) & 0x80808080u);
+    return 8u * (y & 3u) + 7u - (y >> 2);
 }
 
-// 32 spins of word w (and sign plane s for Blume-Capel) -> 32 bytes
 template <int MODEL>
 __device__ __forceinline__ void expand_word(uint32_t w, uint32_t s, uint4 &lo, uint4 &hi)
 {
     uint32_t o[8];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-        const uint32_t n = (w >> (4 * q)) & 0xFu;
-        o[q] = MODEL == 0 ? ising_bytes(n) : bc_bytes(n, (s >> (4 * q)) & 0xFu);
+    for (int k = 0; k < 8; ++k) {
+        const uint32_t m = sign_bytes(w << k);
+        if (MODEL == 0) o[k] = 0xB8B8B8B8u ^ (m & 0x80808080u);
+        else o[k] = m & (0x38383838u | (sign_bytes(s << k) & 0x80808080u));
     }
     lo = make_uint4(o[0], o[1], o[2], o[3]);
     hi = make_uint4(o[4], o[5], o[6], o[7]);
@@ -222,52 +230,58 @@ __global__ void __launch_bounds__(TC_THREADS, 1) corr_tc_kernel(const CorrTCArgs
                 xr[q] = (srow & 7u) | (h << 2 << 8);          // low byte: row & 7, bits 8..: first chunk h * 4
             }
             const size_t step = AXIS == 1 ? 2u : (size_t)TC_KC * a.wpr;      // words per contraction step
-            // words of step kc (w) and kc + 1 (wn) in registers; the loads of step kc + 2 are issued at
-            // the END of step kc, after the proxy fence (which would otherwise wait for them), and are
-            // in flight during all of step kc + 1
-            uint2 w[TC_PER_THREAD], sgn[TC_PER_THREAD], wn[TC_PER_THREAD], sn[TC_PER_THREAD];
+            // The packed words of the next TC_PF contraction steps live in registers (a ring indexed by
+            // kc % TC_PF, the loop unrolled by TC_PF so that the index is static): the loads of step
+            // kc + TC_PF are issued at the end of step kc, after the proxy fence (which would otherwise
+            // wait for them).  A producer iteration is a few hundred cycles of work, far less than a
+            // global-load latency under load: with a distance of one step (round 2's first version)
+            // 40 % of all stall samples sat on the first use of the loaded word.
+            constexpr int TC_PF = MODEL == 0 ? 4 : 3;
+            uint2 wb[TC_PF][TC_PER_THREAD], sb[TC_PF][TC_PER_THREAD];
 #pragma unroll
-            for (int q = 0; q < TC_PER_THREAD; ++q) {
-                w[q] = sgn[q] = wn[q] = sn[q] = make_uint2(0u, 0u);
-                if (kc_zero[q] > 0u) {
-                    w[q] = *reinterpret_cast<const uint2 *>(src[q]);
-                    if (MODEL) sgn[q] = *reinterpret_cast<const uint2 *>(src[q] + pw);
-                }
-                if (n_kc > 1u && kc_zero[q] > 1u) {
-                    wn[q] = *reinterpret_cast<const uint2 *>(src[q] + step);
-                    if (MODEL) sn[q] = *reinterpret_cast<const uint2 *>(src[q] + step + pw);
-                }
-            }
-            for (uint32_t kc = 0; kc < n_kc; ++kc) {
-                mbar_wait(empty0 + 8 * stage, phase ^ 1u);
-                const uint32_t st = smem_u32(smem) + stage * TC_STAGE_BYTES;
+            for (int u = 0; u < TC_PF; ++u)
 #pragma unroll
                 for (int q = 0; q < TC_PER_THREAD; ++q) {
-                    uint4 o[4];
-                    if (kc >= kc_zero[q]) {
-                        o[0] = o[1] = o[2] = o[3] = make_uint4(0u, 0u, 0u, 0u);
-                    } else {
-                        expand_word<MODEL>(w[q].x, sgn[q].x, o[0], o[1]);
-                        expand_word<MODEL>(w[q].y, sgn[q].y, o[2], o[3]);
+                    wb[u][q] = sb[u][q] = make_uint2(0u, 0u);
+                    if ((uint32_t)u < n_kc && (uint32_t)u < kc_zero[q]) {
+                        wb[u][q] = *reinterpret_cast<const uint2 *>(src[q] + (size_t)u * step);
+                        if (MODEL) sb[u][q] = *reinterpret_cast<const uint2 *>(src[q] + (size_t)u * step + pw);
                     }
-                    const uint32_t r7 = xr[q] & 7u, c0 = xr[q] >> 8;
-#pragma unroll
-                    for (int e = 0; e < 4; ++e)
-                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + dst[q] + (((c0 + (uint32_t)e) ^ r7) << 4)),
-                                     "r"(o[e].x), "r"(o[e].y), "r"(o[e].z), "r"(o[e].w) : "memory");
                 }
-                fence_proxy_async();                          // generic-proxy writes -> visible to the tensor core
-                __syncwarp();
-                if (lane == 0) mbar_arrive(full0 + 8 * stage);
-                if (++stage == TC_STAGES) { stage = 0; phase ^= 1u; }
+            for (uint32_t kc0 = 0; kc0 < n_kc; kc0 += TC_PF) {
 #pragma unroll
-                for (int q = 0; q < TC_PER_THREAD; ++q) {
-                    w[q] = wn[q];
-                    sgn[q] = sn[q];
-                    wn[q] = sn[q] = make_uint2(0u, 0u);
-                    if (kc + 2 < n_kc && kc + 2 < kc_zero[q]) {
-                        wn[q] = *reinterpret_cast<const uint2 *>(src[q] + (size_t)(kc + 2) * step);
-                        if (MODEL) sn[q] = *reinterpret_cast<const uint2 *>(src[q] + (size_t)(kc + 2) * step + pw);
+                for (int u = 0; u < TC_PF; ++u) {
+                    const uint32_t kc = kc0 + (uint32_t)u;
+                    if (kc >= n_kc) break;
+                    mbar_wait(empty0 + 8 * stage, phase ^ 1u);
+                    const uint32_t st = smem_u32(smem) + stage * TC_STAGE_BYTES;
+#pragma unroll
+                    for (int q = 0; q < TC_PER_THREAD; ++q) {
+                        uint4 o[4];
+                        if (kc >= kc_zero[q]) {
+                            o[0] = o[1] = o[2] = o[3] = make_uint4(0u, 0u, 0u, 0u);
+                        } else {
+                            expand_word<MODEL>(wb[u][q].x, sb[u][q].x, o[0], o[1]);
+                            expand_word<MODEL>(wb[u][q].y, sb[u][q].y, o[2], o[3]);
+                        }
+                        const uint32_t r7 = xr[q] & 7u, c0 = xr[q] >> 8;
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + dst[q] + (((c0 + (uint32_t)e) ^ r7) << 4)),
+                                         "r"(o[e].x), "r"(o[e].y), "r"(o[e].z), "r"(o[e].w) : "memory");
+                    }
+                    fence_proxy_async();                      // generic-proxy writes -> visible to the tensor core
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(full0 + 8 * stage);
+                    if (++stage == TC_STAGES) { stage = 0; phase ^= 1u; }
+                    const uint32_t nk = kc + (uint32_t)TC_PF;
+#pragma unroll
+                    for (int q = 0; q < TC_PER_THREAD; ++q) {
+                        wb[u][q] = sb[u][q] = make_uint2(0u, 0u);
+                        if (nk < n_kc && nk < kc_zero[q]) {
+                            wb[u][q] = *reinterpret_cast<const uint2 *>(src[q] + (size_t)nk * step);
+                            if (MODEL) sb[u][q] = *reinterpret_cast<const uint2 *>(src[q] + (size_t)nk * step + pw);
+                        }
                     }
                 }
             }
@@ -279,7 +293,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) corr_tc_kernel(const CorrTCArgs
                 fence_after_sync();
                 const uint32_t m = warp * 32u + lane;         // base position index in the tile
                 // position of byte index x inside a 128-block: [64 even | 64 odd] for the x axis
-                const int pm = AXIS == 1 ? (int)m : (int)(m < 64u ? 2u * m : 2u * (m - 64u) + 1u);
+                // (and inside each 32-byte group the byte order of expand_word)
+                const int pm = AXIS == 1 ? (int)m : (int)(2u * ((m & 32u) + tc_spin_of_byte(m & 31u)) + (m >> 6));
 #pragma unroll 1
                 for (uint32_t cb = 0; cb < (uint32_t)(TC_NT * TC_N); cb += 16u) {
                     uint32_t v[16];
@@ -297,7 +312,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) corr_tc_kernel(const CorrTCArgs
                         if (AXIS == 1) pn = (int)n;
                         else {
                             const uint32_t nb = n & 127u;
-                            pn = (int)((n & ~127u) + (nb < 64u ? 2u * nb : 2u * (nb - 64u) + 1u));
+                            pn = (int)((n & ~127u) + 2u * ((nb & 32u) + tc_spin_of_byte(nb & 31u)) + (nb >> 6));
                         }
                         const int d = pn - pm;                 // r - 512 pass, in (-128, 512)
                         const long long r = (long long)d + (long long)pass * (TC_NT * TC_N);

@@ -18,8 +18,9 @@
 //     inside the one launch with no barrier at all (lanes of a warp run in lock step).  BASELINE
 //     config 1 (L = 64, 2000 sweeps) is then one launch instead of 4000.
 //
-// Same arithmetic as ising_march.cuh (class masks, folded Philox planes, brx.idx plane compare);
-// ties are resolved in place (state lives in registers, so there is nothing to patch later).
+// Same arithmetic as ising_march.cuh (class masks, folded Philox planes, plane compare by brx.idx or
+// with the plane cases compiled in); in ising_tiny_kernel the lanes of a replica resolve its ties
+// together before the next half-sweep (state lives in registers, so there is nothing to patch later).
 #pragma once
 #include "ising_march.cuh"
 #include "ising_persist.cuh"
@@ -110,14 +111,30 @@ __global__ void __launch_bounds__(BLOCK_KERNEL_THREADS) ising_block_kernel(const
 // owns rows 4l .. 4l+3 of both colours (4 WPR words per colour).  With P = i (L/2) + p the RNG
 // unit is G = P >> 7: L = 64: G = i >> 2 = l (rows 4l..4l+3 are the block's words x, y, z, w);
 // L = 128: G = i >> 1 = 2l + u, u = 0, 1 (rows 4l+2u, 4l+2u+1: words (row even: 0, 1; odd: 2, 3)).
-template <int COLOUR, int WPR>
+// what PlaneLoop (ising_march.cuh) reads from its argument
+struct TinyPlaneView {
+    const PlaneFold &F;
+    const RoundKeys &K;
+    const uint32_t (&pcase)[8];
+};
+
+// Ties (top byte of u32 equal to the threshold's; 2^-8 per deciding lane) are resolved by the
+// replica's lanes TOGETHER: the words that hold ties are queued in shared memory (one ballot per
+// word, as in WarpTieQueue), then every lane takes one entry, evaluates the tail blocks of its tied
+// bits and leaves the accepted flips in a per-word buffer that the owner reads back.  A lane that
+// looped over its own ties alone would make the warp pay max-over-lanes(ties) tail blocks per
+// half-sweep (~2.5) instead of ~1.
+//   q    [LANES * NW] entries (tied lanes of the word, their dE = 8 mask, word offset, -)
+//   fbuf [LANES * NW] accepted flips per word of the replica's colour
+template <int COLOUR, int WPR, int PC>
 __device__ __forceinline__ void tiny_half_sweep(uint32_t (&T)[4 * WPR], const uint32_t (&O)[4 * WPR],
                                                 const RoundKeys &K, uint32_t t, const SweepParams &p,
-                                                uint32_t ln)
+                                                uint32_t ln, uint4 *q, uint32_t *fbuf)
 {
     constexpr uint32_t LANES = 16 * WPR;
     PlaneFold F;
     build_plane_fold(K, t, (uint32_t)COLOUR, TAG_ACC_PLANE, F);
+    const TinyPlaneView view{F, K, p.pcase};
     // opposite-colour rows 4l-1 (last row of the lane above) and 4l+4 (first row of the lane below)
     uint32_t up[WPR], dn[WPR];
 #pragma unroll
@@ -131,8 +148,8 @@ __device__ __forceinline__ void tiny_half_sweep(uint32_t (&T)[4 * WPR], const ui
     for (int u = 0; u < WPR; ++u) {
         uint32_t uc8[4], uacc[4], ueq[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int r = WPR == 1 ? q : 2 * u + (q >> 1), w = WPR == 1 ? 0 : (q & 1), x = r * WPR + w;
+        for (int qq = 0; qq < 4; ++qq) {
+            const int r = WPR == 1 ? qq : 2 * u + (qq >> 1), w = WPR == 1 ? 0 : (qq & 1), x = r * WPR + w;
             const uint32_t U = r == 0 ? up[w] : O[(r > 0 ? r - 1 : 0) * WPR + w];
             const uint32_t D = r == 3 ? dn[w] : O[(r < 3 ? r + 1 : 3) * WPR + w];
             const uint32_t C = O[x];
@@ -145,65 +162,79 @@ __device__ __forceinline__ void tiny_half_sweep(uint32_t (&T)[4 * WPR], const ui
             const uint32_t k4 = lop3<0x90>(nd, s1, S);               // k == 4
             // classes whose threshold is 2^32 flip unconditionally (masks are ~0 otherwise)
             need[x] = ((nd & ~k4) & p.mask4) | (k4 & p.mask8);
-            uc8[q] = k4 & p.mask8;
-            ueq[q] = need[x];
-            uacc[q] = 0;
+            uc8[qq] = k4 & p.mask8;
+            ueq[qq] = need[x];
+            uacc[qq] = 0;
         }
         const uint32_t G = WPR == 1 ? ln : 2u * ln + (uint32_t)u;
         const PlaneShared ps = plane_shared(G, F);
+        PlaneLoop<PC, 7>::run(view, ps, uc8, uacc, ueq);
 #pragma unroll
-        for (int k = 7; k >= 0; --k) {
-            const uint4 b4 = plane_block(ps, F.fb[0] ^ ((uint32_t)k << 16), F, K);
-            plane_compare(p.pcase[k], uc8, b4, uacc, ueq);
-        }
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int r = WPR == 1 ? q : 2 * u + (q >> 1), w = WPR == 1 ? 0 : (q & 1), x = r * WPR + w;
-            c8[x] = uc8[q]; acc[x] = uacc[q]; eq[x] = ueq[q];
+        for (int qq = 0; qq < 4; ++qq) {
+            const int r = WPR == 1 ? qq : 2 * u + (qq >> 1), w = WPR == 1 ? 0 : (qq & 1), x = r * WPR + w;
+            c8[x] = uc8[qq]; acc[x] = uacc[qq]; eq[x] = ueq[qq];
         }
     }
-    // Ties (top byte of u32 equal to the threshold's; 2^-8 per deciding lane): ONE loop over all
-    // words of the lane, so that the warp pays max-over-lanes(ties of the lane) tail blocks per
-    // half-sweep and not one divergent pass per word.
-    while (true) {
-        uint32_t m = eq[0];
-        int x = 0;
+    // ---- ties: queue the words (group = the LANES lanes of this replica), resolve together ----
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t gmask = WPR == 1 ? 0xffffu << (lane & 16u) : 0xffffffffu;
+    const uint32_t below = gmask & ((1u << lane) - 1u);
+    uint32_t pending = 0;
 #pragma unroll
-        for (int j = 1; j < NW; ++j)
-            if (m == 0) { m = eq[j]; x = j; }
-        if (m == 0) break;
-        const uint32_t bit = __ffs(m) - 1;
-        uint32_t cls = 0;
+    for (int x = 0; x < NW; ++x) {
+        const bool has = eq[x] != 0;
+        const uint32_t m = __ballot_sync(0xffffffffu, has) & gmask;
+        if (has) q[pending + __popc(m & below)] = make_uint4(eq[x], c8[x], ln * (uint32_t)NW + (uint32_t)x, 0u);
+        pending += __popc(m);
+    }
+    __syncwarp();
+    if (__any_sync(0xffffffffu, pending != 0u)) {
+        for (uint32_t base = 0; __any_sync(0xffffffffu, base < pending); base += LANES) {
+            const uint32_t idx = base + ln;
+            if (idx < pending) {
+                const uint4 e = q[idx];
+                uint32_t ties = e.x, flip = 0;
+                while (ties) {
+                    const uint32_t bit = __ffs(ties) - 1;
+                    ties &= ties - 1;
+                    const uint32_t P = (e.z << 5) + bit;             // word offset i * wpr + w = 4 ln WPR + x
+                    const uint4 blk = philox4x32_10(P, 0u, t, (uint32_t)COLOUR | (TAG_ACC_TAIL << 8), K);
+                    const unsigned long long thr = ((e.y >> bit) & 1u) ? p.thr8 : p.thr4;
+                    const unsigned long long u56 = ((unsigned long long)(blk.x >> 8) << 32) | blk.y;
+                    if (u56 < (thr & 0x00ffffffffffffffull)) flip |= 1u << bit;
+                }
+                fbuf[e.z] = flip;
+            }
+        }
+        __syncwarp();
 #pragma unroll
-        for (int j = 0; j < NW; ++j)
-            if (x == j) { cls = c8[j]; eq[j] = m & (m - 1); }
-        const uint32_t P = ((4u * ln * WPR + (uint32_t)x) << 5) + bit;       // word offset i * wpr + w = 4 ln WPR + x
-        const uint4 blk = philox4x32_10(P, 0u, t, (uint32_t)COLOUR | (TAG_ACC_TAIL << 8), K);
-        const unsigned long long thr = ((cls >> bit) & 1u) ? p.thr8 : p.thr4;
-        const unsigned long long u56 = ((unsigned long long)(blk.x >> 8) << 32) | blk.y;
-        const uint32_t hit = (u56 < (thr & 0x00ffffffffffffffull)) ? (1u << bit) : 0u;
-#pragma unroll
-        for (int j = 0; j < NW; ++j)
-            if (x == j) acc[j] |= hit;
+        for (int x = 0; x < NW; ++x)
+            if (eq[x]) acc[x] |= fbuf[ln * (uint32_t)NW + (uint32_t)x];
+        __syncwarp();                                            // before the next half-sweep reuses q / fbuf
     }
 #pragma unroll
     for (int x = 0; x < NW; ++x) T[x] = lop3<0x4B>(T[x], need[x], acc[x]);       // T ^ (~need | acc)
 }
 
 // resident blocks of 128 threads per SM: 4 (<= 128 registers) measured fastest for L = 64; L = 128
-// keeps twice the state per lane and would spill under that cap
-template <int WPR>
+// keeps twice the state per lane and would spill under that cap.  PC >= 0: every sweep of the call
+// has the packed plane cases PC (ising_march.cuh) compiled in.
+template <int WPR, int PC = -1>
 __global__ void __launch_bounds__(128, WPR == 1 ? 4 : 3) ising_tiny_kernel(uint32_t *buf, const RoundKeys *keys,
                                                          const SweepParams *sp, uint32_t n_rep,
                                                          uint32_t t0, uint32_t n_sweeps)
 {
     constexpr uint32_t L = 64 * WPR, LANES = 16 * WPR, NW = 4 * WPR;
+    __shared__ uint4 s_q[128 * NW];                           // [group][LANES * NW]
+    __shared__ uint32_t s_f[128 * NW];
     const uint32_t gt = blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t rep = gt / LANES, ln = gt % LANES;
     if ((gt & ~31u) / LANES >= n_rep) return;                 // the whole warp is past the last replica
     const bool live = rep < n_rep;                            // L = 64: a warp may hold one live half
     const uint32_t r_eff = live ? rep : n_rep - 1u;           // dead lanes shadow the last replica
     uint32_t *base = buf + (size_t)r_eff * (2u * L * WPR) + (size_t)(4u * ln) * WPR;
+    uint4 *q = s_q + (threadIdx.x / LANES) * (LANES * NW);
+    uint32_t *fbuf = s_f + (threadIdx.x / LANES) * (LANES * NW);
     const RoundKeys K = keys[r_eff];
     uint32_t s0[NW], s1[NW];                                  // colour 0 / 1, rows 4 ln .. 4 ln + 3
 #pragma unroll
@@ -216,8 +247,8 @@ __global__ void __launch_bounds__(128, WPR == 1 ? 4 : 3) ising_tiny_kernel(uint3
 #pragma unroll 1
     for (uint32_t sw = 0; sw < n_sweeps; ++sw) {
         const SweepParams p = sp[sw];
-        tiny_half_sweep<0, WPR>(s0, s1, K, t0 + sw, p, ln);   // black sees the old white
-        tiny_half_sweep<1, WPR>(s1, s0, K, t0 + sw, p, ln);   // white sees the new black
+        tiny_half_sweep<0, WPR, PC>(s0, s1, K, t0 + sw, p, ln, q, fbuf);   // black sees the old white
+        tiny_half_sweep<1, WPR, PC>(s1, s0, K, t0 + sw, p, ln, q, fbuf);   // white sees the new black
     }
     if (live) {
 #pragma unroll

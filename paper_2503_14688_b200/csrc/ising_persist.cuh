@@ -1,16 +1,21 @@
 // ising_persist.cuh -- many sweeps of a cache-resident Ising lattice in ONE cooperative kernel.
 //
-// SURVEY.md section 8(f) NEXT-4 ("persistent multi-sweep kernels for cache-resident sizes").  For
-// L <= 8192 a half-sweep is a few microseconds: the grid does not fill the GPU and the time is
-// the latency of one thread's rows plus the launch gap.  Measured gain over back-to-back launches
-// (512 sweeps per call): 1358 -> 1528 updates/ns at L = 4096, 340 -> 391 at 2048, 85 -> 99 at 1024,
-// 2724 -> 2764 at 8192: the row latency (~1.5 us per row, 2 rows per thread), not the launch,
-// dominates.  Here the grid is launched once (cudaLaunchCooperativeKernel, every block resident), loops over the
-// sweeps and colours itself and separates the half-sweeps with a grid-wide barrier; the lattice
-// stays in L2.  What is computed is exactly what n launches of ising_march_kernel compute: the
-// same march_thread() (or, for the smallest lattices, row_thread()) runs, with the per-half-sweep arguments (sweep index, colour, folded
-// Philox constants, thresholds) rebuilt in shared memory by one thread per block from a
-// per-sweep table the host uploads.
+// SURVEY.md section 8(f) NEXT-4 ("persistent multi-sweep kernels for cache-resident sizes").  The grid
+// is launched once (cudaLaunchCooperativeKernel, every block resident), loops over the sweeps and
+// colours itself and separates the half-sweeps with a grid-wide barrier; the lattice stays in L2.
+// What is computed is exactly what n launches of ising_march_kernel compute: the same march_thread()
+// (or, for the smallest lattices, row_thread()) runs, with the per-half-sweep arguments (sweep index,
+// colour, folded Philox constants, thresholds) rebuilt in shared memory by one thread per block from
+// a per-sweep table the host uploads.
+//
+// Measured (B200, updates/ns, persistent vs two launches per sweep, >= 2 s timed, round 2):
+//   L = 4096: 1650 vs 1366;  8192: 2090 vs 2732;  16384: 3733 vs 4091.
+// It wins where a half-sweep is a few microseconds and the launch gap shows (L <= 4352: one row per
+// thread, the whole lattice in flight at once); from L = 8192 on back-to-back launches overlap well,
+// while the persistent variant pays for its arguments living in registers instead of the constant
+// bank (108-127 registers against 63: half the resident warps) and for the grid barrier.  lattice_sweep
+// therefore takes this path by itself only for L <= 4352; larger lattices (L <= 16384) take it on
+// request (lattice_set_persist_blocks), which is what the parity tests of that variant do.
 #pragma once
 #include <cooperative_groups.h>
 
@@ -25,7 +30,9 @@ struct SweepParams {          // what changes from sweep to sweep (built on the 
 };
 
 #ifdef __CUDACC__
-template <bool EDGE, bool ONE_ROW>
+// PC >= 0: every sweep of the call has the packed plane cases PC (a constant-beta run at one of the
+// specialised temperatures, ising_march.cuh): the plane compare is compiled in as in the per-launch kernels.
+template <bool EDGE, bool ONE_ROW, int PC = -1>
 __global__ void __launch_bounds__(256) ising_persist_kernel(const IsingMarchArgs a0, uint32_t *buf0,
                                                             uint32_t *buf1, const SweepParams *sp,
                                                             uint32_t n_sweeps)
@@ -54,14 +61,25 @@ __global__ void __launch_bounds__(256) ising_persist_kernel(const IsingMarchArgs
                 build_plane_fold(a0.K, a.t, colour, TAG_ACC_PLANE, a.F);
             }
             __syncthreads();
-            WarpTieQueue<false> queue{a, s_q[warp], lane, 0u};
+            WarpTieQueue<false> queue{a, s_q[warp], lane, 0u};     // ties (rare) read the shared copy
+            // the marching code reads the launch-constant fields (shape, Philox round keys) from the
+            // kernel parameters, i.e. as constant-bank operands exactly like ising_march_kernel; only
+            // what changes per half-sweep comes from shared memory into registers
+            IsingMarchArgs al = a0;
+            al.tgt = a.tgt; al.opp = a.opp; al.t = a.t; al.colour = colour;
+            al.F.fa = a.F.fa; al.F.fh = a.F.fh; al.F.fl = a.F.fl; al.F.fb[0] = a.F.fb[0];
+            if (EDGE) { al.mask4 = a.mask4; al.mask8 = a.mask8; }
+            if (PC < 0) {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) al.pcase[k] = a.pcase[k];
+            }
             for (uint32_t g = blockIdx.x * 256u + threadIdx.x; g - lane < a0.threads; g += stride) {
                 if (ONE_ROW) {
-                    if (colour == 0) row_thread<0, EDGE>(a, g, queue);
-                    else row_thread<1, EDGE>(a, g, queue);
+                    if (colour == 0) row_thread<0, EDGE>(al, g, queue);
+                    else row_thread<1, EDGE>(al, g, queue);
                 } else {
-                    if (colour == 0) march_thread<0, EDGE, false>(a, g, queue);
-                    else march_thread<1, EDGE, false>(a, g, queue);
+                    if (colour == 0) march_thread<0, EDGE, false, PC>(al, g, queue);
+                    else march_thread<1, EDGE, false, PC>(al, g, queue);
                 }
             }
             queue.drain();

@@ -19,6 +19,7 @@
 #include "ising.cuh"
 #include "ising_march.cuh"
 #include "ising_persist.cuh"
+#include "bc_persist.cuh"
 #include "ising_batch.cuh"
 #include "measure.cuh"
 #include "corr_tc.cuh"
@@ -64,6 +65,9 @@ struct lattice {
     size_t sp_cap;             // entries
     int persist_blocks;        // co-resident blocks of ising_persist_kernel (0: not yet queried, -1: unavailable)
     uint32_t persist_cap;      // lattice_set_persist_blocks: upper bound on the grid (0: none)
+    bool persist_off;          // lattice_set_persist_blocks(UINT32_MAX): never take the persistent path
+    void *d_bsp;               // per-sweep parameters of bc_persist_kernel (BCSweepParams)
+    size_t bsp_cap;            // entries
     int measure_path;          // lattice_set_measure_path: 0 auto, 1 XOR/popcount kernels, 2 tensor cores
     // batch of independent replicas (lattice_create_batch): the batch handle owns one child handle
     // per replica (buf offset, own seed / round keys); a child has parent != nullptr
@@ -294,6 +298,23 @@ bool bc_table_is_integer_dE(const lattice *lat)
     return true;
 }
 
+// truth tables over the class bits (F, Y1, H0) of bc_march.cuh for the current thresholds: bit k of
+// the class's threshold (lut[k]), "always" (lut_always), and the 2^64-scale thresholds for ties
+void bc_fill_integer_dE_luts(const lattice *lat, uint32_t (&lut)[8], uint32_t &lut_always, unsigned long long (&thr)[8])
+{
+    for (int k = 0; k < 8; ++k) lut[k] = 0;
+    lut_always = 0;
+    for (int F = 0; F < 2; ++F)
+        for (int x = 1; x <= 4; ++x) {
+            const uint32_t cls = (uint32_t)(F << 2) | (uint32_t)((x >= 3) << 1) | (uint32_t)(x & 1);
+            const int e = bc_entry(F ? BC_FLIP : BC_VACATE, x);
+            thr[cls] = lat->thrT[e];
+            if (lat->alwT[e]) { lut_always |= 1u << cls; continue; }
+            for (int k = 0; k < 8; ++k)
+                if ((lat->thrT[e] >> (63 - k)) & 1u) lut[k] |= 1u << cls;
+        }
+}
+
 // bc_march_row_gen applies when x = -4 is "always" for vacate and occupy (|Delta| <= 4) and every
 // flip with x <= 0 is (dE = 2x <= 0: any Delta)
 bool bc_table_is_general_ok(const lattice *lat)
@@ -329,17 +350,7 @@ int launch_bc_march(lattice *lat, int colour, bool gen = false)
     a.mir_dn_sg = lat->slab ? lat->mir_dn[colour][1] : nullptr;
     a.R = march_rows(lat->n_own, nq);
     a.threads = nq * (lat->n_own / a.R);
-    for (int k = 0; k < 8; ++k) a.lut[k] = 0;
-    a.lut_always = 0;
-    for (int F = 0; F < 2; ++F)
-        for (int x = 1; x <= 4; ++x) {
-            const uint32_t cls = (uint32_t)(F << 2) | (uint32_t)((x >= 3) << 1) | (uint32_t)(x & 1);
-            const int e = bc_entry(F ? BC_FLIP : BC_VACATE, x);
-            a.thr[cls] = lat->thrT[e];
-            if (lat->alwT[e]) { a.lut_always |= 1u << cls; continue; }
-            for (int k = 0; k < 8; ++k)
-                if ((lat->thrT[e] >> (63 - k)) & 1u) a.lut[k] |= 1u << cls;
-        }
+    bc_fill_integer_dE_luts(lat, a.lut, a.lut_always, a.thr);
     // general crystal field: per move type an 8-entry table indexed by (hA, h1, h0) (bc_march.cuh)
     for (int k = 0; k < 8; ++k) a.lutA[k] = a.lutB[k] = 0;
     a.lutA_always = a.lutB_always = 0;
@@ -580,6 +591,7 @@ static void free_handle(lattice *lat)
     if (lat->d_win) cudaFree(lat->d_win);
     if (lat->d_rlist) cudaFree(lat->d_rlist);
     if (lat->d_sp) cudaFree(lat->d_sp);
+    if (lat->d_bsp) cudaFree(lat->d_bsp);
     if (lat->d_keys) cudaFree(lat->d_keys);
     if (lat->h_keys) std::free(lat->h_keys);
     if (lat->bk) std::free(lat->bk);
@@ -827,7 +839,7 @@ int lattice_half_sweep(lattice_t *lat, int colour, double beta)
 
 // Per-sweep parameters of the in-kernel sweep loops (ising_persist_kernel, ising_tiny_kernel): the
 // thresholds of beta[0..n) on the device, in lat->d_sp.  *edge: some sweep has an "always" class.
-static int upload_sweep_params(lattice *lat, uint64_t n, const double *beta, bool *edge)
+static int upload_sweep_params(lattice *lat, uint64_t n, const double *beta, bool *edge, int *pc_all = nullptr)
 {
     if (lat->sp_cap < n) {
         if (lat->d_sp) cudaFree(lat->d_sp);
@@ -850,6 +862,10 @@ static int upload_sweep_params(lattice *lat, uint64_t n, const double *beta, boo
         for (int q = 0; q < 8; ++q)
             p.pcase[q] = (uint32_t)((p.thr4 >> (63 - q)) & 1u) | ((uint32_t)((p.thr8 >> (63 - q)) & 1u) << 1);
         *edge = *edge || always4 || always8;
+        if (pc_all) {
+            const int pc = ising_packed_pc(p.pcase);
+            *pc_all = (k == 0 || *pc_all == pc) ? pc : -1;
+        }
     }
     // pageable source: the copy is staged before the call returns, so h can be freed right away
     const cudaError_t ce = cudaMemcpyAsync(lat->d_sp, h, n * sizeof(SweepParams), cudaMemcpyHostToDevice, lat->stream);
@@ -858,37 +874,118 @@ static int upload_sweep_params(lattice *lat, uint64_t n, const double *beta, boo
     return LATTICE_OK;
 }
 
-// Cache-resident Ising lattices: all n sweeps in one cooperative launch (ising_persist.cuh).
+// Largest lattice side the persistent multi-sweep kernels take: Ising 32 MiB, Blume-Capel 64 MiB
+// (BASELINE config 3), both inside the 126 MB L2.
+static const uint32_t PERSIST_MAX_L = 16384u;
+
+// Grid of a persistent kernel over `groups` groups of 256 threads: at most the co-resident blocks (and
+// the caller's cap), and among the grids with the same number of rounds per half-sweep the smallest,
+// so that every block strides over the same number of groups (444 blocks over 512 groups would leave
+// 376 of them idle in the second round).
+static unsigned persist_grid(const lattice *lat, unsigned groups)
+{
+    unsigned most = (unsigned)lat->persist_blocks;
+    if (lat->persist_cap && most > lat->persist_cap) most = lat->persist_cap;
+    if (groups <= most) return groups;
+    const unsigned rounds = (groups + most - 1u) / most;
+    return (groups + rounds - 1u) / rounds;
+}
+
+// Co-resident blocks of a cooperative kernel on the current device (0 if unavailable)
+static int coop_blocks(const void *fn)
+{
+    int dev = 0, coop = 0, sms = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 256, 0) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        return 0;
+    }
+    return per_sm * sms;
+}
+
+// Cache-resident Blume-Capel lattices with Delta = 0 type tables: all n sweeps in one cooperative
+// launch (bc_persist.cuh).  Returns 1 if the path does not apply.
+static int sweep_persistent_bc(lattice *lat, uint64_t n, const double *beta)
+{
+    if (lat->persist_blocks == 0) {
+        const int nb = coop_blocks((const void *)bc_persist_kernel);
+        lat->persist_blocks = nb > 0 ? nb : -1;
+    }
+    if (lat->persist_blocks < 0) return 1;
+    if (n > 16384) return 1;                     // the caller chunks; keeps the parameter table small
+    BCSweepParams *h = (BCSweepParams *)std::malloc(n * sizeof(BCSweepParams));
+    if (!h) return LATTICE_ENOMEM;
+    for (uint64_t k = 0; k < n; ++k) {
+        refresh_thresholds(lat, beta[k]);
+        if (!bc_table_is_integer_dE(lat)) { std::free(h); return 1; }
+        std::memset(&h[k], 0, sizeof h[k]);
+        bc_fill_integer_dE_luts(lat, h[k].lut, h[k].lut_always, h[k].thr);
+    }
+    if (lat->bsp_cap < n) {
+        if (lat->d_bsp) cudaFree(lat->d_bsp);
+        lat->d_bsp = nullptr; lat->bsp_cap = 0;
+        const size_t cap = n < 1024 ? 1024 : n;
+        if (cudaMalloc(&lat->d_bsp, cap * sizeof(BCSweepParams)) != cudaSuccess) { cudaGetLastError(); std::free(h); return LATTICE_ENOMEM; }
+        lat->bsp_cap = cap;
+    }
+    const cudaError_t ce = cudaMemcpyAsync(lat->d_bsp, h, n * sizeof(BCSweepParams), cudaMemcpyHostToDevice, lat->stream);
+    std::free(h);
+    if (ce != cudaSuccess) return cuda_fail(lat, ce, "sweep parameter upload");
+
+    const uint32_t L = lat->L, wpr = lat->wpr, nq = wpr / 4u;
+    BCMarchArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.L = L; a.wpr = wpr; a.t = (uint32_t)lat->t;
+    a.R = march_rows(L, nq);
+    a.threads = nq * (L / a.R);
+    a.share_v = 1;
+    a.K = lat->K;
+    uint32_t *buf = lat->buf;
+    const BCSweepParams *sp = (const BCSweepParams *)lat->d_bsp;
+    uint32_t ns = (uint32_t)n;
+    const unsigned blocks = persist_grid(lat, (a.threads + 255u) / 256u);
+    void *args[] = {&a, &buf, &sp, &ns};
+    const cudaError_t le = cudaLaunchCooperativeKernel((const void *)bc_persist_kernel, dim3(blocks), dim3(256), args, 0, lat->stream);
+    if (le != cudaSuccess) return cuda_fail(lat, le, "cudaLaunchCooperativeKernel");
+    lat->launches += 1;
+    lat->t += n;
+    return LATTICE_OK;
+}
+
+// Cache-resident lattices: all n sweeps in one cooperative launch (ising_persist.cuh, bc_persist.cuh).
 // Returns 1 if the path does not apply (the caller then launches the half-sweeps one by one).
 static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
 {
-    if (lat->model != LATTICE_ISING || lat->scheme < 1 || lat->slab || lat->view || lat->n_rep || (lat->wpr % 4u) != 0 ||
-        lat->L > 8192u || n < 2 || lat->persist_blocks < 0)
+    if (lat->scheme < 1 || lat->slab || lat->view || lat->n_rep || (lat->wpr % 4u) != 0 || lat->L > PERSIST_MAX_L ||
+        n < 2 || lat->persist_blocks < 0 || lat->persist_off)
         return 1;
+    // automatic only where it is measured faster than two launches per sweep (ising_persist.cuh):
+    // Ising lattices small enough for one row per thread; otherwise on request (persist_cap > 0)
+    const bool automatic = lat->model == LATTICE_ISING && ising_one_row(lat);
+    if (!automatic && lat->persist_cap == 0) return 1;
+    if (lat->model == LATTICE_BLUME_CAPEL) return sweep_persistent_bc(lat, n, beta);
     if (lat->persist_blocks == 0) {
-        int dev = 0, coop = 0, sms = 0, per_sm = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop ||
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_persist_kernel<false, false>, 256, 0) != cudaSuccess ||
-            per_sm < 1) {
-            cudaGetLastError();
-            lat->persist_blocks = -1;
-            return 1;
+        int nb = coop_blocks((const void *)ising_persist_kernel<false, false>);
+        const void *others[] = {(const void *)ising_persist_kernel<true, false>, (const void *)ising_persist_kernel<false, true>,
+                                (const void *)ising_persist_kernel<true, true>
+#define LAT_PC_FN(V) , (const void *)ising_persist_kernel<false, false, V>
+                                LAT_ISING_PC_LIST(LAT_PC_FN)
+#undef LAT_PC_FN
+        };
+        for (const void *fn : others) {
+            const int o = coop_blocks(fn);
+            if (o < nb) nb = o;
         }
-        int o[3] = {0, 0, 0};
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o[0], ising_persist_kernel<true, false>, 256, 0);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o[1], ising_persist_kernel<false, true>, 256, 0);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o[2], ising_persist_kernel<true, true>, 256, 0);
-        for (int k = 0; k < 3; ++k)
-            if (o[k] < per_sm) per_sm = o[k];
-        if (per_sm < 1) { lat->persist_blocks = -1; return 1; }
-        lat->persist_blocks = per_sm * sms;
+        lat->persist_blocks = nb > 0 ? nb : -1;
+        if (nb <= 0) return 1;
     }
     const uint32_t L = lat->L, wpr = lat->wpr, nq = wpr / 4u;
     const size_t pw = (size_t)L * wpr;
     bool edge = false;
-    const int urc = upload_sweep_params(lat, n, beta, &edge);
+    int pc = -2;                                 // packed plane cases shared by every sweep of the call (-1: they differ)
+    const int urc = upload_sweep_params(lat, n, beta, &edge, &pc);
     if (urc != LATTICE_OK) return urc;
 
     IsingMarchArgs a;
@@ -901,15 +998,23 @@ static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
     uint32_t *buf0 = lat->buf, *buf1 = lat->buf + pw;
     const SweepParams *sp = lat->d_sp;
     uint32_t ns = (uint32_t)n;
-    unsigned blocks = (a.threads + 255u) / 256u;
-    if (blocks > (unsigned)lat->persist_blocks) blocks = (unsigned)lat->persist_blocks;
-    if (lat->persist_cap && blocks > lat->persist_cap) blocks = lat->persist_cap;
+    const unsigned blocks = persist_grid(lat, (a.threads + 255u) / 256u);
     void *args[] = {&a, &buf0, &buf1, &sp, &ns};
     const void *fn = one_row ? (edge ? (const void *)ising_persist_kernel<true, true> : (const void *)ising_persist_kernel<false, true>)
                              : (edge ? (const void *)ising_persist_kernel<true, false> : (const void *)ising_persist_kernel<false, false>);
+    bool spec = false;
+    if (!one_row && !edge) {
+        switch (pc) {
+#define LAT_PC_CASE(V) case V: fn = (const void *)ising_persist_kernel<false, false, V>; spec = true; break;
+        LAT_ISING_PC_LIST(LAT_PC_CASE)
+#undef LAT_PC_CASE
+        default: break;
+        }
+    }
     const cudaError_t le = cudaLaunchCooperativeKernel(fn, dim3(blocks), dim3(256), args, 0, lat->stream);
     if (le != cudaSuccess) return cuda_fail(lat, le, "cudaLaunchCooperativeKernel");
     lat->launches += 1;
+    if (spec) lat->spec_launches += 1;
     lat->t += n;
     return LATTICE_OK;
 }
@@ -1006,17 +1111,27 @@ static int sweep_batch(lattice *lat, uint64_t n, const double *beta)
         for (uint64_t done = 0; done < n;) {
             const uint64_t chunk = n - done < 65536 ? n - done : 65536;
             bool edge = false;
-            const int rc = upload_sweep_params(lat, chunk, beta + done, &edge);
+            int pc = -2;                         // packed plane cases shared by every sweep of the chunk (-1: they differ)
+            const int rc = upload_sweep_params(lat, chunk, beta + done, &edge, &pc);
             if (rc) return rc;
             const uint32_t lanes = 16u * lat->wpr;
             const unsigned long long threads = (unsigned long long)lat->n_rep * lanes;
             const unsigned blocks = (unsigned)((threads + 127u) / 128u);
-            if (lat->wpr == 1u)
-                ising_tiny_kernel<1><<<blocks, 128, 0, lat->stream>>>(lat->buf, lat->d_keys, lat->d_sp, lat->n_rep,
-                                                                       (uint32_t)lat->t, (uint32_t)chunk);
-            else
-                ising_tiny_kernel<2><<<blocks, 128, 0, lat->stream>>>(lat->buf, lat->d_keys, lat->d_sp, lat->n_rep,
-                                                                       (uint32_t)lat->t, (uint32_t)chunk);
+#define LAT_TINY(W, V) ising_tiny_kernel<W, V><<<blocks, 128, 0, lat->stream>>>(lat->buf, lat->d_keys, lat->d_sp, lat->n_rep, \
+                                                                             (uint32_t)lat->t, (uint32_t)chunk)
+            bool spec = false;
+            if (!edge) {
+                switch (pc) {
+#define LAT_PC_CASE(V) case V: if (lat->wpr == 1u) LAT_TINY(1, V); else LAT_TINY(2, V); spec = true; break;
+                LAT_ISING_PC_LIST(LAT_PC_CASE)
+#undef LAT_PC_CASE
+                default: break;
+                }
+            }
+            if (spec) lat->spec_launches += 1;
+            else if (lat->wpr == 1u) LAT_TINY(1, -1);
+            else LAT_TINY(2, -1);
+#undef LAT_TINY
             lat->launches += 1;
             CU(lat, cudaGetLastError());
             lat->t += chunk;
@@ -1071,8 +1186,9 @@ int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta)
         if (std::isnan(beta[k]) || beta[k] < 0.0) return LATTICE_EINVAL;
     if (lat->n_rep) return sweep_batch(lat, n, beta);
     for (uint64_t done = 0; done < n;) {
-        // cache-resident Ising lattices: up to 65536 sweeps per cooperative launch
-        const uint64_t chunk = n - done < 65536 ? n - done : 65536;
+        // cache-resident lattices: up to 65536 (Blume-Capel: 16384) sweeps per cooperative launch
+        const uint64_t cap = lat->model == LATTICE_ISING ? 65536 : 16384;
+        const uint64_t chunk = n - done < cap ? n - done : cap;
         const int rc = sweep_persistent(lat, chunk, beta + done);
         if (rc == LATTICE_OK) { done += chunk; continue; }
         if (rc != 1) return rc;
@@ -1543,7 +1659,8 @@ int lattice_set_measure_path(lattice_t *lat, int path)
 int lattice_set_persist_blocks(lattice_t *lat, uint32_t max_blocks)
 {
     if (!lat) return LATTICE_EINVAL;
-    lat->persist_cap = max_blocks;
+    lat->persist_off = max_blocks == 0xffffffffu;
+    lat->persist_cap = lat->persist_off ? 0u : max_blocks;
     return LATTICE_OK;
 }
 

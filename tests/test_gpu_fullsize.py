@@ -178,7 +178,13 @@ def test_config3_blume_capel_L16384_first_sweeps_whole_lattice():
     g = lat.Lattice(w.L, w.model, w.delta, w.seed)
     o = oracle.OracleLattice(w.L, w.model, w.delta, w.seed)
     beta = w.beta_schedule(4)
-    g.sweep(beta)
+    g.set_persist_blocks(1 << 20)                 # bc_persist_kernel on request: one cooperative launch
+    n0 = g.launches
+    g.sweep(beta[:2])
+    assert g.launches - n0 == 1
+    g.set_persist_blocks(0)                       # the default at this size: two launches per sweep
+    g.sweep(beta[2:])
+    assert g.launches - n0 == 5
     o.sweep(beta)
     for i0 in (0, 8191, 16384 - 512):            # compare in row bands to bound host memory
         assert np.array_equal(g.get_spins(i0, 0, 512, w.L), o.get_spins(i0, 0, 512, w.L))

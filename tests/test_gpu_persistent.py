@@ -25,6 +25,7 @@ from paper_2503_14688_b200 import workloads
 pytestmark = pytest.mark.gpu
 BETA_C = workloads.BETA_C_ISING
 NCPU = os.cpu_count() or 1
+FORCE = 1 << 20            # lattice_set_persist_blocks: take the persistent path wherever it exists
 
 
 @pytest.fixture(autouse=True)
@@ -40,6 +41,7 @@ def test_persistent_marching_variant_against_oracle_and_single_launches(L):
     edge = [BETA_C] * 5 + [0.0] + [BETA_C] * 6 + [BETA_C / 1.01] * 4         # 16 sweeps, one at beta = 0
     plain = [BETA_C] * 3 + [0.5]                                             # no "always" class
     g = lat.Lattice(L, lat.ISING, 0.0, seed)          # persistent kernel, one launch per call
+    g.set_persist_blocks(FORCE)                       # (automatic only for L <= 4352: on request here)
     s = lat.Lattice(L, lat.ISING, 0.0, seed)          # the same sweeps, one per call
     o = oracle.OracleLattice(L, lat.ISING, 0.0, seed)
     for sched in (edge, plain):
@@ -63,7 +65,7 @@ def test_persistent_marching_variant_against_oracle_and_single_launches(L):
     assert g.launches - n0 == 1
     o.sweep(more)
     assert np.array_equal(g.get_spins(), o.get_spins())
-    g.set_persist_blocks(0)
+    g.set_persist_blocks(FORCE)
     Mg, Qg, Sxg, Syg = g.measure(64)
     Mo, Qo, Sxo, Syo = o.measure(64)
     assert (Mg, Qg) == (Mo, Qo) and np.array_equal(Sxg, Sxo) and np.array_equal(Syg, Syo)
@@ -79,6 +81,91 @@ def test_persistent_one_row_variant_with_capped_grid(L):
     sched = [BETA_C] * 6 + [0.0, BETA_C]
     g.sweep(sched)
     o.sweep(sched)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    g.close(); o.close()
+
+
+def test_persistent_ising_L16384_specialised_and_generic():
+    """8192 < L <= 16384: one cooperative launch per call; a constant-beta_c call
+    runs the plane-case specialised instantiation, a mixed schedule the generic one.  Whole-lattice
+    measurements and sampled row bands against the oracle."""
+    L, seed = 16384, 1638400
+    g = lat.Lattice(L, lat.ISING, 0.0, seed)
+    n0 = g.launches
+    g.sweep([BETA_C] * 2)
+    assert g.launches - n0 == 4                       # by default two launches per sweep at this size
+    g.close()
+    g = lat.Lattice(L, lat.ISING, 0.0, seed)
+    g.set_persist_blocks(FORCE)
+    o = oracle.OracleLattice(L, lat.ISING, 0.0, seed)
+    for sched, spec in (([BETA_C] * 3, 1), ([BETA_C, 0.0, 0.3], 0)):
+        n0, s0 = g.launches, g.specialised_launches
+        g.sweep(sched)
+        assert g.launches - n0 == 1 and g.specialised_launches - s0 == spec
+        o.sweep(sched)
+        for i0 in (0, 8191, L - 256):
+            assert np.array_equal(g.get_spins(i0, 0, 256, L), o.get_spins(i0, 0, 256, L))
+    Mg, Qg, Sxg, Syg = g.measure(8)
+    Mo, Qo, Sxo, Syo = o.measure(8)
+    assert (Mg, Qg) == (Mo, Qo) and np.array_equal(Sxg, Sxo) and np.array_equal(Syg, Syo)
+    g.close(); o.close()
+
+
+@pytest.mark.parametrize("L", [256, 1024, 2048])
+def test_persistent_blume_capel_against_oracle_and_single_launches(L):
+    """bc_persist_kernel (Delta = 0 type tables, L <= 16384, on request): lattice_sweep(n >= 2) is one launch and
+    equals the oracle and the same sweeps issued one per call; beta = 0 (every class "always") and
+    a changing beta are in the schedule; then with the grid capped so that blocks stride."""
+    seed = 77000 + L
+    bb = workloads.BETA_BC
+    sched = [bb] * 4 + [0.0] + [0.9 * bb, 0.95 * bb, bb, 1.3 * bb] + [bb] * 3
+    g = lat.Lattice(L, lat.BLUME_CAPEL, 0.0, seed)
+    g.set_persist_blocks(FORCE)                       # Blume-Capel: on request only
+    s = lat.Lattice(L, lat.BLUME_CAPEL, 0.0, seed)
+    o = oracle.OracleLattice(L, lat.BLUME_CAPEL, 0.0, seed)
+    n0 = g.launches
+    g.sweep(sched)
+    assert g.launches - n0 == 1
+    n0 = s.launches
+    for b in sched:
+        s.sweep([b])
+    assert s.launches - n0 == 2 * len(sched)
+    o.sweep(sched)
+    want = o.get_spins()
+    assert np.array_equal(g.get_spins(), want)
+    assert np.array_equal(s.get_spins(), want)
+    g.set_persist_blocks(5)
+    more = [bb, 0.0, bb, 1.1 * bb]
+    n0 = g.launches
+    g.sweep(more)
+    assert g.launches - n0 == 1
+    o.sweep(more)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    # the knob that turns the persistent path off: two launches per sweep again, same result
+    g.set_persist_blocks(0xffffffff)
+    n0 = g.launches
+    g.sweep(more)
+    assert g.launches - n0 == 2 * len(more)
+    o.sweep(more)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    assert g.time == o.time
+    Mg, Qg, Sxg, Syg = g.measure(32)
+    Mo, Qo, Sxo, Syo = o.measure(32)
+    assert (Mg, Qg) == (Mo, Qo) and np.array_equal(Sxg, Sxo) and np.array_equal(Syg, Syo)
+    g.close(); s.close(); o.close()
+
+
+def test_persistent_blume_capel_falls_back_for_a_crystal_field():
+    """Delta != 0 tables do not have the Delta = 0 structure: lattice_sweep(n) keeps the per-launch
+    path (the general marching kernel) and stays bit-exact."""
+    L, seed, delta, beta = 512, 4242, 0.7, 1.2
+    g = lat.Lattice(L, lat.BLUME_CAPEL, delta, seed)
+    g.set_persist_blocks(FORCE)
+    o = oracle.OracleLattice(L, lat.BLUME_CAPEL, delta, seed)
+    n0 = g.launches
+    g.sweep([beta] * 5)
+    assert g.launches - n0 == 10
+    o.sweep([beta] * 5)
     assert np.array_equal(g.get_spins(), o.get_spins())
     g.close(); o.close()
 
