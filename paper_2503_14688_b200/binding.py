@@ -79,7 +79,8 @@ def lib() -> C.CDLL:
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.build()
+    # LATTICE_LIB: a prebuilt library to load instead of building paper_2503_14688_b200/liblattice.so
+    path = os.environ.get("LATTICE_LIB") or _build.build()
     if not os.path.exists(path):
         raise RuntimeError(f"CUDA library {path} is missing and could not be built")
     L = C.CDLL(path)

@@ -213,9 +213,19 @@ __global__ void __launch_bounds__(TC_THREADS, 1) corr_tc_kernel(const CorrTCArgs
                     // smem row = contraction index (lattice row), 128-column blocks along MN:
                     // block 0 = base columns, blocks 1..4 = the pass's partner columns; the second
                     // 128-column block of an N tile sits TC_KC rows (16 KiB) further (MN-major LBO)
-                    const uint32_t kk = it % TC_KC, rest = it / TC_KC;
-                    h = rest & 1u;
-                    const uint32_t mb = rest >> 1;            // 0..4
+                    // chunks 0..255: the base block (mb = 0), one 8-byte word pair per (row, half);
+                    // chunks 256..1279: the four partner blocks, with the block index varying faster
+                    // than the upper bits of the row: the 32 lanes of a load instruction then read the
+                    // 4 x 8 contiguous bytes of 8 rows (8 lines) instead of 8 bytes of 32 rows, while the
+                    // 8 lanes of a quarter-warp still store to 8 consecutive rows (conflict-free)
+                    uint32_t kk, mb;
+                    if (it < 2u * TC_KC) { kk = it % TC_KC; h = it / TC_KC; mb = 0u; }
+                    else {
+                        const uint32_t b = it - 2u * TC_KC;
+                        kk = ((b >> 5) & 15u) * 8u + (b & 7u);
+                        mb = 1u + ((b >> 3) & 3u);
+                        h = b >> 9;
+                    }
                     blk = mb == 0 ? 0u : 1u + (mb - 1u) / 2u;
                     srow = kk + ((mb == 0 ? 0u : (mb - 1u) & 1u) * TC_KC);
                     row_l = a.i0 + kk;                        // + TC_KC rows per step; never wraps
@@ -230,6 +240,67 @@ __global__ void __launch_bounds__(TC_THREADS, 1) corr_tc_kernel(const CorrTCArgs
                 xr[q] = (srow & 7u) | (h << 2 << 8);          // low byte: row & 7, bits 8..: first chunk h * 4
             }
             const size_t step = AXIS == 1 ? 2u : (size_t)TC_KC * a.wpr;      // words per contraction step
+            if constexpr (AXIS == 1) {
+                // y axis: a thread's consecutive steps read consecutive 8-byte pieces of one lattice row,
+                // so it loads 16 bytes = two steps at a time (rows are 16-byte aligned: L % 256 == 0, and
+                // n_kc = L / 128 is even).  Every lane of a load reads another row -- 32 lines, 32
+                // wavefronts of the L1 data pipe whatever the width -- and that pipe (stores of the
+                // expanded bytes + operand reads of the tensor core + these loads) is what binds the
+                // kernel (profiles/r2_corr_tc.md): half as many loads is what counts.  Ring of TC_PF2
+                // such loads per chunk, reloaded for step kc + 2 TC_PF2 after the second of its steps.
+                constexpr int TC_PF2 = 2;
+                uint4 wb[TC_PF2][TC_PER_THREAD], sb[TC_PF2][TC_PER_THREAD];
+#pragma unroll
+                for (int u = 0; u < TC_PF2; ++u)
+#pragma unroll
+                    for (int q = 0; q < TC_PER_THREAD; ++q) {
+                        wb[u][q] = sb[u][q] = make_uint4(0u, 0u, 0u, 0u);
+                        if (2u * (uint32_t)u < n_kc && kc_zero[q] != 0u) {
+                            wb[u][q] = *reinterpret_cast<const uint4 *>(src[q] + 4 * u);
+                            if (MODEL) sb[u][q] = *reinterpret_cast<const uint4 *>(src[q] + 4 * u + pw);
+                        }
+                    }
+                for (uint32_t kc0 = 0; kc0 < n_kc; kc0 += 2u * TC_PF2) {
+#pragma unroll
+                    for (int uv = 0; uv < 2 * TC_PF2; ++uv) {
+                        const int u = uv >> 1, v = uv & 1;
+                        const uint32_t kc = kc0 + (uint32_t)uv;
+                        if (kc >= n_kc) break;
+                        mbar_wait(empty0 + 8 * stage, phase ^ 1u);
+                        const uint32_t st = smem_u32(smem) + stage * TC_STAGE_BYTES;
+#pragma unroll
+                        for (int q = 0; q < TC_PER_THREAD; ++q) {
+                            uint4 o[4];
+                            if (kc_zero[q] == 0u) {
+                                o[0] = o[1] = o[2] = o[3] = make_uint4(0u, 0u, 0u, 0u);
+                            } else {
+                                expand_word<MODEL>(v ? wb[u][q].z : wb[u][q].x, v ? sb[u][q].z : sb[u][q].x, o[0], o[1]);
+                                expand_word<MODEL>(v ? wb[u][q].w : wb[u][q].y, v ? sb[u][q].w : sb[u][q].y, o[2], o[3]);
+                            }
+                            const uint32_t r7 = xr[q] & 7u, c0 = xr[q] >> 8;
+#pragma unroll
+                            for (int e = 0; e < 4; ++e)
+                                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + dst[q] + (((c0 + (uint32_t)e) ^ r7) << 4)),
+                                             "r"(o[e].x), "r"(o[e].y), "r"(o[e].z), "r"(o[e].w) : "memory");
+                        }
+                        fence_proxy_async();                  // generic-proxy writes -> visible to the tensor core
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(full0 + 8 * stage);
+                        if (++stage == TC_STAGES) { stage = 0; phase ^= 1u; }
+                        if (v == 1) {
+                            const uint32_t nk = kc0 + 2u * (uint32_t)u + 2u * TC_PF2;
+#pragma unroll
+                            for (int q = 0; q < TC_PER_THREAD; ++q) {
+                                wb[u][q] = sb[u][q] = make_uint4(0u, 0u, 0u, 0u);
+                                if (nk < n_kc && kc_zero[q] != 0u) {
+                                    wb[u][q] = *reinterpret_cast<const uint4 *>(src[q] + 2 * (size_t)nk);
+                                    if (MODEL) sb[u][q] = *reinterpret_cast<const uint4 *>(src[q] + 2 * (size_t)nk + pw);
+                                }
+                            }
+                        }
+                    }
+                }
+            } else {
             // The packed words of the next TC_PF contraction steps live in registers (a ring indexed by
             // kc % TC_PF, the loop unrolled by TC_PF so that the index is static): the loads of step
             // kc + TC_PF are issued at the end of step kc, after the proxy fence (which would otherwise
@@ -284,6 +355,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) corr_tc_kernel(const CorrTCArgs
                         }
                     }
                 }
+            }
             }
             // ===== epilogue (warps 0-3: TMEM lane quarter = warp) =====
             if (warp < 4) {

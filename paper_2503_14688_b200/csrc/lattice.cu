@@ -1291,7 +1291,7 @@ static int fetch_counts(lattice *lat, const unsigned long long *src, size_t entr
 static bool corr_tc_applies(const lattice *lat, uint64_t n_rows, uint32_t r_max)
 {
     if (lat->measure_path == 1) return false;
-    const bool shape_ok = (lat->L % 128u) == 0 && lat->L >= 1024u && n_rows >= 1 && !lat->slab;
+    const bool shape_ok = (lat->L % 256u) == 0 && lat->L >= 1024u && n_rows >= 1 && !lat->slab;
     if (lat->measure_path == 2) return shape_ok;
     return shape_ok && lat->L >= 4096u && n_rows >= 512 && r_max >= 48;
 }
@@ -1651,7 +1651,7 @@ int lattice_plane_case_specialised(int model, double delta, double beta)
 int lattice_set_measure_path(lattice_t *lat, int path)
 {
     if (!lat || path < 0 || path > 2) return LATTICE_EINVAL;
-    if (path == 2 && ((lat->L % 128u) != 0 || lat->L < 1024u || lat->slab)) return LATTICE_EINVAL;
+    if (path == 2 && ((lat->L % 256u) != 0 || lat->L < 1024u || lat->slab)) return LATTICE_EINVAL;
     lat->measure_path = path;
     return LATTICE_OK;
 }

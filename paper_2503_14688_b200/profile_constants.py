@@ -23,15 +23,15 @@ SOURCES = {
 #: model -> constants read from the named capture
 CAPTURED = {
     0: {"kernel": "ising_march_kernel",
-        "executed_half_rate_instr_per_update": 3.39,      # (pipe_alu + IMAD.WIDE/HI thread-instr) / updates
-        "dram_bytes_per_update": 0.383,                   # (dram__bytes_read + dram__bytes_write) / updates
-        "profile": "profiles/r1e_ising_march_full.md", "commit": "5291d27",
-        "sources_sha256": "r1e"},
+        "executed_half_rate_instr_per_update": 3.21,      # (ALU-pipe + IMAD.WIDE/HI thread-instr) / updates, SASS page
+        "dram_bytes_per_update": 0.383,                   # (dram__bytes_read + dram__bytes_write) / updates at L = 2^20
+        "profile": "profiles/r2_ising_march.md + profiles/r2_launches_default.md", "commit": "e1060ac",
+        "sources_sha256": "01d681f2d6da49703698b8d24fdf470e4c84f57c4811b7f0eaff6f99018958df"},
     1: {"kernel": "bc_march_kernel",
-        "executed_half_rate_instr_per_update": 5.30,
-        "dram_bytes_per_update": 0.667,
-        "profile": "profiles/r1e_bc_march_full.md", "commit": "5291d27",
-        "sources_sha256": "r1e"},
+        "executed_half_rate_instr_per_update": 4.77,
+        "dram_bytes_per_update": 0.768,                   # at L = 2^19 (launch list); 0.669 at L = 2^15 (partly L2-resident)
+        "profile": "profiles/r2_bc_march.md + profiles/r2_launches_default.md", "commit": "e1060ac",
+        "sources_sha256": "366565743a070e83f6f4f3aff8562ed257163d8e2fe76f2ad90fa0aebcb59dc5"},
 }
 
 #: Algorithmic half-rate thread-instructions per update: the floor of the method under the RNG
