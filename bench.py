@@ -616,6 +616,9 @@ def main():
                     help="skip the Blume-Capel workloads the default invocation also times")
     ap.add_argument("--no-batches", action="store_true",
                     help="skip the batched-replica workloads the default invocation also times")
+    ap.add_argument("--delta", type=float, default=None,
+                    help="override the workload's crystal field Delta (Blume-Capel; e.g. the general marching kernel)")
+    ap.add_argument("--beta", type=float, default=None, help="override the workload's beta schedule with a constant")
     ap.add_argument("--no-persistent", action="store_true",
                     help="cache-resident lattices: two launches per sweep instead of the persistent multi-sweep kernel (A/B)")
     ap.add_argument("--batches-only", action="store_true",
@@ -661,6 +664,14 @@ def main():
         return
 
     w = workloads.CONFIGS[args.workload]
+    if args.delta is not None or args.beta is not None:
+        import dataclasses
+        kw = {}
+        if args.delta is not None:
+            kw["delta"] = args.delta
+        if args.beta is not None:
+            kw.update(protocol=1, beta_f=args.beta)
+        w = dataclasses.replace(w, name=w.name + "".join(f"@{k}={v}" for k, v in kw.items()), **kw)
     res = bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, measure_pass=True, worst_case=True)
 
     # the metric's second half: Blume-Capel at the paper's size and BASELINE config 5b, same process

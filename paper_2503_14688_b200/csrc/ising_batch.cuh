@@ -27,6 +27,10 @@
 
 namespace lat {
 
+#ifndef LAT_TINY_MINB
+#define LAT_TINY_MINB 4        // resident blocks per SM of ising_tiny_kernel<1> (measured: 4 > 6; see below)
+#endif
+
 constexpr int BATCH_CHUNK = 128;             // replicas per launch of the marching batch kernel
 
 struct BatchKeys {                           // 10 KiB of kernel parameters
@@ -220,7 +224,7 @@ __device__ __forceinline__ void tiny_half_sweep(uint32_t (&T)[4 * WPR], const ui
 // keeps twice the state per lane and would spill under that cap.  PC >= 0: every sweep of the call
 // has the packed plane cases PC (ising_march.cuh) compiled in.
 template <int WPR, int PC = -1>
-__global__ void __launch_bounds__(128, WPR == 1 ? 4 : 3) ising_tiny_kernel(uint32_t *buf, const RoundKeys *keys,
+__global__ void __launch_bounds__(128, WPR == 1 ? LAT_TINY_MINB : 3) ising_tiny_kernel(uint32_t *buf, const RoundKeys *keys,
                                                          const SweepParams *sp, uint32_t n_rep,
                                                          uint32_t t0, uint32_t n_sweeps)
 {

@@ -1471,6 +1471,7 @@ int lattice_measure_list(lattice_t *lat, uint64_t i0, uint64_t n_rows, const uin
         MeasListArgs b;
         b.buf = lat->buf; b.L = lat->rows; b.wpr = lat->wpr; b.i0 = (uint32_t)i0; b.rlist = lat->d_rlist; b.n_r = n_r;
         b.mq = 1u; b.cnt = lat->d_cnt; b.n = nblk;
+        b.axes = 3u;
         const unsigned long long threads = 2ull * nblk * lat->wpr;
         const dim3 grid((unsigned)((threads + 127) / 128), chunks);
         if (lat->model == LATTICE_ISING) measure_list_kernel<0><<<grid, 128, 0, lat->stream>>>(b);

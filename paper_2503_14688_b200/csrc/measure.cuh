@@ -435,6 +435,7 @@ struct MeasListArgs {
     const uint32_t *rlist;           // device, n_r entries, each in [1, L/2]
     uint32_t n_r;
     uint32_t mq;                     // also count M, Q (chunk 0)
+    uint32_t axes;                   // measure_list_kernel: bit 0 = x axis, bit 1 = y axis
     unsigned long long *cnt;
 };
 
@@ -493,10 +494,22 @@ __global__ void __launch_bounds__(128) measure_list_kernel(const MeasListArgs a)
             const uint32_t r = a.rlist[q];
             const uint32_t *p0 = (r & 1u) ? op0 : bp0, *p1 = (r & 1u) ? op1 : bp1;
             uint32_t X[MEAS_NB], Y[MEAS_NB];
-            {   // y axis
+            if (a.axes & 2u) {   // y axis
                 uint32_t row = ib0 + r;                                // < 2 L
                 if (row >= a.L) row -= a.L;
                 unsigned long long o = (unsigned long long)row * a.wpr + k;
+                if (row + MEAS_NB <= a.L) {
+                    // the 16 partner rows do not wrap: one running pointer, no per-row checks (the
+                    // address arithmetic of the general form below cost more than the counting)
+                    const uint32_t *q0 = p0 + o, *q1 = p1 + o;
+#pragma unroll
+                    for (int j = 0; j < MEAS_NB; ++j) {
+                        const uint32_t w0 = *q0;
+                        if (MODEL == 0) X[j] = B0[j] ^ w0;
+                        else { X[j] = B0[j] & w0; Y[j] = X[j] & (B1[j] ^ *q1); }
+                        q0 += a.wpr; q1 += a.wpr;
+                    }
+                } else {
 #pragma unroll
                 for (int j = 0; j < MEAS_NB; ++j) {
                     const uint32_t w0 = p0[o];
@@ -504,28 +517,34 @@ __global__ void __launch_bounds__(128) measure_list_kernel(const MeasListArgs a)
                     else { X[j] = B0[j] & w0; Y[j] = X[j] & (B1[j] ^ p1[o]); }
                     o += a.wpr; if (o >= plane_words) o -= plane_words;
                 }
+                }
                 const uint32_t c0 = weighted_popc16(X);
                 const uint32_t c1 = MODEL ? weighted_popc16(Y) : 0u;
                 add_r(s_cnt[1], q - q0, mask, leader, lane, c0, c1, MODEL != 0);
             }
-            {   // x axis: rows j and j+1 have parities par0 and par0 ^ 1
+            if (a.axes & 1u) {   // x axis: rows j and j+1 have parities par0 and par0 ^ 1
                 const uint32_t sA = (r >> 1) + ((r & 1u) ? par0 : 0u), sB = (r >> 1) + ((r & 1u) ? (par0 ^ 1u) : 0u);
                 uint32_t kA = k + (sA >> 5), kB = k + (sB >> 5);     // s >> 5 <= wpr / 2
                 if (kA >= a.wpr) kA -= a.wpr;
                 if (kB >= a.wpr) kB -= a.wpr;
                 const uint32_t kA1 = (kA + 1 == a.wpr) ? 0 : kA + 1, kB1 = (kB + 1 == a.wpr) ? 0 : kB + 1;
                 const uint32_t bA = sA & 31u, bB = sB & 31u;
-                unsigned long long o = ob;
+                // four running pointers (rows of either parity: first and second word), advanced by
+                // two rows per use: the 64-bit index arithmetic of `p0[o + ka]` per load cost more than
+                // the counting
+                const uint32_t *pa = p0 + ob + kA, *pa1 = p0 + ob + kA1;
+                const uint32_t *pb = p0 + ob + a.wpr + kB, *pb1 = p0 + ob + a.wpr + kB1;
+                const size_t two = 2 * (size_t)a.wpr, dpl = (size_t)(p1 - p0);
 #pragma unroll
-                for (int j = 0; j < MEAS_NB; ++j) {
-                    const uint32_t ka = (j & 1) ? kB : kA, ka1 = (j & 1) ? kB1 : kA1, bs = (j & 1) ? bB : bA;
-                    const uint32_t w0 = __funnelshift_r(p0[o + ka], p0[o + ka1], bs);
-                    if (MODEL == 0) X[j] = B0[j] ^ w0;
+                for (int j = 0; j < MEAS_NB; j += 2) {
+                    const uint32_t wA = __funnelshift_r(*pa, *pa1, bA), wB = __funnelshift_r(*pb, *pb1, bB);
+                    if (MODEL == 0) { X[j] = B0[j] ^ wA; X[j + 1] = B0[j + 1] ^ wB; }
                     else {
-                        const uint32_t w1 = __funnelshift_r(p1[o + ka], p1[o + ka1], bs);
-                        X[j] = B0[j] & w0; Y[j] = X[j] & (B1[j] ^ w1);
+                        const uint32_t vA = __funnelshift_r(pa[dpl], pa1[dpl], bA), vB = __funnelshift_r(pb[dpl], pb1[dpl], bB);
+                        X[j] = B0[j] & wA; Y[j] = X[j] & (B1[j] ^ vA);
+                        X[j + 1] = B0[j + 1] & wB; Y[j + 1] = X[j + 1] & (B1[j + 1] ^ vB);
                     }
-                    o += a.wpr;
+                    pa += two; pa1 += two; pb += two; pb1 += two;
                 }
                 const uint32_t c0 = weighted_popc16(X);
                 const uint32_t c1 = MODEL ? weighted_popc16(Y) : 0u;
