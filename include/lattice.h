@@ -228,12 +228,14 @@ uint64_t lattice_time(const lattice_t *lat);
 int lattice_set_time(lattice_t *lat, uint64_t t);
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 uint64_t lattice_launches(const lattice_t *lat);
-/* Launch-time specialisation of the Ising half-sweep: how many of the handle's launches ran a
- * kernel instantiated for the plane cases of their beta (the LOP3 truth tables of the bit-serial
- * threshold compare as compile-time constants, no per-plane dispatch), and whether such an
- * instantiation exists for (model, delta, beta) -- it does for beta_c = ln(1 + sqrt 2)/2
- * (PAPER.md:40), for T_1 = 1.66 and T_2 = 2.27414861561203 of the two-step protocol (Table II,
- * PAPER.md:144-146) and for any beta whose thresholds share their top bytes with one of these.
+/* Launch-time specialisation of the half-sweeps: how many of the handle's launches ran a kernel
+ * instantiated for the plane cases of their beta (the LOP3 truth tables of the bit-serial threshold
+ * compare as compile-time constants, no per-plane dispatch), and whether such an instantiation
+ * exists for (model, delta, beta).  Ising: beta_c = ln(1 + sqrt 2)/2, T_1 = 1.66 and
+ * T_2 = 2.27414861561203 of the two-step protocol (Table II).  Blume-Capel at
+ * Delta = 0: T = 1.6934 (BASELINE config 3), T_c = 1.69355839821214427 (Table I),
+ * T_2 = 1.69661396797728 and T_1 = 1.24 (Table II), the plateau of config 5b's
+ * ramp.  Any beta whose thresholds share their top bytes with one of these takes the same kernel.
  * Results never depend on which kernel runs. */
 uint64_t lattice_specialised_launches(const lattice_t *lat);
 int lattice_plane_case_specialised(int model, double delta, double beta);

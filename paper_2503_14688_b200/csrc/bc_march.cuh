@@ -98,6 +98,47 @@ __device__ __forceinline__ void lut3_dispatch(uint32_t lut, const uint32_t (&a)[
 #undef LAT_LR
 #undef LAT_TR
 
+// Launch-time specialisation (as for the Ising kernel, ising_march.cuh): the eight per-plane truth
+// tables depend only on the top bytes of the eight class thresholds, i.e. on beta.  For the
+// temperatures the workloads run at, LS >= 0 selects a set of tables compiled in: every dispatched
+// LOP3 becomes a LOP3 with an immediate, the eight 256-way brx.idx jumps are gone and the plane loop is
+// unrolled.  All sets have lut_always == 0 (no class threshold is 2^32).  LS < 0: the generic path.
+//   0: T = 1.6934 (BASELINE config 3), T_c = 1.69355839821214427 (Table I) and
+//      T_2 = 1.69661396797728 of the two-step protocol (Table II)
+//   1: beta = (1/1.6934)/1.01, the plateau of BASELINE config 5b's ramp
+//   2: T_1 = 1.24 of the two-step protocol
+constexpr int BC_LUT_SETS = 3;
+__host__ __device__ constexpr uint32_t bc_lut_set(int ls, int k)
+{
+    constexpr uint32_t T[BC_LUT_SETS][8] = {{0x02, 0x21, 0x08, 0x14, 0x3f, 0xa3, 0xe9, 0x8a},
+                                            {0x02, 0x21, 0x08, 0x14, 0x3f, 0xab, 0xe3, 0xa1},
+                                            {0x00, 0x02, 0x23, 0x2b, 0x14, 0x08, 0xbf, 0x21}};
+    return T[ls][k];
+}
+
+#ifdef __CUDACC__
+// planes K, K-1, ..., 0 with the truth tables of set LS as LOP3 immediates
+template <int LS, int K>
+struct BCPlaneLoop {
+    template <class Args>
+    static __device__ __forceinline__ void run(const Args &a, const PlaneShared &ps, const uint32_t (&Fm)[4],
+                                               const uint32_t (&Y1)[4], const uint32_t (&H0)[4],
+                                               uint32_t (&acc)[4], uint32_t (&eq)[4])
+    {
+        const uint4 b4 = plane_block(ps, a.F.fb[0] ^ ((uint32_t)K << 16), a.F, a.K);
+        const uint32_t b[4] = {b4.x, b4.y, b4.z, b4.w};
+        constexpr int LUT = (int)bc_lut_set(LS, K);
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            const uint32_t tau = LUT == 0 ? 0u : lop3<LUT>(Fm[w], Y1[w], H0[w]);
+            acc[w] = maj3m(tau, ~b[w], acc[w]);
+            eq[w] &= ~(b[w] ^ tau);
+        }
+        if constexpr (K > 0) BCPlaneLoop<LS, K - 1>::run(a, ps, Fm, Y1, H0, acc, eq);
+    }
+};
+#endif
+
 // Per-warp queue of words that contain tied lanes (same scheme as WarpTieQueue in
 // ising_march.cuh).  Two 128-bit halves per entry:
 //   [0] = (tied lanes, F, Y1, H0 of the word)    [1] = (nz-toggle mask, sg-toggle mask, word offset)
@@ -186,7 +227,7 @@ __device__ __forceinline__ void bcm_load(const uint32_t *nzp, const uint32_t *sg
 // One row of one 128-bit run.  PAR == 0: side neighbour at p-1 (En, Es = word before the run),
 // PAR == 1: at p+1 (word after it).  Stores the updated words (ties treated as rejections) and
 // queues the ties.
-template <int PAR, bool SLAB, class Args>
+template <int PAR, bool SLAB, int LS, class Args>
 __device__ __forceinline__ void bc_march_row(const Args &a, uint32_t G, unsigned long long wo,
                                              uint32_t *tn, uint32_t *ts,
                                              const BCRow &U, const BCRow &C, const BCRow &D,
@@ -237,7 +278,8 @@ __device__ __forceinline__ void bc_march_row(const Args &a, uint32_t G, unsigned
         }
     }
     uint32_t alw[4], acc[4], eq[4];
-    lut3_dispatch(a.lut_always, Fm, Y1, H0, alw);
+    if constexpr (LS >= 0) { alw[0] = alw[1] = alw[2] = alw[3] = 0u; }      // the sets have lut_always == 0
+    else lut3_dispatch(a.lut_always, Fm, Y1, H0, alw);
 #pragma unroll
     for (int w = 0; w < 4; ++w) {
         const uint32_t need = pos[w] & ~alw[w];
@@ -246,16 +288,20 @@ __device__ __forceinline__ void bc_march_row(const Args &a, uint32_t G, unsigned
         eq[w] = need;
         acc[w] = 0;
     }
+    if constexpr (LS >= 0) {
+        BCPlaneLoop<LS, 7>::run(a, ps, Fm, Y1, H0, acc, eq);
+    } else {
 #pragma unroll 1                     // unrolling replicates the 256-entry tables: slower (I-cache)
-    for (int k = 7; k >= 0; --k) {
-        const uint4 b4 = plane_block(ps, a.F.fb[0] ^ ((uint32_t)k << 16), a.F, a.K);
-        const uint32_t b[4] = {b4.x, b4.y, b4.z, b4.w};
-        uint32_t tau[4];
-        lut3_dispatch(a.lut_k(k), Fm, Y1, H0, tau);
+        for (int k = 7; k >= 0; --k) {
+            const uint4 b4 = plane_block(ps, a.F.fb[0] ^ ((uint32_t)k << 16), a.F, a.K);
+            const uint32_t b[4] = {b4.x, b4.y, b4.z, b4.w};
+            uint32_t tau[4];
+            lut3_dispatch(a.lut_k(k), Fm, Y1, H0, tau);
 #pragma unroll
-        for (int w = 0; w < 4; ++w) {
-            acc[w] = maj3m(tau[w], ~b[w], acc[w]);
-            eq[w] &= ~(b[w] ^ tau[w]);
+            for (int w = 0; w < 4; ++w) {
+                acc[w] = maj3m(tau[w], ~b[w], acc[w]);
+                eq[w] &= ~(b[w] ^ tau[w]);
+            }
         }
     }
 #pragma unroll
@@ -450,14 +496,14 @@ __device__ __forceinline__ void bc_march_row_gen(const BCMarchArgs &a, uint32_t 
 }
 
 // GEN = false: the integer-dE (Delta = 0 type) rows above; GEN = true: bc_march_row_gen
-template <bool GEN, int PAR, bool SLAB, class Args, class Queue>
+template <bool GEN, int PAR, bool SLAB, int LS, class Args, class Queue>
 __device__ __forceinline__ void bc_row(const Args &a, uint32_t G, unsigned long long wo, uint32_t *tn,
                                        uint32_t *ts, const BCRow &U, const BCRow &C, const BCRow &D, uint32_t En,
                                        uint32_t Es, Queue &queue, uint32_t *mir_nz = nullptr,
                                        uint32_t *mir_sg = nullptr, uint32_t mir_tag = 0)
 {
     if constexpr (GEN) bc_march_row_gen<PAR, SLAB>(a, G, wo, tn, ts, U, C, D, En, Es, queue, mir_nz, mir_sg, mir_tag);
-    else bc_march_row<PAR, SLAB>(a, G, wo, tn, ts, U, C, D, En, Es, queue, mir_nz, mir_sg, mir_tag);
+    else bc_march_row<PAR, SLAB, LS>(a, G, wo, tn, ts, U, C, D, En, Es, queue, mir_nz, mir_sg, mir_tag);
 }
 
 template <bool GEN, bool SLAB>
@@ -467,7 +513,7 @@ struct BCQueueOf<true, SLAB> { using type = BCTieQueueGen<SLAB>; };
 
 // The march of one thread: rows i0 .. i0+R-1 of run q, g = s * (wpr/4) + q (ties are queued, not
 // drained) -- shared by bc_march_kernel and bc_persist_kernel (bc_persist.cuh).
-template <int COLOUR, bool SLAB, bool GEN, class Args, class Queue>
+template <int COLOUR, bool SLAB, bool GEN, int LS = -1, class Args, class Queue>
 __device__ __forceinline__ void bc_march_thread(const Args &a, uint32_t g, Queue &queue)
 {
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
@@ -496,10 +542,10 @@ __device__ __forceinline__ void bc_march_thread(const Args &a, uint32_t g, Queue
             bcm_load(dn, dn + pw, kw, D);
             const uint32_t ke = COLOUR == 0 ? ke0 : ke1;
             if (SLAB && top && r == 0)
-                bc_row<GEN, COLOUR, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
+                bc_row<GEN, COLOUR, SLAB, LS>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
                                      a.mir_up_nz + kw, a.mir_up_sg + kw, (kw << 4) | (1u << 30));
             else
-                bc_row<GEN, COLOUR, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+                bc_row<GEN, COLOUR, SLAB, LS>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
             U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
         {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
@@ -508,16 +554,16 @@ __device__ __forceinline__ void bc_march_thread(const Args &a, uint32_t g, Queue
             bcm_load(dn, dn + pw, kw, D);
             const uint32_t ke = COLOUR == 0 ? ke1 : ke0;
             if (SLAB && bot && r + 2 == a.R)
-                bc_row<GEN, COLOUR ^ 1, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
+                bc_row<GEN, COLOUR ^ 1, SLAB, LS>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue,
                                          a.mir_dn_nz + kw, a.mir_dn_sg + kw, (kw << 4) | (2u << 30));
             else
-                bc_row<GEN, COLOUR ^ 1, SLAB>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
+                bc_row<GEN, COLOUR ^ 1, SLAB, LS>(a, G, wo, tn, tn + pw, U, C, D, on[ke], on[pw + ke], queue);
             U = C; C = D; on = dn; tn += wpr; wo += wpr; G += nq;
         }
     }
 }
 
-template <int COLOUR, bool SLAB, bool GEN = false>
+template <int COLOUR, bool SLAB, bool GEN = false, int LS = -1>
 __global__ void __launch_bounds__(256, GEN ? 2 : 3) bc_march_kernel(const BCMarchArgs a)
 {
     // the general queue (3 x 16 bytes per entry, 60 KiB per block) exceeds the static limit: dynamic
@@ -527,7 +573,7 @@ __global__ void __launch_bounds__(256, GEN ? 2 : 3) bc_march_kernel(const BCMarc
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;
     if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
     typename BCQueueOf<GEN, SLAB>::type queue{a, GEN ? s_dyn + warp * (3 * TIE_Q_SLOTS) : s_fix[GEN ? 0 : warp], lane, 0u};
-    bc_march_thread<COLOUR, SLAB, GEN>(a, g, queue);
+    bc_march_thread<COLOUR, SLAB, GEN, LS>(a, g, queue);
     queue.drain();
 }
 

@@ -315,6 +315,18 @@ void bc_fill_integer_dE_luts(const lattice *lat, uint32_t (&lut)[8], uint32_t &l
         }
 }
 
+// index of the compiled-in set of truth tables (bc_march.cuh) equal to these, or -1
+int bc_lut_set_index(const uint32_t (&lut)[8], uint32_t lut_always)
+{
+    if (lut_always) return -1;
+    for (int ls = 0; ls < BC_LUT_SETS; ++ls) {
+        bool same = true;
+        for (int k = 0; k < 8; ++k) same = same && lut[k] == bc_lut_set(ls, k);
+        if (same) return ls;
+    }
+    return -1;
+}
+
 // bc_march_row_gen applies when x = -4 is "always" for vacate and occupy (|Delta| <= 4) and every
 // flip with x <= 0 is (dE = 2x <= 0: any Delta)
 bool bc_table_is_general_ok(const lattice *lat)
@@ -397,7 +409,22 @@ int launch_bc_march(lattice *lat, int colour, bool gen = false)
         else { if (colour == 0) LAT_LAUNCH_BC(0, true, false); else LAT_LAUNCH_BC(1, true, false); }
     } else {
         if (gen) { if (colour == 0) LAT_LAUNCH_BC(0, false, true); else LAT_LAUNCH_BC(1, false, true); }
-        else { if (colour == 0) LAT_LAUNCH_BC(0, false, false); else LAT_LAUNCH_BC(1, false, false); }
+        else {
+            // launch-time specialisation: a kernel with this beta's truth tables compiled in
+            switch (bc_lut_set_index(a.lut, a.lut_always)) {
+#define LAT_LS_CASE(V)                                                                                         \
+            case V:                                                                                            \
+                if (colour == 0) bc_march_kernel<0, false, false, V><<<blocks, 256, dyn, lat->stream>>>(a);    \
+                else bc_march_kernel<1, false, false, V><<<blocks, 256, dyn, lat->stream>>>(a);                \
+                lat->spec_launches += 1;                                                                       \
+                break;
+            LAT_LS_CASE(0) LAT_LS_CASE(1) LAT_LS_CASE(2)
+#undef LAT_LS_CASE
+            default:
+                if (colour == 0) LAT_LAUNCH_BC(0, false, false); else LAT_LAUNCH_BC(1, false, false);
+                break;
+            }
+        }
     }
 #undef LAT_LAUNCH_BC
     lat->launches += 1;
@@ -1105,40 +1132,45 @@ static int launch_half_sweep_batch(lattice *lat, int colour)
 
 // n sweeps of every replica.  L = 64, 128 (Ising, bit-plane schemes): the whole call is ONE launch of
 // ising_tiny_kernel, replicas resident in registers.  Otherwise two (chunked) launches per sweep.
+// L = 64, 128 (Ising, bit-plane schemes): n sweeps of n_rep replicas in ONE launch of ising_tiny_kernel,
+// every replica resident in the registers of a (half-)warp.  lat->d_keys holds their round keys.
+static int sweep_tiny(lattice *lat, uint32_t n_rep, uint64_t n, const double *beta)
+{
+    for (uint64_t done = 0; done < n;) {
+        const uint64_t chunk = n - done < 65536 ? n - done : 65536;
+        bool edge = false;
+        int pc = -2;                         // packed plane cases shared by every sweep of the chunk (-1: they differ)
+        const int rc = upload_sweep_params(lat, chunk, beta + done, &edge, &pc);
+        if (rc) return rc;
+        const uint32_t lanes = 16u * lat->wpr;
+        const unsigned long long threads = (unsigned long long)n_rep * lanes;
+        const unsigned blocks = (unsigned)((threads + 127u) / 128u);
+#define LAT_TINY(W, V) ising_tiny_kernel<W, V><<<blocks, 128, 0, lat->stream>>>(lat->buf, lat->d_keys, lat->d_sp, n_rep, \
+                                                                             (uint32_t)lat->t, (uint32_t)chunk)
+        bool spec = false;
+        if (!edge) {
+            switch (pc) {
+#define LAT_PC_CASE(V) case V: if (lat->wpr == 1u) LAT_TINY(1, V); else LAT_TINY(2, V); spec = true; break;
+            LAT_ISING_PC_LIST(LAT_PC_CASE)
+#undef LAT_PC_CASE
+            default: break;
+            }
+        }
+        if (spec) lat->spec_launches += 1;
+        else if (lat->wpr == 1u) LAT_TINY(1, -1);
+        else LAT_TINY(2, -1);
+#undef LAT_TINY
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+        lat->t += chunk;
+        done += chunk;
+    }
+    return LATTICE_OK;
+}
+
 static int sweep_batch(lattice *lat, uint64_t n, const double *beta)
 {
-    if (lat->model == LATTICE_ISING && lat->scheme >= 1 && lat->wpr <= 2u) {
-        for (uint64_t done = 0; done < n;) {
-            const uint64_t chunk = n - done < 65536 ? n - done : 65536;
-            bool edge = false;
-            int pc = -2;                         // packed plane cases shared by every sweep of the chunk (-1: they differ)
-            const int rc = upload_sweep_params(lat, chunk, beta + done, &edge, &pc);
-            if (rc) return rc;
-            const uint32_t lanes = 16u * lat->wpr;
-            const unsigned long long threads = (unsigned long long)lat->n_rep * lanes;
-            const unsigned blocks = (unsigned)((threads + 127u) / 128u);
-#define LAT_TINY(W, V) ising_tiny_kernel<W, V><<<blocks, 128, 0, lat->stream>>>(lat->buf, lat->d_keys, lat->d_sp, lat->n_rep, \
-                                                                             (uint32_t)lat->t, (uint32_t)chunk)
-            bool spec = false;
-            if (!edge) {
-                switch (pc) {
-#define LAT_PC_CASE(V) case V: if (lat->wpr == 1u) LAT_TINY(1, V); else LAT_TINY(2, V); spec = true; break;
-                LAT_ISING_PC_LIST(LAT_PC_CASE)
-#undef LAT_PC_CASE
-                default: break;
-                }
-            }
-            if (spec) lat->spec_launches += 1;
-            else if (lat->wpr == 1u) LAT_TINY(1, -1);
-            else LAT_TINY(2, -1);
-#undef LAT_TINY
-            lat->launches += 1;
-            CU(lat, cudaGetLastError());
-            lat->t += chunk;
-            done += chunk;
-        }
-        return LATTICE_OK;
-    }
+    if (lat->model == LATTICE_ISING && lat->scheme >= 1 && lat->wpr <= 2u) return sweep_tiny(lat, lat->n_rep, n, beta);
     if (lat->model == LATTICE_ISING && lat->scheme >= 1 && (lat->wpr % 4u) == 0 && lat->L <= 1024u && n >= 2) {
         // one block per replica, all sweeps of the chunk in one launch (ising_block_kernel)
         for (uint64_t done = 0; done < n;) {
@@ -1185,6 +1217,16 @@ int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta)
     for (uint64_t k = 0; k < n; ++k)
         if (std::isnan(beta[k]) || beta[k] < 0.0) return LATTICE_EINVAL;
     if (lat->n_rep) return sweep_batch(lat, n, beta);
+    if (lat->model == LATTICE_ISING && lat->scheme >= 1 && lat->wpr <= 2u && !lat->slab && !lat->view && n >= 2 &&
+        !lat->persist_off) {
+        // a single L = 64 / 128 lattice (BASELINE config 1): the register-resident kernel of the batch
+        // path with one replica -- all n sweeps in one launch instead of 2 n launches of 2048 updates
+        if (!lat->d_keys) {
+            if (cudaMalloc(&lat->d_keys, sizeof(RoundKeys)) != cudaSuccess) { cudaGetLastError(); return LATTICE_ENOMEM; }
+            CU(lat, cudaMemcpyAsync(lat->d_keys, &lat->K, sizeof(RoundKeys), cudaMemcpyHostToDevice, lat->stream));
+        }
+        return sweep_tiny(lat, 1u, n, beta);
+    }
     for (uint64_t done = 0; done < n;) {
         // cache-resident lattices: up to 65536 (Blume-Capel: 16384) sweeps per cooperative launch
         const uint64_t cap = lat->model == LATTICE_ISING ? 65536 : 16384;
@@ -1633,8 +1675,19 @@ uint64_t lattice_specialised_launches(const lattice_t *lat) { return lat ? lat->
 
 int lattice_plane_case_specialised(int model, double delta, double beta)
 {
-    if (model != LATTICE_ISING || std::isnan(beta) || beta < 0.0) return 0;
-    (void)delta;
+    if (std::isnan(beta) || beta < 0.0) return 0;
+    if (model == LATTICE_BLUME_CAPEL) {
+        if (std::isnan(delta)) return 0;
+        lattice tmp{};                                       // thresholds only: scheme 1 tables
+        tmp.model = LATTICE_BLUME_CAPEL; tmp.delta = delta; tmp.scheme = 1;
+        refresh_thresholds(&tmp, beta);
+        if (!bc_table_is_integer_dE(&tmp)) return 0;
+        uint32_t lut[8], lut_always = 0;
+        unsigned long long thr[8];
+        bc_fill_integer_dE_luts(&tmp, lut, lut_always, thr);
+        return bc_lut_set_index(lut, lut_always) >= 0 ? 1 : 0;
+    }
+    if (model != LATTICE_ISING) return 0;
     uint64_t thr[2];
     build_thresholds(LATTICE_ISING, 0.0, beta, thr);
     if (thr[0] >= TWO32 || thr[1] >= TWO32) return 0;

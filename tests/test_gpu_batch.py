@@ -56,6 +56,31 @@ def test_tiny_replicas_all_sweeps_in_one_launch(L, n_rep, scheme):
     b.close()
 
 
+@pytest.mark.parametrize("L", [64, 128])
+def test_single_small_lattice_takes_the_register_resident_kernel(L):
+    """A plain (non-batch) Ising lattice with L = 64 / 128: lattice_sweep(n >= 2) is one launch of
+    ising_tiny_kernel with one replica, equal to the oracle and to one sweep per call."""
+    g = lat.Lattice(L, lat.ISING, 0.0, 4711 + L)
+    s = lat.Lattice(L, lat.ISING, 0.0, 4711 + L)
+    o = oracle.OracleLattice(L, lat.ISING, 0.0, 4711 + L)
+    for sched in ([BETA_C] * 40, [BETA_C, 0.0, 0.3, math.inf, 1e-9, BETA_C / 1.01] * 3):
+        n0 = g.launches
+        g.sweep(sched)
+        assert g.launches - n0 == 1
+        n0 = s.launches
+        for b in sched:
+            s.sweep([b])
+        assert s.launches - n0 == 2 * len(sched)
+        o.sweep(sched)
+        assert np.array_equal(g.get_spins(), o.get_spins())
+        assert np.array_equal(s.get_spins(), o.get_spins())
+    assert g.time == s.time == o.time
+    Mg, Qg, Sxg, Syg = g.measure(L // 2)
+    Mo, Qo, Sxo, Syo = o.measure(L // 2)
+    assert (Mg, Qg) == (Mo, Qo) and np.array_equal(Sxg, Sxo) and np.array_equal(Syg, Syo)
+    g.close(); s.close(); o.close()
+
+
 def test_config1_as_a_batch_is_one_launch_and_equals_the_single_lattice():
     """BASELINE config 1 (L = 64, 2000 sweeps at beta_c): replica 0 carries the config's own seed."""
     w = workloads.CONFIGS["ising_L64"]

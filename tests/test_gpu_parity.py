@@ -109,6 +109,38 @@ def test_half_sweeps_and_extreme_temperatures(model, scheme):
         assert np.array_equal(g.get_spins(), o.get_spins()), beta
 
 
+@pytest.mark.parametrize("scheme", [1, 2])
+def test_blume_capel_table_specialised_kernels_are_bit_identical(scheme):
+    """The Blume-Capel counterpart: truth tables compiled in for T = 1.6934 / T_c / T_2 (one set), the
+    plateau of config 5b's ramp and T_1 = 1.24 of the two-step protocol (Table II, PAPER.md:148-152);
+    any other beta, and any Delta != 0, takes the dispatching kernel."""
+    from paper_2503_14688_b200 import workloads
+    sp = lat.lib().lattice_plane_case_specialised
+    specials = [workloads.BETA_BC, 1.0 / 1.69355839821214427017, 1.0 / 1.69661396797728, workloads.BETA_BC / 1.01,
+                1.0 / 1.24]
+    for b in specials:
+        assert sp(lat.BLUME_CAPEL, 0.0, b) == 1
+    assert sp(lat.BLUME_CAPEL, 0.0, 0.3) == 0 and sp(lat.BLUME_CAPEL, 0.0, 0.0) == 0
+    assert sp(lat.BLUME_CAPEL, 0.7, workloads.BETA_BC) == 0
+    L = 1024
+    g = lat.Lattice(L, lat.BLUME_CAPEL, 0.0, 70707, scheme)
+    o = oracle.OracleLattice(L, lat.BLUME_CAPEL, 0.0, 70707, scheme)
+    sched = [specials[0], specials[0], 0.3, specials[3], specials[4], 0.0, specials[1], 0.55, specials[2], specials[4]]
+    for b in sched:                                   # one sweep per call: two plain launches each
+        g.sweep([b])
+    o.sweep(sched)
+    assert g.specialised_launches == 2 * sum(1 for b in sched if b in specials)
+    assert np.array_equal(g.get_spins(), o.get_spins())
+    for fill in (1, 0, -1):                           # ordered states: every lane deciding, ties most frequent
+        g.fill(fill)
+        o.set_spins(np.full((L, L), fill, dtype=np.int8))
+        for b in (specials[0], specials[3], specials[4]):
+            g.sweep([b]); o.sweep([b])
+        assert np.array_equal(g.get_spins(), o.get_spins()), fill
+    _same_measure(g, o, 48, L, 0.0)
+    g.close(); o.close()
+
+
 def test_plane_case_specialised_kernels_are_bit_identical():
     """Launch-time specialisation (compile-time LOP3 truth tables for the betas the workloads run at):
     the specialised instantiations run -- the launch-kind counter says so -- and give the oracle's
