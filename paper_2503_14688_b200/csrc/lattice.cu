@@ -23,6 +23,7 @@
 #include "ising_batch.cuh"
 #include "measure.cuh"
 #include "corr_tc.cuh"
+#include "corr_tc2.cuh"
 #include "philox.cuh"
 #include "ubench.cuh"
 
@@ -1334,7 +1335,7 @@ static bool corr_tc_applies(const lattice *lat, uint64_t n_rows, uint32_t r_max)
 {
     if (lat->measure_path == 1) return false;
     const bool shape_ok = (lat->L % 256u) == 0 && lat->L >= 1024u && n_rows >= 1 && !lat->slab;
-    if (lat->measure_path == 2) return shape_ok;
+    if (lat->measure_path >= 2) return shape_ok;
     return shape_ok && lat->L >= 4096u && n_rows >= 512 && r_max >= 48;
 }
 
@@ -1346,6 +1347,10 @@ static int enqueue_corr_tc(lattice *lat, unsigned long long *cnt, uint64_t i0, u
         cudaFuncSetAttribute(corr_tc_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
         cudaFuncSetAttribute(corr_tc_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
         cudaFuncSetAttribute(corr_tc_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
+        cudaFuncSetAttribute(corr_tc2_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM_BYTES);
+        cudaFuncSetAttribute(corr_tc2_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM_BYTES);
+        cudaFuncSetAttribute(corr_tc2_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM_BYTES);
+        cudaFuncSetAttribute(corr_tc2_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM_BYTES);
         opted = true;
     }
     int dev = 0, sms = 148;
@@ -1357,18 +1362,32 @@ static int enqueue_corr_tc(lattice *lat, unsigned long long *cnt, uint64_t i0, u
     CorrTCArgs a;
     a.buf = lat->buf; a.L = lat->L; a.rows = lat->rows; a.wpr = lat->wpr;
     a.i0 = (uint32_t)i0; a.n_rows = (uint32_t)n_rows; a.r_max = r_max; a.s_stride = 2;
-    a.n_pass = (r_max + TC_M + TC_NT * TC_N - 1) / (TC_NT * TC_N);
+    const bool pairs = lat->measure_path == 3;       // CTA pairs (corr_tc2.cuh) only on request: measured slower so far
+    const uint32_t tile = pairs ? 2u * T2_M : (uint32_t)TC_M;
+    a.n_pass = (r_max + tile + TC_NT * TC_N - 1) / (TC_NT * TC_N);
     for (int axis = 1; axis >= 0; --axis) {
-        a.n_tiles = axis == 1 ? (uint32_t)((n_rows + TC_M - 1) / TC_M) : lat->L / TC_M;
+        a.n_tiles = axis == 1 ? (uint32_t)((n_rows + tile - 1) / tile) : lat->L / tile;
         a.n_items = a.n_tiles * a.n_pass;
         a.S = (long long *)(cnt + 2 + (axis == 1 ? 2 * (size_t)r_max : 0));
-        const unsigned grid = a.n_items < (unsigned)sms ? a.n_items : (unsigned)sms;
-        if (lat->model == LATTICE_ISING) {
-            if (axis == 1) corr_tc_kernel<0, 1><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
-            else corr_tc_kernel<0, 0><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+        if (pairs) {
+            const unsigned most = (unsigned)sms / 2u;
+            const unsigned grid = 2u * (a.n_items < most ? a.n_items : most);       // clusters of two CTAs
+            if (lat->model == LATTICE_ISING) {
+                if (axis == 1) corr_tc2_kernel<0, 1><<<grid, T2_THREADS, T2_SMEM_BYTES, lat->stream>>>(a);
+                else corr_tc2_kernel<0, 0><<<grid, T2_THREADS, T2_SMEM_BYTES, lat->stream>>>(a);
+            } else {
+                if (axis == 1) corr_tc2_kernel<1, 1><<<grid, T2_THREADS, T2_SMEM_BYTES, lat->stream>>>(a);
+                else corr_tc2_kernel<1, 0><<<grid, T2_THREADS, T2_SMEM_BYTES, lat->stream>>>(a);
+            }
         } else {
-            if (axis == 1) corr_tc_kernel<1, 1><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
-            else corr_tc_kernel<1, 0><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+            const unsigned grid = a.n_items < (unsigned)sms ? a.n_items : (unsigned)sms;
+            if (lat->model == LATTICE_ISING) {
+                if (axis == 1) corr_tc_kernel<0, 1><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+                else corr_tc_kernel<0, 0><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+            } else {
+                if (axis == 1) corr_tc_kernel<1, 1><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+                else corr_tc_kernel<1, 0><<<grid, TC_THREADS, TC_SMEM_BYTES, lat->stream>>>(a);
+            }
         }
         lat->launches += 1;
         CU(lat, cudaGetLastError());
@@ -1704,8 +1723,8 @@ int lattice_plane_case_specialised(int model, double delta, double beta)
 
 int lattice_set_measure_path(lattice_t *lat, int path)
 {
-    if (!lat || path < 0 || path > 2) return LATTICE_EINVAL;
-    if (path == 2 && ((lat->L % 256u) != 0 || lat->L < 1024u || lat->slab)) return LATTICE_EINVAL;
+    if (!lat || path < 0 || path > 3) return LATTICE_EINVAL;
+    if (path >= 2 && ((lat->L % 256u) != 0 || lat->L < 1024u || lat->slab)) return LATTICE_EINVAL;
     lat->measure_path = path;
     return LATTICE_OK;
 }

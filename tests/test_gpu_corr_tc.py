@@ -35,23 +35,30 @@ def test_tensor_core_correlations_equal_oracle_and_popcount_path(L, r_max, model
     pop = g.measure(r_max)
     g.set_measure_path(2)
     tc = g.measure(r_max)
-    for got in (pop, tc):
+    g.set_measure_path(3)                           # CTA pairs (tcgen05 cta_group::2, csrc/corr_tc2.cuh)
+    tc2 = g.measure(r_max)
+    for got in (pop, tc, tc2):
         assert (got[0], got[1]) == (want[0], want[1])
         assert np.array_equal(got[2], want[2]), np.nonzero(got[2] != want[2])[0][:8]
         assert np.array_equal(got[3], want[3]), np.nonzero(got[3] != want[3])[0][:8]
     # row ranges: partner rows wrap periodically, base rows end inside a 128-row tile
     for i0, n in ((0, 128), (5, 300), (L - 77, 77), (L // 2 - 1, 1)):
         ws = o.measure(min(r_max, 200), (i0, n))
-        gs = g.measure(min(r_max, 200), (i0, n))
-        assert (gs[0], gs[1]) == (ws[0], ws[1]) and np.array_equal(gs[2], ws[2]) and np.array_equal(gs[3], ws[3]), (i0, n)
+        for path in (2, 3):
+            g.set_measure_path(path)
+            gs = g.measure(min(r_max, 200), (i0, n))
+            assert (gs[0], gs[1]) == (ws[0], ws[1]) and np.array_equal(gs[2], ws[2]) and np.array_equal(gs[3], ws[3]), (i0, n, path)
     # ordered and striped states: |G| = L, every accumulator at its extreme
     i, j = np.indices((L, L))
     for s in (np.ones((L, L), np.int8), np.where(i % 2 == 0, 1, -1).astype(np.int8),
               np.where(j % 4 < 2, 1, -1).astype(np.int8)):
         g.set_spins(s)
         o.set_spins(s)
-        a, b = g.measure(r_max), o.measure(r_max)
-        assert (a[0], a[1]) == (b[0], b[1]) and np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3])
+        b = o.measure(r_max)
+        for path in (2, 3):
+            g.set_measure_path(path)
+            a = g.measure(r_max)
+            assert (a[0], a[1]) == (b[0], b[1]) and np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3]), path
     g.close(); o.close()
 
 
@@ -60,7 +67,9 @@ def test_tensor_core_path_selection_and_errors():
     with pytest.raises(lat.LatticeError):
         g.set_measure_path(2)                       # L < 1024
     with pytest.raises(lat.LatticeError):
-        g.set_measure_path(3)
+        g.set_measure_path(3)                       # CTA pairs: the same shape conditions
+    with pytest.raises(lat.LatticeError):
+        g.set_measure_path(4)
     g.set_measure_path(1)
     g.close()
     b = lat.LatticeBatch(1024, np.arange(3, dtype=np.uint64) + 5)
