@@ -243,9 +243,10 @@ int lattice_plane_case_specialised(int model, double delta, double beta);
  *   0 (default) automatic: the tensor-core path for L >= 4096, >= 512 base rows and r_max >= 48,
  *     else the XOR/popcount kernels;
  *   1 always the XOR/popcount kernels (north_star (c));
- *   2 always the tensor cores (EINVAL unless L is a multiple of 256, L >= 1024, not a slab);
- *   3 the tensor cores with CTA pairs (tcgen05 cta_group::2, csrc/corr_tc2.cuh; same conditions):
- *     exact as well, measured slower than path 2 so far and therefore never chosen automatically.
+ *   2 always the tensor cores (EINVAL unless L is a multiple of 256, L >= 1024, not a slab): CTA pairs
+ *     (tcgen05 cta_group::2, csrc/corr_tc2.cuh) on the y axis, one CTA per item (csrc/corr_tc.cuh) on
+ *     the x axis -- the combination measured fastest;
+ *   3 / 4 CTA pairs / single CTAs on both axes (same conditions; for tests and measurements).
  * The tensor-core path (csrc/corr_tc.cuh) evaluates dense C(r <= r_max), Eq. 2, as
  * the band of the row / column Gram matrix with tcgen05.mma on fp8 copies of the spins (exactly
  * representable; fp32 accumulators hold exact integers up to 2^24 > L); both paths return the same

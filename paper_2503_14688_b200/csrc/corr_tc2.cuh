@@ -160,10 +160,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T2_THREADS, 1) corr_
                 row_l = i % a.rows;
                 word = 0u;                                        // + 2 words (64 packed positions) per step
             } else {
-                const uint32_t rest = it / T2_KC;                 // 0..5
-                srow = it % T2_KC;                                // contraction index = lattice row of the stage
-                h = rest & 1u;
-                mb = rest >> 1;
+                // chunks 0..511: the two partner blocks, the block index varying faster than the upper bits
+                // of the row, so that the 32 lanes of a load read 16 rows x 2 blocks (16 lines, the blocks of a
+                // row are 32 bytes apart) while a quarter-warp still stores to 8 consecutive rows;
+                // chunks 512..767: the base block (srow = contraction index = lattice row of the stage)
+                if (it < 4u * T2_KC) {
+                    srow = ((it >> 4) & 15u) * 8u + (it & 7u);
+                    mb = 1u + ((it >> 3) & 1u);
+                    h = it >> 8;
+                } else {
+                    srow = it % T2_KC;
+                    mb = 0u;
+                    h = (it - 4u * T2_KC) / T2_KC;
+                }
                 row_l = a.i0 + srow;                              // + T2_KC rows per step; never wraps
                 kc_zero = srow < a.n_rows ? (a.n_rows - srow + T2_KC - 1) / T2_KC : 0u;
                 const uint32_t col0 = (mb == 0 ? p0 + T2_M * rank : w0 + (mb - 1u) * T2_N + T2_M * rank) % a.L;

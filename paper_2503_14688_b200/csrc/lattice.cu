@@ -24,6 +24,7 @@
 #include "measure.cuh"
 #include "corr_tc.cuh"
 #include "corr_tc2.cuh"
+#include "corr_transpose.cuh"
 #include "philox.cuh"
 #include "ubench.cuh"
 
@@ -68,6 +69,8 @@ struct lattice {
     uint32_t persist_cap;      // lattice_set_persist_blocks: upper bound on the grid (0: none)
     bool persist_off;          // lattice_set_persist_blocks(UINT32_MAX): never take the persistent path
     void *d_bsp;               // per-sweep parameters of bc_persist_kernel (BCSweepParams)
+    uint32_t *d_tr;            // transposed band of rows for the x-axis correlations (corr_transpose.cuh)
+    size_t tr_cap;             // bytes
     size_t bsp_cap;            // entries
     int measure_path;          // lattice_set_measure_path: 0 auto, 1 XOR/popcount kernels, 2 tensor cores
     // batch of independent replicas (lattice_create_batch): the batch handle owns one child handle
@@ -620,6 +623,7 @@ static void free_handle(lattice *lat)
     if (lat->d_rlist) cudaFree(lat->d_rlist);
     if (lat->d_sp) cudaFree(lat->d_sp);
     if (lat->d_bsp) cudaFree(lat->d_bsp);
+    if (lat->d_tr) cudaFree(lat->d_tr);
     if (lat->d_keys) cudaFree(lat->d_keys);
     if (lat->h_keys) std::free(lat->h_keys);
     if (lat->bk) std::free(lat->bk);
@@ -953,6 +957,7 @@ static int sweep_persistent_bc(lattice *lat, uint64_t n, const double *beta)
     }
     if (lat->bsp_cap < n) {
         if (lat->d_bsp) cudaFree(lat->d_bsp);
+    if (lat->d_tr) cudaFree(lat->d_tr);
         lat->d_bsp = nullptr; lat->bsp_cap = 0;
         const size_t cap = n < 1024 ? 1024 : n;
         if (cudaMalloc(&lat->d_bsp, cap * sizeof(BCSweepParams)) != cudaSuccess) { cudaGetLastError(); std::free(h); return LATTICE_ENOMEM; }
@@ -1362,10 +1367,58 @@ static int enqueue_corr_tc(lattice *lat, unsigned long long *cnt, uint64_t i0, u
     CorrTCArgs a;
     a.buf = lat->buf; a.L = lat->L; a.rows = lat->rows; a.wpr = lat->wpr;
     a.i0 = (uint32_t)i0; a.n_rows = (uint32_t)n_rows; a.r_max = r_max; a.s_stride = 2;
-    const bool pairs = lat->measure_path == 3;       // CTA pairs (corr_tc2.cuh) only on request: measured slower so far
-    const uint32_t tile = pairs ? 2u * T2_M : (uint32_t)TC_M;
-    a.n_pass = (r_max + tile + TC_NT * TC_N - 1) / (TC_NT * TC_N);
+    // x axis on a transposed copy, band by band (corr_transpose.cuh), with the y-axis pair kernel: whole
+    // 512-row bands of an even first row when a lattice row is a whole number of 32-word groups; the
+    // remaining rows (and any other shape, or no memory for the copy) take the MN-major kernel below
+    uint64_t x_done = 0;
+    if ((lat->measure_path == 0 || lat->measure_path == 2) && (lat->wpr % 32u) == 0 && (i0 % 2u) == 0 && n_rows >= 512) {
+        const uint32_t planes = lat->model == LATTICE_ISING ? 2u : 4u;
+        const uint64_t full = n_rows / 512u * 512u;
+        const uint32_t Bmax = full < 65536u ? (uint32_t)full : 65536u;
+        const size_t need = (size_t)planes * lat->L * (Bmax / 64u) * sizeof(uint32_t);
+        if (lat->tr_cap < need) {
+            if (lat->d_tr) cudaFree(lat->d_tr);
+            lat->d_tr = nullptr; lat->tr_cap = 0;
+            if (cudaMalloc(&lat->d_tr, need) == cudaSuccess) lat->tr_cap = need;
+            else cudaGetLastError();
+        }
+        if (lat->tr_cap >= need) {
+            for (uint64_t b0 = 0; b0 < full; b0 += Bmax) {
+                const uint32_t B = full - b0 < Bmax ? (uint32_t)(full - b0) : Bmax;
+                TransposeArgs t;
+                t.src = lat->buf; t.dst = lat->d_tr; t.rows = lat->rows; t.wpr = lat->wpr;
+                t.i0 = (uint32_t)(i0 + b0); t.B = B; t.L = lat->L; t.bc = lat->model == LATTICE_ISING ? 0u : 1u;
+                band_transpose_kernel<<<dim3(lat->wpr / 32u, B / 512u, planes * 2u), 256, 0, lat->stream>>>(t);
+                lat->launches += 1;
+                CU(lat, cudaGetLastError());
+                CorrTCArgs x;
+                x.buf = lat->d_tr; x.L = B; x.rows = lat->L; x.wpr = B / 64u;
+                x.i0 = 0; x.n_rows = lat->L; x.r_max = r_max; x.s_stride = 2;
+                x.n_pass = (r_max + 2u * T2_M + TC_NT * TC_N - 1) / (TC_NT * TC_N);
+                x.n_tiles = (lat->L + 2u * T2_M - 1) / (2u * T2_M);
+                x.n_items = x.n_tiles * x.n_pass;
+                x.S = (long long *)(cnt + 2);
+                const unsigned most = (unsigned)sms / 2u;
+                const unsigned grid = 2u * (x.n_items < most ? x.n_items : most);
+                if (lat->model == LATTICE_ISING) corr_tc2_kernel<0, 1><<<grid, T2_THREADS, T2_SMEM_BYTES, lat->stream>>>(x);
+                else corr_tc2_kernel<1, 1><<<grid, T2_THREADS, T2_SMEM_BYTES, lat->stream>>>(x);
+                lat->launches += 1;
+                CU(lat, cudaGetLastError());
+            }
+            x_done = full;
+        }
+    }
     for (int axis = 1; axis >= 0; --axis) {
+        if (axis == 0) {
+            if (x_done == n_rows) break;
+            a.i0 = (uint32_t)(i0 + x_done); a.n_rows = (uint32_t)(n_rows - x_done);
+        }
+        // CTA pairs (corr_tc2.cuh) on the y axis, one CTA per item (corr_tc.cuh) on the x axis: what is
+        // measured fastest at L = 2^20 (y: 3.9 s against 5.0 s; x: 7.0 s against 6.0 s, where the pair
+        // kernel reads more DRAM sectors).  Paths 3 / 4 force pairs / single CTAs on both axes (tests).
+        const bool pairs = lat->measure_path == 3 || (lat->measure_path != 4 && axis == 1);
+        const uint32_t tile = pairs ? 2u * T2_M : (uint32_t)TC_M;
+        a.n_pass = (r_max + tile + TC_NT * TC_N - 1) / (TC_NT * TC_N);
         a.n_tiles = axis == 1 ? (uint32_t)((n_rows + tile - 1) / tile) : lat->L / tile;
         a.n_items = a.n_tiles * a.n_pass;
         a.S = (long long *)(cnt + 2 + (axis == 1 ? 2 * (size_t)r_max : 0));
@@ -1723,7 +1776,7 @@ int lattice_plane_case_specialised(int model, double delta, double beta)
 
 int lattice_set_measure_path(lattice_t *lat, int path)
 {
-    if (!lat || path < 0 || path > 3) return LATTICE_EINVAL;
+    if (!lat || path < 0 || path > 4) return LATTICE_EINVAL;
     if (path >= 2 && ((lat->L % 256u) != 0 || lat->L < 1024u || lat->slab)) return LATTICE_EINVAL;
     lat->measure_path = path;
     return LATTICE_OK;

@@ -35,16 +35,18 @@ def test_tensor_core_correlations_equal_oracle_and_popcount_path(L, r_max, model
     pop = g.measure(r_max)
     g.set_measure_path(2)
     tc = g.measure(r_max)
-    g.set_measure_path(3)                           # CTA pairs (tcgen05 cta_group::2, csrc/corr_tc2.cuh)
+    g.set_measure_path(3)                           # CTA pairs (tcgen05 cta_group::2, csrc/corr_tc2.cuh) on both axes
     tc2 = g.measure(r_max)
-    for got in (pop, tc, tc2):
+    g.set_measure_path(4)                           # one CTA per item (csrc/corr_tc.cuh) on both axes
+    tc1 = g.measure(r_max)
+    for got in (pop, tc, tc2, tc1):
         assert (got[0], got[1]) == (want[0], want[1])
         assert np.array_equal(got[2], want[2]), np.nonzero(got[2] != want[2])[0][:8]
         assert np.array_equal(got[3], want[3]), np.nonzero(got[3] != want[3])[0][:8]
     # row ranges: partner rows wrap periodically, base rows end inside a 128-row tile
     for i0, n in ((0, 128), (5, 300), (L - 77, 77), (L // 2 - 1, 1)):
         ws = o.measure(min(r_max, 200), (i0, n))
-        for path in (2, 3):
+        for path in (2, 3, 4):
             g.set_measure_path(path)
             gs = g.measure(min(r_max, 200), (i0, n))
             assert (gs[0], gs[1]) == (ws[0], ws[1]) and np.array_equal(gs[2], ws[2]) and np.array_equal(gs[3], ws[3]), (i0, n, path)
@@ -55,10 +57,32 @@ def test_tensor_core_correlations_equal_oracle_and_popcount_path(L, r_max, model
         g.set_spins(s)
         o.set_spins(s)
         b = o.measure(r_max)
-        for path in (2, 3):
+        for path in (2, 3, 4):
             g.set_measure_path(path)
             a = g.measure(r_max)
             assert (a[0], a[1]) == (b[0], b[1]) and np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3]), path
+    g.close(); o.close()
+
+
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+def test_x_axis_on_the_transposed_bands(model):
+    """L a multiple of 2048: the x axis of the tensor-core path runs the y-axis pair kernel on a
+    transposed copy of whole 512-row bands (csrc/corr_transpose.cuh) and the MN-major kernel on the
+    rows that are left; odd first rows and short ranges take the MN-major kernel alone.  All of it
+    against the oracle."""
+    L, r_max = 4096, 300
+    g = lat.Lattice(L, model, 0.0, 27182)
+    o = oracle.OracleLattice(L, model, 0.0, 27182)
+    beta = workloads.BETA_C_ISING if model == lat.ISING else workloads.BETA_BC
+    g.sweep([beta] * 8)
+    o.sweep([beta] * 8)
+    g.set_measure_path(2)
+    for rows in (None, (0, 1536), (1024, 700), (1, 600), (2048, 2048), (3584, 512)):
+        n0 = g.launches
+        a, b = g.measure(r_max, rows), o.measure(r_max, rows)
+        assert (a[0], a[1]) == (b[0], b[1]) and np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3]), rows
+        if rows in (None, (2048, 2048), (3584, 512)):
+            assert g.launches - n0 == 1 + 1 + 2           # M/Q, y axis, transpose + x axis on the copy
     g.close(); o.close()
 
 
@@ -69,7 +93,7 @@ def test_tensor_core_path_selection_and_errors():
     with pytest.raises(lat.LatticeError):
         g.set_measure_path(3)                       # CTA pairs: the same shape conditions
     with pytest.raises(lat.LatticeError):
-        g.set_measure_path(4)
+        g.set_measure_path(5)
     g.set_measure_path(1)
     g.close()
     b = lat.LatticeBatch(1024, np.arange(3, dtype=np.uint64) + 5)
