@@ -440,7 +440,7 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
     if measure_pass and rank == 0:
         r_meas = w.r_max if args.measure_rmax < 0 else args.measure_rmax
         r_meas = max(1, min(r_meas, L // 2))
-        # the tensor-core path (csrc/corr_tc.cuh) does C(r <= 4096) at L = 2^20 in ~12 s: the default run
+        # the tensor-core path (csrc/corr_tc2.cuh) does C(r <= 4096) at L = 2^20 in ~8 s: the default run
         # measures the workload's full r_max; only where that path does not apply (L < 4096) and the
         # XOR/popcount kernels would take long is r_max bounded (an explicit --measure-rmax is honoured)
         words = L * L // 32
@@ -464,7 +464,7 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
             same = all(int(Sxl[k]) == int(Sx[r - 1]) and int(Syl[k]) == int(Sy[r - 1]) for k, r in enumerate(rl))
             sparse = {"points": len(rl), "r_last": rl[-1], "ms": ev2.elapsed_time(ev3), "equals_dense": bool(same and Ml == M)}
         meas = {"r_max": r_meas, "ms": ev0.elapsed_time(ev1), "t": g.time, "M": M,
-                "path": "tensor cores (tcgen05 banded Gram, csrc/corr_tc.cuh)" if (L >= 4096 and r_meas >= 48)
+                "path": "tensor cores (tcgen05 banded Gram: CTA pairs, x axis on transposed bands; csrc/corr_tc2.cuh, corr_transpose.cuh)" if (L >= 4096 and r_meas >= 48)
                         else "XOR/popcount kernels (csrc/measure.cuh)",
                 "e": lat.energy(Sx, Sy, Q, w.delta, L), "xi": xi_v, "r_cut": r_cut, "sparse_list": sparse}
     # ---- worst-case input: the all-up state (every site has 4 aligned neighbours, so every

@@ -247,10 +247,14 @@ int lattice_plane_case_specialised(int model, double delta, double beta);
  *     (tcgen05 cta_group::2, csrc/corr_tc2.cuh) on the y axis, one CTA per item (csrc/corr_tc.cuh) on
  *     the x axis -- the combination measured fastest;
  *   3 / 4 CTA pairs / single CTAs on both axes (same conditions; for tests and measurements).
- * The tensor-core path (csrc/corr_tc.cuh) evaluates dense C(r <= r_max), Eq. 2, as
- * the band of the row / column Gram matrix with tcgen05.mma on fp8 copies of the spins (exactly
- * representable; fp32 accumulators hold exact integers up to 2^24 > L); both paths return the same
- * exact integer counts. */
+ * The tensor-core path evaluates dense C(r <= r_max), Eq. 2, as the band of the row /
+ * column Gram matrix with tcgen05.mma on fp8 copies of the spins (exactly representable; fp32
+ * accumulators hold exact integers up to 2^24 > L); all paths return the same exact integer counts.
+ * Device memory: for lattices with L a multiple of 2048 the x axis is evaluated on a transposed copy
+ * of up to 65536 rows at a time (csrc/corr_transpose.cuh), which the library allocates on first use
+ * and keeps until lattice_destroy: lattice_state_bytes(L, model) * min(n_rows, 65536) / L bytes
+ * (8 GiB at L = 2^20).  If that allocation fails the copy-free kernel is used instead (slower, same
+ * counts). */
 int lattice_set_measure_path(lattice_t *lat, int path);
 /* The persistent multi-sweep kernels: lattice_sweep(n >= 2) on a
  * cache-resident lattice can run all n sweeps in ONE cooperative launch with a grid barrier per

@@ -1,5 +1,9 @@
 // corr_tc.cuh -- dense axis correlations S_x(r), S_y(r), r <= r_max, on the 5th-generation tensor
-// cores (tcgen05 + TMEM).
+// cores (tcgen05 + TMEM): the one-CTA-per-item kernel.  Since round 2's last third the CTA-pair
+// kernel of corr_tc2.cuh (which reuses the helpers and the operand encoding defined here) takes the y
+// axis and, on transposed bands (corr_transpose.cuh), the x axis; this kernel keeps the x axis of rows
+// that are not whole 512-row bands, of odd first rows and of lattices with L not a multiple of 2048 (its
+// MN-major operands need no copy), and both axes on request (lattice_set_measure_path 4).
 //
 // Paper: C(r;t), Eq. 2, along the lattice axes.  Dense in r this IS a dense
 // contraction: S_y(r) = sum_i G[i, i+r] with the band of the row Gram matrix

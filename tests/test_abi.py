@@ -190,4 +190,12 @@ def test_plane_case_specialisations_match_the_config_betas():
     assert f(w.model, 0.0, w.beta_1) == 1 and f(w.model, 0.0, w.beta_f) == 1
     w = workloads.CONFIGS["ising_L2p16_ramp"]
     assert f(w.model, 0.0, w.beta_f) == 1                       # the plateau after the ramp
-    assert f(lat.ISING, 0.0, 0.2) == 0 and f(lat.BLUME_CAPEL, 0.0, workloads.BETA_BC) == 0
+    assert f(lat.ISING, 0.0, 0.2) == 0
+    # Blume-Capel: the truth-table sets of bc_march.cuh (config 3, the paper's T_c, both two-step temperatures,
+    # the plateau of config 5b's ramp); no set for another beta or for a crystal field
+    for name in ("bc_L16384", "bc_L2p19", "bc_L2p15_ramp"):
+        w = workloads.CONFIGS[name]
+        assert f(w.model, w.delta, w.beta_f) == 1, name
+    w = workloads.CONFIGS["bc_L2p16_twostep"]
+    assert f(w.model, 0.0, w.beta_1) == 1 and f(w.model, 0.0, w.beta_f) == 1
+    assert f(lat.BLUME_CAPEL, 0.0, 0.3) == 0 and f(lat.BLUME_CAPEL, 0.7, workloads.BETA_BC) == 0

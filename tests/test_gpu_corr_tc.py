@@ -86,6 +86,29 @@ def test_x_axis_on_the_transposed_bands(model):
     g.close(); o.close()
 
 
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+def test_tensor_core_path_on_a_view(model):
+    """A measurement-only view (not periodic along y; how a slab measures C(r) for r > 1): base rows
+    0..1023 of a buffer holding rows 0..1023+r_max of an L = 4096 lattice take the tensor-core path by
+    themselves (x axis on the transposed band) and give the oracle's partial sums."""
+    L, n, r_max = 4096, 1024, 300
+    g = lat.Lattice(L, model, 0.0, 16180)
+    o = oracle.OracleLattice(L, model, 0.0, 16180)
+    beta = workloads.BETA_C_ISING if model == lat.ISING else workloads.BETA_BC
+    g.sweep([beta] * 6)
+    o.sweep([beta] * 6)
+    planes = 2 if model == lat.ISING else 4
+    rows = n + r_max
+    import torch
+    g.synchronize()
+    view = g.buf.view(planes, L, L // 64 * 4)[:, :rows].contiguous()
+    torch.cuda.synchronize()
+    M, Q, Sx, Sy = lat.measure_buffer(L, model, rows, n, r_max, view.data_ptr(), view.numel(), g.stream.cuda_stream)
+    Mo, Qo, Sxo, Syo = o.measure(r_max, (0, n))
+    assert (M, Q) == (Mo, Qo) and np.array_equal(Sx, Sxo) and np.array_equal(Sy, Syo)
+    g.close(); o.close()
+
+
 def test_tensor_core_path_selection_and_errors():
     g = lat.Lattice(256, lat.ISING, 0.0, 1)
     with pytest.raises(lat.LatticeError):
