@@ -103,7 +103,8 @@ def test_tensor_core_path_on_a_view(model):
     g.synchronize()
     view = g.buf.view(planes, L, L // 64 * 4)[:, :rows].contiguous()
     torch.cuda.synchronize()
-    M, Q, Sx, Sy = lat.measure_buffer(L, model, rows, n, r_max, view.data_ptr(), view.numel(), g.stream.cuda_stream)
+    M, Q, Sx, Sy = lat.binding.measure_buffer(L, model, rows, n, r_max, view.data_ptr(), view.numel(),
+                                                 g.stream.cuda_stream)
     Mo, Qo, Sxo, Syo = o.measure(r_max, (0, n))
     assert (M, Q) == (Mo, Qo) and np.array_equal(Sx, Sxo) and np.array_equal(Sy, Syo)
     g.close(); o.close()
