@@ -130,6 +130,20 @@ int lattice_create_slab(lattice_t **out, uint32_t L, int model, double delta, ui
 int lattice_slab_set_neighbours(lattice_t *lat, void *device_up_buf, uint32_t up_n_rows,
                                 void *device_down_buf, uint32_t down_n_rows);
 
+/* Device-side ordering of the colours (csrc/slab_flags.cuh): instead of the caller waiting between the
+ * half-sweeps, every slab publishes the number of half-sweeps it has completed, 2 t + colour + 1 after
+ * colour `colour` of sweep t, in a 64-bit word of device memory (8-byte aligned, e.g. behind its slab
+ * buffer), and every half-sweep launch of this handle is preceded by a one-thread kernel that waits
+ * until both neighbours' words have reached the previous half-sweep, and followed by one that
+ * publishes its own (release, system scope).  The neighbours' words may be peer-GPU or IPC memory.
+ * lattice_slab_set_flags publishes 2 * lattice_time() (so does lattice_set_time); the caller makes sure
+ * that every slab has done so before the first half-sweep (one host barrier at set-up), and that all
+ * slabs are given the same sequence of half-sweeps.  Three NULLs switch back to host ordering.
+ * The wait is bounded (~17 s, then the kernel traps: ECUDA on the next call).
+ * Errors: EINVAL (NULL handle, some but not all pointers NULL, misaligned), ESTATE (not a slab), ECUDA. */
+int lattice_slab_set_flags(lattice_t *lat, void *device_my_flag, const void *device_up_flag,
+                           const void *device_down_flag);
+
 /* A measurement-only handle over a caller-assembled buffer [colour(/plane)][rows][L/64] that is
  * NOT periodic along y: lattice_measure_rows(view, i0, n, r_max, ...) requires
  * i0 + n + r_max <= rows (partner rows i + r are read from the buffer as they are); the x axis

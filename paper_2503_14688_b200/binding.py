@@ -37,6 +37,7 @@ SIGNATURES = {
     "lattice_slab_bytes": (C.c_size_t, [C.c_uint32, C.c_int, C.c_uint32]),
     "lattice_create_slab": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_double, C.c_uint64,
                                       C.c_uint32, C.c_uint32, _vp, C.c_size_t, _vp]),
+    "lattice_slab_set_flags": (C.c_int, [_vp, _vp, _vp, _vp]),
     "lattice_slab_set_neighbours": (C.c_int, [_vp, _vp, C.c_uint32, _vp, C.c_uint32]),
     "lattice_view": (C.c_int, [C.POINTER(_vp), C.c_uint32, C.c_int, C.c_uint32, _vp, C.c_size_t, _vp]),
     "lattice_device_copy": (C.c_int, [_vp, _vp, C.c_size_t, _vp]),
@@ -90,6 +91,9 @@ def lib() -> C.CDLL:
         fn.argtypes = args
     _lib = L
     return L
+
+
+FLAG_BYTES = 64            # room behind a slab buffer for its 64-bit flag word (keeps 16-byte alignment)
 
 
 class LatticeError(RuntimeError):
@@ -212,6 +216,9 @@ class Lattice:
             nbytes = int(lib().lattice_slab_bytes(self.L, self.model, self.slab[1]))
         if nbytes == 0:
             raise LatticeError("lattice_state_bytes", EINVAL, f"L={L} model={model} slab={slab}")
+        self.state_nbytes = nbytes
+        if self.slab is not None:
+            nbytes += FLAG_BYTES                     # the slab's flag word lives behind its rows (set_flags)
         self._torch = torch
         self.device = torch.device(device)
         self._own_ptr = None
@@ -298,8 +305,22 @@ class Lattice:
         self._check(lib().lattice_slab_set_neighbours(self._h, _vp(up_ptr), up_rows, _vp(down_ptr), down_rows),
                     "lattice_slab_set_neighbours")
 
+    @property
+    def flag_ptr(self) -> int:
+        """Device address of this slab's flag word (behind its rows)."""
+        return self.data_ptr + self.state_nbytes
+
+    def set_flags(self, up_flag_ptr: int, down_flag_ptr: int) -> None:
+        """Row-slab mode: order the colours on the device (include/lattice.h, lattice_slab_set_flags).
+        The neighbours' flag words are `neighbour.flag_ptr` (or the address of the neighbour's buffer
+        opened from its IPC handle + its slab bytes)."""
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_slab_set_flags(self._h, _vp(self.flag_ptr), _vp(up_flag_ptr), _vp(down_flag_ptr)),
+                        "lattice_slab_set_flags")
+
     def set_time(self, t: int) -> None:
-        self._check(lib().lattice_set_time(self._h, int(t)), "lattice_set_time")
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_set_time(self._h, int(t)), "lattice_set_time")
 
     def sweep(self, beta) -> None:
         """Run len(beta) sweeps; beta is a host fp64 array (one entry per sweep)."""
@@ -433,8 +454,22 @@ class LatticeBatch:
     def launches(self) -> int:
         return int(lib().lattice_launches(self._h))
 
+    @property
+    def flag_ptr(self) -> int:
+        """Device address of this slab's flag word (behind its rows)."""
+        return self.data_ptr + self.state_nbytes
+
+    def set_flags(self, up_flag_ptr: int, down_flag_ptr: int) -> None:
+        """Row-slab mode: order the colours on the device (include/lattice.h, lattice_slab_set_flags).
+        The neighbours' flag words are `neighbour.flag_ptr` (or the address of the neighbour's buffer
+        opened from its IPC handle + its slab bytes)."""
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_slab_set_flags(self._h, _vp(self.flag_ptr), _vp(up_flag_ptr), _vp(down_flag_ptr)),
+                        "lattice_slab_set_flags")
+
     def set_time(self, t: int) -> None:
-        self._check(lib().lattice_set_time(self._h, int(t)), "lattice_set_time")
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_set_time(self._h, int(t)), "lattice_set_time")
 
     def sweep(self, beta) -> None:
         b = np.ascontiguousarray(np.atleast_1d(beta), dtype=np.float64)

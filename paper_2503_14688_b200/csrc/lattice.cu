@@ -27,6 +27,7 @@
 #include "corr_transpose.cuh"
 #include "philox.cuh"
 #include "ubench.cuh"
+#include "slab_flags.cuh"
 
 using namespace lat;
 
@@ -39,6 +40,8 @@ struct lattice {
     bool view;                 // handle over a caller-assembled [planes][rows][wpr] buffer: measurement only
     uint32_t *mir_up[2][2], *mir_dn[2][2];   // slab: per colour and plane, the neighbours' halo rows
     bool have_nbr;
+    unsigned long long *flag_my;             // lattice_slab_set_flags: completed half-sweeps of this slab ...
+    const unsigned long long *flag_up, *flag_dn;   // ... and of the neighbours (peer / IPC memory); null: host-ordered
     uint32_t wpr;              // words per row per colour (per plane)
     int model;
     double delta;
@@ -441,12 +444,23 @@ int launch_half_sweep(lattice *lat, int colour)
     if (lat->view || lat->n_rep) return LATTICE_ESTATE;
     if (lat->slab) {
         if (!lat->have_nbr) return LATTICE_ESTATE;
-        if (lat->model == LATTICE_ISING) return launch_ising_march(lat, colour);
         // Blume-Capel slabs run only the marching kernels: the Delta = 0 type table, or any table
         // with |Delta| <= 4 (bc_march.cuh)
-        if (bc_table_is_integer_dE(lat)) return launch_bc_march(lat, colour);
-        if (bc_table_is_general_ok(lat)) return launch_bc_march(lat, colour, true);
-        return LATTICE_EINVAL;
+        const bool bc_int = lat->model == LATTICE_BLUME_CAPEL && bc_table_is_integer_dE(lat);
+        if (lat->model == LATTICE_BLUME_CAPEL && !bc_int && !bc_table_is_general_ok(lat)) return LATTICE_EINVAL;
+        const unsigned long long h = 2ull * lat->t + (unsigned)colour + 1ull;     // this half-sweep's number
+        if (lat->flag_my) {                      // device-side ordering (slab_flags.cuh)
+            slab_wait_kernel<<<1, 1, 0, lat->stream>>>(lat->flag_up, lat->flag_dn, h - 1ull);
+            lat->launches += 1;
+        }
+        const int rc = lat->model == LATTICE_ISING ? launch_ising_march(lat, colour) : launch_bc_march(lat, colour, !bc_int);
+        if (rc) return rc;
+        if (lat->flag_my) {
+            slab_publish_kernel<<<1, 1, 0, lat->stream>>>(lat->flag_my, h);
+            lat->launches += 1;
+            CU(lat, cudaGetLastError());
+        }
+        return LATTICE_OK;
     }
     if (lat->model == LATTICE_BLUME_CAPEL && lat->scheme >= 1 && (lat->wpr % 4u) == 0) {
         if (bc_table_is_integer_dE(lat)) return launch_bc_march(lat, colour);
@@ -1732,6 +1746,30 @@ int lattice_set_time(lattice_t *lat, uint64_t t)
     if (!lat || t >= TWO32) return LATTICE_EINVAL;
     if (lat->view || lat->parent) return LATTICE_ESTATE;
     lat->t = t;
+    if (lat->flag_my) {                          // the slab's published count follows (2 t half-sweeps done)
+        slab_publish_kernel<<<1, 1, 0, lat->stream>>>(lat->flag_my, 2ull * t);
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+    }
+    return LATTICE_OK;
+}
+
+int lattice_slab_set_flags(lattice_t *lat, void *device_my_flag, const void *device_up_flag, const void *device_down_flag)
+{
+    if (!lat) return LATTICE_EINVAL;
+    if (!lat->slab) return LATTICE_ESTATE;
+    if (!device_my_flag && !device_up_flag && !device_down_flag) {           // back to host-ordered colours
+        lat->flag_my = nullptr; lat->flag_up = lat->flag_dn = nullptr;
+        return LATTICE_OK;
+    }
+    if (!device_my_flag || !device_up_flag || !device_down_flag) return LATTICE_EINVAL;
+    if (((uintptr_t)device_my_flag | (uintptr_t)device_up_flag | (uintptr_t)device_down_flag) & 7u) return LATTICE_EINVAL;
+    lat->flag_my = (unsigned long long *)device_my_flag;
+    lat->flag_up = (const unsigned long long *)device_up_flag;
+    lat->flag_dn = (const unsigned long long *)device_down_flag;
+    slab_publish_kernel<<<1, 1, 0, lat->stream>>>(lat->flag_my, 2ull * lat->t);
+    lat->launches += 1;
+    CU(lat, cudaGetLastError());
     return LATTICE_OK;
 }
 

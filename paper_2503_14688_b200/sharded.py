@@ -22,7 +22,10 @@ from . import binding as lat
 
 class ShardedLattice:
     def __init__(self, L: int, n_slabs: int, seed: int = 0, devices=None, model: int = lat.ISING,
-                 delta: float = 0.0):
+                 delta: float = 0.0, device_flags: bool = False):
+        """device_flags = True: the colours are ordered on the device (lattice_slab_set_flags: every
+        half-sweep launch waits for the neighbours' published counts) instead of by stream order /
+        events from the host."""
         import torch
         if n_slabs < 1 or L % n_slabs:
             raise ValueError("n_slabs must divide L")
@@ -41,12 +44,18 @@ class ShardedLattice:
                 if nb.device != s.device:
                     lat.enable_peer_access(s.device.index, nb.device.index)
             s.set_neighbours(up, down)
+        self.device_flags = bool(device_flags)
+        if self.device_flags:
+            for k, s in enumerate(self.slabs):
+                s.set_flags(self.slabs[(k - 1) % n_slabs].flag_ptr, self.slabs[(k + 1) % n_slabs].flag_ptr)
         self._t = 0
-        self.synchronize()
+        self.synchronize()                            # every slab has published its count before any sweep
 
     # -- ordering -------------------------------------------------------------------------------
     def _fence(self) -> None:
         """All slabs have finished (and mirrored) the colour just launched before the next starts."""
+        if self.device_flags:
+            return                                    # ordered on the device (slab_flags.cuh)
         if not self._multi_device:
             streams = {s.stream.cuda_stream for s in self.slabs}
             if len(streams) == 1:
@@ -104,11 +113,11 @@ class ShardedLattice:
             # own rows, then r_max rows from the slabs below (possibly several, periodic)
             pieces = []
             for p in range(planes):
-                own = s.buf.view(planes, rows + 2, wpr * 4)[p, 1:rows + 1]
+                own = s.buf[:s.state_nbytes].view(planes, rows + 2, wpr * 4)[p, 1:rows + 1]
                 ext, need, j = [own], r_max, k
                 while need > 0:
                     j = (j + 1) % self.n
-                    nb = self.slabs[j].buf.view(planes, rows + 2, wpr * 4)[p, 1:1 + min(need, rows)]
+                    nb = self.slabs[j].buf[:self.slabs[j].state_nbytes].view(planes, rows + 2, wpr * 4)[p, 1:1 + min(need, rows)]
                     ext.append(nb.to(s.device))
                     need -= min(need, rows)
                 pieces.append(torch.cat(ext, dim=0))
@@ -155,7 +164,10 @@ class SlabRank:
     all-reduce of the measurement counts."""
 
     def __init__(self, L: int, seed: int = 0, model: int = lat.ISING, delta: float = 0.0,
-                 device: str = "cuda:0", group=None):
+                 device: str = "cuda:0", group=None, device_flags: bool = False):
+        """device_flags = True: no barrier per half-sweep; the ranks' kernels wait for each other's
+        published counts (lattice_slab_set_flags).  For one rank per PHYSICAL GPU only: ranks that
+        share a GPU must not run kernels that wait on one another."""
         import torch
         import torch.distributed as dist
         self._torch, self._dist, self.group = torch, dist, group
@@ -177,8 +189,15 @@ class SlabRank:
             self._opened = [p_up] if self.world == 2 else [p_up, p_down]
             self._down_ptr = p_down
             self.lat.set_neighbour_ptrs(p_up, rows, p_down, rows)
+        self.device_flags = bool(device_flags)
+        if self.device_flags:
+            nb = self.lat.state_nbytes                # every rank's slab has the same size
+            if self.world == 1:
+                self.lat.set_flags(self.lat.flag_ptr, self.lat.flag_ptr)
+            else:
+                self.lat.set_flags(p_up + nb, p_down + nb)
         self._t = 0
-        self._fence()
+        self._fence()                                 # every rank has published its count
 
     def _fence(self) -> None:
         self.lat.synchronize()
@@ -193,7 +212,8 @@ class SlabRank:
         for b in np.atleast_1d(np.asarray(beta, dtype=np.float64)):
             for colour in (0, 1):
                 self.lat.half_sweep(colour, float(b))
-                self._fence()                        # every rank's mirrors have landed
+                if not self.device_flags:
+                    self._fence()                    # every rank's mirrors have landed
             self._t += 1
             self.lat.set_time(self._t)
 

@@ -105,6 +105,46 @@ def test_sharded_across_physical_devices(model):
     sh.close(); g.close()
 
 
+@pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
+def test_device_side_flags_order_the_colours(model):
+    """lattice_slab_set_flags: every half-sweep launch is wait kernel + marching kernel + publish kernel.
+    All slabs share one device and one stream here, so the neighbours' counts are always there when a
+    wait kernel runs (a wait that really spins must not be run on one GPU: B200_PROFILING.md); what is
+    checked is the published arithmetic, the launch sequence and that nothing else changes: spins equal
+    the host-ordered sharded lattice, the unsharded one and the oracle."""
+    import torch
+    L, n = 1024, 4
+    beta = BETA_C if model == lat.ISING else workloads.BETA_BC
+    sh = ShardedLattice(L, n, seed=99, model=model, device_flags=True)
+    ho = ShardedLattice(L, n, seed=99, model=model)
+    o = oracle.OracleLattice(L, model, 0.0, 99)
+    sched = [beta] * 5 + [0.0, beta, 0.7 * beta]
+    n0 = sh.slabs[0].launches
+    sh.sweep(sched)
+    ho.sweep(sched)
+    o.sweep(sched)
+    # per sweep and slab: 2 x (wait + march + publish) + the publish of set_time
+    assert sh.slabs[0].launches - n0 == len(sched) * 7
+    sh.synchronize()
+    for s in sh.slabs:
+        flag = s.buf[s.state_nbytes:s.state_nbytes + 8].view(torch.int64).item()
+        assert flag == 2 * len(sched)
+    want = o.get_spins()
+    assert np.array_equal(sh.get_spins(), want)
+    assert np.array_equal(ho.get_spins(), want)
+    assert sh.measure(1) == ho.measure(1)
+    # a checkpoint-style time change republishes the count
+    for d in (sh, ho):
+        for s in d.slabs:
+            s.set_time(100)
+        d._t = 100
+        d.sweep([beta] * 2)
+    sh.synchronize()
+    assert sh.slabs[2].buf[sh.slabs[2].state_nbytes:sh.slabs[2].state_nbytes + 8].view(torch.int64).item() == 204
+    assert np.array_equal(sh.get_spins(), ho.get_spins())
+    sh.close(); ho.close(); o.close()
+
+
 def test_slab_api_errors():
     L = 256
     with pytest.raises(lat.LatticeError):
