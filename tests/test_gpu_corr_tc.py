@@ -64,6 +64,21 @@ def test_tensor_core_correlations_equal_oracle_and_popcount_path(L, r_max, model
     g.close(); o.close()
 
 
+def test_transposed_bands_with_a_row_length_that_is_not_a_power_of_two():
+    """L = 6144 = 3 * 2048: 96 words per row, 24 pair tiles, the partner windows wrap at a tile boundary."""
+    L, r_max = 6144, 600
+    g = lat.Lattice(L, lat.ISING, 0.0, 14142)
+    o = oracle.OracleLattice(L, lat.ISING, 0.0, 14142)
+    g.sweep([workloads.BETA_C_ISING] * 5)
+    o.sweep([workloads.BETA_C_ISING] * 5)
+    for path in (2, 3, 4):
+        g.set_measure_path(path)
+        for rows in (None, (2048, 3072)):
+            a, b = g.measure(r_max, rows), o.measure(r_max, rows)
+            assert (a[0], a[1]) == (b[0], b[1]) and np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3]), (path, rows)
+    g.close(); o.close()
+
+
 @pytest.mark.parametrize("model", [lat.ISING, lat.BLUME_CAPEL])
 def test_x_axis_on_the_transposed_bands(model):
     """L a multiple of 2048: the x axis of the tensor-core path runs the y-axis pair kernel on a
