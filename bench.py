@@ -36,7 +36,9 @@ One JSON line is printed by rank 0:
   cpu_baseline  the oracle, as it stands, on the host cores over bounded samples: `value` is the
             all-cores figure for the timed model and RNG scheme; `matrix` holds 1 thread and all
             cores x schemes 0/1 x both models, `cpu_model` the CPU
-  measure   the measurement pass (M, Q, C(r) on both axes) timed separately after the sweeps
+  measure   the measurement pass (M, Q, C(r) on both axes) timed separately after the sweeps; on the
+            tensor-core path with its own `roofline` ("bound": "tensor"): band-Gram flops / time against
+            2 x the measured sustained bf16 peak (fp8 operands)
 
 N > 1 (torchrun): the path is specified for one GPU with no collectives (BASELINE.json
 north_star), so every rank runs an independent replica (own seed) -- "replicas only", weak
@@ -463,7 +465,25 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
             torch.cuda.synchronize(dev)
             same = all(int(Sxl[k]) == int(Sx[r - 1]) and int(Syl[k]) == int(Sy[r - 1]) for k, r in enumerate(rl))
             sparse = {"points": len(rl), "r_last": rl[-1], "ms": ev2.elapsed_time(ev3), "equals_dense": bool(same and Ml == M)}
-        meas = {"r_max": r_meas, "ms": ev0.elapsed_time(ev1), "t": g.time, "M": M,
+        tc_roofline = None
+        if L >= 4096 and r_meas >= 48:
+            # dense C(r) as the band of the row / column Gram matrix (csrc/corr_tc2.cuh): per axis L / 256 pair
+            # tiles x ceil((r_max + 256) / 512) passes of 256 x 512 outputs, contraction length L
+            passes = (r_meas + 256 + 511) // 512
+            flop = 2.0 * 2 * (L // 256) * passes * 256 * 512 * L
+            tf = flop / (ev0.elapsed_time(ev1) * 1e-3) / 1e12
+            try:
+                with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                    mp = json.load(f)
+                bf16 = float(mp.get("bf16_tflops_sustained") or mp["bf16_tflops"])
+                src = "2 x the sustained bf16 TFLOP/s of MEASURED_PEAKS.json (the guide's nominal fp8 : bf16 ratio)"
+            except Exception:
+                bf16, src = 2250.0, "2 x the nominal 2250 bf16 TFLOP/s (no MEASURED_PEAKS.json)"
+            tc_roofline = {"bound": "tensor", "kernel": "corr_tc2_kernel (+ band_transpose_kernel, measure_mq_kernel)",
+                           "achieved": tf, "peak": 2.0 * bf16, "unit": "TFLOP/s", "frac": tf / (2.0 * bf16),
+                           "dtype": "fp8 e4m3 operands, fp32 accumulate (exact integers)", "peak_source": src,
+                           "flop": flop, "traffic": None}
+        meas = {"r_max": r_meas, "ms": ev0.elapsed_time(ev1), "t": g.time, "M": M, "roofline": tc_roofline,
                 "path": "tensor cores (tcgen05 banded Gram: CTA pairs, x axis on transposed bands; csrc/corr_tc2.cuh, corr_transpose.cuh)" if (L >= 4096 and r_meas >= 48)
                         else "XOR/popcount kernels (csrc/measure.cuh)",
                 "e": lat.energy(Sx, Sy, Q, w.delta, L), "xi": xi_v, "r_cut": r_cut, "sparse_list": sparse}
