@@ -643,6 +643,7 @@ def main():
                     help="cache-resident lattices: two launches per sweep instead of the persistent multi-sweep kernel (A/B)")
     ap.add_argument("--batches-only", action="store_true",
                     help="time only the batched-replica workloads (profiling aid: prints their JSON object)")
+    ap.add_argument("--batch-shapes", default="", help="with --batches-only: LxN[,LxN...] instead of the two default shapes")
     ap.add_argument("--measure-rmax", type=int, default=-1,
                     help="r_max of the separately timed measurement pass (-1: the workload's)")
     ap.add_argument("--measure-list", type=int, default=64,
@@ -678,8 +679,10 @@ def main():
     cdev = dev if args.dist_backend == "nccl" else "cpu"   # where the plumbing tensors live
 
     if args.batches_only:
-        out = {name: bench_batch(name, Lb, nb, args, lat, torch, dev)
-               for name, Lb, nb in (("ising_L4096_x64", 4096, 64), ("ising_L64_x4096", 64, 4096))}
+        shapes = [("ising_L4096_x64", 4096, 64), ("ising_L64_x4096", 64, 4096)]
+        if args.batch_shapes:
+            shapes = [(f"ising_L{a}_x{b}", int(a), int(b)) for a, b in (x.split("x") for x in args.batch_shapes.split(","))]
+        out = {name: bench_batch(name, Lb, nb, args, lat, torch, dev) for name, Lb, nb in shapes}
         print(json.dumps({"batched_replicas": out}))
         return
 

@@ -74,19 +74,34 @@ __global__ void __launch_bounds__(256) measure_mq_kernel(const MeasArgs a)
 {
     const uint32_t rep = blockIdx.x / a.bpr, bx = blockIdx.x - rep * a.bpr;
     const uint32_t *buf = a.buf + rep * a.rep_words;
-    const unsigned long long total = 2ull * a.n_rows * a.wpr;
+    // the base rows of one colour (and plane) are one contiguous range of n_rows * wpr words
+    const unsigned long long n = (unsigned long long)a.n_rows * a.wpr, stride = (unsigned long long)a.bpr * blockDim.x;
+    const size_t off = (size_t)a.i0 * a.wpr;
     unsigned long long c0 = 0, c1 = 0;
-    for (unsigned long long g = (unsigned long long)bx * blockDim.x + threadIdx.x; g < total;
-         g += (unsigned long long)a.bpr * blockDim.x) {
-        const uint32_t colour = (uint32_t)(g / ((unsigned long long)a.n_rows * a.wpr));
-        const unsigned long long rem = g % ((unsigned long long)a.n_rows * a.wpr);
-        const size_t off = ((size_t)a.i0 * a.wpr) + rem;
-        if (a.model == 0) {
-            c0 += __popc(plane_ptr(a, buf, colour, 0)[off]);
+    for (uint32_t colour = 0; colour < 2; ++colour) {
+        const uint32_t *p0 = plane_ptr(a, buf, colour, 0) + off, *p1 = plane_ptr(a, buf, colour, 1) + off;
+        if ((a.wpr & 3u) == 0) {                 // 16-byte loads (rows are whole 128-bit runs)
+            const uint4 *q0 = reinterpret_cast<const uint4 *>(p0), *q1 = reinterpret_cast<const uint4 *>(p1);
+            for (unsigned long long g = (unsigned long long)bx * blockDim.x + threadIdx.x; g < n / 4; g += stride) {
+                const uint4 nz = q0[g];
+                if (a.model == 0) {
+                    c0 += __popc(nz.x) + __popc(nz.y) + __popc(nz.z) + __popc(nz.w);
+                } else {
+                    const uint4 sg = q1[g];
+                    c0 += __popc(nz.x & ~sg.x) + __popc(nz.y & ~sg.y) + __popc(nz.z & ~sg.z) + __popc(nz.w & ~sg.w);
+                    c1 += __popc(nz.x & sg.x) + __popc(nz.y & sg.y) + __popc(nz.z & sg.z) + __popc(nz.w & sg.w);
+                }
+            }
         } else {
-            const uint32_t nz = plane_ptr(a, buf, colour, 0)[off], sg = plane_ptr(a, buf, colour, 1)[off];
-            c0 += __popc(nz & ~sg);
-            c1 += __popc(nz & sg);
+            for (unsigned long long g = (unsigned long long)bx * blockDim.x + threadIdx.x; g < n; g += stride) {
+                if (a.model == 0) {
+                    c0 += __popc(p0[g]);
+                } else {
+                    const uint32_t nz = p0[g], sg = p1[g];
+                    c0 += __popc(nz & ~sg);
+                    c1 += __popc(nz & sg);
+                }
+            }
         }
     }
     block_add2(c0, c1, a.cnt + rep * a.cnt_stride);
