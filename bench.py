@@ -567,6 +567,8 @@ def bench_batch(name, L, n_rep, args, lat, torch, dev):
     --min-seconds, clock-sampled; e2e adds lattice_measure_batch(r_max = 1) per step."""
     seeds = np.arange(n_rep, dtype=np.uint64) * 1000 + np.uint64(workloads.SEED_BASE + 31)
     b = lat.LatticeBatch(L, seeds, lat.ISING, 0.0, args.scheme, device=str(dev))
+    if args.no_persistent:                          # A/B: two launches per sweep instead of the in-kernel sweep loops
+        lat.lib().lattice_set_persist_blocks(b._h, 0xffffffff)
     K = args.steps
     beta = workloads.BETA_C_ISING
 

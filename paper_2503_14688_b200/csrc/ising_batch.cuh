@@ -10,7 +10,7 @@
 //     (L a multiple of 256): blockIdx.y is the replica; its ten round keys come from a table in
 //     the kernel parameters, indexed by blockIdx.y, i.e. uniform-register operands of the Philox
 //     XORs exactly like the single-lattice kernel's launch constants (no extra registers);
-//   * ising_block_kernel -- 256 <= L <= 1024: one thread block per replica runs ALL n sweeps of the
+//   * ising_block_kernel -- 256 <= L <= 512: one thread block per replica runs ALL n sweeps of the
 //     call, a block barrier between the colours instead of a launch;
 //   * ising_tiny_kernel -- L = 64 and 128 (one or two words per row): a half-warp (L = 64) or a
 //     warp (L = 128) owns a whole replica IN REGISTERS, each lane four consecutive rows = whole
@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(256) ising_march_batch_kernel(const IsingMarch
     queue.drain();
 }
 
-// ---- 256 <= L <= 1024: one thread block per replica, all sweeps of the call in one launch --------
+// ---- 256 <= L <= 512: one thread block per replica, all sweeps of the call in one launch ---------
 //
 // A half-sweep of such a replica is a few thousand thread-rows: launched on its own it costs more
 // in launch latency than in work.  Here block b owns replica b for the whole call: its threads take
