@@ -70,7 +70,7 @@ __global__ void __launch_bounds__(256) ising_march_batch_kernel(const IsingMarch
 constexpr int BLOCK_KERNEL_THREADS = 512;
 
 template <bool EDGE>
-__global__ void __launch_bounds__(BLOCK_KERNEL_THREADS) ising_block_kernel(const IsingMarchArgs a0, uint32_t *buf,
+__global__ void __launch_bounds__(BLOCK_KERNEL_THREADS, 2) ising_block_kernel(const IsingMarchArgs a0, uint32_t *buf,
                                                                            const RoundKeys *keys,
                                                                            const SweepParams *sp, uint32_t n_sweeps,
                                                                            unsigned long long rep_words)
