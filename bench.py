@@ -362,6 +362,8 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
                     device=str(dev))
     if args.no_persistent:
         g.set_persist_blocks(0xffffffff)
+    if args.force_persistent:
+        g.set_persist_blocks(1 << 20)
     updates_per_sweep = L * L
     K, W = args.steps, args.warmup
 
@@ -643,6 +645,8 @@ def main():
     ap.add_argument("--beta", type=float, default=None, help="override the workload's beta schedule with a constant")
     ap.add_argument("--no-persistent", action="store_true",
                     help="cache-resident lattices: two launches per sweep instead of the persistent multi-sweep kernel (A/B)")
+    ap.add_argument("--force-persistent", action="store_true",
+                    help="cache-resident lattices: take the persistent multi-sweep kernel wherever it exists (A/B)")
     ap.add_argument("--batches-only", action="store_true",
                     help="time only the batched-replica workloads (profiling aid: prints their JSON object)")
     ap.add_argument("--batch-shapes", default="", help="with --batches-only: LxN[,LxN...] instead of the two default shapes")

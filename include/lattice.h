@@ -274,7 +274,7 @@ int lattice_set_measure_path(lattice_t *lat, int path);
  * cache-resident lattice can run all n sweeps in ONE cooperative launch with a grid barrier per
  * half-sweep.  max_blocks selects when:
  *   0 (default)   automatic: only where it is measured faster than two launches per sweep, i.e. Ising
- *                 lattices with L <= 4352;
+ *                 lattices with L <= 8192;
  *   1..2^32-2     on request, for any Ising lattice with L <= 16384 and any Blume-Capel lattice with
  *                 L <= 16384 and Delta = 0 type threshold tables, with at most max_blocks blocks (fewer
  *                 blocks than 256-thread groups of work: every block strides over several groups);

@@ -33,7 +33,7 @@ struct BCPersistArgs : BCMarchArgs {
     __device__ __forceinline__ uint32_t lut_k(int k) const { return lut_s[k]; }
 };
 
-__global__ void __launch_bounds__(256, 3) bc_persist_kernel(const BCMarchArgs a0, uint32_t *buf, const BCSweepParams *sp,
+__global__ void __launch_bounds__(256, 2) bc_persist_kernel(const BCMarchArgs a0, uint32_t *buf, const BCSweepParams *sp,
                                                             uint32_t n_sweeps)
 {
     namespace cg = cooperative_groups;

@@ -8,14 +8,16 @@
 // colour, folded Philox constants, thresholds) rebuilt in shared memory by one thread per block from
 // a per-sweep table the host uploads.
 //
-// Measured (B200, updates/ns, persistent vs two launches per sweep, >= 2 s timed, round 2):
-//   L = 4096: 1650 vs 1366;  8192: 2090 vs 2732;  16384: 3733 vs 4091.
-// It wins where a half-sweep is a few microseconds and the launch gap shows (L <= 4352: one row per
-// thread, the whole lattice in flight at once); from L = 8192 on back-to-back launches overlap well,
-// while the persistent variant pays for its arguments living in registers instead of the constant
-// bank (108-127 registers against 63: half the resident warps) and for the grid barrier.  lattice_sweep
-// therefore takes this path by itself only for L <= 4352; larger lattices (L <= 16384) take it on
-// request (lattice_set_persist_blocks), which is what the parity tests of that variant do.
+// Measured (B200, updates/ns, persistent vs two launches per sweep, >= 2 s timed, round 2, grids sized
+// so that every block strides over the same number of 256-thread groups):
+//   L = 4096: 1677 vs 1366;  8192: 2997 vs 2732;  16384: 4112 vs 4094.
+// It wins where a half-sweep is a few microseconds and the launch gap shows; at L = 16384 back-to-back
+// launches overlap as well, and the persistent variant pays for its arguments living in registers
+// instead of the constant bank (108-127 registers against 63: half the resident warps) and for the
+// grid barrier.  lattice_sweep therefore takes this path by itself for L <= 8192; L = 16384 takes it on
+// request (lattice_set_persist_blocks), which is what the parity tests of that variant do.  (With a
+// grid of simply "all resident blocks" L = 8192 ran at 2090: 444 blocks over 512 groups leave most of
+// them idle in the second round.)
 #pragma once
 #include <cooperative_groups.h>
 

@@ -1009,8 +1009,8 @@ static int sweep_persistent(lattice *lat, uint64_t n, const double *beta)
         n < 2 || lat->persist_blocks < 0 || lat->persist_off)
         return 1;
     // automatic only where it is measured faster than two launches per sweep (ising_persist.cuh):
-    // Ising lattices small enough for one row per thread; otherwise on request (persist_cap > 0)
-    const bool automatic = lat->model == LATTICE_ISING && ising_one_row(lat);
+    // Ising lattices with L <= 8192; otherwise on request (persist_cap > 0)
+    const bool automatic = lat->model == LATTICE_ISING && lat->L <= 8192u;
     if (!automatic && lat->persist_cap == 0) return 1;
     if (lat->model == LATTICE_BLUME_CAPEL) return sweep_persistent_bc(lat, n, beta);
     if (lat->persist_blocks == 0) {

@@ -41,7 +41,7 @@ def test_persistent_marching_variant_against_oracle_and_single_launches(L):
     edge = [BETA_C] * 5 + [0.0] + [BETA_C] * 6 + [BETA_C / 1.01] * 4         # 16 sweeps, one at beta = 0
     plain = [BETA_C] * 3 + [0.5]                                             # no "always" class
     g = lat.Lattice(L, lat.ISING, 0.0, seed)          # persistent kernel, one launch per call
-    g.set_persist_blocks(FORCE)                       # (automatic only for L <= 4352: on request here)
+    g.set_persist_blocks(FORCE)                       # (automatic for L <= 8192; forced here all the same)
     s = lat.Lattice(L, lat.ISING, 0.0, seed)          # the same sweeps, one per call
     o = oracle.OracleLattice(L, lat.ISING, 0.0, seed)
     for sched in (edge, plain):
