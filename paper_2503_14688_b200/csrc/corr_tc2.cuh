@@ -105,6 +105,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T2_THREADS, 1) corr_
     __shared__ __align__(8) unsigned long long bars[2 * T2_STAGES + 2];
     __shared__ uint32_t tmem_base_s;
 
+    // two producer groups, each owning pairs of stages (below): measured -4 % for Ising (7.6 -> 7.4 s at
+    // L = 2^20), +6 % for Blume-Capel (its second plane costs registers: spills under the 80-register cap)
+    constexpr bool T2_GROUPS = AXIS == 1 && MODEL == 0;
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
     const uint32_t rank = cluster_rank();                     // 0 = leader (issues the MMAs)
     const uint32_t full0 = smem_u32(&bars[0]), empty0 = smem_u32(&bars[T2_STAGES]),
@@ -113,7 +116,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T2_THREADS, 1) corr_
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < T2_STAGES; ++s) {
-            mbar_init(full0 + 8 * s, 2 * (T2_PRODUCERS / 32));    // one arrive per producer warp of both CTAs
+            // one arrive per producer warp that fills the stage, in both CTAs: all 24 warps (x axis), or the
+            // 12 warps of the group that owns the stage (Ising y axis, below)
+            mbar_init(full0 + 8 * s, T2_GROUPS ? T2_PRODUCERS / 32 : 2 * (T2_PRODUCERS / 32));
             mbar_init(empty0 + 8 * s, 1);                         // tcgen05.commit (multicast)
         }
         mbar_init(accf, 1);
@@ -144,7 +149,132 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T2_THREADS, 1) corr_
         // first base position of the pair's tile; this CTA's own base block starts 128 * rank further
         const uint32_t p0 = (AXIS == 1 ? a.i0 : 0u) + tile * (2u * T2_M);
         const uint32_t w0 = p0 + pass * (T2_NT * T2_N);           // first partner position of the pass
-        if (warp < T2_PRODUCERS / 32) {
+        // ===== epilogue (warps 0-3: TMEM lane quarter = warp): this CTA's 128 base positions =====
+        auto epilogue = [&]() {
+            if (warp < 4) {
+            for (uint32_t t = threadIdx.x; t < (uint32_t)T2_HIST; t += 128u) hist[t] = 0;
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            mbar_wait_cluster(accf, acc_phase);
+            fence_after_sync();
+            const uint32_t m = warp * 32u + lane;             // base position index in this CTA's block
+            // position of byte index x inside a 128-block: natural for y; [64 even | 64 odd] and the
+            // byte order of expand_word inside each 32-byte group for x (corr_tc.cuh)
+            const int pm = (int)(T2_M * rank) +
+                           (AXIS == 1 ? (int)m : (int)(2u * ((m & 32u) + tc_spin_of_byte(m & 31u)) + (m >> 6)));
+#pragma unroll 1
+            for (uint32_t cb = 0; cb < (uint32_t)(T2_NT * T2_N); cb += 16u) {
+                uint32_t v[16];
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+                             "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]),
+                               "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]),
+                               "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                             : "r"(tmem + ((warp * 32u) << 16) + cb));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    // column n of the accumulators <-> partner position: N tile n >> 8, inside it the
+                    // leader's 128 partner rows first, then the peer's: the natural order of the window
+                    const uint32_t n = cb + (uint32_t)e;
+                    int pn;
+                    if (AXIS == 1) pn = (int)n;
+                    else {
+                        const uint32_t nb = n & 127u;
+                        pn = (int)((n & ~127u) + 2u * ((nb & 32u) + tc_spin_of_byte(nb & 31u)) + (nb >> 6));
+                    }
+                    const int d = pn - pm;                     // r - 512 pass, in (-256, 512)
+                    const long long r = (long long)d + (long long)pass * (T2_NT * T2_N);
+                    const int val = __float2int_rn(__uint_as_float(v[e]));
+                    if (r >= 1 && r <= (long long)a.r_max && val) atomicAdd(&hist[d + (2 * T2_M - 1)], val);
+                }
+            }
+            // this CTA's accumulators are read: tell the leader (it waits for both CTAs)
+            fence_before_sync();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tfree_leader);
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            for (uint32_t t = threadIdx.x; t < (uint32_t)T2_HIST; t += 128u) {
+                const long long r = (long long)t - (2 * T2_M - 1) + (long long)pass * (T2_NT * T2_N);
+                if (hist[t] && r >= 1 && r <= (long long)a.r_max)
+                    atomicAdd((unsigned long long *)(a.S + (r - 1) * a.s_stride), (unsigned long long)(long long)hist[t]);
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+        }
+        };
+        if (T2_GROUPS && warp < T2_PRODUCERS / 32) {
+            // ===== producers, Ising y axis: two groups of 12 warps; group g fills the stage PAIRS 4 j + 2 g, 4 j + 2 g + 1
+            // of the item (one 16-byte load = both stages of a pair), two 64-byte chunks per thread and
+            // stage.  The per-stage overhead of a warp (barrier wait, proxy fence, arrive) is paid once per
+            // two chunks, and one group expands while the other waits for its stores to drain.
+            constexpr uint32_t GRP = T2_PRODUCERS / 2;            // 384 threads
+            const uint32_t grp = threadIdx.x / GRP, tg = threadIdx.x - grp * GRP;
+            const uint32_t *src[2];
+            uint32_t dst[2], r7[2], c0[2];
+            bool zero[2];
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const uint32_t it = tg + (uint32_t)q * GRP, tr = it >> 1, h = it & 1u;   // 0..127 base rows, 128..383 partner rows
+                const uint32_t mb = tr / T2_M, srow = tr % T2_M;
+                uint32_t i;
+                zero[q] = false;
+                if (mb == 0) { i = p0 + T2_M * rank + srow; zero[q] = i >= a.i0 + a.n_rows; }
+                else i = w0 + (mb - 1u) * T2_N + T2_M * rank + srow;
+                const uint32_t row_l = i % a.rows, c = (row_l & 1u) ^ h;
+                src[q] = a.buf + (MODEL == 0 ? (size_t)c * pw : (size_t)(2u * c) * pw) + (size_t)row_l * a.wpr;
+                dst[q] = mb * T2_BLK_BYTES + (srow >> 3) * 1024u + (srow & 7u) * 128u;
+                r7[q] = srow & 7u; c0[q] = h << 2;
+            }
+            uint4 cur[2], curs[2], nxt[2], nxts[2];
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                cur[q] = curs[q] = nxt[q] = nxts[q] = make_uint4(0u, 0u, 0u, 0u);
+                const uint32_t k0 = 2u * grp, k1 = k0 + 4u;                              // first stages of the first two pairs
+                if (!zero[q] && k0 < n_kc) {
+                    cur[q] = *reinterpret_cast<const uint4 *>(src[q] + 2 * (size_t)k0);
+                    if (MODEL) curs[q] = *reinterpret_cast<const uint4 *>(src[q] + 2 * (size_t)k0 + pw);
+                }
+                if (!zero[q] && k1 < n_kc) {
+                    nxt[q] = *reinterpret_cast<const uint4 *>(src[q] + 2 * (size_t)k1);
+                    if (MODEL) nxts[q] = *reinterpret_cast<const uint4 *>(src[q] + 2 * (size_t)k1 + pw);
+                }
+            }
+            for (uint32_t kp = 2u * grp; kp < n_kc; kp += 4u) {
+#pragma unroll
+                for (int v = 0; v < 2; ++v) {
+                    const uint32_t sg = sbase + kp + (uint32_t)v, slot = sg % T2_STAGES;
+                    mbar_wait_cluster(empty0 + 8 * slot, ((sg / T2_STAGES) & 1u) ^ 1u);
+                    const uint32_t st = smem_u32(smem) + slot * T2_STAGE_BYTES;
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) {
+                        uint4 o[4];
+                        if (zero[q]) o[0] = o[1] = o[2] = o[3] = make_uint4(0u, 0u, 0u, 0u);
+                        else {
+                            expand_word<MODEL>(v ? cur[q].z : cur[q].x, v ? curs[q].z : curs[q].x, o[0], o[1]);
+                            expand_word<MODEL>(v ? cur[q].w : cur[q].y, v ? curs[q].w : curs[q].y, o[2], o[3]);
+                        }
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(st + dst[q] + (((c0[q] + (uint32_t)e) ^ r7[q]) << 4)),
+                                         "r"(o[e].x), "r"(o[e].y), "r"(o[e].z), "r"(o[e].w) : "memory");
+                    }
+                    fence_proxy_async();                          // generic-proxy writes -> visible to the tensor core
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(full0_leader + 8 * slot);
+                }
+                const uint32_t nk = kp + 8u;                      // the pair after the next one
+#pragma unroll
+                for (int q = 0; q < 2; ++q) {
+                    cur[q] = nxt[q]; curs[q] = nxts[q];
+                    nxt[q] = nxts[q] = make_uint4(0u, 0u, 0u, 0u);
+                    if (!zero[q] && nk < n_kc) {
+                        nxt[q] = *reinterpret_cast<const uint4 *>(src[q] + 2 * (size_t)nk);
+                        if (MODEL) nxts[q] = *reinterpret_cast<const uint4 *>(src[q] + 2 * (size_t)nk + pw);
+                    }
+                }
+            }
+            epilogue();
+            acc_phase ^= 1u;
+        } else if (warp < T2_PRODUCERS / 32) {
             // ===== producers: one 64-byte chunk of the stage per thread =====
             // blocks of 128 smem rows: 0 = this CTA's base block, 1 + nt = this CTA's half of N tile nt
             const uint32_t it = threadIdx.x;
@@ -261,56 +391,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(T2_THREADS, 1) corr_
                     }
                 }
             }
-            // ===== epilogue (warps 0-3: TMEM lane quarter = warp): this CTA's 128 base positions =====
-            if (warp < 4) {
-                for (uint32_t t = threadIdx.x; t < (uint32_t)T2_HIST; t += 128u) hist[t] = 0;
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                mbar_wait_cluster(accf, acc_phase);
-                fence_after_sync();
-                const uint32_t m = warp * 32u + lane;             // base position index in this CTA's block
-                // position of byte index x inside a 128-block: natural for y; [64 even | 64 odd] and the
-                // byte order of expand_word inside each 32-byte group for x (corr_tc.cuh)
-                const int pm = (int)(T2_M * rank) +
-                               (AXIS == 1 ? (int)m : (int)(2u * ((m & 32u) + tc_spin_of_byte(m & 31u)) + (m >> 6)));
-#pragma unroll 1
-                for (uint32_t cb = 0; cb < (uint32_t)(T2_NT * T2_N); cb += 16u) {
-                    uint32_t v[16];
-                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-                                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]),
-                                   "=r"(v[7]), "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]),
-                                   "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                                 : "r"(tmem + ((warp * 32u) << 16) + cb));
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                    for (int e = 0; e < 16; ++e) {
-                        // column n of the accumulators <-> partner position: N tile n >> 8, inside it the
-                        // leader's 128 partner rows first, then the peer's: the natural order of the window
-                        const uint32_t n = cb + (uint32_t)e;
-                        int pn;
-                        if (AXIS == 1) pn = (int)n;
-                        else {
-                            const uint32_t nb = n & 127u;
-                            pn = (int)((n & ~127u) + 2u * ((nb & 32u) + tc_spin_of_byte(nb & 31u)) + (nb >> 6));
-                        }
-                        const int d = pn - pm;                     // r - 512 pass, in (-256, 512)
-                        const long long r = (long long)d + (long long)pass * (T2_NT * T2_N);
-                        const int val = __float2int_rn(__uint_as_float(v[e]));
-                        if (r >= 1 && r <= (long long)a.r_max && val) atomicAdd(&hist[d + (2 * T2_M - 1)], val);
-                    }
-                }
-                // this CTA's accumulators are read: tell the leader (it waits for both CTAs)
-                fence_before_sync();
-                __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(tfree_leader);
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                for (uint32_t t = threadIdx.x; t < (uint32_t)T2_HIST; t += 128u) {
-                    const long long r = (long long)t - (2 * T2_M - 1) + (long long)pass * (T2_NT * T2_N);
-                    if (hist[t] && r >= 1 && r <= (long long)a.r_max)
-                        atomicAdd((unsigned long long *)(a.S + (r - 1) * a.s_stride), (unsigned long long)(long long)hist[t]);
-                }
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-            }
+            epilogue();
             acc_phase ^= 1u;
         } else if (rank == 0) {
             // ===== MMA issuer: one elected thread of the leader CTA =====
