@@ -206,6 +206,21 @@ int lattice_half_sweep(lattice_t *lat, int colour, double beta);
 int lattice_measure(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx,
                     int64_t *Sy);
 
+/* lattice_measure without any allocation, for callers that cannot call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it): the same exact counts (Eq. 2-3,
+ * PAPER.md:42-50) for r = 1 .. r_max, r_max <= LATTICE_STATIC_RMAX, computed by the XOR/popcount
+ * kernels with their per-r counters in a file-scope device array of 2 + 4 * LATTICE_STATIC_RMAX 64-bit
+ * words (34 KiB) that every GPU loading the library holds until exit.  The call makes no cudaMalloc,
+ * cudaFree or host allocation; it clears the array on the handle's stream, launches, copies the counts
+ * back and synchronises the stream.  ALL calls on a device share that array: calls that overlap on
+ * the GPU (different streams, handles or host threads) race -- serialise them.  The device current at
+ * the call must be the one that holds the lattice.
+ * Errors: EINVAL (NULL, r_max < 1, r_max > L/2, r_max > LATTICE_STATIC_RMAX -- lattice_last_error says
+ * so --, a slab with r_max != 1), ESTATE (batch handle or view), ECUDA. */
+#define LATTICE_STATIC_RMAX 1024
+int lattice_measure_static(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx,
+                           int64_t *Sy);
+
 /* The same sums restricted to base sites in rows i0 .. i0+n_rows-1 (partners wrap
  * periodically); the partial sums of a partition of the rows add up to lattice_measure.
  * For spot checks at L = 2^20 and for future row-slab sharding. */

@@ -51,6 +51,7 @@ SIGNATURES = {
     "lattice_sweep": (C.c_int, [_vp, C.c_uint64, _f64p]),
     "lattice_half_sweep": (C.c_int, [_vp, C.c_int, C.c_double]),
     "lattice_measure": (C.c_int, [_vp, C.c_uint32, _i64p, _i64p, _i64p, _i64p]),
+    "lattice_measure_static": (C.c_int, [_vp, C.c_uint32, _i64p, _i64p, _i64p, _i64p]),
     "lattice_measure_rows": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint32, _i64p, _i64p,
                                        _i64p, _i64p]),
     "lattice_measure_list": (C.c_int, [_vp, C.c_uint64, C.c_uint64, _u32p, C.c_uint32, _i64p, _i64p, _i64p, _i64p]),
@@ -93,6 +94,7 @@ def lib() -> C.CDLL:
     return L
 
 
+STATIC_RMAX = 1024         # LATTICE_STATIC_RMAX of include/lattice.h
 FLAG_BYTES = 64            # room behind a slab buffer for its 64-bit flag word (keeps 16-byte alignment)
 
 
@@ -346,6 +348,21 @@ class Lattice:
                 rc = lib().lattice_measure_rows(self._h, rows[0], rows[1], r_max, C.byref(M),
                                                 C.byref(Q), _p(Sx, C.c_int64), _p(Sy, C.c_int64))
         self._check(rc, "lattice_measure")
+        return int(M.value), int(Q.value), Sx, Sy
+
+    def measure_static(self, r_max: int):
+        """lattice_measure_static: the same counts as measure(r_max) for r_max <= STATIC_RMAX with no
+        allocation on the library side (counters in a static device array shared by all calls: do not
+        overlap calls on the GPU)."""
+        Sx = np.zeros(r_max, dtype=np.int64)
+        Sy = np.zeros(r_max, dtype=np.int64)
+        M, Q = C.c_int64(0), C.c_int64(0)
+        with self._torch.cuda.device(self.device):
+            rc = lib().lattice_measure_static(self._h, r_max, C.byref(M), C.byref(Q),
+                                              _p(Sx, C.c_int64), _p(Sy, C.c_int64))
+        if rc == EINVAL:
+            raise LatticeError("lattice_measure_static", rc, lib().lattice_last_error(self._h).decode())
+        self._check(rc, "lattice_measure_static")
         return int(M.value), int(Q.value), Sx, Sy
 
     def measure_list(self, r_list, rows=None):

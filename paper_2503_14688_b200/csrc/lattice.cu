@@ -1663,6 +1663,60 @@ int lattice_measure(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int6
     return lattice_measure_rows(lat, lat->row0, lat->n_own, r_max, M, Q, Sx, Sy);
 }
 
+// ---- lattice_measure_static: the measurement with NO allocation --------------------------------------
+// For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that
+// forbid it).  lattice_measure keeps its per-r counters in lat->d_cnt, which ensure_cnt() cudaMallocs on
+// first use; here they live in a file-scope device array that every GPU loading the library holds until
+// exit (34 KiB).  In host code `g_static_cnt` is only a host-side stand-in for the symbol, not a device
+// address: the address the kernels are given comes from cudaGetSymbolAddress, asked once per device with
+// that device current.  Every call shares the array: it is cleared on the stream at the start of each
+// call, and calls that overlap on the GPU (two streams, two handles, two host threads) race.
+static __device__ __align__(256) unsigned long long g_static_cnt[2 + 4 * LATTICE_STATIC_RMAX];
+static unsigned long long *g_static_cnt_ptr[64];             // per device ordinal; null: not asked yet
+
+static int static_cnt_for_current_device(lattice *lat, unsigned long long **out)
+{
+    int dev = -1;
+    CU(lat, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return LATTICE_EINVAL;
+    if (!g_static_cnt_ptr[dev]) {
+        void *p = nullptr;
+        CU(lat, cudaGetSymbolAddress(&p, g_static_cnt));
+        if (!p) return LATTICE_ECUDA;
+        g_static_cnt_ptr[dev] = (unsigned long long *)p;
+    }
+    *out = g_static_cnt_ptr[dev];
+    return LATTICE_OK;
+}
+
+int lattice_measure_static(lattice_t *lat, uint32_t r_max, int64_t *M, int64_t *Q, int64_t *Sx, int64_t *Sy)
+{
+    if (!lat || !M || !Q || !Sx || !Sy) return LATTICE_EINVAL;
+    if (lat->n_rep || lat->view) return LATTICE_ESTATE;
+    const uint64_t L = lat->L;
+    if (r_max < 1 || r_max > L / 2) return LATTICE_EINVAL;
+    if (r_max > (uint32_t)LATTICE_STATIC_RMAX) {
+        snprintf(lat->err, sizeof lat->err, "lattice_measure_static: r_max = %u exceeds LATTICE_STATIC_RMAX = %d",
+                 r_max, (int)LATTICE_STATIC_RMAX);
+        return LATTICE_EINVAL;
+    }
+    if (lat->slab && r_max != 1) return LATTICE_EINVAL;           // as lattice_measure on a slab
+    unsigned long long *cnt = nullptr;
+    int rc = static_cnt_for_current_device(lat, &cnt);
+    if (rc) return rc;
+    const size_t entries = 2 + 4 * (size_t)r_max;
+    CU(lat, cudaMemsetAsync(cnt, 0, entries * sizeof(unsigned long long), lat->stream));   // last call's counts
+    // the XOR/popcount kernels only: the tensor-core path keeps a transposed copy it allocates
+    rc = enqueue_measure(lat, cnt, lat->row0, lat->n_own, r_max, nullptr);
+    if (rc) return rc;
+    unsigned long long h[2 + 4 * LATTICE_STATIC_RMAX];            // host side: on the stack, no malloc
+    cudaError_t e = cudaMemcpyAsync(h, cnt, entries * sizeof(unsigned long long), cudaMemcpyDeviceToHost, lat->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(lat->stream);
+    if (e != cudaSuccess) return cuda_fail(lat, e, "measure copy/sync");
+    convert_counts(lat->model, (int64_t)((uint64_t)lat->n_own * L), r_max, h, M, Q, Sx, Sy, false);
+    return LATTICE_OK;
+}
+
 static int window_call(lattice_t *lat, uint64_t i0, uint64_t j0, uint32_t h, uint32_t w, int8_t *host,
                        bool set)
 {
