@@ -31,7 +31,7 @@ One JSON line is printed by rank 0:
             size (L = 2^19) and for BASELINE config 5b (L = 2^15, beta ramp), each
             with its own value, e2e, roofline, roofline_hbm and clocks
   batched_replicas  (default invocation, 1 GPU) aggregate updates/ns of 64 replicas of L = 4096 and
-            4096 replicas of L = 64 in one batch handle each (lattice_create_batch): the shapes of
+            8192 replicas of L = 64 in one batch handle each (lattice_create_batch): the shapes of
             BASELINE configs 2 and 1, which fill the GPU only as batches
   cpu_baseline  the oracle, as it stands, on the host cores over bounded samples: `value` is the
             all-cores figure for the timed model and RNG scheme; `matrix` holds 1 thread and all
@@ -685,7 +685,7 @@ def main():
     cdev = dev if args.dist_backend == "nccl" else "cpu"   # where the plumbing tensors live
 
     if args.batches_only:
-        shapes = [("ising_L4096_x64", 4096, 64), ("ising_L64_x4096", 64, 4096)]
+        shapes = [("ising_L4096_x64", 4096, 64), ("ising_L64_x8192", 64, 8192)]
         if args.batch_shapes:
             shapes = [(f"ising_L{a}_x{b}", int(a), int(b)) for a, b in (x.split("x") for x in args.batch_shapes.split(","))]
         out = {name: bench_batch(name, Lb, nb, args, lat, torch, dev) for name, Lb, nb in shapes}
@@ -717,7 +717,7 @@ def main():
     # cache-resident sizes fill the GPU only as batches of replicas (BASELINE configs 1 and 2's shapes)
     batches = {}
     if world == 1 and not args.no_batches and args.workload == "ising_L2p20" and not args.L:
-        for name, Lb, nb in (("ising_L4096_x64", 4096, 64), ("ising_L64_x4096", 64, 4096)):
+        for name, Lb, nb in (("ising_L4096_x64", 4096, 64), ("ising_L64_x8192", 64, 8192)):
             batches[name] = bench_batch(name, Lb, nb, args, lat, torch, dev)
 
     if rank != 0:
