@@ -16,7 +16,7 @@ One JSON line is printed by rank 0:
   value     whole-job spin updates/ns, device-timed (CUDA events), lattice resident in HBM
   e2e       the same metric through the C-ABI with host buffers every step: the step's beta goes
             in as a host fp64 array and the step's result (M, Q, S_x(1), S_y(1) -> e, m) comes
-            back to host memory (lattice_sweep + lattice_measure), all inside the timed region
+            back to host memory (lattice_sweep_record), all inside the timed region
   roofline  the binding roofline of the dominant kernel (the half-sweep): "bound": "alu" --
             ALGORITHMIC thread-instructions of the half-rate dispatch class per launch (hand
             count) / mean launch time measured here, against a peak MEASURED
@@ -392,8 +392,8 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
     e2e_out = {}
 
     def step_e2e(t, n):
-        g.sweep(sched(t, n))                    # host fp64 beta in
-        e2e_out["r"] = g.measure(1)             # host int64 counts out (synchronises)
+        # host fp64 beta in, host int64 counts out (synchronises): one C-ABI call, lattice_sweep_record
+        e2e_out["r"] = g.sweep_record(sched(t, n))
 
     peaks = dispatch_peak(lat, torch, dev, g.stream.cuda_stream)
 
@@ -558,7 +558,9 @@ def bench_workload(w, args, lat, torch, dev, rank, world, cdev, replicas, *, mea
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * sps,
                 "d2h_bytes_per_step": 8 * (2 + 4 * 1), "ms_per_step": e2e_ms / K, "clocks": e2e_clocks,
-                "what": f"lattice_sweep({sps}, host beta[{sps}]) + lattice_measure(r_max=1) -> host int64, per step"},
+                "what": f"lattice_sweep_record({sps}, host beta[{sps}]) -> host int64 (M, Q, S_x(1), S_y(1)), per step: the "
+                        f"sweeps and the r = 1 record (fused into the last white half-sweep for Ising marching lattices, "
+                        f"else lattice_sweep + lattice_measure(1))"},
         "roofline": roofline, "roofline_hbm": roofline_hbm, "worst_case": worst, "measure": meas,
     }
 

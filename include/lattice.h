@@ -194,6 +194,17 @@ int lattice_set_rng_scheme(lattice_t *lat, int scheme);
  * Errors: EINVAL (NULL beta with n > 0, NaN or negative beta, t+n >= 2^32), ECUDA. */
 int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta);
 
+/* lattice_sweep(n, beta) followed by the r = 1 record of the resulting state -- what a run that logs
+ * e(t), m(t) every step does (Eq. 3): *M, *Q, *Sx1 = S_x(1), *Sy1 = S_y(1) exactly as
+ * lattice_measure(lat, 1, ...) would return them after the sweeps.  For Ising lattices on the marching
+ * kernel (L a multiple of 256, L > 4352, bit-plane RNG schemes, not a slab) the record is counted inside
+ * the last white half-sweep, where the four neighbour words of every white site are in registers (every
+ * bond joins a white and a black site): no separate pass over the lattice.  Any other handle runs
+ * lattice_sweep and lattice_measure(1).  Host outputs; synchronises the stream.  n == 0 measures only.
+ * Errors: as lattice_sweep and lattice_measure; ESTATE for batch handles and views. */
+int lattice_sweep_record(lattice_t *lat, uint64_t n, const double *beta, int64_t *M, int64_t *Q,
+                         int64_t *Sx1, int64_t *Sy1);
+
 /* One colour (0 = black first, 1 = white) of sweep t at inverse temperature beta, without
  * advancing t.  lattice_sweep(1, &beta) == half_sweep(0), half_sweep(1), t += 1.  For tests. */
 int lattice_half_sweep(lattice_t *lat, int colour, double beta);

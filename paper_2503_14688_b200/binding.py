@@ -49,6 +49,7 @@ SIGNATURES = {
     "lattice_ipc_close": (C.c_int, [_vp]),
     "lattice_set_rng_scheme": (C.c_int, [_vp, C.c_int]),
     "lattice_sweep": (C.c_int, [_vp, C.c_uint64, _f64p]),
+    "lattice_sweep_record": (C.c_int, [_vp, C.c_uint64, _f64p, _i64p, _i64p, _i64p, _i64p]),
     "lattice_half_sweep": (C.c_int, [_vp, C.c_int, C.c_double]),
     "lattice_measure": (C.c_int, [_vp, C.c_uint32, _i64p, _i64p, _i64p, _i64p]),
     "lattice_measure_static": (C.c_int, [_vp, C.c_uint32, _i64p, _i64p, _i64p, _i64p]),
@@ -329,6 +330,16 @@ class Lattice:
         b = np.ascontiguousarray(np.atleast_1d(beta), dtype=np.float64)
         with self._torch.cuda.device(self.device):
             self._check(lib().lattice_sweep(self._h, b.size, _p(b, C.c_double)), "lattice_sweep")
+
+    def sweep_record(self, beta):
+        """Run len(beta) sweeps and return the r = 1 record (M, Q, S_x(1), S_y(1)) of the final state
+        (lattice_sweep_record: counted inside the last white half-sweep where that kernel exists)."""
+        b = np.ascontiguousarray(np.atleast_1d(beta), dtype=np.float64)
+        M, Q, Sx, Sy = C.c_int64(0), C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        with self._torch.cuda.device(self.device):
+            self._check(lib().lattice_sweep_record(self._h, b.size, _p(b, C.c_double), C.byref(M), C.byref(Q),
+                                                   C.byref(Sx), C.byref(Sy)), "lattice_sweep_record")
+        return int(M.value), int(Q.value), int(Sx.value), int(Sy.value)
 
     def half_sweep(self, colour: int, beta: float) -> None:
         with self._torch.cuda.device(self.device):

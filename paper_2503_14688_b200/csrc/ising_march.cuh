@@ -50,7 +50,10 @@ struct IsingMarchArgs {
     uint32_t threads;         // (wpr/4) * (L/R), a multiple of 32
     PlaneFold F;              // folded ACC_PLANE stream of (t, colour)
     RoundKeys K;
+    unsigned long long *rec;  // REC kernels: [REC_SLOTS][4] counters (anti-aligned x bonds, y bonds, up whites, up blacks)
 };
+
+constexpr int REC_SLOTS = 64;  // blocks spread their record atomics over this many counter sets
 
 __host__ __device__ __forceinline__ uint32_t fsl1(uint32_t lo, uint32_t hi)   // (hi:lo << 1) high word
 {
@@ -152,11 +155,15 @@ struct PlaneLoop {
 // 31 entries are pending before a row and a row adds at most 4 x 32.
 constexpr int TIE_Q_SLOTS = 160;
 
-template <bool SLAB>
+// REC (the fused r = 1 record of the white half-sweep, see march_row): a late flip changes the four
+// bonds of its site, which the row has already counted with the unflipped value; the resolving thread
+// re-reads the neighbour words (rare path) and keeps the differences in rx, ry, rm.
+template <bool SLAB, bool REC = false>
 struct WarpTieQueue {
     const IsingMarchArgs &a;
     uint4 *q;                  // [TIE_Q_SLOTS] this warp's slice
     uint32_t lane, pending;
+    int rx, ry, rm;            // REC: corrections to the anti-aligned x / y bond counts and the up-white count
 
     // entry.w = word offset bits 32..35 | column word << 4 | mirror flag << 30 (1 = up, 2 = down)
     __device__ __forceinline__ void resolve(uint32_t idx)
@@ -177,7 +184,20 @@ struct WarpTieQueue {
             if (u56 < (thr & 0x00ffffffffffffffull)) flip |= 1u << bit;
         }
         if (flip) {
-            atomicXor(a.tgt + wo, flip);
+            const uint32_t was = atomicXor(a.tgt + wo, flip);
+            if constexpr (REC) {
+                const uint32_t now = was ^ flip;
+                const uint32_t row = (uint32_t)(wo / a.wpr), k = (uint32_t)(wo - (unsigned long long)row * a.wpr);
+                const uint32_t *rp = a.opp + (unsigned long long)row * a.wpr;
+                const uint32_t C = rp[k];
+                const uint32_t U = a.opp[(unsigned long long)(row == 0 ? a.L - 1 : row - 1) * a.wpr + k];
+                const uint32_t D = a.opp[(unsigned long long)(row + 1 == a.L ? 0 : row + 1) * a.wpr + k];
+                const uint32_t S = ((row + a.colour) & 1u) == 0 ? fsl1(rp[k == 0 ? a.wpr - 1 : k - 1], C)
+                                                                : fsr1(C, rp[k + 1 == a.wpr ? 0 : k + 1]);
+                rx += __popc((now ^ C) & flip) + __popc((now ^ S) & flip) - __popc((was ^ C) & flip) - __popc((was ^ S) & flip);
+                ry += __popc((now ^ U) & flip) + __popc((now ^ D) & flip) - __popc((was ^ U) & flip) - __popc((was ^ D) & flip);
+                rm += __popc(now & flip) - __popc(was & flip);
+            }
             const uint32_t mf = SLAB ? e.w >> 30 : 0u;
             if (mf) {
                 // the mirror row may be peer-GPU memory: order this late flip after the plain
@@ -225,10 +245,23 @@ struct WarpTieQueue {
 // and queues the ties.  EDGE: some class has threshold 2^32 (beta = 0): mask it out of `need`.
 // mir / mir_tag: slab mode only -- where this row is mirrored (null: nowhere) and the queue tag
 // (column word << 4 | flag << 30) that lets a late flip reach the mirror too.
-template <int PAR, bool EDGE, bool SLAB, int PC = -1>
+// REC: what the fused r = 1 record of a thread adds up (march_row<.., REC = true>, white half-sweep)
+struct RecAcc {
+    uint32_t ax, ay, mw, mb;  // anti-aligned x bonds, y bonds, up spins of this colour, of the other colour
+};
+
+// REC = true (white half-sweep only): the row also counts the r = 1 record.  Every bond of the lattice
+// joins one white and one black site, so summing over the white sites their two horizontal bonds
+// (black words C and S) and two vertical bonds (U and D) counts every bond once: with the black rows
+// final and the white word as stored, anti-aligned pairs of an axis = popc(n1 ^ n2) + 2 popc((T ^ n1) &
+// (T ^ n2)); S_axis(1) = L^2 - 2 anti, M = 2 (up whites + up blacks) - L^2.  Per word 4 LOP3 + 1 SHF +
+// 6 POPC: ~5 % of the half-sweep instead of a separate 24 ms pass over the lattice (Eq. 2-3,
+// PAPER.md:42-50).  Late tie flips are corrected in WarpTieQueue::resolve.
+template <int PAR, bool EDGE, bool SLAB, int PC = -1, bool REC = false, class Queue>
 __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, unsigned long long wo, uint32_t *tp,
                                           const uint4 &U4, const uint4 &C4, const uint4 &D4, uint32_t E,
-                                          WarpTieQueue<SLAB> &queue, uint32_t *mir = nullptr, uint32_t mir_tag = 0)
+                                          Queue &queue, uint32_t *mir = nullptr, uint32_t mir_tag = 0,
+                                          RecAcc *rec = nullptr)
 {
     const uint4 T4 = *reinterpret_cast<const uint4 *>(tp);       // tp == a.tgt + wo
     uint32_t T[4] = {T4.x, T4.y, T4.z, T4.w};
@@ -265,6 +298,18 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
 #pragma unroll
     for (int w = 0; w < 4; ++w) T[w] = lop3<0x4B>(T[w], need[w], acc[w]);    // T ^ (~need | acc)
     *reinterpret_cast<uint4 *>(tp) = make_uint4(T[0], T[1], T[2], T[3]);
+    if constexpr (REC) {
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            uint32_t S;
+            if (PAR == 0) S = fsl1(w == 0 ? E : C[w > 0 ? w - 1 : 0], C[w]);
+            else S = fsr1(C[w], w == 3 ? E : C[w < 3 ? w + 1 : 0]);
+            rec->ax += __popc(C[w] ^ S) + 2u * __popc(lop3<0x18>(T[w], C[w], S));      // (T ^ C) & (T ^ S)
+            rec->ay += __popc(U[w] ^ D[w]) + 2u * __popc(lop3<0x18>(T[w], U[w], D[w]));
+            rec->mw += __popc(T[w]);
+            rec->mb += __popc(C[w]);
+        }
+    }
     if (SLAB && mir) {
         *reinterpret_cast<uint4 *>(mir) = make_uint4(T[0], T[1], T[2], T[3]);
         __threadfence_system();      // before any late flip of this row (resolve) reaches the mirror
@@ -274,8 +319,8 @@ __device__ __forceinline__ void march_row(const IsingMarchArgs &a, uint32_t G, u
 
 // The march of one thread: rows i0 .. i0+R-1 of run q, g = s * (wpr/4) + q (ties are queued, not
 // drained).
-template <int COLOUR, bool EDGE, bool SLAB, int PC = -1>
-__device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g, WarpTieQueue<SLAB> &queue)
+template <int COLOUR, bool EDGE, bool SLAB, int PC = -1, bool REC = false, class Queue>
+__device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g, Queue &queue, RecAcc *rec = nullptr)
 {
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2;
     const uint32_t q = g % nq, s = g / nq;
@@ -307,7 +352,7 @@ __device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g
             if (SLAB && top && r == 0)
                 march_row<COLOUR, EDGE, SLAB, PC>(a, G, wo, tp, U, C, D, E, queue, a.mir_up + kw, (kw << 4) | (1u << 30));
             else
-                march_row<COLOUR, EDGE, SLAB, PC>(a, G, wo, tp, U, C, D, E, queue);
+                march_row<COLOUR, EDGE, SLAB, PC, REC>(a, G, wo, tp, U, C, D, E, queue, nullptr, 0, rec);
             U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
         {   // row i0 + r + 1: the other parity; its row i + 1 wraps to row 0 at the lattice end
@@ -318,7 +363,7 @@ __device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g
             if (SLAB && bot && r + 2 == a.R)
                 march_row<COLOUR ^ 1, EDGE, SLAB, PC>(a, G, wo, tp, U, C, D, E, queue, a.mir_dn + kw, (kw << 4) | (2u << 30));
             else
-                march_row<COLOUR ^ 1, EDGE, SLAB, PC>(a, G, wo, tp, U, C, D, E, queue);
+                march_row<COLOUR ^ 1, EDGE, SLAB, PC, REC>(a, G, wo, tp, U, C, D, E, queue, nullptr, 0, rec);
             U = C; C = D; op = dn; tp += wpr; wo += wpr; G += nq;
         }
     }
@@ -329,8 +374,8 @@ __device__ __forceinline__ void march_thread(const IsingMarchArgs &a, uint32_t g
 // even though every thread now loads all three neighbour rows itself).  g enumerates
 // (row slot s, run q) with the even rows first and the odd rows after them, so that every warp
 // works on rows of one parity (wpr/4 * L/2 is a multiple of 32) and the branch is warp-uniform.
-template <int COLOUR, bool EDGE>
-__device__ __forceinline__ void row_thread(const IsingMarchArgs &a, uint32_t g, WarpTieQueue<false> &queue)
+template <int COLOUR, bool EDGE, class Queue>
+__device__ __forceinline__ void row_thread(const IsingMarchArgs &a, uint32_t g, Queue &queue)
 {
     const uint32_t L = a.L, wpr = a.wpr, nq = wpr >> 2, half = L >> 1;
     const uint32_t q = g % nq, s = g / nq;
@@ -369,16 +414,38 @@ __global__ void __launch_bounds__(256) ising_row_kernel(const IsingMarchArgs a)
 //   0xAD10  T_2 = 2.27414861561203 of the same protocol, and beta_c/1.01 (plateau of config 5a)
 #define LAT_ISING_PC_LIST(X) X(0xF910) X(0x7440) X(0xAD10)
 
-template <int COLOUR, bool EDGE, bool SLAB, int PC = -1>
+template <int COLOUR, bool EDGE, bool SLAB, int PC = -1, bool REC = false>
 __global__ void __launch_bounds__(256) ising_march_kernel(const IsingMarchArgs a)
 {
     __shared__ uint4 s_q[8][TIE_Q_SLOTS];
+    __shared__ unsigned int s_rec[4];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
     const uint32_t g = blockIdx.x * 256u + threadIdx.x;
+    if constexpr (REC) {
+        if (threadIdx.x < 4) s_rec[threadIdx.x] = 0;
+        __syncthreads();
+    }
     if (g - lane >= a.threads) return;          // a.threads is a multiple of 32: whole warps only
-    WarpTieQueue<SLAB> queue{a, s_q[warp], lane, 0u};
-    march_thread<COLOUR, EDGE, SLAB, PC>(a, g, queue);
+    WarpTieQueue<SLAB, REC> queue{a, s_q[warp], lane, 0u};
+    RecAcc rec{0u, 0u, 0u, 0u};
+    march_thread<COLOUR, EDGE, SLAB, PC, REC>(a, g, queue, &rec);
     queue.drain();
+    if constexpr (REC) {
+        // thread -> warp (REDUX) -> block (shared atomics) -> one of REC_SLOTS counter sets; a thread's
+        // sums may be "negative" (it only corrected late flips of other threads' rows): the sums are
+        // modulo 2^32 and a warp's total is the exact count of its own rows
+        const uint32_t v[4] = {__reduce_add_sync(0xffffffffu, rec.ax + (uint32_t)queue.rx),
+                               __reduce_add_sync(0xffffffffu, rec.ay + (uint32_t)queue.ry),
+                               __reduce_add_sync(0xffffffffu, rec.mw + (uint32_t)queue.rm),
+                               __reduce_add_sync(0xffffffffu, rec.mb)};
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) atomicAdd(&s_rec[k], v[k]);
+        }
+        __syncthreads();                        // warps that returned above have exited: they do not count
+        if (threadIdx.x < 4)
+            atomicAdd(a.rec + (blockIdx.x % REC_SLOTS) * 4u + threadIdx.x, (unsigned long long)s_rec[threadIdx.x]);
+    }
 }
 #endif
 

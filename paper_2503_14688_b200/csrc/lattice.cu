@@ -217,7 +217,9 @@ static int ising_packed_pc(const uint32_t (&pcase)[8])
     return pc;
 }
 
-int launch_ising_march(lattice *lat, int colour)
+// rec != nullptr (white half-sweep of a whole lattice on the marching kernel only): also count the r = 1
+// record into rec[REC_SLOTS][4] (ising_march.cuh, REC)
+int launch_ising_march(lattice *lat, int colour, unsigned long long *rec = nullptr)
 {
     const uint32_t wpr = lat->wpr, nq = wpr / 4u;
     const size_t pw = (size_t)lat->rows * wpr;
@@ -240,9 +242,30 @@ int launch_ising_march(lattice *lat, int colour)
     a.R = march_rows(lat->n_own, nq);
     a.threads = nq * (lat->n_own / a.R);
     a.K = lat->K;
+    a.rec = rec;
     build_plane_fold(lat->K, a.t, a.colour, TAG_ACC_PLANE, a.F);
     const unsigned blocks = (a.threads + 255u) / 256u;
     const bool edge = always4 || always8;
+    if (rec) {
+        if (lat->slab || colour != 1 || ising_one_row(lat)) return LATTICE_EINVAL;
+        bool done = false;
+        if (!edge) {
+            switch (ising_packed_pc(a.pcase)) {
+#define LAT_PC_CASE(V) case V: ising_march_kernel<1, false, false, V, true><<<blocks, 256, 0, lat->stream>>>(a); done = true; break;
+            LAT_ISING_PC_LIST(LAT_PC_CASE)
+#undef LAT_PC_CASE
+            default: break;
+            }
+            if (done) lat->spec_launches += 1;
+        }
+        if (!done) {
+            if (edge) ising_march_kernel<1, true, false, -1, true><<<blocks, 256, 0, lat->stream>>>(a);
+            else ising_march_kernel<1, false, false, -1, true><<<blocks, 256, 0, lat->stream>>>(a);
+        }
+        lat->launches += 1;
+        CU(lat, cudaGetLastError());
+        return LATTICE_OK;
+    }
 #define LAT_LAUNCH_MARCH(C, E, S) ising_march_kernel<C, E, S><<<blocks, 256, 0, lat->stream>>>(a)
     if (lat->slab) {
         if (colour == 0) { if (edge) LAT_LAUNCH_MARCH(0, true, true); else LAT_LAUNCH_MARCH(0, false, true); }
@@ -1267,6 +1290,49 @@ int lattice_sweep(lattice_t *lat, uint64_t n, const double *beta)
         }
         break;
     }
+    return LATTICE_OK;
+}
+
+// n sweeps followed by the r = 1 record of the final state, with the record counted INSIDE the last
+// white half-sweep where that kernel exists (Ising, bit-plane schemes, whole lattice on the marching
+// kernel, i.e. L a multiple of 256 and L > 4352); otherwise lattice_sweep + lattice_measure(1).
+int lattice_sweep_record(lattice_t *lat, uint64_t n, const double *beta, int64_t *M, int64_t *Q, int64_t *Sx1,
+                         int64_t *Sy1)
+{
+    if (!lat || !M || !Q || !Sx1 || !Sy1 || (n && !beta)) return LATTICE_EINVAL;
+    if (lat->parent || lat->n_rep || lat->view) return LATTICE_ESTATE;
+    const bool fused = n >= 1 && lat->model == LATTICE_ISING && lat->scheme >= 1 && (lat->wpr % 4u) == 0 && !lat->slab &&
+                       !ising_one_row(lat);
+    if (!fused) {
+        const int rc = lattice_sweep(lat, n, beta);
+        if (rc) return rc;
+        return lattice_measure(lat, 1, M, Q, Sx1, Sy1);
+    }
+    int rc = lattice_sweep(lat, n - 1, beta);                       // validates all but the last beta
+    if (rc) return rc;
+    const double b = beta[n - 1];
+    if (std::isnan(b) || b < 0.0 || lat->t + 1 >= TWO32) return LATTICE_EINVAL;
+    const size_t entries = (size_t)REC_SLOTS * 4;
+    rc = ensure_cnt(lat, entries);
+    if (rc) return rc;
+    CU(lat, cudaMemsetAsync(lat->d_cnt, 0, entries * sizeof(unsigned long long), lat->stream));
+    refresh_thresholds(lat, b);
+    rc = launch_half_sweep(lat, 0);
+    if (rc) return rc;
+    rc = launch_ising_march(lat, 1, lat->d_cnt);
+    if (rc) return rc;
+    lat->t += 1;
+    unsigned long long h[REC_SLOTS * 4];
+    cudaError_t e = cudaMemcpyAsync(h, lat->d_cnt, sizeof h, cudaMemcpyDeviceToHost, lat->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(lat->stream);
+    if (e != cudaSuccess) return cuda_fail(lat, e, "record copy/sync");
+    unsigned long long ax = 0, ay = 0, mw = 0, mb = 0;
+    for (int k = 0; k < REC_SLOTS; ++k) { ax += h[4 * k]; ay += h[4 * k + 1]; mw += h[4 * k + 2]; mb += h[4 * k + 3]; }
+    const int64_t N = (int64_t)lat->L * (int64_t)lat->L;
+    *M = 2 * (int64_t)(mw + mb) - N;
+    *Q = N;
+    *Sx1 = N - 2 * (int64_t)ax;
+    *Sy1 = N - 2 * (int64_t)ay;
     return LATTICE_OK;
 }
 
