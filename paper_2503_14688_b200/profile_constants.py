@@ -25,13 +25,13 @@ CAPTURED = {
     0: {"kernel": "ising_march_kernel",
         "executed_half_rate_instr_per_update": 3.21,      # (ALU-pipe + IMAD.WIDE/HI thread-instr) / updates, SASS page
         "dram_bytes_per_update": 0.383,                   # (dram__bytes_read + dram__bytes_write) / updates at L = 2^20
-        "profile": "profiles/r2_ising_march.md + profiles/r2_launches_default.md", "commit": "e1060ac",
-        "sources_sha256": "01d681f2d6da49703698b8d24fdf470e4c84f57c4811b7f0eaff6f99018958df"},
+        "profile": "profiles/r2_ising_march.md + profiles/r2_launches_default.md", "commit": "628ec9c",
+        "sources_sha256": "2409eae7a91bbd271cf2918bdd840392e292198010a17babc312a02761846a75"},
     1: {"kernel": "bc_march_kernel",
         "executed_half_rate_instr_per_update": 4.65,     # tables compiled in (LS >= 0); 4.77 with the dispatching kernel
         "dram_bytes_per_update": 0.768,                   # at L = 2^19 (launch list); 0.669 at L = 2^15 (partly L2-resident)
-        "profile": "profiles/r2_bc_march.md + profiles/r2_launches_default.md", "commit": "deef1e5",
-        "sources_sha256": "cfcb415b1045923498fc6138aecccde54c402ed7f70c743103bb9c5570bea577"},
+        "profile": "profiles/r2_bc_march.md + profiles/r2_launches_default.md", "commit": "628ec9c",
+        "sources_sha256": "e53bde8a311852275e9e46dec8dca1350233819e23768e4f3f56738bb2de0d45"},
 }
 
 #: Algorithmic half-rate thread-instructions per update: the floor of the method under the RNG
