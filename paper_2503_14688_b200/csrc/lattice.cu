@@ -100,6 +100,17 @@ int cuda_fail(lattice *lat, cudaError_t e, const char *what)
     return LATTICE_ECUDA;
 }
 
+// cudaFuncSetAttribute applies to the device that is current: opt-ins for more than 48 KiB of dynamic
+// shared memory are remembered per device ordinal, not per process (one process may drive several GPUs)
+bool first_use_on_current_device(bool (&seen)[64])
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return true; }
+    if (seen[dev]) return false;
+    seen[dev] = true;
+    return true;
+}
+
 #define CU(lat, call)                                                   \
     do {                                                                \
         cudaError_t e_ = (call);                                        \
@@ -424,13 +435,12 @@ int launch_bc_march(lattice *lat, int colour, bool gen = false)
     const unsigned blocks = (a.threads + 255u) / 256u;
     const size_t dyn = gen ? (size_t)8 * 3 * TIE_Q_SLOTS * sizeof(uint4) : 0;       // the general tie queue
     if (gen) {
-        static bool opted = false;                       // > 48 KiB of dynamic shared memory: opt in once
-        if (!opted) {
+        static bool opted[64];                           // > 48 KiB of dynamic shared memory: opt in once per device
+        if (first_use_on_current_device(opted)) {
             cudaFuncSetAttribute(bc_march_kernel<0, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
             cudaFuncSetAttribute(bc_march_kernel<1, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
             cudaFuncSetAttribute(bc_march_kernel<0, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
             cudaFuncSetAttribute(bc_march_kernel<1, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-            opted = true;
         }
     }
 #define LAT_LAUNCH_BC(C, S, G) bc_march_kernel<C, S, G><<<blocks, 256, dyn, lat->stream>>>(a)
@@ -1429,8 +1439,8 @@ static bool corr_tc_applies(const lattice *lat, uint64_t n_rows, uint32_t r_max)
 
 static int enqueue_corr_tc(lattice *lat, unsigned long long *cnt, uint64_t i0, uint64_t n_rows, uint32_t r_max)
 {
-    static bool opted = false;
-    if (!opted) {
+    static bool opted[64];
+    if (first_use_on_current_device(opted)) {
         cudaFuncSetAttribute(corr_tc_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
         cudaFuncSetAttribute(corr_tc_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
         cudaFuncSetAttribute(corr_tc_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM_BYTES);
@@ -1439,7 +1449,6 @@ static int enqueue_corr_tc(lattice *lat, unsigned long long *cnt, uint64_t i0, u
         cudaFuncSetAttribute(corr_tc2_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM_BYTES);
         cudaFuncSetAttribute(corr_tc2_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM_BYTES);
         cudaFuncSetAttribute(corr_tc2_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, T2_SMEM_BYTES);
-        opted = true;
     }
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
