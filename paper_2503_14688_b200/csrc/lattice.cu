@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "bc.cuh"
@@ -102,8 +103,11 @@ int cuda_fail(lattice *lat, cudaError_t e, const char *what)
 
 // cudaFuncSetAttribute applies to the device that is current: opt-ins for more than 48 KiB of dynamic
 // shared memory are remembered per device ordinal, not per process (one process may drive several GPUs)
+std::mutex g_setup_mutex;      // per-process set-up state shared by all handles (different handles may be used from different threads)
+
 bool first_use_on_current_device(bool (&seen)[64])
 {
+    std::lock_guard<std::mutex> lock(g_setup_mutex);
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return true; }
     if (seen[dev]) return false;
@@ -1751,6 +1755,7 @@ static unsigned long long *g_static_cnt_ptr[64];             // per device ordin
 
 static int static_cnt_for_current_device(lattice *lat, unsigned long long **out)
 {
+    std::lock_guard<std::mutex> lock(g_setup_mutex);
     int dev = -1;
     CU(lat, cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64) return LATTICE_EINVAL;
