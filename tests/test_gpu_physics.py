@@ -97,6 +97,41 @@ def test_dynamic_exponent_z_from_replicas_matches_the_paper():
     ex = np.array([x.mean() for x in e]) + math.sqrt(2)
     slope = math.log(ex[-1] / ex[6]) / math.log(times[-1] / times[6])
     assert abs(slope + 1 / Z) < 0.06
+    # xi and E of the same runs with ONE z (the joint fit of Fig. 3)
+    keep = [k for k, t in enumerate(times) if t >= 16]
+    E_mean = np.array([e[k].mean() for k in keep])
+    E_err = np.array([e[k].std(ddof=1) / math.sqrt(len(e[k])) for k in keep])
+    tk = [times[k] for k in keep]
+    joint = analysis.fit_z_joint([{"kind": "xi", "t": tk, "xi": fit["xi"][keep], "xi_err": fit["xi_err"][keep]},
+                                  {"kind": "E", "t": tk, "E": E_mean, "E_err": E_err}])
+    assert joint["dof"] == 2 * len(keep) - 6 and joint["Q"] > 0.01, joint
+    assert abs(joint["z"] - Z) < 0.08, joint
+
+
+def test_dynamic_exponent_z_from_the_energy_matches_the_paper():
+    """z from the local observable alone (Eq. 6 / D2): 32 independent quenches of
+    an L = 8192 Ising lattice to T_c as ONE batch handle (lattice_create_batch), e(t) recorded at 45
+    quarter-octave times 16 <= t <= 2^15 (15 s of GPU), E - E_eq = b t^(-1/z) + b' t^(-2/z) + b''
+    t^(-(omega + 1/nu)/z) with E_eq = -sqrt 2 exact, jackknife over the runs.  This build's numbers
+    (seeded, they repeat): z = 2.175(13), chi^2/dof = 37.0/41, Q = 0.65 -- the paper's 2.1676(1) within
+    one sigma."""
+    L, n_rep, t_end = 8192, 32, 1 << 15
+    seeds = np.arange(n_rep, dtype=np.uint64) * 104729 + 2503146890
+    b = lat.LatticeBatch(L, seeds)
+    times = sorted({int(round(2 ** (k / 4))) for k in range(16, 4 * 15 + 1)})
+    E = []
+    for t in times:
+        b.sweep(np.full(t - b.time, workloads.BETA_C_ISING))
+        M, Q, Sx, Sy = b.measure(1)
+        E.append(-(Sx[:, 0] + Sy[:, 0]) / float(L * L))
+    b.close()
+    fit = analysis.fit_z_energy_jackknife(times, E, t_min=16)
+    assert fit["dof"] == len(times) - 4 and fit["Q"] > 0.05 and fit["chi2"] / fit["dof"] < 1.6, fit
+    assert 0 < fit["z_err"] < 0.03
+    assert abs(fit["z"] - Z) < max(3 * fit["z_err"], 0.03), fit
+    assert fit["b"] > 0                                   # approach from above (PAPER.md:60)
+    e_mean = fit["E"]
+    assert (np.diff(e_mean) < 0).all() and e_mean[-1] > -math.sqrt(2)
 
 
 @pytest.mark.parametrize("name,e_plateau", [("ising_L2p16_ramp", -1.3583), ("bc_L2p15_ramp", -1.0993)])
